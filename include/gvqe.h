@@ -1,0 +1,124 @@
+/*
+ * gvqe.h -- C ABI of libgvqe: batched statevector VQE energy engine for NVIDIA B200 (sm_100a).
+ *
+ * Hot path of Graph-VQE (arxiv/paper_2607_02749; citations are lines of /root/reference/PAPER.md):
+ *   |psi(theta)> = U(theta)|0>^N  for a hardware-efficient RY/RZ + CZ/CNOT ansatz   PAPER.md:169-179 (Eq. 7, 8)
+ *   E(theta) = <psi|H|psi>,  H = sum_k c_k P_k,  c_k real, P_k in {I,X,Y,Z}^N        PAPER.md:135 (Eq. 4), 148-153 (Eq. 6)
+ *   E = sum_j <psi|H_j|psi> over any partition of the terms ("Hamiltonian batching")  PAPER.md:214-219 (Eq. 12)
+ *   restricted objective: only the block's parameters move                          PAPER.md:207-212 (Eq. 11)
+ *   dE/dtheta_i = 1/2 [E(theta + pi/2 e_i) - E(theta - pi/2 e_i)]                     PAPER.md:221-225 (Eq. 13)
+ *
+ * Conventions: qubit q <-> bit q of the amplitude index (LSB = qubit 0); character j
+ * of a Pauli string acts on qubit j; R_y, R_z exactly as Eq. 7; ops are applied in list order.
+ *
+ * Memory: every "host" pointer is ordinary host memory, borrowed for the duration of the call (inputs are
+ * copied).  ALL device memory is the caller's workspace (gvqe_set_workspace); the library allocates none.
+ * Errors: every call returns a gvqe_status; gvqe_last_error gives the message.  There is no CPU fallback:
+ * a missing/failed CUDA device is GVQE_ERR_CUDA.  Results are deterministic: identical inputs give
+ * bit-identical outputs (no floating-point atomics).  A context is not thread-safe.
+ */
+#ifndef GVQE_H
+#define GVQE_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gvqe_ctx gvqe_ctx; /* opaque, owned by the library, freed by gvqe_destroy */
+
+typedef enum {
+    GVQE_OK = 0,
+    GVQE_ERR_INVALID_ARG = 1,
+    GVQE_ERR_NO_HAMILTONIAN = 2,
+    GVQE_ERR_WORKSPACE = 3,
+    GVQE_ERR_UNSUPPORTED = 4,
+    GVQE_ERR_CUDA = 5
+} gvqe_status;
+
+typedef enum { GVQE_C64 = 0, GVQE_C128 = 1 } gvqe_precision;
+typedef enum { GVQE_OP_RY = 0, GVQE_OP_RZ = 1, GVQE_OP_CZ = 2, GVQE_OP_CNOT = 3 } gvqe_opkind;
+
+/* One gate.  RY/RZ: qubit q0, angle params[param], q1 = -1.  CZ: qubits q0,q1, param = -1.
+ * CNOT: target q0, control q1, param = -1.  A parameter may drive at most one gate (Eq. 13 is then exact). */
+typedef struct { int32_t kind, q0, q1, param; } gvqe_op;
+
+/* Layered ansatz: for l in 0..n_layers-1: RY(theta[2Nl+q]) all q, RZ(theta[2Nl+N+q]) all q,
+ * entanglers (q,q+1) ascending (CNOT: control q, target q+1), then (N-1 -> 0) if topology == 1;
+ * finally RY(theta[2ND+q]) (and RZ(theta[2ND+N+q]) if final_rot == 2, which gives Eq. 8's P = 2N(D+1)). */
+typedef struct {
+    int32_t n_layers;  /* D >= 0 */
+    int32_t entangler; /* GVQE_OP_CZ or GVQE_OP_CNOT */
+    int32_t topology;  /* 0 linear chain, 1 ring */
+    int32_t final_rot; /* 1 = RY only, 2 = RY then RZ */
+} gvqe_layout;
+
+/* Create a context (host only; touches no GPU).  1 <= n_qubits <= 34.  *out receives the context. */
+gvqe_status gvqe_create(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, gvqe_ctx **out);
+/* Same from an explicit op list (host, n_ops entries; params are indices in [0, n_params)). */
+gvqe_status gvqe_create_ops(int n_qubits, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec,
+                            gvqe_ctx **out);
+int gvqe_num_params(const gvqe_ctx *ctx);
+int gvqe_num_qubits(const gvqe_ctx *ctx);
+
+/* Hamiltonian, Eq. 6.  paulis: host, n_terms * n_qubits characters of "IXYZ" (no separators, character j of a
+ * term acts on qubit j); coeffs: host, n_terms finite doubles.  Identity and duplicate terms are legal.
+ * Host work only (parse -> masks -> flip-mask groups); device tables are (re)built on the next energy call. */
+gvqe_status gvqe_set_hamiltonian(gvqe_ctx *ctx, int n_terms, const char *paulis, const double *coeffs);
+/* Same from masks: x_mask = qubits with X or Y, z_mask = qubits with Z or Y (so Y = both bits). */
+gvqe_status gvqe_set_hamiltonian_masks(gvqe_ctx *ctx, int n_terms, const uint64_t *x_mask, const uint64_t *z_mask,
+                                       const double *coeffs);
+/* Integer side of the grouping (bit-exact contract): per term x_mask, z_mask, n_Y mod 4, group index; groups are
+ * the distinct x_mask values in ascending unsigned order (group_mask[g]).  Output arrays are host, caller-owned,
+ * sized n_terms (group_mask: n_terms is always enough); any may be NULL. */
+gvqe_status gvqe_get_grouping(const gvqe_ctx *ctx, uint64_t *x_mask, uint64_t *z_mask, uint8_t *ny_mod4,
+                              int32_t *group_of_term, int32_t *n_groups, uint64_t *group_mask);
+
+/* Device workspace.  gvqe_workspace_bytes: bytes needed to keep `batch_in_flight` statevectors resident (plus
+ * tables and scratch); 0 on error.  Call after gvqe_set_hamiltonian.  gvqe_set_workspace: device_ptr is DEVICE
+ * memory (256-byte aligned) owned by the caller, which must stay valid until gvqe_destroy or the next
+ * gvqe_set_workspace; too small for one statevector -> GVQE_ERR_WORKSPACE.  Larger batches are streamed in
+ * chunks of as many statevectors as fit (at most max_in_flight if that was set > 0). */
+size_t gvqe_workspace_bytes(const gvqe_ctx *ctx, int batch_in_flight);
+gvqe_status gvqe_set_workspace(gvqe_ctx *ctx, void *device_ptr, size_t bytes);
+gvqe_status gvqe_set_max_in_flight(gvqe_ctx *ctx, int max_in_flight);
+
+/* E[b] = <psi(params[b])|H|psi(params[b])>, Eq. 4.  params: HOST, B x P row-major doubles (finite); E: HOST, B
+ * doubles.  cuda_stream: a cudaStream_t (NULL = default stream).  Returns after E is on the host. */
+gvqe_status gvqe_energy_batch(gvqe_ctx *ctx, const double *params, int B, double *E, void *cuda_stream);
+/* Same with DEVICE pointers (params_dev: B x P doubles, E_dev: B doubles); asynchronous on the stream, no host
+ * copies or synchronisation.  This is the entry the device-resident timing uses. */
+gvqe_status gvqe_energy_batch_device(gvqe_ctx *ctx, const double *params_dev, int B, double *E_dev, void *cuda_stream);
+
+/* Eq. 13 over the parameters with mask[p] != 0 (Eq. 11: the cluster's parameters).  params: HOST, P doubles;
+ * mask: HOST, P bytes; dE: HOST, P doubles (0 where mask is 0); E0: HOST, optional (NULL allowed), receives
+ * E(params).  The 2|mask|+1 evaluations run as one batch (row 0 = theta, rows 2j+1 / 2j+2 = +/- pi/2 on the
+ * j-th masked parameter). */
+gvqe_status gvqe_param_shift_grad(gvqe_ctx *ctx, const double *params, const uint8_t *mask, double *dE, double *E0,
+                                  void *cuda_stream);
+
+/* Test hook: amplitudes (interleaved re,im in the context's precision, 2^n of them) of in-flight slot `slot`
+ * as left by the last energy call, copied to host_out (HOST). */
+gvqe_status gvqe_get_state(gvqe_ctx *ctx, int slot, void *host_out);
+
+/* Introspection of the compiled schedule (host; for tests and traffic accounting).
+ * gvqe_schedule_info: number of fused gate blocks, number of off-diagonal passes, statevectors in flight.
+ * gvqe_dump_schedule: writes a text description of every block/stage/op into buf (NUL-terminated, truncated to
+ * cap); returns the full length needed. */
+gvqe_status gvqe_schedule_info(const gvqe_ctx *ctx, int32_t *n_gate_blocks, int32_t *n_offdiag_passes,
+                               int32_t *in_flight);
+size_t gvqe_dump_schedule(const gvqe_ctx *ctx, char *buf, size_t cap);
+/* The order in which the device executes the input ops (indices into the op list, each exactly once; the
+ * compiler only reorders ops that commute).  order: host, cap entries; returns the number of ops. */
+int gvqe_get_exec_order(const gvqe_ctx *ctx, int32_t *order, int cap);
+/* Kernel launches issued by this context since creation (for bench.py's gpu_launches). */
+uint64_t gvqe_launch_count(const gvqe_ctx *ctx);
+
+const char *gvqe_last_error(const gvqe_ctx *ctx);
+void gvqe_destroy(gvqe_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GVQE_H */

@@ -1,0 +1,404 @@
+// schedule.cpp -- host-side schedule compiler (see schedule.h, program.h).
+//
+// Two levels of the same greedy "take what commutes forward" pass:
+//   block level: choose tile bits T; an op can run in this block if every qubit it acts on NON-diagonally
+//                (RY qubit, CNOT target) is in T and it commutes with every earlier op that was left behind.
+//   stage level: inside a block choose register bits Rset (subset of T); non-diagonal ops need their qubit in
+//                Rset; diagonal ops (RZ, CZ) are collected and flushed as one merged diagonal segment.
+// Commutation rule used: two ops commute if on every qubit they share BOTH act diagonally (RZ, CZ and the
+// control side of a CNOT are diagonal in the computational basis).  So a skipped op marks the qubits it touches
+// diagonally as "no later non-diagonal op" (nd) and the qubits it touches non-diagonally as fully blocked.
+#include "schedule.h"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+
+namespace gv {
+namespace {
+
+struct Acts { int nq; int q[2]; bool diag[2]; };
+
+inline Acts acts_of(const HostOp &o)
+{
+    Acts a{};
+    switch (o.kind) {
+    case 0: a.nq = 1; a.q[0] = o.q0; a.diag[0] = false; break;                                   // RY
+    case 1: a.nq = 1; a.q[0] = o.q0; a.diag[0] = true; break;                                    // RZ
+    case 2: a.nq = 2; a.q[0] = o.q0; a.q[1] = o.q1; a.diag[0] = a.diag[1] = true; break;          // CZ
+    default: a.nq = 2; a.q[0] = o.q0; a.diag[0] = false; a.q[1] = o.q1; a.diag[1] = true; break;  // CNOT
+    }
+    return a;
+}
+inline bool is_diag(const HostOp &o) { return o.kind == 1 || o.kind == 2; }
+
+// ---- block level -------------------------------------------------------------------------------------------
+struct BlockTake { std::vector<int> taken; int n_nondiag = 0; };
+
+void block_take(const std::vector<HostOp> &ops, const std::vector<int> &pending, uint64_t T, int n, BlockTake &out)
+{
+    out.taken.clear();
+    out.n_nondiag = 0;
+    uint64_t full = 0, nd = 0;
+    const uint64_t all = (n >= 64) ? ~0ull : ((1ull << n) - 1);
+    for (int idx : pending) {
+        const HostOp &o = ops[idx];
+        const Acts a = acts_of(o);
+        bool ok = true;
+        for (int i = 0; i < a.nq; ++i) {
+            const uint64_t b = 1ull << a.q[i];
+            if (full & b) ok = false;
+            if (!a.diag[i] && ((nd & b) || !(T & b))) ok = false;
+        }
+        if (ok) {
+            out.taken.push_back(idx);
+            if (!is_diag(o)) ++out.n_nondiag;
+        } else {
+            for (int i = 0; i < a.nq; ++i) {
+                const uint64_t b = 1ull << a.q[i];
+                if (a.diag[i]) nd |= b; else full |= b;
+            }
+            if ((full & all) == all) break;
+        }
+    }
+}
+
+int count_runs(uint64_t T)
+{
+    int runs = 0;
+    while (T) {
+        const int lo = __builtin_ctzll(T);
+        uint64_t t = T >> lo;
+        int len = 0;
+        while (t & 1) { t >>= 1; ++len; }
+        ++runs;
+        T &= ~(((len >= 64) ? ~0ull : ((1ull << len) - 1)) << lo);
+    }
+    return runs;
+}
+
+// candidate tile-bit sets: [0,f) + every contiguous window of k-f qubits + "first needed" set
+void block_candidates(const std::vector<HostOp> &ops, const std::vector<int> &pending, int n, int k, int f,
+                      std::vector<uint64_t> &cand)
+{
+    cand.clear();
+    if (n <= k) { cand.push_back((1ull << n) - 1); return; }
+    const uint64_t low = (1ull << f) - 1;
+    const int h = k - f;
+    for (int a = f; a + h <= n; ++a) cand.push_back(low | (((1ull << h) - 1) << a));
+    // first-needed: non-diagonal qubits >= f in pending order
+    uint64_t T = low;
+    int cnt = 0;
+    for (int idx : pending) {
+        const Acts a = acts_of(ops[idx]);
+        for (int i = 0; i < a.nq && cnt < h; ++i)
+            if (!a.diag[i] && a.q[i] >= f && !(T >> a.q[i] & 1)) { T |= 1ull << a.q[i]; ++cnt; }
+        if (cnt >= h) break;
+    }
+    // pad next to already chosen bits (keeps the number of runs small), then anywhere
+    for (int pass = 0; pass < 2 && cnt < h; ++pass)
+        for (int q = f; q < n && cnt < h; ++q) {
+            if (T >> q & 1) continue;
+            const bool adj = (q > 0 && (T >> (q - 1) & 1)) || (q + 1 < n && (T >> (q + 1) & 1));
+            if (pass == 1 || adj) { T |= 1ull << q; ++cnt; }
+        }
+    if (count_runs(T) <= MAX_RUNS && std::find(cand.begin(), cand.end(), T) == cand.end()) cand.push_back(T);
+}
+
+}  // namespace
+}  // namespace gv
+
+// ---- stage level -------------------------------------------------------------------------------------------
+namespace gv {
+namespace {
+
+struct StageItem { bool is_seg; int op; std::vector<int> seg_ops; };  // op / seg_ops index the block's op list
+
+struct StageTake {
+    std::vector<StageItem> items;
+    std::vector<int> carry;      // diagonal ops taken but not yet flushed
+    std::vector<int> rest;       // ops left for later stages (block-list positions)
+    int n_nondiag = 0, n_seg = 0;
+};
+
+// bops: the block's ops in execution order; L: positions (into bops) still to run; carry: pending diagonals.
+// Rset: register qubits (global ids).  flush_anywhere: allow a diagonal flush after a non-diagonal op of this stage.
+void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, const std::vector<int> &carry_in,
+                uint64_t Rset, bool flush_anywhere, StageTake &out)
+{
+    out.items.clear(); out.rest.clear(); out.n_nondiag = 0; out.n_seg = 0;
+    std::vector<int> pend = carry_in;
+    uint64_t pend_touch = 0;
+    for (int p : pend) { const Acts a = acts_of(bops[p]); for (int i = 0; i < a.nq; ++i) pend_touch |= 1ull << a.q[i]; }
+    uint64_t full = 0, nd = 0;
+    for (int pos : L) {
+        const HostOp &o = bops[pos];
+        const Acts a = acts_of(o);
+        bool ok = true;
+        uint64_t ndq = 0;
+        for (int i = 0; i < a.nq; ++i) {
+            const uint64_t b = 1ull << a.q[i];
+            if (full & b) ok = false;
+            if (!a.diag[i]) { ndq |= b; if ((nd & b) || !(Rset & b)) ok = false; }
+        }
+        if (ok && !is_diag(o) && (pend_touch & ndq) && !flush_anywhere && out.n_nondiag > 0) ok = false;
+        if (ok) {
+            if (is_diag(o)) {
+                pend.push_back(pos);
+                for (int i = 0; i < a.nq; ++i) pend_touch |= 1ull << a.q[i];
+            } else {
+                if (pend_touch & ndq) {  // a pending diagonal touches a qubit this op changes: flush first
+                    StageItem s; s.is_seg = true; s.op = -1; s.seg_ops.swap(pend);
+                    out.items.push_back(std::move(s)); ++out.n_seg;
+                    pend.clear(); pend_touch = 0;
+                }
+                StageItem it; it.is_seg = false; it.op = pos;
+                out.items.push_back(std::move(it)); ++out.n_nondiag;
+            }
+        } else {
+            out.rest.push_back(pos);
+            for (int i = 0; i < a.nq; ++i) {
+                const uint64_t b = 1ull << a.q[i];
+                if (a.diag[i]) nd |= b; else full |= b;
+            }
+        }
+    }
+    out.carry.swap(pend);
+}
+
+}  // namespace
+}  // namespace gv
+
+// ---- driver --------------------------------------------------------------------------------------------------
+namespace gv {
+namespace {
+
+// local bit position of global qubit q inside tile-bit set T
+inline int local_pos(uint64_t T, int q) { return __builtin_popcountll(T & ((1ull << q) - 1)); }
+
+void stage_candidates(const std::vector<HostOp> &bops, const std::vector<int> &L, uint64_t T, int k, int R,
+                      std::vector<uint64_t> &cand)
+{
+    cand.clear();
+    std::vector<int> tq;  // local -> global
+    for (int q = 0; q < 64; ++q) if (T >> q & 1) tq.push_back(q);
+    for (int p = 0; p + R <= k; ++p) {
+        uint64_t s = 0;
+        for (int j = 0; j < R; ++j) s |= 1ull << tq[p + j];
+        cand.push_back(s);
+    }
+    uint64_t s = 0; int cnt = 0;
+    for (int pos : L) {
+        const Acts a = acts_of(bops[pos]);
+        for (int i = 0; i < a.nq && cnt < R; ++i)
+            if (!a.diag[i] && !(s >> a.q[i] & 1)) { s |= 1ull << a.q[i]; ++cnt; }
+        if (cnt >= R) break;
+    }
+    for (int p = 0; p < k && cnt < R; ++p) if (!(s >> tq[p] & 1)) { s |= 1ull << tq[p]; ++cnt; }
+    if (std::find(cand.begin(), cand.end(), s) == cand.end()) cand.push_back(s);
+}
+
+// bank-conflict proxy for the swizzle phys = j ^ ((j >> 4) & 15): lanes vary the lowest 4 non-register local bits;
+// a pair (b, b+4) with both bits lane-varying collides.
+int conflict_penalty(uint64_t T, uint64_t Rset, int k)
+{
+    int lane_bits[4], nl = 0;
+    for (int p = 0; p < k && nl < 4; ++p) {
+        int q = -1, c = 0;
+        for (int g = 0; g < 64; ++g) if (T >> g & 1) { if (c == p) { q = g; break; } ++c; }
+        if (!(Rset >> q & 1)) lane_bits[nl++] = p;
+    }
+    int pen = 0;
+    for (int i = 0; i < nl; ++i) for (int j = 0; j < nl; ++j)
+        if (lane_bits[i] < 4 && lane_bits[j] == lane_bits[i] + 4) ++pen;
+    return pen;
+}
+
+}  // namespace
+
+bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &P, std::string &err)
+{
+    P = Program();
+    if (n < 1 || n > 40) { err = "schedule: bad qubit count"; return false; }
+    if (R < 1 || R > MAX_R) { err = "schedule: bad register-bit count"; return false; }
+    if (k > n) k = n;
+    if (k < R) { err = "schedule: tile smaller than register block"; return false; }
+    if (f > k) f = k;
+    if (n > k && k - f < 1) { err = "schedule: no free tile bits"; return false; }
+    P.n = n; P.k = k; P.f = f; P.R = R;
+    for (const HostOp &o : ops) {
+        const bool two = (o.kind == 2 || o.kind == 3);
+        if (o.kind < 0 || o.kind > 3 || o.q0 < 0 || o.q0 >= n || (two && (o.q1 < 0 || o.q1 >= n || o.q1 == o.q0))) {
+            err = "schedule: bad op"; return false;
+        }
+    }
+    std::vector<int> pending(ops.size());
+    for (size_t i = 0; i < ops.size(); ++i) pending[i] = (int)i;
+    std::vector<uint64_t> cand;
+    BlockTake bt, best;
+    bool first = true;
+    while (!pending.empty() || first) {
+        // ---- choose T
+        block_candidates(ops, pending, n, k, f, cand);
+        uint64_t bestT = cand[0];
+        best.taken.clear(); best.n_nondiag = -1;
+        for (uint64_t T : cand) {
+            block_take(ops, pending, T, n, bt);
+            if (bt.n_nondiag > best.n_nondiag ||
+                (bt.n_nondiag == best.n_nondiag && bt.taken.size() > best.taken.size())) {
+                best = bt; bestT = T;
+            }
+        }
+        if (best.taken.empty() && !pending.empty()) { err = "schedule: no progress (internal)"; return false; }
+        const uint64_t T = bestT;
+        // ---- block header
+        Block B; memset(&B, 0, sizeof B);
+        B.k = (uint8_t)k; B.source_zero = first ? 1 : 0;
+        {
+            int lp = 0, nr = 0;
+            for (int q = 0; q < n;) {
+                if (!(T >> q & 1)) { ++q; continue; }
+                int len = 0; while (q + len < n && (T >> (q + len) & 1)) ++len;
+                if (nr >= MAX_RUNS) { err = "schedule: too many tile runs (internal)"; return false; }
+                B.runs[nr].lpos = (uint8_t)lp; B.runs[nr].gpos = (uint8_t)q; B.runs[nr].len = (uint8_t)len; ++nr;
+                lp += len; q += len;
+            }
+            B.n_runs = (uint8_t)nr;
+        }
+        B.stage_begin = (uint32_t)P.stages.size();
+        // ---- stages
+        std::vector<HostOp> bops; bops.reserve(best.taken.size());
+        for (int idx : best.taken) bops.push_back(ops[idx]);
+        std::vector<int> L(bops.size()); for (size_t i = 0; i < bops.size(); ++i) L[i] = (int)i;
+        std::vector<int> carry;
+        std::vector<uint64_t> rc;
+        StageTake st, sbest;
+        uint32_t max_seg = 0;
+        while (!L.empty() || !carry.empty()) {
+            bool any_nd = false;
+            for (int pos : L) if (!is_diag(bops[pos])) { any_nd = true; break; }
+            uint64_t Rset = 0;
+            if (!any_nd) {  // only diagonals left: one closing segment
+                for (int pos : L) carry.push_back(pos);
+                L.clear();
+                sbest.items.clear(); sbest.rest.clear(); sbest.carry.clear();
+                StageItem s; s.is_seg = true; s.op = -1; s.seg_ops = carry;
+                sbest.items.push_back(s);
+                int cnt = 0; for (int q = 0; q < n && cnt < R; ++q) if (T >> q & 1) { Rset |= 1ull << q; ++cnt; }
+            } else {
+                stage_candidates(bops, L, T, k, R, rc);
+                double bscore = -1e30;
+                for (uint64_t rs : rc) for (int fa = 0; fa < 2; ++fa) {
+                    stage_take(bops, L, carry, rs, fa != 0, st);
+                    if (st.n_nondiag == 0) continue;
+                    const double score = st.n_nondiag - 2.0 * st.n_seg - 0.01 * conflict_penalty(T, rs, k);
+                    if (score > bscore) { bscore = score; sbest = st; Rset = rs; }
+                }
+                if (bscore < -1e29) { err = "schedule: stage made no progress (internal)"; return false; }
+                if (sbest.rest.empty() && !sbest.carry.empty()) {  // last stage of the block: flush what is pending
+                    StageItem s; s.is_seg = true; s.op = -1; s.seg_ops = sbest.carry;
+                    sbest.items.push_back(s); sbest.carry.clear();
+                }
+            }
+            // ---- emit the stage
+            Stage S; memset(&S, 0, sizeof S);
+            {
+                int slot = 0;
+                for (int q = 0; q < n; ++q) if (Rset >> q & 1) {
+                    S.regq[slot] = (uint8_t)q; S.regbit[slot] = (uint8_t)local_pos(T, q); ++slot;
+                }
+            }
+            auto slot_of = [&](int q) -> int { for (int s = 0; s < R; ++s) if (S.regq[s] == q) return s; return 255; };
+            S.op_begin = (uint32_t)P.mops.size();
+            S.seg_begin = (uint32_t)P.segs.size();
+            uint32_t nseg = 0;
+            for (const StageItem &it : sbest.items) {
+                MicroOp m; memset(&m, 0, sizeof m);
+                if (it.is_seg) {
+                    DiagSeg sg; sg.rz_begin = (uint32_t)P.rzs.size(); sg.cz_begin = (uint32_t)P.czs.size();
+                    for (int pos : it.seg_ops) {
+                        const HostOp &o = bops[pos];
+                        P.exec_order.push_back(best.taken[pos]);
+                        if (o.kind == 1) {
+                            DiagRZ r; r.qubit = (uint8_t)o.q0; r.slot = (uint8_t)slot_of(o.q0); r.pad = 0; r.param = o.param;
+                            P.rzs.push_back(r);
+                        } else {
+                            DiagCZ c; c.q0 = (uint8_t)o.q0; c.q1 = (uint8_t)o.q1;
+                            c.s0 = (uint8_t)slot_of(o.q0); c.s1 = (uint8_t)slot_of(o.q1);
+                            P.czs.push_back(c);
+                        }
+                    }
+                    sg.rz_end = (uint32_t)P.rzs.size(); sg.cz_end = (uint32_t)P.czs.size();
+                    m.kind = MOP_DIAG; m.param = (int32_t)P.segs.size();
+                    P.segs.push_back(sg); ++nseg;
+                } else {
+                    const HostOp &o = bops[it.op];
+                    P.exec_order.push_back(best.taken[it.op]);
+                    if (o.kind == 0) { m.kind = MOP_RY; m.a = (uint8_t)slot_of(o.q0); m.param = o.param; }
+                    else {
+                        m.kind = MOP_CX; m.a = (uint8_t)slot_of(o.q0);
+                        const int cs = slot_of(o.q1);
+                        if (cs != 255) { m.b = (uint8_t)cs; m.c = CTL_REG; } else { m.b = (uint8_t)o.q1; m.c = CTL_FIXED; }
+                        m.param = -1;
+                    }
+                }
+                P.mops.push_back(m);
+            }
+            S.op_end = (uint32_t)P.mops.size();
+            S.n_seg = (uint8_t)nseg;
+            if (nseg > 255) { err = "schedule: too many diagonal segments in a stage"; return false; }
+            max_seg = std::max(max_seg, nseg);
+            P.stages.push_back(S);
+            L = sbest.rest; carry = sbest.carry;
+        }
+        B.stage_end = (uint32_t)P.stages.size();
+        B.max_seg = max_seg;
+        P.blocks.push_back(B);
+        P.block_ops.push_back(best.taken);
+        // ---- remove taken ops
+        std::vector<char> gone(ops.size(), 0);
+        for (int idx : best.taken) gone[idx] = 1;
+        std::vector<int> np; np.reserve(pending.size());
+        for (int idx : pending) if (!gone[idx]) np.push_back(idx);
+        pending.swap(np);
+        first = false;
+    }
+    return true;
+}
+
+std::string dump_program(const Program &p)
+{
+    std::string s;
+    char buf[256];
+    snprintf(buf, sizeof buf, "program n=%d k=%d f=%d R=%d blocks=%zu stages=%zu mops=%zu segs=%zu\n", p.n, p.k, p.f, p.R,
+             p.blocks.size(), p.stages.size(), p.mops.size(), p.segs.size());
+    s += buf;
+    for (size_t b = 0; b < p.blocks.size(); ++b) {
+        const Block &B = p.blocks[b];
+        snprintf(buf, sizeof buf, "block %zu k=%d zero=%d runs=", b, B.k, B.source_zero); s += buf;
+        for (int r = 0; r < B.n_runs; ++r) {
+            snprintf(buf, sizeof buf, "%d:%d+%d ", B.runs[r].lpos, B.runs[r].gpos, B.runs[r].len); s += buf;
+        }
+        s += "\n";
+        for (uint32_t si = B.stage_begin; si < B.stage_end; ++si) {
+            const Stage &S = p.stages[si];
+            s += " stage R=";
+            for (int j = 0; j < p.R; ++j) { snprintf(buf, sizeof buf, "%d/%d ", S.regbit[j], S.regq[j]); s += buf; }
+            s += ":";
+            for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
+                const MicroOp &m = p.mops[oi];
+                if (m.kind == MOP_RY) snprintf(buf, sizeof buf, " RY(s%d,p%d)", m.a, m.param);
+                else if (m.kind == MOP_CX) snprintf(buf, sizeof buf, " CX(t=s%d,c=%s%d)", m.a, m.c == CTL_REG ? "s" : "q", m.b);
+                else {
+                    const DiagSeg &g = p.segs[m.param];
+                    snprintf(buf, sizeof buf, " DIAG(#%d rz=%u cz=%u)", m.param, g.rz_end - g.rz_begin, g.cz_end - g.cz_begin);
+                }
+                s += buf;
+            }
+            s += "\n";
+        }
+    }
+    return s;
+}
+
+}  // namespace gv
