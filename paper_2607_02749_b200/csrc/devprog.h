@@ -1,0 +1,87 @@
+// devprog.h -- device-side encoding of the compiled schedule and of the Hamiltonian passes.
+// Plain PODs shared by the host lowering (lower.cpp, hamiltonian.cpp) and the kernels (kernels.cuh); the host
+// builds arrays of these, uploads them into the caller's workspace, and every thread block copies the slice it
+// needs into shared memory before it touches the state.                       SURVEY.md section 8(a) a0, a3-a7.
+#pragma once
+#include <stdint.h>
+
+#include "program.h"
+
+namespace gv {
+
+constexpr int DEV_MAX_R = 5;
+
+// ---- gate engine ------------------------------------------------------------------------------------------
+struct DOp {                 // 8 bytes; one register-level micro-op of a stage
+    uint8_t kind;            // MOP_RY, MOP_CX, MOP_DIAG
+    uint8_t a;               // RY: register slot; CX: target slot
+    uint8_t b;               // CX: control register slot (CTL_REG) or global qubit (CTL_FIXED)
+    uint8_t c;               // CX: CTL_REG / CTL_FIXED
+    int32_t idx;             // RY: block-local (cos,sin) index; DIAG: block-local segment index
+};
+
+struct DTrz {                // RZ on a qubit that is not a register bit of the stage (thread- or tile-constant)
+    uint8_t qubit;           // global qubit
+    uint8_t pad;             // 0: thread/tile-constant; s+1: a further RZ on register slot s of the same segment
+    uint16_t cs;             // block-local (cos,sin) index
+};
+
+struct DSeg {                // one merged diagonal segment (all its RZ and CZ, Eq. 7 phases and CZ signs)
+    uint16_t trz_begin, trz_end;        // DTrz entries (block-local)
+    uint16_t tcz_begin, tcz_end;        // CZ pairs with no register bit: 64-bit masks with two bits set
+    int16_t reg_rz[DEV_MAX_R];          // per register slot: block-local (cos,sin) index of its RZ, or -1
+    uint16_t pad;
+    uint32_t regreg_neg;                // bit r set: amplitude with register index r changes sign (reg-reg CZ)
+    uint32_t pad2;
+    uint64_t nbr[DEV_MAX_R];            // per slot: global qubits CZ-coupled to it that are not register bits
+};
+
+struct DStage {              // 16 bytes
+    uint8_t regbit[DEV_MAX_R];          // local bit position (inside the tile) of each register slot, ascending
+    uint8_t pad[3];
+    uint16_t op_begin, op_end;          // DOp entries (block-local)
+    uint32_t pad2;
+};
+
+struct DBlock {              // one HBM round trip over every statevector in flight
+    uint8_t k;               // tile bits
+    uint8_t n_runs;
+    uint8_t source_zero;     // 1: tile starts as |0...0> restricted to the tile (no global read)
+    uint8_t n_stages;
+    Run runs[MAX_RUNS];      // local bits [lpos,lpos+len) <-> global qubits [gpos,gpos+len)
+    uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off;   // offsets into the device arrays
+    uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs;
+    uint32_t smem_prog_bytes;                                         // shared memory the slice needs
+};
+
+// ---- Hamiltonian engine -----------------------------------------------------------------------------------
+struct DTerm {               // one Pauli term of an off-diagonal group, 32 bytes
+    double cr, ci;           // c_k * i^{n_Y}
+    uint64_t zout;           // z_mask bits outside the pass's tile bits (sign is constant per tile)
+    uint32_t zu;             // z_mask bits inside the tile, compressed to the group's table index space
+    uint32_t pad;
+};
+
+struct URun { uint8_t lpos, len, shift, pad; };   // table index bits: ((j >> lpos) & ((1<<len)-1)) << shift
+
+struct DGroup {              // one flip mask inside a pass, 36 bytes
+    uint32_t m_loc;          // flip mask in local tile coordinates (non-zero)
+    uint32_t term_begin, term_end;
+    uint32_t tab_off;        // offset of the group's W table in the shared-memory table area
+    uint8_t ubits;           // table has 2^ubits entries (table mode)
+    uint8_t n_uruns;
+    uint8_t pivot;           // highest set bit of m_loc
+    uint8_t direct;          // 1: no table; W is summed term by term per pair and DTerm.zu is the LOCAL z mask
+    uint8_t last_in_batch;   // 1: tables of groups up to and including this one are built together
+    uint8_t pad[3];
+    URun uruns[3];
+};
+
+struct DPass {               // one read-only sweep over the state
+    uint8_t k, n_runs, with_diag, pad;
+    Run runs[MAX_RUNS];
+    uint32_t group_begin, group_end;
+    uint32_t pad2[2];
+};
+
+}  // namespace gv

@@ -1,0 +1,224 @@
+// hamiltonian.cpp -- see hamiltonian.h.
+#include "hamiltonian.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+
+namespace gv {
+namespace {
+
+bool finish(Hamiltonian &H, std::string &err)
+{
+    const uint64_t all = H.n >= 64 ? ~0ull : ((1ull << H.n) - 1);
+    H.abs_sum = 0.0;
+    std::vector<uint64_t> masks;
+    masks.reserve(H.terms.size());
+    for (const HostTerm &t : H.terms) {
+        if (!std::isfinite(t.c)) { err = "hamiltonian: coefficient is not finite"; return false; }
+        if ((t.x | t.z) & ~all) { err = "hamiltonian: mask has bits outside the register"; return false; }
+        H.abs_sum += std::fabs(t.c);
+        masks.push_back(t.x);
+    }
+    std::sort(masks.begin(), masks.end());
+    masks.erase(std::unique(masks.begin(), masks.end()), masks.end());
+    H.group_mask = masks;
+    H.group_of_term.resize(H.terms.size());
+    for (size_t k = 0; k < H.terms.size(); ++k)
+        H.group_of_term[k] = (int32_t)(std::lower_bound(masks.begin(), masks.end(), H.terms[k].x) - masks.begin());
+    std::map<uint64_t, double> dz;   // ordered; each entry summed in input order -> deterministic
+    for (const HostTerm &t : H.terms) if (t.x == 0) dz[t.z] += t.c;
+    H.diag_z.clear(); H.diag_c.clear();
+    for (const auto &kv : dz) { H.diag_z.push_back(kv.first); H.diag_c.push_back(kv.second); }
+    return true;
+}
+
+inline int local_pos(uint64_t T, int q) { return __builtin_popcountll(T & ((1ull << q) - 1)); }
+
+uint32_t compress(uint64_t v, uint64_t T)   // bits of v at the positions of T, packed (software pext)
+{
+    uint32_t out = 0; int o = 0;
+    while (T) {
+        const int q = __builtin_ctzll(T);
+        if (v >> q & 1) out |= 1u << o;
+        ++o; T &= T - 1;
+    }
+    return out;
+}
+
+int runs_of(uint64_t T, Run *runs, int cap)   // returns number of runs (may exceed cap; only cap are written)
+{
+    int nr = 0, lp = 0;
+    for (int q = 0; q < 64;) {
+        if (!(T >> q & 1)) { ++q; continue; }
+        int len = 0; while (q + len < 64 && (T >> (q + len) & 1)) ++len;
+        if (nr < cap) { runs[nr].lpos = (uint8_t)lp; runs[nr].gpos = (uint8_t)q; runs[nr].len = (uint8_t)len; runs[nr].pad = 0; }
+        ++nr; lp += len; q += len;
+    }
+    return nr;
+}
+
+// fill `Thi` (bits >= f) up to `h` bits: first next to bits already chosen (or next to the low block), then anywhere
+uint64_t fill_bits(uint64_t Thi, int n, int f, int h)
+{
+    int cnt = __builtin_popcountll(Thi);
+    const uint64_t low = f ? ((1ull << f) - 1) : 0;
+    for (int pass = 0; pass < 2 && cnt < h; ++pass) {
+        bool grew = true;
+        while (grew && cnt < h) {
+            grew = false;
+            for (int q = f; q < n && cnt < h; ++q) {
+                if (Thi >> q & 1) continue;
+                const uint64_t T = Thi | low;
+                const bool adj = (q > 0 && (T >> (q - 1) & 1)) || (q + 1 < n && (T >> (q + 1) & 1));
+                if (pass == 1 || adj) { Thi |= 1ull << q; ++cnt; grew = true; }
+            }
+        }
+    }
+    return Thi;
+}
+
+}  // namespace
+
+bool hamiltonian_from_paulis(int n, int M, const char *paulis, const double *coeffs, Hamiltonian &H, std::string &err)
+{
+    H = Hamiltonian(); H.n = n;
+    H.terms.resize((size_t)M);
+    for (int k = 0; k < M; ++k) {
+        HostTerm t{0, 0, 0, coeffs[k]};
+        const char *s = paulis + (size_t)k * n;
+        for (int j = 0; j < n; ++j) {
+            switch (s[j]) {
+            case 'I': break;
+            case 'X': t.x |= 1ull << j; break;
+            case 'Z': t.z |= 1ull << j; break;
+            case 'Y': t.x |= 1ull << j; t.z |= 1ull << j; ++t.ny; break;
+            default: err = "hamiltonian: bad Pauli character (expected I, X, Y or Z)"; return false;
+            }
+        }
+        H.terms[k] = t;
+    }
+    return finish(H, err);
+}
+
+bool hamiltonian_from_masks(int n, int M, const uint64_t *xm, const uint64_t *zm, const double *coeffs, Hamiltonian &H,
+                            std::string &err)
+{
+    H = Hamiltonian(); H.n = n;
+    H.terms.resize((size_t)M);
+    for (int k = 0; k < M; ++k) H.terms[k] = HostTerm{xm[k], zm[k], __builtin_popcountll(xm[k] & zm[k]), coeffs[k]};
+    return finish(H, err);
+}
+
+bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint32_t tab_cap, ExpectPlan &plan,
+                      std::string &err)
+{
+    plan = ExpectPlan();
+    if (k > n) k = n;
+    if (f > k) f = k;
+    plan.k = k;
+    const uint64_t low = f ? ((1ull << f) - 1) : 0;
+    const int h = k - f;
+    // off-diagonal groups in canonical order, their terms in input order
+    std::vector<uint64_t> gm;
+    for (uint64_t m : H.group_mask) if (m) gm.push_back(m);
+    std::vector<std::vector<int>> gterms(gm.size());
+    for (size_t t = 0; t < H.terms.size(); ++t) {
+        if (!H.terms[t].x) continue;
+        const size_t g = std::lower_bound(gm.begin(), gm.end(), H.terms[t].x) - gm.begin();
+        gterms[g].push_back((int)t);
+    }
+    // ---- choose the tile-bit set of every pass
+    std::vector<uint64_t> passT;
+    std::vector<std::vector<int>> passG;
+    if (n <= k || gm.empty()) {
+        passT.push_back(n <= k ? ((1ull << n) - 1) : ((1ull << k) - 1));
+        passG.emplace_back();
+        for (size_t g = 0; g < gm.size(); ++g) passG[0].push_back((int)g);
+    } else {
+        std::vector<char> done(gm.size(), 0);
+        size_t left = gm.size();
+        Run tmp[MAX_RUNS];
+        while (left) {
+            uint64_t Thi = 0;
+            std::vector<int> mine;
+            for (;;) {
+                int best = -1, best_add = 1 << 30;
+                for (size_t g = 0; g < gm.size(); ++g) {
+                    if (done[g]) continue;
+                    const uint64_t need = gm[g] & ~low;
+                    const int add = __builtin_popcountll(need & ~Thi);
+                    if (add >= best_add) continue;
+                    const uint64_t cand = Thi | need;
+                    if (__builtin_popcountll(cand) > h) continue;
+                    if (runs_of(fill_bits(cand, n, f, h) | low, tmp, MAX_RUNS) > MAX_RUNS) continue;
+                    best = (int)g; best_add = add;
+                    if (add == 0) break;
+                }
+                if (best < 0) break;
+                Thi |= gm[best] & ~low; done[best] = 1; --left; mine.push_back(best);
+            }
+            if (mine.empty()) {
+                err = "hamiltonian: a flip mask does not fit one tile (too many or too scattered X/Y positions)";
+                return false;
+            }
+            std::sort(mine.begin(), mine.end());
+            passT.push_back(fill_bits(Thi, n, f, h) | low);
+            passG.push_back(mine);
+        }
+    }
+    // ---- encode
+    for (size_t p = 0; p < passT.size(); ++p) {
+        const uint64_t T = passT[p];
+        DPass dp; memset(&dp, 0, sizeof dp);
+        dp.k = (uint8_t)k; dp.with_diag = (p == 0) ? 1 : 0;
+        const int nr = runs_of(T, dp.runs, MAX_RUNS);
+        if (nr > MAX_RUNS) { err = "hamiltonian: too many tile runs (internal)"; return false; }
+        dp.n_runs = (uint8_t)nr;
+        dp.group_begin = (uint32_t)plan.groups.size();
+        uint32_t tab_used = 0;
+        for (int g : passG[p]) {
+            DGroup dg; memset(&dg, 0, sizeof dg);
+            dg.m_loc = compress(gm[g], T);
+            dg.pivot = (uint8_t)(31 - __builtin_clz(dg.m_loc));
+            uint64_t U = 0;
+            for (int t : gterms[g]) U |= H.terms[t].z;
+            U &= T;
+            const uint32_t Uloc = compress(U, T);
+            Run ur[4];
+            const int nur = runs_of(Uloc, ur, 4);
+            const int ubits = __builtin_popcount(Uloc);
+            const bool table = (ubits <= umax) && (nur <= 3) && ((1u << ubits) <= tab_cap);
+            dg.direct = table ? 0 : 1;
+            dg.term_begin = (uint32_t)plan.terms.size();
+            if (table) {
+                dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)nur;
+                for (int r = 0; r < nur; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
+                if (tab_used + (1u << ubits) > tab_cap) {   // close the batch before this group
+                    if (!plan.groups.empty() && plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
+                    tab_used = 0;
+                }
+                dg.tab_off = tab_used; tab_used += 1u << ubits;
+            }
+            for (int t : gterms[g]) {
+                const HostTerm &ht = H.terms[t];
+                DTerm dt; memset(&dt, 0, sizeof dt);
+                static const double pr[4] = {1, 0, -1, 0}, pim[4] = {0, 1, 0, -1};
+                dt.cr = ht.c * pr[ht.ny & 3]; dt.ci = ht.c * pim[ht.ny & 3];
+                dt.zout = ht.z & ~T;
+                const uint32_t zloc = compress(ht.z & T, T);
+                dt.zu = table ? compress(zloc, Uloc) : zloc;
+                plan.terms.push_back(dt);
+            }
+            dg.term_end = (uint32_t)plan.terms.size();
+            plan.groups.push_back(dg);
+        }
+        if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
+        dp.group_end = (uint32_t)plan.groups.size();
+        plan.passes.push_back(dp);
+    }
+    return true;
+}
+
+}  // namespace gv

@@ -1,0 +1,284 @@
+// kernels.cu -- __global__ wrappers and launchers (see kernels.cuh for the per-thread code).  sm_100a only.
+#include <cuda_runtime.h>
+
+#include "kernels.cuh"
+#include "kernels.h"
+
+namespace gv {
+
+// ---- parameter expansion: (cos(theta/2), sin(theta/2)) in fp64, stored in working precision ----
+template <typename T>
+__global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *__restrict__ cs, uint64_t count)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    double s, c;
+    sincos(0.5 * params[i], &s, &c);
+    cs[i] = cx<T>{(T)c, (T)s};
+}
+
+// ---- fused gate block: one HBM round trip, all stages of the block in shared memory ---------
+template <typename T, int R, int MAXT>
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))
+gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    DBlock *sb = reinterpret_cast<DBlock *>(smem);
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    {
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(da.blocks + bi);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(sb);
+        for (uint32_t i = tid; i < sizeof(DBlock) / 4; i += nthr) dst[i] = src[i];
+    }
+    __syncthreads();
+    ProgView<T> pv;
+    pv.bind(smem + HDR_BYTES, *sb);
+    cx<T> *tile = reinterpret_cast<cx<T> *>(smem + HDR_BYTES + sb->smem_prog_bytes);
+    const uint32_t b = blockIdx.y;
+    cx<T> *state = states + (uint64_t)b * stride;
+    const int k = sb->k, n_runs = sb->n_runs;
+    const uint64_t xbase = tile_base(blockIdx.x, sb->runs, n_runs);
+    const bool zero = sb->source_zero != 0;
+    if (zero && xbase != 0) {   // |0...0> has no weight in this tile and gates act inside tiles: stays zero
+        tile_zero_store<T>(state, xbase, sb->runs, n_runs, k, tid, nthr);
+        return;
+    }
+    gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
+    if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
+    else tile_load<T>(tile, state, xbase, sb->runs, n_runs, k, tid, nthr);
+    __syncthreads();
+    if (zero) {
+        if (tid == 0) tile[0] = cx<T>{T(1), T(0)};
+        __syncthreads();
+    }
+    const int ns = sb->n_stages;
+    for (int s = 0; s < ns; ++s) {
+        gate_stage<T, R>(pv, pv.stages[s], tile, tid, xbase, sb->runs, n_runs);
+        __syncthreads();
+    }
+    tile_store<T>(tile, state, xbase, sb->runs, n_runs, k, tid, nthr);
+}
+
+// ---- expectation pass: read-only sweep, diagonal table + every flip-mask group of the pass --
+__device__ __forceinline__ double block_sum(double v, double *red)
+{
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) red[w] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0) for (int i = 0; i < (int)(blockDim.x >> 5); ++i) s += red[i];
+    return s;   // valid on thread 0
+}
+
+template <typename T, typename TT>
+__global__ void __launch_bounds__(256, 2)
+expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
+                   const cx<T> *states, uint64_t stride, const TT *__restrict__ table, double *partial,
+                   uint32_t slots_per_b, uint32_t slot_off)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ double red[32];
+    DPass *sp = reinterpret_cast<DPass *>(smem);
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    {
+        const uint32_t *src = reinterpret_cast<const uint32_t *>(passes + pi);
+        uint32_t *dst = reinterpret_cast<uint32_t *>(sp);
+        for (uint32_t i = tid; i < sizeof(DPass) / 4; i += nthr) dst[i] = src[i];
+    }
+    __syncthreads();
+    cx<T> *tab = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);
+    cx<T> *tile = tab + EXPECT_TAB_CAP;
+    const uint32_t b = blockIdx.y;
+    const cx<T> *state = states + (uint64_t)b * stride;
+    const int k = sp->k, n_runs = sp->n_runs;
+    const uint64_t xbase = tile_base(blockIdx.x, sp->runs, n_runs);
+    double acc = expect_load<T, TT>(tile, state, table, sp->with_diag != 0, xbase, sp->runs, n_runs, k, tid, nthr);
+    __syncthreads();
+    uint32_t g = sp->group_begin;
+    const uint32_t gend = sp->group_end;
+    while (g < gend) {
+        uint32_t ge = g;
+        while (!groups[ge].last_in_batch) ++ge;
+        for (uint32_t gi = g; gi <= ge; ++gi) {
+            const DGroup dg = groups[gi];
+            if (dg.direct) continue;
+            for (uint32_t u = tid; u < (1u << dg.ubits); u += nthr)
+                tab[dg.tab_off + u] = group_table_entry<T>(dg, terms, xbase, u);
+        }
+        __syncthreads();
+        for (uint32_t gi = g; gi <= ge; ++gi) {
+            const DGroup dg = groups[gi];
+            acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
+        }
+        __syncthreads();
+        g = ge + 1;
+    }
+    const double s = block_sum(acc, red);
+    if (tid == 0) partial[(uint64_t)b * slots_per_b + slot_off + blockIdx.x] = s;
+}
+
+// ---- second-stage deterministic reduction ------------------------------------------------------
+__global__ void __launch_bounds__(256) reduce_kernel(const double *__restrict__ partial, uint32_t slots_per_b, double *E)
+{
+    __shared__ double red[32];
+    const double *p = partial + (uint64_t)blockIdx.x * slots_per_b;
+    double v = 0.0;
+    for (uint32_t i = threadIdx.x; i < slots_per_b; i += blockDim.x) v += p[i];
+    const double s = block_sum(v, red);
+    if (threadIdx.x == 0) E[blockIdx.x] = s;
+}
+
+// ---- diagonal energy table: scatter c at index z, then in-place Walsh-Hadamard butterflies -------
+template <typename TT>
+__global__ void table_scatter_kernel(TT *table, const uint64_t *__restrict__ z, const double *__restrict__ c, uint32_t count)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) table[z[i]] = (TT)c[i];
+}
+
+template <typename TT>
+__global__ void __launch_bounds__(256) fwht_pass_kernel(TT *table, TileDesc td, uint32_t bitmask)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    TT *tile = reinterpret_cast<TT *>(smem);
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    const int k = td.k, n_runs = td.n_runs;
+    const uint64_t xbase = tile_base(blockIdx.x, td.runs, n_runs);
+    for (uint32_t j = tid; j < (1u << k); j += nthr) tile[j] = table[xbase | scatter_runs(j, td.runs, n_runs)];
+    __syncthreads();
+    for (int p = 0; p < k; ++p) {
+        if (!((bitmask >> p) & 1u)) continue;
+        for (uint32_t i = tid; i < (1u << (k - 1)); i += nthr) {
+            const uint32_t j = insert_zero(i, p);
+            const TT u = tile[j], v = tile[j | (1u << p)];
+            tile[j] = u + v;
+            tile[j | (1u << p)] = u - v;
+        }
+        __syncthreads();
+    }
+    for (uint32_t j = tid; j < (1u << k); j += nthr) table[xbase | scatter_runs(j, td.runs, n_runs)] = tile[j];
+}
+
+// ================================================ launchers ===================================================
+namespace {
+
+template <typename T, int R, int MAXT>
+int gate_launch_t(const GateLaunch &g, int bi, int k, uint32_t smem_prog, int n, void *states, uint64_t stride,
+                  const void *cs, int P, int batch, cudaStream_t st)
+{
+    DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx};
+    const size_t smem = HDR_BYTES + smem_prog + ((size_t)sizeof(cx<T>) << k);
+    dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
+    gate_block_kernel<T, R, MAXT><<<grid, 1u << (k - R), smem, st>>>(da, bi, (cx<T> *)states, stride, (const cx<T> *)cs, P);
+    return (int)cudaGetLastError();
+}
+
+template <typename F> int set_smem(F f, int bytes)
+{
+    return (int)cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
+}  // namespace
+
+int kernels_init(void)
+{
+    const int big = 200 * 1024;
+    int e = 0;
+    e |= set_smem(gate_block_kernel<float, 5, 256>, big);
+    e |= set_smem(gate_block_kernel<float, 4, 256>, big);
+    e |= set_smem(gate_block_kernel<float, 4, 512>, big);
+    e |= set_smem(gate_block_kernel<float, 3, 512>, big);
+    e |= set_smem(gate_block_kernel<double, 4, 256>, big);
+    e |= set_smem(gate_block_kernel<double, 3, 256>, big);
+    e |= set_smem(gate_block_kernel<double, 3, 512>, big);
+    e |= set_smem(gate_block_kernel<double, 5, 256>, big);
+    e |= set_smem(expect_pass_kernel<float, float>, big);
+    e |= set_smem(expect_pass_kernel<double, double>, big);
+    e |= set_smem(fwht_pass_kernel<float>, big);
+    e |= set_smem(fwht_pass_kernel<double>, big);
+    return e;
+}
+
+int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches)
+{
+    if (!count) return 0;
+    const unsigned nb = (unsigned)((count + 255) / 256);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (prec == 0) expand_params_kernel<float><<<nb, 256, 0, st>>>(params, (cx<float> *)cs, count);
+    else expand_params_kernel<double><<<nb, 256, 0, st>>>(params, (cx<double> *)cs, count);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+int launch_gate_block(int prec, int R, const GateLaunch &g, int bi, int k, uint32_t smem_prog, int n, void *states,
+                      uint64_t stride, const void *cs, int P, int batch, void *stream, uint64_t *launches)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    const int thr = 1 << (k - R);
+    ++*launches;
+    if (prec == 0) {
+        if (R == 5 && thr <= 256) return gate_launch_t<float, 5, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 4 && thr <= 256) return gate_launch_t<float, 4, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 4 && thr <= 512) return gate_launch_t<float, 4, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 3 && thr <= 512) return gate_launch_t<float, 3, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+    } else {
+        if (R == 4 && thr <= 256) return gate_launch_t<double, 4, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 3 && thr <= 256) return gate_launch_t<double, 3, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 3 && thr <= 512) return gate_launch_t<double, 3, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 5 && thr <= 256) return gate_launch_t<double, 5, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+    }
+    --*launches;
+    return (int)cudaErrorInvalidConfiguration;
+}
+
+int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
+                       const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                       uint32_t slot_off, int batch, void *stream, uint64_t *launches)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
+    const size_t esz = prec == 0 ? sizeof(cx<float>) : sizeof(cx<double>);
+    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * esz + (esz << k);
+    const int thr = (1 << k) >= 2048 ? 256 : ((1 << k) / 8 < 32 ? 32 : (1 << k) / 8);
+    if (prec == 0)
+        expect_pass_kernel<float, float><<<grid, thr, smem, st>>>(passes, pi, groups, terms, (const cx<float> *)states, stride,
+                                                                  (const float *)table, partial, slots_per_b, slot_off);
+    else
+        expect_pass_kernel<double, double><<<grid, thr, smem, st>>>(passes, pi, groups, terms, (const cx<double> *)states,
+                                                                    stride, (const double *)table, partial, slots_per_b, slot_off);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+int launch_reduce(const double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches)
+{
+    reduce_kernel<<<batch, 256, 0, (cudaStream_t)stream>>>(partial, slots_per_b, E);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+int launch_table_scatter(int prec, void *table, const uint64_t *z, const double *c, uint32_t count, void *stream,
+                         uint64_t *launches)
+{
+    if (!count) return 0;
+    const unsigned nb = (count + 255) / 256;
+    if (prec == 0) table_scatter_kernel<float><<<nb, 256, 0, (cudaStream_t)stream>>>((float *)table, z, c, count);
+    else table_scatter_kernel<double><<<nb, 256, 0, (cudaStream_t)stream>>>((double *)table, z, c, count);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches)
+{
+    const unsigned nb = (unsigned)(1ull << (n - td.k));
+    const int thr = (1 << td.k) >= 512 ? 256 : 32;
+    if (prec == 0)
+        fwht_pass_kernel<float><<<nb, thr, sizeof(float) << td.k, (cudaStream_t)stream>>>((float *)table, td, bitmask);
+    else
+        fwht_pass_kernel<double><<<nb, thr, sizeof(double) << td.k, (cudaStream_t)stream>>>((double *)table, td, bitmask);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+}  // namespace gv

@@ -1,0 +1,387 @@
+// kernels.cuh -- per-thread device code of the gate engine and the Hamiltonian engine (sm_100a).
+//
+// Everything here is written per thread (tid explicit) and split at the points where the thread block
+// synchronises, so the __global__ wrappers in kernels.cu are a plain sequence  phase; __syncthreads(); phase; ...
+// Operations follow /root/reference/PAPER.md: R_y, R_z of Eq. 7, the entangling layer
+// (PAPER.md:169), |psi> = U(theta)|0>, E = sum_k c_k <P_k> (Eq. 4, 6) evaluated
+// as a partition of the terms (Eq. 12).  Index convention: qubit q <-> bit q of the amplitude index.
+#pragma once
+#include <stdint.h>
+
+#include "devprog.h"
+
+#ifdef GVQE_EMU   // host emulation used only by developer probes; never part of the library build
+#define GV_DEV inline
+#define GV_UNROLL
+static inline int gv_popcll(uint64_t v) { return __builtin_popcountll(v); }
+static inline int gv_popc(uint32_t v) { return __builtin_popcount(v); }
+#else
+#define GV_DEV __device__ __forceinline__
+#define GV_UNROLL _Pragma("unroll")
+GV_DEV int gv_popcll(uint64_t v) { return __popcll(v); }
+GV_DEV int gv_popc(uint32_t v) { return __popc(v); }
+#endif
+
+namespace gv {
+
+template <typename T> struct alignas(2 * sizeof(T)) cx { T x, y; };
+
+template <typename T> GV_DEV cx<T> cmul(cx<T> a, cx<T> b) { return cx<T>{a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x}; }
+template <typename T> GV_DEV cx<T> cneg(cx<T> a) { return cx<T>{-a.x, -a.y}; }
+
+// Shared-memory swizzle: XOR-fold the higher index bits into the low FB bits (FB = log2 of the elements one
+// 128-byte wavefront holds: 16 complex64, 8 complex128).  Linear over GF(2): phys(a ^ b) = phys(a) ^ phys(b).
+template <typename T> GV_DEV uint32_t phys(uint32_t j)
+{
+    constexpr int FB = sizeof(T) == 4 ? 4 : 3;
+    constexpr uint32_t M = (1u << FB) - 1;
+    uint32_t p = j;
+    GV_UNROLL
+    for (int sh = FB; sh < 16; sh += FB) p ^= (j >> sh) & M;
+    return p;
+}
+
+GV_DEV uint64_t scatter_runs(uint32_t j, const Run *runs, int n_runs)
+{
+    uint64_t x = 0;
+    for (int r = 0; r < n_runs; ++r)
+        x |= (uint64_t)((j >> runs[r].lpos) & ((1u << runs[r].len) - 1u)) << runs[r].gpos;
+    return x;
+}
+
+// Global index of local index 0 of tile number `tile`: the tile bits fill the positions the runs leave free.
+GV_DEV uint64_t tile_base(uint64_t tile, const Run *runs, int n_runs)
+{
+    uint64_t x = 0;
+    int gpos = 0;
+    for (int r = 0; r < n_runs; ++r) {
+        const int gap = (int)runs[r].gpos - gpos;
+        if (gap > 0) { x |= (tile & ((1ull << gap) - 1ull)) << gpos; tile >>= gap; }
+        gpos = runs[r].gpos + runs[r].len;
+    }
+    x |= tile << gpos;
+    return x;
+}
+
+GV_DEV uint32_t insert_zero(uint32_t i, uint32_t pos) { return ((i >> pos) << (pos + 1)) | (i & ((1u << pos) - 1u)); }
+
+struct DevArrays {
+    const DBlock *blocks; const DStage *stages; const DOp *ops; const DSeg *segs; const DTrz *trzs;
+    const uint64_t *tczs; const int32_t *csidx;
+};
+
+GV_DEV uint32_t al16u(uint32_t v) { return (v + 15u) & ~15u; }
+
+template <typename T> struct ProgView {
+    cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz;
+    GV_DEV void bind(unsigned char *p, const DBlock &b)
+    {
+        cs = (cx<T> *)p;        p += al16u(b.n_cs * (uint32_t)sizeof(cx<T>));
+        tcz = (uint64_t *)p;    p += al16u(b.n_tcz * 8u);
+        segs = (DSeg *)p;       p += al16u(b.n_segs * (uint32_t)sizeof(DSeg));
+        stages = (DStage *)p;   p += al16u(b.n_stages * (uint32_t)sizeof(DStage));
+        ops = (DOp *)p;         p += al16u(b.n_ops * (uint32_t)sizeof(DOp));
+        trz = (DTrz *)p;
+    }
+};
+
+// Copy the block's program slice into shared memory and gather this batch row's (cos, sin) values.
+template <typename T>
+GV_DEV void gate_prologue(ProgView<T> &pv, const DBlock &b, const DevArrays &da, const cx<T> *cs_row, uint32_t tid,
+                          uint32_t nthr)
+{
+    for (uint32_t i = tid; i < b.n_cs; i += nthr) pv.cs[i] = cs_row[da.csidx[b.cs_off + i]];
+    for (uint32_t i = tid; i < b.n_tcz; i += nthr) pv.tcz[i] = da.tczs[b.tcz_off + i];
+    for (uint32_t i = tid; i < b.n_segs; i += nthr) pv.segs[i] = da.segs[b.seg_off + i];
+    for (uint32_t i = tid; i < b.n_stages; i += nthr) pv.stages[i] = da.stages[b.stage_off + i];
+    for (uint32_t i = tid; i < b.n_ops; i += nthr) pv.ops[i] = da.ops[b.op_off + i];
+    for (uint32_t i = tid; i < b.n_trz; i += nthr) pv.trz[i] = da.trzs[b.trz_off + i];
+}
+
+// ---- tile <-> global -------------------------------------------------------------------------------------
+template <typename T> struct alignas(16) vec16 { cx<T> v[16 / sizeof(cx<T>)]; };
+
+template <typename T>
+GV_DEV void tile_load(cx<T> *tile, const cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k,
+                      uint32_t tid, uint32_t nthr)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t nchunk = (1u << k) / V;
+    for (uint32_t c = tid; c < nchunk; c += nthr) {
+        const uint32_t j = c * V;
+        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
+        const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + x);
+        const uint32_t p = phys<T>(j);
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v.v[e];
+    }
+}
+
+template <typename T>
+GV_DEV void tile_store(const cx<T> *tile, cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k,
+                       uint32_t tid, uint32_t nthr)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t nchunk = (1u << k) / V;
+    for (uint32_t c = tid; c < nchunk; c += nthr) {
+        const uint32_t j = c * V;
+        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
+        const uint32_t p = phys<T>(j);
+        vec16<T> v;
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) v.v[e] = tile[p ^ e];
+        *reinterpret_cast<vec16<T> *>(state + x) = v;
+    }
+}
+
+template <typename T>
+GV_DEV void tile_zero_store(cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k, uint32_t tid, uint32_t nthr)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t nchunk = (1u << k) / V;
+    vec16<T> v;
+    GV_UNROLL
+    for (uint32_t e = 0; e < V; ++e) v.v[e] = cx<T>{T(0), T(0)};
+    for (uint32_t c = tid; c < nchunk; c += nthr) {
+        const uint64_t x = xbase | scatter_runs(c * V, runs, n_runs);
+        *reinterpret_cast<vec16<T> *>(state + x) = v;
+    }
+}
+
+template <typename T> GV_DEV void tile_init_zero_state(cx<T> *tile, int k, uint32_t tid, uint32_t nthr)
+{
+    for (uint32_t j = tid; j < (1u << k); j += nthr) tile[j] = cx<T>{T(0), T(0)};
+}
+
+// ---- register-level gates (Eq. 7) ------------------------------------------------------------------------
+// R_y(theta) = [[c,-s],[s,c]] on register slot S, c = cos(theta/2), s = sin(theta/2).
+template <typename T, int R, int S> GV_DEV void ry_slot(cx<T> *a, T c, T s)
+{
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
+        if (r & (1 << S)) continue;
+        const cx<T> u = a[r], v = a[r | (1 << S)];
+        a[r] = cx<T>{c * u.x - s * v.x, c * u.y - s * v.y};
+        a[r | (1 << S)] = cx<T>{s * u.x + c * v.x, s * u.y + c * v.y};
+    }
+}
+
+// CNOT with target slot S: swap the pair when the control bit is set.
+template <typename T, int R, int S> GV_DEV void cx_slot(cx<T> *a, bool fixed, bool fixed_bit, uint32_t ctl_mask)
+{
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
+        if (r & (1 << S)) continue;
+        const bool on = fixed ? fixed_bit : ((r & ctl_mask) != 0);
+        const cx<T> u = a[r], v = a[r | (1 << S)];
+        a[r] = on ? v : u;
+        a[r | (1 << S)] = on ? u : v;
+    }
+}
+
+template <typename T, int R> GV_DEV void ry_dispatch(cx<T> *a, int slot, T c, T s)
+{
+    switch (slot) {
+    case 0: ry_slot<T, R, 0>(a, c, s); break;
+    case 1: if constexpr (R > 1) ry_slot<T, R, 1>(a, c, s); break;
+    case 2: if constexpr (R > 2) ry_slot<T, R, 2>(a, c, s); break;
+    case 3: if constexpr (R > 3) ry_slot<T, R, 3>(a, c, s); break;
+    case 4: if constexpr (R > 4) ry_slot<T, R, 4>(a, c, s); break;
+    default: break;
+    }
+}
+
+template <typename T, int R> GV_DEV void cx_dispatch(cx<T> *a, int slot, bool fixed, bool fixed_bit, uint32_t ctl_mask)
+{
+    switch (slot) {
+    case 0: cx_slot<T, R, 0>(a, fixed, fixed_bit, ctl_mask); break;
+    case 1: if constexpr (R > 1) cx_slot<T, R, 1>(a, fixed, fixed_bit, ctl_mask); break;
+    case 2: if constexpr (R > 2) cx_slot<T, R, 2>(a, fixed, fixed_bit, ctl_mask); break;
+    case 3: if constexpr (R > 3) cx_slot<T, R, 3>(a, fixed, fixed_bit, ctl_mask); break;
+    case 4: if constexpr (R > 4) cx_slot<T, R, 4>(a, fixed, fixed_bit, ctl_mask); break;
+    default: break;
+    }
+}
+
+// Merged diagonal segment: every R_z phase (Eq. 7: e^{-i phi/2} on bit 0, e^{+i phi/2} on bit 1) and every CZ sign
+// of the segment as ONE complex factor per amplitude.  The factor of amplitude (thread index x, register index r)
+// splits into a thread part, a table over the low register slots and a table over the high register slots.
+template <typename T, int R> GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint64_t x)
+{
+    constexpr int RL = R / 2, RH = R - RL;
+    cx<T> ph{T(1), T(0)};
+    cx<T> F0[R], F1[R];
+    GV_UNROLL
+    for (int s = 0; s < R; ++s) {
+        const int i = sg.reg_rz[s];
+        if (i >= 0) { const cx<T> cs = pv.cs[i]; F0[s] = cx<T>{cs.x, -cs.y}; F1[s] = cs; }
+        else { F0[s] = cx<T>{T(1), T(0)}; F1[s] = F0[s]; }
+    }
+    for (uint32_t e = sg.trz_begin; e < sg.trz_end; ++e) {
+        const DTrz t = pv.trz[e];
+        const cx<T> cs = pv.cs[t.cs];
+        if (t.pad == 0) {
+            const bool bit = (x >> t.qubit) & 1ull;
+            ph = cmul(ph, cx<T>{cs.x, bit ? cs.y : -cs.y});
+        } else {   // a further R_z on a register slot that already has one in this segment
+            GV_UNROLL
+            for (int s = 0; s < R; ++s)
+                if (t.pad - 1 == s) { F0[s] = cmul(F0[s], cx<T>{cs.x, -cs.y}); F1[s] = cmul(F1[s], cs); }
+        }
+    }
+    uint32_t par = 0;
+    for (uint32_t e = sg.tcz_begin; e < sg.tcz_end; ++e) { const uint64_t m = pv.tcz[e]; par ^= ((x & m) == m) ? 1u : 0u; }
+    if (par) ph = cneg(ph);
+    GV_UNROLL
+    for (int s = 0; s < R; ++s)
+        if (gv_popcll(x & sg.nbr[s]) & 1) F1[s] = cneg(F1[s]);
+    cx<T> tlo[1 << RL], thi[1 << RH];
+    tlo[0] = ph;
+    GV_UNROLL
+    for (int s = 0; s < RL; ++s) {
+        GV_UNROLL
+        for (int e = 0; e < (1 << s); ++e) { tlo[e | (1 << s)] = cmul(tlo[e], F1[s]); tlo[e] = cmul(tlo[e], F0[s]); }
+    }
+    thi[0] = cx<T>{T(1), T(0)};
+    GV_UNROLL
+    for (int s = 0; s < RH; ++s) {
+        GV_UNROLL
+        for (int e = 0; e < (1 << s); ++e) { thi[e | (1 << s)] = cmul(thi[e], F1[RL + s]); thi[e] = cmul(thi[e], F0[RL + s]); }
+    }
+    const uint32_t neg = sg.regreg_neg;
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
+        cx<T> w = cmul(tlo[r & ((1 << RL) - 1)], thi[r >> RL]);
+        if ((neg >> r) & 1u) w = cneg(w);
+        a[r] = cmul(a[r], w);
+    }
+}
+
+// One stage: 2^R amplitudes per thread in registers, all micro-ops of the stage, back to shared memory.
+template <typename T, int R>
+GV_DEV void gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uint32_t tid, uint64_t xbase,
+                       const Run *runs, int n_runs)
+{
+    constexpr int NR = 1 << R;
+    uint32_t j = tid;
+    uint32_t po[R];
+    GV_UNROLL
+    for (int s = 0; s < R; ++s) {
+        const uint32_t pos = st.regbit[s];
+        j = insert_zero(j, pos);
+        po[s] = phys<T>(1u << pos);
+    }
+    const uint32_t pj = phys<T>(j);
+    cx<T> a[NR];
+    GV_UNROLL
+    for (int r = 0; r < NR; ++r) {
+        uint32_t o = 0;
+        GV_UNROLL
+        for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
+        a[r] = tile[pj ^ o];
+    }
+    const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
+    for (uint32_t oi = st.op_begin; oi < st.op_end; ++oi) {
+        const DOp o = pv.ops[oi];
+        if (o.kind == MOP_RY) {
+            const cx<T> cs = pv.cs[o.idx];
+            ry_dispatch<T, R>(a, o.a, cs.x, cs.y);
+        } else if (o.kind == MOP_CX) {
+            const bool fixed = (o.c == CTL_FIXED);
+            const bool fb = fixed ? (((x >> o.b) & 1ull) != 0) : false;
+            cx_dispatch<T, R>(a, o.a, fixed, fb, fixed ? 0u : (1u << o.b));
+        } else {
+            diag_apply<T, R>(a, pv, pv.segs[o.idx], x);
+        }
+    }
+    GV_UNROLL
+    for (int r = 0; r < NR; ++r) {
+        uint32_t o = 0;
+        GV_UNROLL
+        for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
+        tile[pj ^ o] = a[r];
+    }
+}
+
+// ---- Hamiltonian engine ----------------------------------------------------------------------------------
+// Diagonal part while the tile is loaded: sum_x |psi[x]|^2 E(x), E = diagonal energy table.
+template <typename T, typename TT>
+GV_DEV double expect_load(cx<T> *tile, const cx<T> *state, const TT *table, bool with_diag, uint64_t xbase,
+                          const Run *runs, int n_runs, int k, uint32_t tid, uint32_t nthr)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t nchunk = (1u << k) / V;
+    double acc = 0.0;
+    for (uint32_t c = tid; c < nchunk; c += nthr) {
+        const uint32_t j = c * V;
+        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
+        const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + x);
+        const uint32_t p = phys<T>(j);
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v.v[e];
+        if (with_diag) {
+            GV_UNROLL
+            for (uint32_t e = 0; e < V; ++e) {
+                const T pr = v.v[e].x * v.v[e].x + v.v[e].y * v.v[e].y;
+                acc += (double)(pr * (T)table[x + e]);
+            }
+        }
+    }
+    return acc;
+}
+
+// W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the
+// sign from the bits outside the tile).  One entry per call.
+template <typename T>
+GV_DEV cx<T> group_table_entry(const DGroup &g, const DTerm *terms, uint64_t xbase, uint32_t u)
+{
+    double wr = 0.0, wi = 0.0;
+    for (uint32_t t = g.term_begin; t < g.term_end; ++t) {
+        const DTerm tm = terms[t];
+        const int par = (gv_popcll(xbase & tm.zout) + gv_popc(u & tm.zu)) & 1;
+        wr += par ? -tm.cr : tm.cr;
+        wi += par ? -tm.ci : tm.ci;
+    }
+    return cx<T>{(T)wr, (T)wi};
+}
+
+// 2 Re sum over pairs (x, x^m), x with the pivot bit clear, of conj(psi[x^m]) W(x) psi[x].
+template <typename T>
+GV_DEV double group_accumulate(const DGroup &g, const DTerm *terms, const cx<T> *tile, const cx<T> *tab, uint64_t xbase,
+                               int k, uint32_t tid, uint32_t nthr)
+{
+    const uint32_t pm = phys<T>(g.m_loc);
+    const uint32_t npair = 1u << (k - 1);
+    double acc = 0.0;
+    T part = T(0);
+    uint32_t cnt = 0;
+    for (uint32_t i = tid; i < npair; i += nthr) {
+        const uint32_t j = insert_zero(i, g.pivot);
+        const uint32_t pj = phys<T>(j);
+        const cx<T> a = tile[pj], b = tile[pj ^ pm];
+        cx<T> w;
+        if (g.direct) {
+            double wr = 0.0, wi = 0.0;
+            for (uint32_t t = g.term_begin; t < g.term_end; ++t) {
+                const DTerm tm = terms[t];
+                const int par = (gv_popcll(xbase & tm.zout) + gv_popc(j & tm.zu)) & 1;
+                wr += par ? -tm.cr : tm.cr;
+                wi += par ? -tm.ci : tm.ci;
+            }
+            w = cx<T>{(T)wr, (T)wi};
+        } else {
+            uint32_t u = 0;
+            for (int r = 0; r < g.n_uruns; ++r)
+                u |= ((j >> g.uruns[r].lpos) & ((1u << g.uruns[r].len) - 1u)) << g.uruns[r].shift;
+            w = tab[g.tab_off + u];
+        }
+        const T tr = b.x * a.x + b.y * a.y;   // conj(b) * a
+        const T ti = b.x * a.y - b.y * a.x;
+        part += w.x * tr - w.y * ti;
+        if (++cnt == 16) { acc += (double)part; part = T(0); cnt = 0; }
+    }
+    acc += (double)part;
+    return 2.0 * acc;
+}
+
+}  // namespace gv

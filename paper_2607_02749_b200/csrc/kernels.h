@@ -1,0 +1,36 @@
+// kernels.h -- host-callable launchers of the sm_100a kernels (kernels.cu).  All pointers are DEVICE pointers into
+// the caller's workspace unless stated otherwise; every launcher enqueues on `stream` and returns the CUDA error
+// of the launch (0 = success).  `launches` is incremented by the number of kernels enqueued.
+#pragma once
+#include <stdint.h>
+
+#include "devprog.h"
+
+namespace gv {
+
+struct TileDesc { uint8_t k, n_runs, pad[2]; Run runs[MAX_RUNS]; };
+
+struct GateLaunch {
+    const DBlock *blocks; const DStage *stages; const DOp *ops; const DSeg *segs; const DTrz *trzs;
+    const uint64_t *tczs; const int32_t *csidx;
+};
+
+constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area
+constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
+constexpr uint32_t HDR_BYTES = 128;         // shared-memory header holding the DBlock / DPass copy
+
+// prec: 0 = complex64 (float), 1 = complex128 (double)
+int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches);
+int launch_gate_block(int prec, int R, const GateLaunch &g, int block_index, int k, uint32_t smem_prog_bytes, int n,
+                      void *states, uint64_t stride_amps, const void *cs, int P, int batch, void *stream,
+                      uint64_t *launches);
+int launch_expect_pass(int prec, const DPass *passes, int pass_index, int k, int n, const DGroup *groups,
+                       const DTerm *terms, const void *states, uint64_t stride_amps, const void *table, double *partial,
+                       uint32_t slots_per_b, uint32_t slot_off, int batch, void *stream, uint64_t *launches);
+int launch_reduce(const double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches);
+int launch_table_scatter(int prec, void *table, const uint64_t *z, const double *c, uint32_t count, void *stream,
+                         uint64_t *launches);
+int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches);
+int kernels_init(void);   // opt-in shared memory sizes; returns the CUDA error
+
+}  // namespace gv

@@ -1,0 +1,126 @@
+// lower.cpp -- see lower.h.  A compiled block is cut into device blocks at stage boundaries whenever its program
+// slice would outgrow the shared-memory budget (same tile bits, one more HBM round trip; results unchanged).
+#include "lower.h"
+
+#include <cstring>
+
+namespace gv {
+
+namespace {
+constexpr uint32_t SLICE_BUDGET = 12 * 1024;   // bytes of shared memory for the program slice of one block
+inline uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
+}  // namespace
+
+uint32_t prog_slice_bytes(uint32_t n_stages, uint32_t n_ops, uint32_t n_segs, uint32_t n_trz, uint32_t n_tcz,
+                          uint32_t n_cs, int scs_bytes)
+{
+    return al16(n_cs * (uint32_t)scs_bytes) + al16(n_tcz * 8u) + al16(n_segs * (uint32_t)sizeof(DSeg)) +
+           al16(n_stages * (uint32_t)sizeof(DStage)) + al16(n_ops * (uint32_t)sizeof(DOp)) +
+           al16(n_trz * (uint32_t)sizeof(DTrz));
+}
+
+bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &err)
+{
+    D = DevProgram();
+    D.n = p.n; D.k = p.k; D.f = p.f; D.R = p.R;
+    if (p.R > DEV_MAX_R) { err = "lower: R too large"; return false; }
+    for (const Block &B : p.blocks) {
+        bool first_piece = true;
+        uint32_t si = B.stage_begin;
+        do {
+            DBlock db; memset(&db, 0, sizeof db);
+            db.k = B.k; db.n_runs = B.n_runs; db.source_zero = (first_piece && B.source_zero) ? 1 : 0;
+            memcpy(db.runs, B.runs, sizeof db.runs);
+            db.stage_off = (uint32_t)D.stages.size(); db.op_off = (uint32_t)D.ops.size();
+            db.seg_off = (uint32_t)D.segs.size(); db.trz_off = (uint32_t)D.trzs.size();
+            db.tcz_off = (uint32_t)D.tczs.size(); db.cs_off = (uint32_t)D.csidx.size();
+            std::vector<int32_t> cs_local;   // parameter index per local slot (deduplicated)
+            auto cs_slot = [&](int32_t param) -> uint32_t {
+                for (size_t i = 0; i < cs_local.size(); ++i) if (cs_local[i] == param) return (uint32_t)i;
+                cs_local.push_back(param);
+                return (uint32_t)cs_local.size() - 1;
+            };
+            uint32_t n_stages = 0;
+            while (si < B.stage_end) {
+                const Stage &S = p.stages[si];
+                // size of this stage's contribution
+                uint32_t add_ops = S.op_end - S.op_begin, add_segs = 0, add_trz = 0, add_tcz = 0, add_cs = 0;
+                for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
+                    const MicroOp &m = p.mops[oi];
+                    if (m.kind == MOP_RY) ++add_cs;
+                    if (m.kind == MOP_DIAG) {
+                        const DiagSeg &g = p.segs[m.param];
+                        ++add_segs; add_trz += g.rz_end - g.rz_begin; add_tcz += g.cz_end - g.cz_begin;
+                        add_cs += g.rz_end - g.rz_begin;
+                    }
+                }
+                const uint32_t tot = prog_slice_bytes(n_stages + 1, (uint32_t)(D.ops.size() - db.op_off) + add_ops,
+                                                      (uint32_t)(D.segs.size() - db.seg_off) + add_segs,
+                                                      (uint32_t)(D.trzs.size() - db.trz_off) + add_trz,
+                                                      (uint32_t)(D.tczs.size() - db.tcz_off) + add_tcz,
+                                                      (uint32_t)cs_local.size() + add_cs, scs_bytes);
+                if (n_stages > 0 && (tot > SLICE_BUDGET || n_stages >= 250)) break;
+                if (tot > 4 * SLICE_BUDGET) { err = "lower: a single stage exceeds the program budget (internal)"; return false; }
+                // ---- emit the stage
+                DStage ds; memset(&ds, 0, sizeof ds);
+                for (int s = 0; s < p.R; ++s) ds.regbit[s] = S.regbit[s];
+                ds.op_begin = (uint16_t)(D.ops.size() - db.op_off);
+                for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
+                    const MicroOp &m = p.mops[oi];
+                    DOp o; o.kind = m.kind; o.a = m.a; o.b = m.b; o.c = m.c; o.idx = -1;
+                    if (m.kind == MOP_RY) o.idx = (int32_t)cs_slot(m.param);
+                    else if (m.kind == MOP_DIAG) {
+                        const DiagSeg &g = p.segs[m.param];
+                        DSeg sg; memset(&sg, 0, sizeof sg);
+                        for (int s = 0; s < DEV_MAX_R; ++s) sg.reg_rz[s] = -1;
+                        sg.trz_begin = (uint16_t)(D.trzs.size() - db.trz_off);
+                        sg.tcz_begin = (uint16_t)(D.tczs.size() - db.tcz_off);
+                        for (uint32_t r = g.rz_begin; r < g.rz_end; ++r) {
+                            const DiagRZ &z = p.rzs[r];
+                            const uint32_t slot = cs_slot(z.param);
+                            if (z.slot != 255 && sg.reg_rz[z.slot] < 0) sg.reg_rz[z.slot] = (int16_t)slot;
+                            else {   // not a register bit (or a second RZ on the same slot): per-thread factor.
+                                DTrz t; t.qubit = z.qubit; t.pad = (uint8_t)(z.slot != 255 ? z.slot + 1 : 0); t.cs = (uint16_t)slot;
+                                D.trzs.push_back(t);
+                            }
+                        }
+                        for (uint32_t c = g.cz_begin; c < g.cz_end; ++c) {
+                            const DiagCZ &z = p.czs[c];
+                            if (z.s0 != 255 && z.s1 != 255) {
+                                static const uint32_t A[5] = {0xAAAAAAAAu, 0xCCCCCCCCu, 0xF0F0F0F0u, 0xFF00FF00u, 0xFFFF0000u};
+                                sg.regreg_neg ^= A[z.s0] & A[z.s1];
+                            } else if (z.s0 != 255) sg.nbr[z.s0] ^= 1ull << z.q1;
+                            else if (z.s1 != 255) sg.nbr[z.s1] ^= 1ull << z.q0;
+                            else D.tczs.push_back((1ull << z.q0) | (1ull << z.q1));
+                        }
+                        sg.trz_end = (uint16_t)(D.trzs.size() - db.trz_off);
+                        sg.tcz_end = (uint16_t)(D.tczs.size() - db.tcz_off);
+                        o.idx = (int32_t)(D.segs.size() - db.seg_off);
+                        D.segs.push_back(sg);
+                    }
+                    D.ops.push_back(o);
+                }
+                ds.op_end = (uint16_t)(D.ops.size() - db.op_off);
+                D.stages.push_back(ds);
+                ++n_stages; ++si;
+            }
+            db.n_stages = (uint8_t)n_stages;
+            db.n_ops = (uint32_t)(D.ops.size() - db.op_off);
+            db.n_segs = (uint32_t)(D.segs.size() - db.seg_off);
+            db.n_trz = (uint32_t)(D.trzs.size() - db.trz_off);
+            db.n_tcz = (uint32_t)(D.tczs.size() - db.tcz_off);
+            db.n_cs = (uint32_t)cs_local.size();
+            for (int32_t v : cs_local) D.csidx.push_back(v);
+            db.smem_prog_bytes = prog_slice_bytes(db.n_stages, db.n_ops, db.n_segs, db.n_trz, db.n_tcz, db.n_cs, scs_bytes);
+            if (db.smem_prog_bytes > D.max_smem_prog) D.max_smem_prog = db.smem_prog_bytes;
+            if (db.n_ops > 65535 || db.n_trz > 65535 || db.n_tcz > 65535 || db.n_cs > 65535) {
+                err = "lower: block too large (internal)"; return false;
+            }
+            D.blocks.push_back(db);
+            first_piece = false;
+        } while (si < B.stage_end);
+    }
+    return true;
+}
+
+}  // namespace gv

@@ -112,6 +112,10 @@ void block_candidates(const std::vector<HostOp> &ops, const std::vector<int> &pe
 namespace gv {
 namespace {
 
+constexpr int MAX_SEG_OPS = 96;    // RZ + CZ entries merged into one diagonal segment
+constexpr int MAX_STAGE_ND = 64;   // RY/CNOT micro-ops per stage
+constexpr int MAX_STAGE_SEG = 12;  // diagonal segments per stage
+
 struct StageItem { bool is_seg; int op; std::vector<int> seg_ops; };  // op / seg_ops index the block's op list
 
 struct StageTake {
@@ -142,6 +146,10 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
             if (!a.diag[i]) { ndq |= b; if ((nd & b) || !(Rset & b)) ok = false; }
         }
         if (ok && !is_diag(o) && (pend_touch & ndq) && !flush_anywhere && out.n_nondiag > 0) ok = false;
+        // size caps (shared-memory slice of the program): an op that does not fit waits for the next stage
+        if (ok && is_diag(o) && (int)pend.size() >= MAX_SEG_OPS) ok = false;
+        if (ok && !is_diag(o) && out.n_nondiag >= MAX_STAGE_ND) ok = false;
+        if (ok && !is_diag(o) && (pend_touch & ndq) && out.n_seg >= MAX_STAGE_SEG) ok = false;
         if (ok) {
             if (is_diag(o)) {
                 pend.push_back(pos);
@@ -278,9 +286,10 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
             bool any_nd = false;
             for (int pos : L) if (!is_diag(bops[pos])) { any_nd = true; break; }
             uint64_t Rset = 0;
-            if (!any_nd) {  // only diagonals left: one closing segment
-                for (int pos : L) carry.push_back(pos);
-                L.clear();
+            if (!any_nd) {  // only diagonals left: closing segment(s), MAX_SEG_OPS at a time
+                size_t take = 0;
+                while (take < L.size() && (int)carry.size() < MAX_SEG_OPS) carry.push_back(L[take++]);
+                L.erase(L.begin(), L.begin() + take);
                 sbest.items.clear(); sbest.rest.clear(); sbest.carry.clear();
                 StageItem s; s.is_seg = true; s.op = -1; s.seg_ops = carry;
                 sbest.items.push_back(s);
@@ -349,7 +358,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
             if (nseg > 255) { err = "schedule: too many diagonal segments in a stage"; return false; }
             max_seg = std::max(max_seg, nseg);
             P.stages.push_back(S);
-            L = sbest.rest; carry = sbest.carry;
+            if (any_nd) { L = sbest.rest; carry = sbest.carry; } else carry.clear();
         }
         B.stage_end = (uint32_t)P.stages.size();
         B.max_seg = max_seg;
