@@ -1,0 +1,224 @@
+"""ctypes binding of libgvqe (include/gvqe.h): argument marshalling only, same names as the C ABI.
+
+Every step of the path runs in the CUDA kernels of libgvqe.so; there is no Python or CPU fallback: a missing
+library raises at import of the symbols, a missing GPU surfaces as GVQE_ERR_CUDA from the first energy call.
+PyTorch is used for the device workspace and the stream only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+from . import build as _build
+
+GVQE_OK, GVQE_ERR_INVALID_ARG, GVQE_ERR_NO_HAMILTONIAN, GVQE_ERR_WORKSPACE, GVQE_ERR_UNSUPPORTED, GVQE_ERR_CUDA = range(6)
+GVQE_C64, GVQE_C128 = 0, 1
+STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "GVQE_ERR_WORKSPACE",
+                "GVQE_ERR_UNSUPPORTED", "GVQE_ERR_CUDA"]
+
+EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
+           "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
+           "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
+           "gvqe_get_state", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
+           "gvqe_last_error", "gvqe_destroy"]
+
+
+class GvqeLayout(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("entangler", C.c_int32), ("topology", C.c_int32), ("final_rot", C.c_int32)]
+
+
+class GvqeError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS_NAMES[status] if 0 <= status < 6 else status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.SO
+
+
+def load():
+    """Load libgvqe.so (built in-tree on first use when nvcc is present).  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_build.SO) or (os.path.exists(_build.NVCC) and _build.needs_build()):
+        _build.build()
+    L = C.CDLL(_build.SO)
+    vp, i32, u64, sz = C.c_void_p, C.c_int, C.c_uint64, C.c_size_t
+    L.gvqe_create.argtypes = [i32, C.POINTER(GvqeLayout), i32, C.POINTER(vp)]
+    L.gvqe_create_ops.argtypes = [i32, vp, i32, i32, i32, C.POINTER(vp)]
+    L.gvqe_num_params.argtypes = [vp]
+    L.gvqe_num_qubits.argtypes = [vp]
+    L.gvqe_set_hamiltonian.argtypes = [vp, i32, C.c_char_p, vp]
+    L.gvqe_set_hamiltonian_masks.argtypes = [vp, i32, vp, vp, vp]
+    L.gvqe_get_grouping.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    L.gvqe_workspace_bytes.argtypes = [vp, i32]
+    L.gvqe_workspace_bytes.restype = sz
+    L.gvqe_set_workspace.argtypes = [vp, vp, sz]
+    L.gvqe_set_max_in_flight.argtypes = [vp, i32]
+    L.gvqe_energy_batch.argtypes = [vp, vp, i32, vp, vp]
+    L.gvqe_energy_batch_device.argtypes = [vp, vp, i32, vp, vp]
+    L.gvqe_param_shift_grad.argtypes = [vp, vp, vp, vp, vp, vp]
+    L.gvqe_get_state.argtypes = [vp, i32, vp]
+    L.gvqe_schedule_info.argtypes = [vp, vp, vp, vp]
+    L.gvqe_dump_schedule.argtypes = [vp, C.c_char_p, sz]
+    L.gvqe_dump_schedule.restype = sz
+    L.gvqe_get_exec_order.argtypes = [vp, vp, i32]
+    L.gvqe_launch_count.argtypes = [vp]
+    L.gvqe_launch_count.restype = u64
+    L.gvqe_last_error.argtypes = [vp]
+    L.gvqe_last_error.restype = C.c_char_p
+    L.gvqe_destroy.argtypes = [vp]
+    L.gvqe_destroy.restype = None
+    _lib = L
+    return L
+
+
+_ENT = {"cz": 2, "cnot": 3}
+_TOPO = {"linear": 0, "ring": 1}
+
+
+class Gvqe:
+    """One libgvqe context.  Method names mirror the C ABI without the gvqe_ prefix."""
+
+    def __init__(self, n_qubits: int, *, layout: Optional[dict] = None, ops=None, n_params: Optional[int] = None,
+                 precision: str = "c128"):
+        self._L = load()
+        self._h = C.c_void_p()
+        self._ws = None
+        prec = {"c64": GVQE_C64, "c128": GVQE_C128}[precision]
+        self.precision = precision
+        if layout is not None:
+            lay = GvqeLayout(int(layout["n_layers"]), _ENT.get(layout["entangler"], layout["entangler"]),
+                             _TOPO.get(layout["topology"], layout["topology"]), int(layout.get("final_rot", 1)))
+            st = self._L.gvqe_create(n_qubits, C.byref(lay), prec, C.byref(self._h))
+        else:
+            o = np.ascontiguousarray(np.asarray(ops, dtype=np.int32).reshape(-1, 4))
+            st = self._L.gvqe_create_ops(n_qubits, o.ctypes.data, len(o), int(n_params), prec, C.byref(self._h))
+        if st != GVQE_OK:
+            raise GvqeError(st, "gvqe_create failed")
+        self.n = n_qubits
+        self.P = self._L.gvqe_num_params(self._h)
+
+    # -- helpers
+    def _check(self, st: int):
+        if st != GVQE_OK:
+            raise GvqeError(st, self._L.gvqe_last_error(self._h).decode())
+
+    def close(self):
+        if self._h:
+            self._L.gvqe_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- C ABI
+    def set_hamiltonian(self, paulis, coeffs):
+        if not isinstance(paulis, (bytes, bytearray)):
+            paulis = ("".join(paulis) if not isinstance(paulis, str) else paulis).encode("ascii")
+        c = np.ascontiguousarray(coeffs, dtype=np.float64)
+        if len(paulis) != len(c) * self.n:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, "paulis must hold n_terms * n_qubits characters")
+        self._check(self._L.gvqe_set_hamiltonian(self._h, len(c), bytes(paulis), c.ctypes.data))
+
+    def set_hamiltonian_masks(self, x_mask, z_mask, coeffs):
+        x = np.ascontiguousarray(x_mask, dtype=np.uint64)
+        z = np.ascontiguousarray(z_mask, dtype=np.uint64)
+        c = np.ascontiguousarray(coeffs, dtype=np.float64)
+        self._check(self._L.gvqe_set_hamiltonian_masks(self._h, len(c), x.ctypes.data, z.ctypes.data, c.ctypes.data))
+
+    def get_grouping(self, n_terms: int):
+        M = max(n_terms, 1)
+        xm, zm = np.zeros(M, np.uint64), np.zeros(M, np.uint64)
+        ny, got, gm = np.zeros(M, np.uint8), np.zeros(M, np.int32), np.zeros(M, np.uint64)
+        ng = C.c_int32(0)
+        self._check(self._L.gvqe_get_grouping(self._h, xm.ctypes.data, zm.ctypes.data, ny.ctypes.data, got.ctypes.data,
+                                              C.addressof(ng), gm.ctypes.data))
+        return xm[:n_terms], zm[:n_terms], ny[:n_terms], got[:n_terms], int(ng.value), gm[:ng.value]
+
+    def workspace_bytes(self, batch_in_flight: int) -> int:
+        return int(self._L.gvqe_workspace_bytes(self._h, int(batch_in_flight)))
+
+    def set_workspace(self, device_ptr: int, nbytes: int):
+        self._check(self._L.gvqe_set_workspace(self._h, C.c_void_p(device_ptr), nbytes))
+
+    def set_max_in_flight(self, m: int):
+        self._check(self._L.gvqe_set_max_in_flight(self._h, int(m)))
+
+    def alloc_workspace(self, batch_in_flight: int, device="cuda:0"):
+        """Convenience: a torch uint8 tensor of workspace_bytes(batch) on `device`, handed to set_workspace."""
+        import torch
+
+        nbytes = self.workspace_bytes(batch_in_flight)
+        if nbytes == 0:
+            raise GvqeError(GVQE_ERR_NO_HAMILTONIAN, "set the Hamiltonian before sizing the workspace")
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=device)
+        ptr = (self._ws.data_ptr() + 255) & ~255
+        self.set_workspace(ptr, nbytes)
+        return self._ws
+
+    def energy_batch(self, params, stream: int = 0, out: Optional[np.ndarray] = None) -> np.ndarray:
+        p = np.ascontiguousarray(params, dtype=np.float64)
+        if p.ndim == 1:
+            p = p.reshape(1, -1) if self.P else p.reshape(len(p), 0)
+        if p.shape[1] != self.P:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, f"params must be [B, {self.P}]")
+        E = out if out is not None else np.empty(p.shape[0], dtype=np.float64)
+        self._check(self._L.gvqe_energy_batch(self._h, p.ctypes.data, p.shape[0], E.ctypes.data, C.c_void_p(stream)))
+        return E
+
+    def energy_batch_ptr(self, params_host_ptr: int, B: int, E_host_ptr: int, stream: int = 0):
+        """Raw host pointers (e.g. pinned torch tensors): no numpy marshalling in the timed path."""
+        self._check(self._L.gvqe_energy_batch(self._h, C.c_void_p(params_host_ptr), B, C.c_void_p(E_host_ptr), C.c_void_p(stream)))
+
+    def energy_batch_device(self, params_dev_ptr: int, B: int, E_dev_ptr: int, stream: int = 0):
+        self._check(self._L.gvqe_energy_batch_device(self._h, C.c_void_p(params_dev_ptr), B, C.c_void_p(E_dev_ptr),
+                                                     C.c_void_p(stream)))
+
+    def param_shift_grad(self, params, mask, stream: int = 0):
+        p = np.ascontiguousarray(params, dtype=np.float64).reshape(-1)
+        m = np.ascontiguousarray(mask, dtype=np.uint8).reshape(-1)
+        if len(p) != self.P or len(m) != self.P:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, f"params and mask must have {self.P} entries")
+        dE = np.zeros(max(self.P, 1), dtype=np.float64)
+        E0 = C.c_double(0.0)
+        self._check(self._L.gvqe_param_shift_grad(self._h, p.ctypes.data, m.ctypes.data, dE.ctypes.data, C.addressof(E0),
+                                                  C.c_void_p(stream)))
+        return dE[:self.P], E0.value
+
+    def get_state(self, slot: int = 0) -> np.ndarray:
+        dt = np.complex64 if self.precision == "c64" else np.complex128
+        out = np.empty(1 << self.n, dtype=dt)
+        self._check(self._L.gvqe_get_state(self._h, slot, out.ctypes.data))
+        return out
+
+    def schedule_info(self):
+        a, b, c = C.c_int32(0), C.c_int32(0), C.c_int32(0)
+        self._check(self._L.gvqe_schedule_info(self._h, C.addressof(a), C.addressof(b), C.addressof(c)))
+        return a.value, b.value, c.value
+
+    def dump_schedule(self) -> str:
+        need = self._L.gvqe_dump_schedule(self._h, None, 0)
+        buf = C.create_string_buffer(need + 1)
+        self._L.gvqe_dump_schedule(self._h, buf, need + 1)
+        return buf.value.decode()
+
+    def get_exec_order(self) -> np.ndarray:
+        m = self._L.gvqe_get_exec_order(self._h, None, 0)
+        o = np.zeros(max(m, 1), dtype=np.int32)
+        self._L.gvqe_get_exec_order(self._h, o.ctypes.data, m)
+        return o[:m]
+
+    def launch_count(self) -> int:
+        return int(self._L.gvqe_launch_count(self._h))

@@ -1,0 +1,495 @@
+// gvqe_api.cpp -- the C ABI of include/gvqe.h on top of the schedule compiler, the Hamiltonian planner and the
+// sm_100a kernels.  Host C++ (compiled by nvcc as host code); allocates no device memory: everything lives in
+// the caller's workspace.  No CPU fallback: every energy is computed by the kernels in kernels.cu.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/gvqe.h"
+#include "hamiltonian.h"
+#include "kernels.h"
+#include "lower.h"
+#include "schedule.h"
+
+using namespace gv;
+
+namespace {
+constexpr int N_MIN_STORE = 10;   // smaller registers are padded with idle qubits (they stay |0>)
+constexpr int N_MAX = 34;
+inline size_t al256(size_t v) { return (v + 255) & ~(size_t)255; }
+int env_int(const char *name, int dflt)
+{
+    const char *s = getenv(name);
+    return (s && *s) ? atoi(s) : dflt;
+}
+}  // namespace
+
+struct gvqe_ctx {
+    int n_user = 0, n_store = 0, prec = 0, P = 0;
+    int K = 0, F = 0, R = 0;
+    std::vector<HostOp> ops;
+    Program prog;
+    DevProgram dev;
+    bool have_h = false;
+    Hamiltonian H;
+    ExpectPlan plan;
+    std::vector<TileDesc> fwht_tiles;
+    std::vector<uint32_t> fwht_masks;
+    // workspace
+    char *ws = nullptr;
+    size_t ws_bytes = 0;
+    int max_in_flight = 0, in_flight = 0;
+    bool dirty = true;          // device arrays / table must be (re)built
+    bool kernels_ready = false;
+    // carved device pointers
+    GateLaunch gl{};
+    DPass *d_passes = nullptr; DGroup *d_groups = nullptr; DTerm *d_terms = nullptr;
+    uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr;
+    void *d_table = nullptr; void *d_states = nullptr; void *d_cs = nullptr;
+    double *d_params = nullptr, *d_partial = nullptr, *d_E = nullptr;
+    uint32_t slots_per_b = 0;
+    uint64_t launches = 0;
+    std::string err;
+    size_t amp_bytes() const { return prec == GVQE_C64 ? 8 : 16; }
+    size_t tab_bytes() const { return prec == GVQE_C64 ? 4 : 8; }
+};
+
+namespace {
+
+gvqe_status fail(gvqe_ctx *c, gvqe_status s, const std::string &m) { if (c) c->err = m; return s; }
+gvqe_status cuda_fail(gvqe_ctx *c, int e, const char *what)
+{
+    c->err = std::string(what) + ": " + cudaGetErrorString((cudaError_t)e);
+    return GVQE_ERR_CUDA;
+}
+
+gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_precision prec, gvqe_ctx **out)
+{
+    if (!out) return GVQE_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (n < 1 || n > N_MAX || (prec != GVQE_C64 && prec != GVQE_C128) || n_params < 0) return GVQE_ERR_INVALID_ARG;
+    std::vector<char> used((size_t)n_params, 0);
+    for (const HostOp &o : ops) {
+        if (o.kind < 0 || o.kind > 3 || o.q0 < 0 || o.q0 >= n) return GVQE_ERR_INVALID_ARG;
+        if (o.kind >= 2 && (o.q1 < 0 || o.q1 >= n || o.q1 == o.q0)) return GVQE_ERR_INVALID_ARG;
+        if (o.kind <= 1) {
+            if (o.param < 0 || o.param >= n_params || used[o.param]) return GVQE_ERR_INVALID_ARG;
+            used[o.param] = 1;   // a parameter drives at most one gate: Eq. 13 is then exact
+        }
+    }
+    gvqe_ctx *c = new gvqe_ctx();
+    c->n_user = n; c->n_store = n < N_MIN_STORE ? N_MIN_STORE : n; c->prec = prec; c->P = n_params; c->ops = ops;
+    c->K = env_int("GVQE_K", prec == GVQE_C64 ? 13 : 12);
+    c->F = env_int("GVQE_F", prec == GVQE_C64 ? 4 : 3);
+    c->R = env_int("GVQE_R", prec == GVQE_C64 ? 5 : 4);
+    if (c->K > c->n_store) c->K = c->n_store;
+    if (c->K < c->R + 5 || c->K > 14 || c->F < 1 || c->F >= c->K || c->K - c->R > 9) { delete c; return GVQE_ERR_INVALID_ARG; }
+    std::string err;
+    if (!compile_program(c->n_store, c->ops, c->K, c->F, c->R, c->prog, err) ||
+        !lower_program(c->prog, (int)c->amp_bytes(), c->dev, err)) {
+        delete c;
+        return GVQE_ERR_UNSUPPORTED;
+    }
+    *out = c;
+    return GVQE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+gvqe_status gvqe_create(int n, const gvqe_layout *L, gvqe_precision prec, gvqe_ctx **out)
+{
+    if (!L || !out || n < 1 || n > N_MAX) return GVQE_ERR_INVALID_ARG;
+    if (L->n_layers < 0 || L->n_layers > 4096 || (L->entangler != GVQE_OP_CZ && L->entangler != GVQE_OP_CNOT) ||
+        (L->topology != 0 && L->topology != 1) || (L->final_rot != 1 && L->final_rot != 2))
+        return GVQE_ERR_INVALID_ARG;
+    // D x (RY layer, RZ layer, entanglers), then the final rotation layer.
+    std::vector<HostOp> ops;
+    const int D = L->n_layers;
+    for (int l = 0; l < D; ++l) {
+        for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RY, q, -1, 2 * n * l + q});
+        for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RZ, q, -1, 2 * n * l + n + q});
+        for (int q = 0; q + 1 < n; ++q) {
+            if (L->entangler == GVQE_OP_CZ) ops.push_back({GVQE_OP_CZ, q, q + 1, -1});
+            else ops.push_back({GVQE_OP_CNOT, q + 1, q, -1});
+        }
+        if (L->topology == 1 && n > 2) {
+            if (L->entangler == GVQE_OP_CZ) ops.push_back({GVQE_OP_CZ, n - 1, 0, -1});
+            else ops.push_back({GVQE_OP_CNOT, 0, n - 1, -1});
+        }
+    }
+    for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RY, q, -1, 2 * n * D + q});
+    if (L->final_rot == 2) for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RZ, q, -1, 2 * n * D + n + q});
+    return build_ctx(n, ops, 2 * n * D + n * L->final_rot, prec, out);
+}
+
+gvqe_status gvqe_create_ops(int n, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec, gvqe_ctx **out)
+{
+    if (n_ops < 0 || (n_ops > 0 && !ops)) return GVQE_ERR_INVALID_ARG;
+    std::vector<HostOp> v((size_t)n_ops);
+    for (int i = 0; i < n_ops; ++i) v[i] = HostOp{ops[i].kind, ops[i].q0, ops[i].q1, ops[i].param};
+    return build_ctx(n, v, n_params, prec, out);
+}
+
+int gvqe_num_params(const gvqe_ctx *c) { return c ? c->P : -1; }
+int gvqe_num_qubits(const gvqe_ctx *c) { return c ? c->n_user : -1; }
+
+static gvqe_status after_hamiltonian(gvqe_ctx *c)
+{
+    std::string err;
+    if (!plan_expectation(c->H, c->n_store, c->K, c->F, EXPECT_UMAX, EXPECT_TAB_CAP, c->plan, err)) {
+        c->have_h = false;
+        return fail(c, GVQE_ERR_UNSUPPORTED, err);
+    }
+    // Walsh-Hadamard passes of the diagonal table: low window first, then windows of new high bits
+    c->fwht_tiles.clear(); c->fwht_masks.clear();
+    const int n = c->n_store, kt = n < 13 ? n : 13, ft = 5;
+    int done = 0;
+    while (done < n) {
+        TileDesc td; memset(&td, 0, sizeof td);
+        td.k = (uint8_t)kt;
+        uint32_t mask;
+        if (done == 0) {
+            td.n_runs = 1; td.runs[0] = Run{0, 0, (uint8_t)kt, 0};
+            mask = (kt >= 32) ? ~0u : ((1u << kt) - 1);
+            done = kt;
+        } else {
+            const int h = kt - ft;
+            int start = done; if (start + h > n) start = n - h;
+            td.n_runs = 2; td.runs[0] = Run{0, 0, (uint8_t)ft, 0}; td.runs[1] = Run{(uint8_t)ft, (uint8_t)start, (uint8_t)h, 0};
+            mask = 0;
+            for (int q = done; q < start + h; ++q) mask |= 1u << (ft + (q - start));
+            done = start + h;
+        }
+        c->fwht_tiles.push_back(td); c->fwht_masks.push_back(mask);
+    }
+    c->have_h = true; c->dirty = true;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_set_hamiltonian(gvqe_ctx *c, int M, const char *paulis, const double *coeffs)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (M < 0 || (M > 0 && (!paulis || !coeffs))) return fail(c, GVQE_ERR_INVALID_ARG, "set_hamiltonian: null input");
+    std::string err;
+    Hamiltonian H;
+    if (!hamiltonian_from_paulis(c->n_user, M, paulis, coeffs, H, err)) return fail(c, GVQE_ERR_INVALID_ARG, err);
+    c->H = H;
+    return after_hamiltonian(c);
+}
+
+gvqe_status gvqe_set_hamiltonian_masks(gvqe_ctx *c, int M, const uint64_t *xm, const uint64_t *zm, const double *coeffs)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (M < 0 || (M > 0 && (!xm || !zm || !coeffs))) return fail(c, GVQE_ERR_INVALID_ARG, "set_hamiltonian_masks: null input");
+    std::string err;
+    Hamiltonian H;
+    if (!hamiltonian_from_masks(c->n_user, M, xm, zm, coeffs, H, err)) return fail(c, GVQE_ERR_INVALID_ARG, err);
+    c->H = H;
+    return after_hamiltonian(c);
+}
+
+gvqe_status gvqe_get_grouping(const gvqe_ctx *c, uint64_t *xm, uint64_t *zm, uint8_t *ny, int32_t *got, int32_t *ng,
+                              uint64_t *gmask)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (!c->have_h) return GVQE_ERR_NO_HAMILTONIAN;
+    const size_t M = c->H.terms.size();
+    for (size_t k = 0; k < M; ++k) {
+        if (xm) xm[k] = c->H.terms[k].x;
+        if (zm) zm[k] = c->H.terms[k].z;
+        if (ny) ny[k] = (uint8_t)(c->H.terms[k].ny & 3);
+        if (got) got[k] = c->H.group_of_term[k];
+    }
+    if (ng) *ng = (int32_t)c->H.group_mask.size();
+    if (gmask) for (size_t g = 0; g < c->H.group_mask.size(); ++g) gmask[g] = c->H.group_mask[g];
+    return GVQE_OK;
+}
+
+}  // extern "C"
+
+// ---- workspace ---------------------------------------------------------------------------------------------
+namespace {
+
+struct Carve {
+    size_t off = 0;
+    size_t take(size_t bytes) { const size_t o = off; off = al256(off + bytes); return o; }
+};
+
+struct Layout {
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, passes, groups, terms, dz, dc, table, fixed_end;
+    size_t per_state;   // state + cs row + params row + partial slots + E
+    size_t state_b, cs_b, params_b, partial_b;
+};
+
+Layout layout_of(const gvqe_ctx *c)
+{
+    Layout L{};
+    Carve cv;
+    const DevProgram &d = c->dev;
+    L.blocks = cv.take(d.blocks.size() * sizeof(DBlock));
+    L.stages = cv.take(d.stages.size() * sizeof(DStage));
+    L.ops = cv.take(d.ops.size() * sizeof(DOp));
+    L.segs = cv.take(d.segs.size() * sizeof(DSeg));
+    L.trzs = cv.take(d.trzs.size() * sizeof(DTrz));
+    L.tczs = cv.take(d.tczs.size() * 8);
+    L.csidx = cv.take(d.csidx.size() * 4);
+    L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
+    L.groups = cv.take(c->plan.groups.size() * sizeof(DGroup));
+    L.terms = cv.take(c->plan.terms.size() * sizeof(DTerm));
+    L.dz = cv.take(c->H.diag_z.size() * 8);
+    L.dc = cv.take(c->H.diag_c.size() * 8);
+    L.table = cv.take(c->tab_bytes() << c->n_store);
+    L.fixed_end = cv.off;
+    const uint64_t tiles = 1ull << (c->n_store - c->plan.k);
+    L.state_b = al256(c->amp_bytes() << c->n_store);
+    L.cs_b = al256((size_t)(c->P > 0 ? c->P : 1) * c->amp_bytes());
+    L.params_b = al256((size_t)(c->P > 0 ? c->P : 1) * 8);
+    L.partial_b = al256((size_t)tiles * c->plan.passes.size() * 8);
+    L.per_state = L.state_b + L.cs_b + L.params_b + L.partial_b + 256 /* E */;
+    return L;
+}
+
+gvqe_status upload(gvqe_ctx *c, void *dst, const void *src, size_t bytes, cudaStream_t st)
+{
+    if (!bytes) return GVQE_OK;
+    const cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, st);
+    return e == cudaSuccess ? GVQE_OK : cuda_fail(c, e, "upload");
+}
+
+// Carve the workspace, upload the compiled program and the Hamiltonian arrays, build the diagonal table.
+gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
+{
+    if (!c->have_h) return fail(c, GVQE_ERR_NO_HAMILTONIAN, "no Hamiltonian set");
+    if (!c->ws) return fail(c, GVQE_ERR_WORKSPACE, "no workspace set");
+    if (!c->dirty) return GVQE_OK;
+    if (!c->kernels_ready) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return cuda_fail(c, e, "cudaGetDevice");
+        const int ke = kernels_init();
+        if (ke) return cuda_fail(c, ke, "kernel attribute setup");
+        c->kernels_ready = true;
+    }
+    const Layout L = layout_of(c);
+    if (c->ws_bytes < L.fixed_end + L.per_state) {
+        char b[160];
+        snprintf(b, sizeof b, "workspace too small: %zu bytes given, %zu needed for one statevector", c->ws_bytes,
+                 L.fixed_end + L.per_state);
+        return fail(c, GVQE_ERR_WORKSPACE, b);
+    }
+    size_t fit = (c->ws_bytes - L.fixed_end) / L.per_state;
+    if (fit > 32768) fit = 32768;
+    if (c->max_in_flight > 0 && fit > (size_t)c->max_in_flight) fit = (size_t)c->max_in_flight;
+    c->in_flight = (int)fit;
+    char *w = c->ws;
+    const DevProgram &d = c->dev;
+    c->gl.blocks = (const DBlock *)(w + L.blocks); c->gl.stages = (const DStage *)(w + L.stages);
+    c->gl.ops = (const DOp *)(w + L.ops); c->gl.segs = (const DSeg *)(w + L.segs);
+    c->gl.trzs = (const DTrz *)(w + L.trzs); c->gl.tczs = (const uint64_t *)(w + L.tczs);
+    c->gl.csidx = (const int32_t *)(w + L.csidx);
+    c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
+    c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
+    c->d_table = w + L.table;
+    char *p = w + L.fixed_end;
+    c->d_states = p; p += L.state_b * fit;
+    c->d_cs = p; p += L.cs_b * fit;
+    c->d_params = (double *)p; p += L.params_b * fit;
+    c->d_partial = (double *)p; p += L.partial_b * fit;
+    c->d_E = (double *)p;
+    c->slots_per_b = (uint32_t)((1ull << (c->n_store - c->plan.k)) * c->plan.passes.size());
+    gvqe_status s;
+#define UP(dst, vec) if ((s = upload(c, (void *)(dst), (vec).data(), (vec).size() * sizeof((vec)[0]), st)) != GVQE_OK) return s
+    UP(c->gl.blocks, d.blocks); UP(c->gl.stages, d.stages); UP(c->gl.ops, d.ops); UP(c->gl.segs, d.segs);
+    UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx);
+    UP(c->d_passes, c->plan.passes); UP(c->d_groups, c->plan.groups); UP(c->d_terms, c->plan.terms);
+    UP(c->d_diag_z, c->H.diag_z); UP(c->d_diag_c, c->H.diag_c);
+#undef UP
+    // diagonal energy table: E(x) = sum_{Z-only k} c_k (-1)^{popcount(x & z_k)} = WHT of the scattered coefficients
+    cudaError_t e = cudaMemsetAsync(c->d_table, 0, c->tab_bytes() << c->n_store, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "table memset");
+    int ke = launch_table_scatter(c->prec, c->d_table, c->d_diag_z, c->d_diag_c, (uint32_t)c->H.diag_z.size(), st, &c->launches);
+    if (ke) return cuda_fail(c, ke, "table scatter");
+    if (!c->H.diag_z.empty())
+        for (size_t i = 0; i < c->fwht_tiles.size(); ++i) {
+            ke = launch_fwht_pass(c->prec, c->d_table, c->fwht_tiles[i], c->fwht_masks[i], c->n_store, st, &c->launches);
+            if (ke) return cuda_fail(c, ke, "table transform");
+        }
+    c->dirty = false;
+    return GVQE_OK;
+}
+
+// One chunk of `nb` statevectors: parameters are already on the device (nb x P doubles).
+gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_dev, cudaStream_t st)
+{
+    const Layout L = layout_of(c);
+    const uint64_t stride = L.state_b / c->amp_bytes();
+    int ke = launch_expand_params(c->prec, params_dev, c->d_cs, (uint64_t)nb * c->P, st, &c->launches);
+    if (ke) return cuda_fail(c, ke, "expand_params");
+    for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
+        ke = launch_gate_block(c->prec, c->R, c->gl, (int)bi, c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
+                               c->n_store, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
+        if (ke) return cuda_fail(c, ke, "gate block");
+    }
+    const uint32_t tiles = 1u << (c->n_store - c->plan.k);
+    for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
+        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_states,
+                                stride, c->d_table, c->d_partial, c->slots_per_b, (uint32_t)pi * tiles, nb, st, &c->launches);
+        if (ke) return cuda_fail(c, ke, "expectation pass");
+    }
+    ke = launch_reduce(c->d_partial, c->slots_per_b, E_dev, nb, st, &c->launches);
+    if (ke) return cuda_fail(c, ke, "reduce");
+    return GVQE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t gvqe_workspace_bytes(const gvqe_ctx *c, int batch)
+{
+    if (!c || !c->have_h || batch < 1) return 0;
+    const Layout L = layout_of(c);
+    return L.fixed_end + L.per_state * (size_t)batch + 256;
+}
+
+gvqe_status gvqe_set_workspace(gvqe_ctx *c, void *ptr, size_t bytes)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (!ptr || ((uintptr_t)ptr & 255)) return fail(c, GVQE_ERR_INVALID_ARG, "workspace must be a 256-byte aligned device pointer");
+    if (c->have_h) {
+        const Layout L = layout_of(c);
+        if (bytes < L.fixed_end + L.per_state) return fail(c, GVQE_ERR_WORKSPACE, "workspace too small for one statevector");
+    } else if (bytes < (c->amp_bytes() << c->n_store)) return fail(c, GVQE_ERR_WORKSPACE, "workspace too small for one statevector");
+    c->ws = (char *)ptr; c->ws_bytes = bytes; c->dirty = true;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_set_max_in_flight(gvqe_ctx *c, int m)
+{
+    if (!c || m < 0) return GVQE_ERR_INVALID_ARG;
+    c->max_in_flight = m; c->dirty = true;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_energy_batch_device(gvqe_ctx *c, const double *params_dev, int B, double *E_dev, void *stream)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (B < 0 || (B > 0 && (!E_dev || (!params_dev && c->P > 0)))) return fail(c, GVQE_ERR_INVALID_ARG, "energy_batch_device: bad arguments");
+    cudaStream_t st = (cudaStream_t)stream;
+    gvqe_status s = ensure_ready(c, st);
+    if (s != GVQE_OK) return s;
+    for (int b0 = 0; b0 < B; b0 += c->in_flight) {
+        const int nb = (B - b0 < c->in_flight) ? (B - b0) : c->in_flight;
+        if ((s = run_chunk(c, params_dev + (size_t)b0 * c->P, nb, E_dev + b0, st)) != GVQE_OK) return s;
+    }
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_energy_batch(gvqe_ctx *c, const double *params, int B, double *E, void *stream)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (B < 0 || (B > 0 && (!E || (!params && c->P > 0)))) return fail(c, GVQE_ERR_INVALID_ARG, "energy_batch: bad arguments");
+    for (size_t i = 0; i < (size_t)B * c->P; ++i)
+        if (!std::isfinite(params[i])) return fail(c, GVQE_ERR_INVALID_ARG, "energy_batch: parameter is not finite");
+    cudaStream_t st = (cudaStream_t)stream;
+    gvqe_status s = ensure_ready(c, st);
+    if (s != GVQE_OK) return s;
+    for (int b0 = 0; b0 < B; b0 += c->in_flight) {
+        const int nb = (B - b0 < c->in_flight) ? (B - b0) : c->in_flight;
+        cudaError_t e = cudaSuccess;
+        if (c->P > 0) e = cudaMemcpyAsync(c->d_params, params + (size_t)b0 * c->P, (size_t)nb * c->P * 8, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
+        if ((s = run_chunk(c, c->d_params, nb, c->d_E, st)) != GVQE_OK) return s;
+        e = cudaMemcpyAsync(E + b0, c->d_E, (size_t)nb * 8, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "E D2H");
+        // d_params / d_E are reused by the next chunk: stream order makes that safe for pinned and pageable hosts
+    }
+    const cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "stream synchronize");
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_param_shift_grad(gvqe_ctx *c, const double *params, const uint8_t *mask, double *dE, double *E0, void *stream)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (c->P > 0 && (!params || !mask || !dE)) return fail(c, GVQE_ERR_INVALID_ARG, "param_shift_grad: null input");
+    std::vector<int> idx;
+    for (int p = 0; p < c->P; ++p) if (mask[p]) idx.push_back(p);
+    const int B = 2 * (int)idx.size() + 1;
+    // Eq. 13: rows theta, theta +/- (pi/2) e_p for the masked p, ascending (reading A8)
+    std::vector<double> rows((size_t)B * c->P), E((size_t)B);
+    for (int b = 0; b < B; ++b) for (int p = 0; p < c->P; ++p) rows[(size_t)b * c->P + p] = params[p];
+    const double half_pi = 1.57079632679489661923;
+    for (size_t j = 0; j < idx.size(); ++j) {
+        rows[(2 * j + 1) * c->P + idx[j]] += half_pi;
+        rows[(2 * j + 2) * c->P + idx[j]] -= half_pi;
+    }
+    const gvqe_status s = gvqe_energy_batch(c, rows.data(), B, E.data(), stream);
+    if (s != GVQE_OK) return s;
+    for (int p = 0; p < c->P; ++p) dE[p] = 0.0;
+    for (size_t j = 0; j < idx.size(); ++j) dE[idx[j]] = 0.5 * (E[2 * j + 1] - E[2 * j + 2]);
+    if (E0) *E0 = E[0];
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_get_state(gvqe_ctx *c, int slot, void *host_out)
+{
+    if (!c || !host_out) return GVQE_ERR_INVALID_ARG;
+    if (c->dirty || !c->ws) return fail(c, GVQE_ERR_WORKSPACE, "get_state: no energy call has run on this workspace");
+    if (slot < 0 || slot >= c->in_flight) return fail(c, GVQE_ERR_INVALID_ARG, "get_state: slot out of range");
+    const Layout L = layout_of(c);
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess)
+        e = cudaMemcpy(host_out, (char *)c->d_states + L.state_b * (size_t)slot, c->amp_bytes() << c->n_user, cudaMemcpyDeviceToHost);
+    return e == cudaSuccess ? GVQE_OK : cuda_fail(c, e, "get_state");
+}
+
+gvqe_status gvqe_schedule_info(const gvqe_ctx *c, int32_t *nb, int32_t *np, int32_t *inflight)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (nb) *nb = (int32_t)c->dev.blocks.size();
+    if (np) *np = c->have_h ? (int32_t)c->plan.passes.size() : 0;
+    if (inflight) *inflight = c->in_flight;
+    return GVQE_OK;
+}
+
+size_t gvqe_dump_schedule(const gvqe_ctx *c, char *buf, size_t cap)
+{
+    if (!c) return 0;
+    std::string s = dump_program(c->prog);
+    char line[256];
+    snprintf(line, sizeof line, "device blocks=%zu max_prog_smem=%u\n", c->dev.blocks.size(), c->dev.max_smem_prog);
+    s += line;
+    if (c->have_h) {
+        for (size_t p = 0; p < c->plan.passes.size(); ++p) {
+            const DPass &dp = c->plan.passes[p];
+            snprintf(line, sizeof line, "pass %zu k=%d diag=%d groups=%u runs=", p, dp.k, dp.with_diag, dp.group_end - dp.group_begin);
+            s += line;
+            for (int r = 0; r < dp.n_runs; ++r) { snprintf(line, sizeof line, "%d:%d+%d ", dp.runs[r].lpos, dp.runs[r].gpos, dp.runs[r].len); s += line; }
+            s += "\n";
+        }
+    }
+    if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }
+    return s.size() + 1;
+}
+
+int gvqe_get_exec_order(const gvqe_ctx *c, int32_t *order, int cap)
+{
+    if (!c) return -1;
+    const int m = (int)c->prog.exec_order.size();
+    if (order) for (int i = 0; i < m && i < cap; ++i) order[i] = c->prog.exec_order[i];
+    return m;
+}
+
+uint64_t gvqe_launch_count(const gvqe_ctx *c) { return c ? c->launches : 0; }
+const char *gvqe_last_error(const gvqe_ctx *c) { return c ? c->err.c_str() : "null context"; }
+void gvqe_destroy(gvqe_ctx *c) { delete c; }
+
+}  // extern "C"
