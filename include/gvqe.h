@@ -115,6 +115,17 @@ int gvqe_get_exec_order(const gvqe_ctx *ctx, int32_t *order, int cap);
 /* Kernel launches issued by this context since creation (for bench.py's gpu_launches). */
 uint64_t gvqe_launch_count(const gvqe_ctx *ctx);
 
+/* Per-phase device timing (CUDA events on the caller's stream around the gate blocks and around the expectation
+ * passes of every chunk).  gvqe_profile_enable(ctx, 1) resets the counters and starts recording, (ctx, 0) stops.
+ * gvqe_profile_read synchronises the recorded events and fills out[8] (host):
+ *   [0] gate-block kernel time, ms      [1] gate-block launches   [2] gate-block algorithmic bytes (SURVEY 8(d):
+ *   2*S per block and state, S for the write-only first block)     [3] expectation-pass kernel time, ms
+ *   [4] expectation-pass launches       [5] expectation algorithmic bytes (S per pass and state + the table once
+ *   per launch of the pass that carries the diagonal part)         [6] other kernels (expand, reduce) time, ms
+ *   [7] chunks recorded. */
+gvqe_status gvqe_profile_enable(gvqe_ctx *ctx, int on);
+gvqe_status gvqe_profile_read(gvqe_ctx *ctx, double *out);
+
 const char *gvqe_last_error(const gvqe_ctx *ctx);
 void gvqe_destroy(gvqe_ctx *ctx);
 

@@ -23,7 +23,7 @@ EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
-           "gvqe_last_error", "gvqe_destroy"]
+           "gvqe_profile_enable", "gvqe_profile_read", "gvqe_last_error", "gvqe_destroy"]
 
 
 class GvqeLayout(C.Structure):
@@ -73,6 +73,8 @@ def load():
     L.gvqe_get_exec_order.argtypes = [vp, vp, i32]
     L.gvqe_launch_count.argtypes = [vp]
     L.gvqe_launch_count.restype = u64
+    L.gvqe_profile_enable.argtypes = [vp, i32]
+    L.gvqe_profile_read.argtypes = [vp, vp]
     L.gvqe_last_error.argtypes = [vp]
     L.gvqe_last_error.restype = C.c_char_p
     L.gvqe_destroy.argtypes = [vp]
@@ -219,6 +221,15 @@ class Gvqe:
         o = np.zeros(max(m, 1), dtype=np.int32)
         self._L.gvqe_get_exec_order(self._h, o.ctypes.data, m)
         return o[:m]
+
+    def profile_enable(self, on: bool):
+        self._check(self._L.gvqe_profile_enable(self._h, 1 if on else 0))
+
+    def profile_read(self) -> dict:
+        o = np.zeros(8, dtype=np.float64)
+        self._check(self._L.gvqe_profile_read(self._h, o.ctypes.data))
+        keys = ["gate_ms", "gate_launches", "gate_bytes", "expect_ms", "expect_launches", "expect_bytes", "other_ms", "chunks"]
+        return dict(zip(keys, o.tolist()))
 
     def launch_count(self) -> int:
         return int(self._L.gvqe_launch_count(self._h))

@@ -54,6 +54,10 @@ struct gvqe_ctx {
     double *d_params = nullptr, *d_partial = nullptr, *d_E = nullptr;
     uint32_t slots_per_b = 0;
     uint64_t launches = 0;
+    // profiling (gvqe_profile_enable): 4 events per chunk
+    bool profiling = false;
+    std::vector<cudaEvent_t> ev;
+    double prof_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     std::string err;
     size_t amp_bytes() const { return prec == GVQE_C64 ? 8 : 16; }
     size_t tab_bytes() const { return prec == GVQE_C64 ? 4 : 8; }
@@ -326,25 +330,50 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
 }
 
 // One chunk of `nb` statevectors: parameters are already on the device (nb x P doubles).
+}  // namespace
+extern "C" gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out);
+namespace {
 gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_dev, cudaStream_t st)
 {
     const Layout L = layout_of(c);
     const uint64_t stride = L.state_b / c->amp_bytes();
+    cudaEvent_t e4[4] = {nullptr, nullptr, nullptr, nullptr};
+    if (c->profiling) {
+        if (c->ev.size() >= 4096) {   // fold what has been recorded so far
+            double tmp[8];
+            gvqe_profile_read(c, tmp);
+        }
+        for (int i = 0; i < 4; ++i) if (cudaEventCreate(&e4[i]) != cudaSuccess) return cuda_fail(c, (int)cudaGetLastError(), "event create");
+    }
     int ke = launch_expand_params(c->prec, params_dev, c->d_cs, (uint64_t)nb * c->P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
+    if (c->profiling) cudaEventRecord(e4[0], st);
     for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
         ke = launch_gate_block(c->prec, c->R, c->gl, (int)bi, c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
                                c->n_store, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "gate block");
     }
+    if (c->profiling) cudaEventRecord(e4[1], st);
     const uint32_t tiles = 1u << (c->n_store - c->plan.k);
     for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
         ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_states,
                                 stride, c->d_table, c->d_partial, c->slots_per_b, (uint32_t)pi * tiles, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "expectation pass");
     }
+    if (c->profiling) cudaEventRecord(e4[2], st);
     ke = launch_reduce(c->d_partial, c->slots_per_b, E_dev, nb, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "reduce");
+    if (c->profiling) {
+        cudaEventRecord(e4[3], st);
+        for (int i = 0; i < 4; ++i) c->ev.push_back(e4[i]);
+        const double S = (double)(c->amp_bytes() << c->n_store);
+        double gb = 0;
+        for (const DBlock &b : c->dev.blocks) gb += (b.source_zero ? 1.0 : 2.0) * S * nb;
+        c->prof_acc[1] += (double)c->dev.blocks.size(); c->prof_acc[2] += gb;
+        c->prof_acc[4] += (double)c->plan.passes.size();
+        c->prof_acc[5] += (double)c->plan.passes.size() * S * nb + (double)(c->tab_bytes() << c->n_store);
+        c->prof_acc[7] += 1.0;
+    }
     return GVQE_OK;
 }
 
@@ -488,8 +517,43 @@ int gvqe_get_exec_order(const gvqe_ctx *c, int32_t *order, int cap)
     return m;
 }
 
+gvqe_status gvqe_profile_enable(gvqe_ctx *c, int on)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (on) {
+        for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+        c->ev.clear();
+        for (double &v : c->prof_acc) v = 0.0;
+    }
+    c->profiling = on != 0;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out)
+{
+    if (!c || !out) return GVQE_ERR_INVALID_ARG;
+    for (size_t i = 0; i + 3 < c->ev.size(); i += 4) {
+        cudaError_t e = cudaEventSynchronize(c->ev[i + 3]);
+        if (e != cudaSuccess) return cuda_fail(c, e, "profile event");
+        float g = 0, x = 0, r = 0;
+        cudaEventElapsedTime(&g, c->ev[i], c->ev[i + 1]);
+        cudaEventElapsedTime(&x, c->ev[i + 1], c->ev[i + 2]);
+        cudaEventElapsedTime(&r, c->ev[i + 2], c->ev[i + 3]);
+        c->prof_acc[0] += g; c->prof_acc[3] += x; c->prof_acc[6] += r;
+    }
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    c->ev.clear();
+    for (int i = 0; i < 8; ++i) out[i] = c->prof_acc[i];
+    return GVQE_OK;
+}
+
 uint64_t gvqe_launch_count(const gvqe_ctx *c) { return c ? c->launches : 0; }
 const char *gvqe_last_error(const gvqe_ctx *c) { return c ? c->err.c_str() : "null context"; }
-void gvqe_destroy(gvqe_ctx *c) { delete c; }
+void gvqe_destroy(gvqe_ctx *c)
+{
+    if (!c) return;
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    delete c;
+}
 
 }  // extern "C"

@@ -1,0 +1,246 @@
+"""GPU parity: libgvqe (through the C ABI) against the CPU oracle on the same seeded inputs.  Run with -m gpu.
+
+Tolerances (BASELINE.json north_star; reading A13):
+  complex128: |dE| <= 1e-10 |E_oracle| + 1e-12 sum|c_k|
+  complex64 : |dE| <= max(1e-4 |E_oracle|, 1e-5 sum|c_k|)
+Masks / grouping are bit-exact (tests/test_host_logic.py, CPU)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import paper_2607_02749_b200 as gv
+from workload import make_workload, layout_ops, num_params, OP_RY, OP_RZ, OP_CZ, OP_CNOT
+from workload.generator import random_ops, random_paulis
+
+pytestmark = pytest.mark.gpu
+
+
+def tol(prec, E_ref, coeffs):
+    s = float(np.sum(np.abs(coeffs)))
+    E_ref = np.abs(np.asarray(E_ref, dtype=np.float64))
+    if prec == "c128":
+        return 1e-10 * E_ref + 1e-12 * max(s, 1e-300)
+    return np.maximum(1e-4 * E_ref, 1e-5 * s)
+
+
+def assert_close(prec, E, E_ref, coeffs, what=""):
+    E, E_ref = np.asarray(E), np.asarray(E_ref)
+    bad = np.abs(E - E_ref) > tol(prec, E_ref, coeffs)
+    assert not bad.any(), f"{what}: max |dE| = {np.max(np.abs(E - E_ref)):.3e}, first bad row {int(np.argmax(bad))}"
+
+
+def ctx_for(w, prec, in_flight=None, ops=False):
+    if ops:
+        g = gv.Gvqe(w.n, ops=w.ops, n_params=w.P, precision=prec)
+    else:
+        g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
+                    precision=prec)
+    g.set_hamiltonian(w.paulis, w.coeffs)
+    g.alloc_workspace(in_flight or min(w.B, 64))
+    return g
+
+
+# ---- BASELINE configs ----------------------------------------------------------------------------------------
+def test_config1_full(orc):
+    """10 qubits, c128, Z-only H, the 2P+1 = 141 row parameter-shift set; every row against T0."""
+    w = make_workload(1)
+    g = ctx_for(w, "c128", 141)
+    E = g.energy_batch(w.params)
+    assert_close("c128", E, orc.energy_batch(w.n, w.ops, w.params, w.paulis, w.coeffs), w.coeffs, "cfg1")
+    dE, E0 = g.param_shift_grad(w.theta, w.mask)
+    dE_o, E0_o = orc.param_shift_grad(w.n, w.ops, w.theta, w.mask, w.paulis, w.coeffs)
+    assert abs(E0 - E0_o) <= tol("c128", E0_o, w.coeffs)
+    assert np.max(np.abs(dE - dE_o)) <= 1e-10 * np.max(np.abs(E)) + 1e-12 * np.sum(np.abs(w.coeffs))
+
+
+def test_config2_full_cluster_gradient(orc):
+    """16 qubits, c128, 1000 terms (15 % X/Y), cluster-restricted gradient over community 0 (36 params, batch 73)."""
+    w = make_workload(2)
+    assert int(w.mask.sum()) == 36 and w.B == 73
+    g = ctx_for(w, "c128", 73)
+    dE, E0 = g.param_shift_grad(w.theta, w.mask)
+    dE_o, E0_o = orc.param_shift_grad(w.n, w.ops, w.theta, w.mask, w.paulis, w.coeffs)
+    assert abs(E0 - E0_o) <= tol("c128", E0_o, w.coeffs)
+    assert np.all(dE[w.mask == 0] == 0.0)
+    assert np.max(np.abs(dE - dE_o)) <= 1e-10 * abs(E0_o) + 1e-12 * np.sum(np.abs(w.coeffs))
+    E = g.energy_batch(w.params)
+    assert_close("c128", E[:8], orc.energy_batch(w.n, w.ops, w.params[:8], w.paulis, w.coeffs), w.coeffs, "cfg2 rows")
+
+
+@pytest.mark.parametrize("prec", ["c64", "c128"])
+def test_config3_full_sampled(orc, prec):
+    """22 qubits, 5000 terms, batch 64 in the bench launch configuration; rows 0, 31, 63 against the oracle
+    (T1 for all three, T0 term-by-term for row 0 on a 300-term subsample of the same Hamiltonian)."""
+    w = make_workload(3)
+    g = ctx_for(w, prec, 64)
+    E = g.energy_batch(w.params)
+    rows = [0, 31, 63]
+    ref = []
+    for b in rows:
+        psi = orc.state(w.n, w.ops, w.params[b])
+        ref.append(orc.t1_energy_of_state(w.n, psi, w.paulis, w.coeffs))
+    assert_close(prec, E[rows], ref, w.coeffs, f"cfg3 {prec}")
+    # T0 on a subsample through the same library path
+    idx = np.arange(0, w.M, 17)
+    pl = w.pauli_list()
+    sub_p = "".join(pl[i] for i in idx).encode()
+    g.set_hamiltonian(sub_p, w.coeffs[idx])
+    g.alloc_workspace(1)
+    E0 = g.energy_batch(w.params[:1])
+    psi = orc.state(w.n, w.ops, w.params[0])
+    assert_close(prec, E0, [orc.energy_of_state(w.n, psi, sub_p, w.coeffs[idx])], w.coeffs[idx], "cfg3 T0 subsample")
+
+
+def test_config4_shape_at_24_qubits(orc):
+    """Config 4 recipe (CNOT ring, pooled flip masks, c64) at 24 qubits, 2 layers: one row against T1."""
+    w = make_workload(4, n=24, M=4000, D=2, batch=2)
+    g = ctx_for(w, "c64", 2)
+    E = g.energy_batch(w.params)
+    psi = orc.state(w.n, w.ops, w.params[1])
+    assert_close("c64", E[1:2], [orc.t1_energy_of_state(w.n, psi, w.paulis, w.coeffs)], w.coeffs, "cfg4@24")
+
+
+def test_config4_full_size_properties():
+    """28 qubits c64, full 20 000-term Hamiltonian, chunks of 8: properties that hold at any size."""
+    w = make_workload(4)
+    g = ctx_for(w, "c64", 8)
+    zsum = sum(c for s, c in zip(w.pauli_list(), w.coeffs) if "X" not in s and "Y" not in s)
+    rows = np.zeros((9, w.P))                                   # 9 rows -> two chunks (8 + 1)
+    rng = np.random.default_rng(4)
+    xs = [0]
+    for b in range(1, 9):                                       # last-layer RY(pi x_q): psi = +-e_x, E = E_diag(x)
+        x = int(rng.integers(0, 1 << w.n))
+        xs.append(x)
+        for q in range(w.n):
+            rows[b, 2 * w.n * w.D + q] = math.pi * ((x >> q) & 1)
+    E = g.energy_batch(rows)
+    zs = [(sum(1 << q for q, ch in enumerate(s) if ch == "Z"), c) for s, c in zip(w.pauli_list(), w.coeffs)
+          if "X" not in s and "Y" not in s]
+    want = [sum(c * (-1) ** bin(x & z).count("1") for z, c in zs) for x in xs]
+    assert abs(want[0] - zsum) < 1e-9
+    assert_close("c64", E, want, w.coeffs, "cfg4 basis states")
+    E2 = g.energy_batch(w.params[:3])                           # random angles: bound and determinism
+    assert np.all(np.abs(E2) <= np.sum(np.abs(w.coeffs)))
+    assert np.array_equal(E2, g.energy_batch(w.params[:3]))
+
+
+# ---- embedding: an n' problem on arbitrary (high) qubits of a larger register equals the n' oracle energy ------------
+@pytest.mark.parametrize("prec,n_big", [("c64", 26), ("c128", 25)])
+def test_embedding_on_high_qubits(orc, prec, n_big):
+    n_s = 12
+    w = make_workload(4, n=n_s, M=300, D=2, batch=2)
+    place = [1, 3, 6, 9, 11, 14, 15, 17, 20, 22, n_big - 2, n_big - 1]
+    ops = w.ops.copy()
+    for o in ops:
+        o[1] = place[o[1]]
+        if o[2] >= 0:
+            o[2] = place[o[2]]
+    pl = []
+    for s in w.pauli_list():
+        t = ["I"] * n_big
+        for q, ch in enumerate(s):
+            t[place[q]] = ch
+        t[0] = "Z"                                               # idle qubit 0 stays |0>: Z contributes +1
+        pl.append("".join(t))
+    g = gv.Gvqe(n_big, ops=ops, n_params=w.P, precision=prec)
+    g.set_hamiltonian("".join(pl).encode(), w.coeffs)
+    g.alloc_workspace(2)
+    E = g.energy_batch(w.params)
+    assert_close(prec, E, orc.energy_batch(n_s, w.ops, w.params, w.paulis, w.coeffs), w.coeffs, "embedding")
+
+
+# ---- randomised small cases: arbitrary op lists and Pauli strings, several tiles, ragged sizes ------------------------
+@pytest.mark.parametrize("seed", range(14))
+def test_random_circuits_and_paulis(orc, seed, monkeypatch):
+    n = 1 + seed
+    monkeypatch.setenv("GVQE_K", str(10 + seed % 3))            # n > k from n = 11 on: multi-tile and strided blocks
+    prec = "c64" if seed % 2 else "c128"
+    ops, P = random_ops(7000 + seed, n, 150)
+    paulis, coeffs = random_paulis(8000 + seed, n, 80, min(n, 6))
+    th = np.random.default_rng(seed).uniform(-math.pi, math.pi, (5, P))
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec)
+    g.set_hamiltonian(paulis, coeffs)
+    g.alloc_workspace(3)                                         # 5 rows in chunks of 3 + 2
+    E = g.energy_batch(th)
+    assert_close(prec, E, orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, f"random n={n}")
+    psi = g.get_state(1)                                         # slot 1 of the last chunk = row 4
+    ref = orc.state(n, ops, th[4])
+    assert np.max(np.abs(psi - ref)) < (1e-12 if prec == "c128" else 2e-5)
+
+
+@pytest.mark.parametrize("n,D,ent,topo,fr,prec", [(13, 3, "cz", "linear", 1, "c64"), (15, 2, "cnot", "ring", 1, "c64"),
+                                                   (14, 2, "cnot", "linear", 2, "c128"), (16, 3, "cz", "ring", 2, "c128"),
+                                                   (17, 2, "cnot", "ring", 1, "c128"), (18, 2, "cz", "linear", 2, "c64")])
+def test_layered_ansatz_variants(orc, n, D, ent, topo, fr, prec):
+    ops = np.array(layout_ops(n, D, ent, topo, fr), dtype=np.int32)
+    P = num_params(n, D, fr)
+    paulis, coeffs = random_paulis(100 + n, n, 120, 5)
+    th = np.random.default_rng(n).uniform(-math.pi, math.pi, (4, P))
+    g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo, final_rot=fr), precision=prec)
+    g.set_hamiltonian(paulis, coeffs)
+    g.alloc_workspace(4)
+    assert_close(prec, g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, "layered")
+
+
+# ---- edge cases ----------------------------------------------------------------------------------------------------
+def test_edge_cases(orc):
+    n = 11
+    ops = np.array(layout_ops(n, 1, "cz", "linear", 1), dtype=np.int32)
+    P = num_params(n, 1, 1)
+    th = np.random.default_rng(0).uniform(-math.pi, math.pi, (3, P))
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision="c128")
+    # empty Hamiltonian, identity only, duplicates, a weight-n string (direct mode), empty batch
+    g.set_hamiltonian(b"", [])
+    g.alloc_workspace(3)
+    assert np.array_equal(g.energy_batch(th), np.zeros(3))
+    g.set_hamiltonian(b"I" * n, [2.5])
+    g.alloc_workspace(3)
+    assert np.allclose(g.energy_batch(th), 2.5, atol=1e-12)
+    strs = ["ZZ" + "I" * (n - 2)] * 3 + ["XYZ" + "I" * (n - 3)] * 2 + ["Y" * n, "X" + "Z" * (n - 1), "Z" * n]
+    cs = np.array([0.5, -1.5, 2.0, 0.3, 0.4, 1.1, -0.7, 0.9])
+    g.set_hamiltonian("".join(strs).encode(), cs)
+    g.alloc_workspace(2)
+    assert_close("c128", g.energy_batch(th), orc.energy_batch(n, ops, th, "".join(strs).encode(), cs), cs, "edge")
+    assert len(g.energy_batch(np.zeros((0, P)))) == 0
+    with pytest.raises(gv.GvqeError):
+        g.energy_batch(np.full((1, P), np.nan))
+    # a circuit with no parameters and no ops at all
+    g0 = gv.Gvqe(3, ops=np.zeros((0, 4), dtype=np.int32), n_params=0, precision="c64")
+    g0.set_hamiltonian(b"ZIZ" + b"XII", [1.0, 1.0])
+    g0.alloc_workspace(1)
+    assert abs(g0.energy_batch(np.zeros((1, 0)))[0] - 1.0) < 1e-6
+
+
+def test_chunking_determinism_and_device_api():
+    import torch
+
+    w = make_workload(3, n=15, M=600, D=3, batch=10)
+    a = ctx_for(w, "c64", 10)
+    b = ctx_for(w, "c64", 10)
+    b.set_max_in_flight(3)
+    Ea, Eb = a.energy_batch(w.params), b.energy_batch(w.params)
+    assert np.array_equal(Ea, Eb)                                # chunking does not change a bit
+    assert np.array_equal(Ea, a.energy_batch(w.params))          # repeated call is bit-identical
+    p_dev = torch.from_numpy(w.params).cuda()
+    E_dev = torch.zeros(10, dtype=torch.float64, device="cuda")
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    a.energy_batch_device(p_dev.data_ptr(), 10, E_dev.data_ptr(), s.cuda_stream)
+    s.synchronize()
+    assert np.array_equal(E_dev.cpu().numpy(), Ea)
+    assert a.launch_count() > 0
+
+
+def test_final_rot_2_is_eq8(orc):
+    """Eq. 8 layout (final layer RY and RZ): P = 2N(D+1)."""
+    n, D = 12, 2
+    ops = np.array(layout_ops(n, D, "cnot", "ring", 2), dtype=np.int32)
+    g = gv.Gvqe(n, layout=dict(n_layers=D, entangler="cnot", topology="ring", final_rot=2), precision="c128")
+    assert g.P == 2 * n * (D + 1)
+    paulis, coeffs = random_paulis(3, n, 60, 4)
+    g.set_hamiltonian(paulis, coeffs)
+    g.alloc_workspace(2)
+    th = np.random.default_rng(1).uniform(-math.pi, math.pi, (2, g.P))
+    assert_close("c128", g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, "eq8")
