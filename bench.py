@@ -1,0 +1,144 @@
+#!/usr/bin/env python
+"""bench.py -- VQE energy evaluations/s of libgvqe on one B200 (BASELINE.json metric), with the HBM roofline of the
+dominant kernel and the CPU oracle timed beside it.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..6] [--impl ours|reference]
+
+A step = one gvqe_energy_batch call: the whole hot path (parameter expansion, every fused gate block, every
+expectation pass, reduction) over one batch of synthetic parameter vectors of the configured workload.  Default
+workload: BASELINE config 4 (28 qubits, complex64, 6 layers RY/RZ + CNOT ring, 20 000 Pauli terms, parameter-shift
+sweep streamed 8 statevectors at a time).  The path does not shard (replicas only): with --gpus N every
+rank runs the same workload on its own GPU on different rows of the sweep, no collective in the data path.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "vqe_energy_evals_per_s"
+UNIT = "evals/s"
+PREC_OF = {1: "c128", 2: "c128", 3: "c64", 4: "c64", 5: "c64", 6: "c128"}
+ROWS_PER_STEP = {1: 141, 2: 73, 3: 64, 4: 8, 5: 1, 6: 1}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index=0):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                o = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                    "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in o.strip().split(",")]
+                if len(f) >= 6:
+                    self.rows.append(f)
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(int(r[0]) for r in self.rows if r[0].isdigit())
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [nm for i, nm in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None,
+                "sm_max_mhz": int(self.rows[0][1]) if self.rows[0][1].isdigit() else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def oracle_sample(cfg, budget_rows=4):
+    """Time the CPU oracle (oracle/, as it stands) on a bounded sample of the workload; returns evals/s and a
+    description.  Small configs: whole evaluations.  Large configs: an evenly spaced sample of the circuit's ops
+    (orc_state) and of the Hamiltonian's terms (orc_energy, term by term), extrapolated linearly in the op and term
+    counts (both loops are plain passes over the 2^n amplitudes, so the cost is linear in each)."""
+    import psutil
+    import oracle
+    from workload import make_workload
+
+    oracle.build()
+    cores = oracle.max_threads()
+    w = make_workload(cfg, batch=1) if cfg >= 3 else make_workload(cfg)
+    n, scale = w.n, 1.0
+    if n <= 16:
+        rows = w.params[:budget_rows]
+        t0 = time.perf_counter()
+        oracle.energy_batch(w.n, w.ops, rows, w.paulis, w.coeffs)
+        dt = time.perf_counter() - t0
+        return len(rows) / dt, cores, f"{len(rows)} full evaluations of config {cfg} (T0, {w.M} terms), {dt:.2f} s"
+    avail = psutil.virtual_memory().available
+    n_s = n
+    while (24 << n_s) > 0.6 * avail and n_s > 20:
+        n_s -= 1
+    if n_s != n:
+        scale = float(1 << (n - n_s))
+        w = make_workload(cfg, n=n_s, batch=1)
+    k_ops, k_t = min(len(w.ops), 24), min(w.M, 8)
+    oi = np.linspace(0, len(w.ops) - 1, k_ops).astype(int)
+    ti = np.linspace(0, w.M - 1, k_t).astype(int)
+    pl = w.pauli_list()
+    sub_p = "".join(pl[i] for i in ti).encode()
+    t0 = time.perf_counter()
+    psi = oracle.state(w.n, w.ops[oi], w.params[0])
+    t_ops = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    oracle.energy_of_state(w.n, psi, sub_p, w.coeffs[ti])
+    t_terms = time.perf_counter() - t0
+    t_eval = scale * (t_ops * len(w.ops) / k_ops + t_terms * w.M / k_t)
+    desc = (f"config {cfg}: {k_ops} of {len(w.ops)} ops ({t_ops:.2f} s) and {k_t} of {w.M} terms ({t_terms:.2f} s) at "
+            f"{w.n} qubits, extrapolated linearly to one full evaluation" + (f" and x{scale:.0f} to {n} qubits" if scale > 1 else ""))
+    return 1.0 / t_eval, cores, desc
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, same metric/config; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    vals = []
+    desc, cores = "", 0
+    for _ in range(max(1, min(args.steps, 3))):
+        v, cores, desc = oracle_sample(args.config, budget_rows=2)
+        vals.append(v)
+    v = float(np.median(vals))
+    rows = ROWS_PER_STEP[args.config]
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * rows / v, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": workload_config(args.config),
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(cfg):
+    from workload import CONFIGS
+    c = CONFIGS[cfg]
+    return {"workload": f"BASELINE config {cfg if cfg < 5 else ('5a' if cfg == 5 else '5b')}: {c['n']} qubits, "
+                        f"{PREC_OF[cfg]}, {c['D']} layers RY/RZ + {c['entangler'].upper()} {c['topology']}, "
+                        f"{c['M']} Pauli terms", "rows_per_step": ROWS_PER_STEP[cfg], "precision": PREC_OF[cfg],
+            "l2": "state buffers in flight exceed the 126 MB L2" if c["n"] >= 24 else "L2-resident working set (see DESIGN.md)",
+            "parallelism": "replicas"}
