@@ -142,3 +142,121 @@ def workload_config(cfg):
                         f"{c['M']} Pauli terms", "rows_per_step": ROWS_PER_STEP[cfg], "precision": PREC_OF[cfg],
             "l2": "state buffers in flight exceed the 126 MB L2" if c["n"] >= 24 else "L2-resident working set (see DESIGN.md)",
             "parallelism": "replicas"}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2607_02749_b200 as gv
+    from workload import make_workload
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg, prec, rows = args.config, PREC_OF[args.config], ROWS_PER_STEP[args.config]
+    w = make_workload(cfg)
+    g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
+                precision=prec)
+    g.set_hamiltonian(w.paulis, w.coeffs)
+    g.alloc_workspace(rows, device=f"cuda:{local}")
+    n_gate_blocks, n_passes, _ = g.schedule_info()
+    stream = torch.cuda.Stream()
+    total = args.warmup + args.steps
+
+    def step_rows(i):   # each step takes the next `rows` rows of the sweep (rank-shifted), wrapping around
+        idx = (np.arange(rows) + (i * world + rank) * rows) % w.B
+        return w.params[idx]
+
+    host_in = [torch.from_numpy(np.ascontiguousarray(step_rows(i))).pin_memory() for i in range(total)]
+    host_out = torch.zeros(rows, dtype=torch.float64).pin_memory()
+    dev_in = [t.cuda(non_blocking=True) for t in host_in]
+    dev_out = torch.zeros(rows, dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn):   # device time of exactly args.steps steps, max over ranks
+        for i in range(args.warmup):
+            fn(i)
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for i in range(args.warmup, total):
+            fn(i)
+        e1.record(stream)
+        barrier()
+        ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = g.launch_count()
+    ms_dev = timed(lambda i: g.energy_batch_device(dev_in[i].data_ptr(), rows, dev_out.data_ptr(), stream.cuda_stream))
+    launches = (g.launch_count() - l0) * args.steps // total
+    sampler.stop_flag = True
+    ms_e2e = timed(lambda i: g.energy_batch_ptr(host_in[i].data_ptr(), rows, host_out.data_ptr(), stream.cuda_stream))
+    clocks = sampler.summary()
+    # per-kernel-class device time (CUDA events inside the library, on the same stream), outside the timed region
+    g.profile_enable(True)
+    for i in range(args.warmup, total):
+        g.energy_batch_device(dev_in[i].data_ptr(), rows, dev_out.data_ptr(), stream.cuda_stream)
+    stream.synchronize()
+    prof = g.profile_read()
+    g.profile_enable(False)
+    if rank != 0:
+        return
+    peak, peak_src = peaks()
+    gate_gbs = prof["gate_bytes"] / (prof["gate_ms"] * 1e-3) / 1e9 if prof["gate_ms"] > 0 else 0.0
+    exp_gbs = prof["expect_bytes"] / (prof["expect_ms"] * 1e-3) / 1e9 if prof["expect_ms"] > 0 else 0.0
+    value = rows * world * args.steps / (ms_dev * 1e-3)
+    e2e = rows * world * args.steps / (ms_e2e * 1e-3)
+    cpu_v, cores, desc = oracle_sample(cfg) if (world == 1 and not args.no_cpu_baseline) else (None, 0, "skipped")
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_dev / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if prec == "c64" else "f64", "data": "synthetic", "config": workload_config(cfg),
+        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": rows * w.P * 8, "d2h_bytes_per_step": rows * 8},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "gate_block_kernel", "achieved": gate_gbs, "peak": peak, "unit": "GB/s",
+                     "frac": gate_gbs / peak, "frac_of_8TBs": gate_gbs / 8000.0, "traffic": None, "peak_source": peak_src,
+                     "launches_per_step": n_gate_blocks,
+                     "avg_launch_ms": prof["gate_ms"] / max(prof["gate_launches"], 1),
+                     "share_of_step": prof["gate_ms"] / max(prof["gate_ms"] + prof["expect_ms"] + prof["other_ms"], 1e-9)},
+        "expectation": {"kernel": "expect_pass_kernel", "achieved": exp_gbs, "unit": "GB/s", "frac": exp_gbs / peak,
+                        "frac_of_8TBs": exp_gbs / 8000.0, "launches_per_step": n_passes,
+                        "avg_launch_ms": prof["expect_ms"] / max(prof["expect_launches"], 1)},
+        "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
