@@ -64,7 +64,7 @@ struct DTerm {               // one Pauli term of an off-diagonal group, 32 byte
 
 struct URun { uint8_t lpos, len, shift, pad; };   // table index bits: ((j >> lpos) & ((1<<len)-1)) << shift
 
-struct DGroup {              // one flip mask inside a pass, 36 bytes
+struct DGroup {              // one flip mask (or a slice of its terms) inside a pass, 52 bytes
     uint32_t m_loc;          // flip mask in local tile coordinates (non-zero)
     uint32_t term_begin, term_end;
     uint32_t tab_off;        // offset of the group's W table in the shared-memory table area
@@ -73,8 +73,12 @@ struct DGroup {              // one flip mask inside a pass, 36 bytes
     uint8_t pivot;           // highest set bit of m_loc
     uint8_t direct;          // 1: no table; W is summed term by term per pair and DTerm.zu is the LOCAL z mask
     uint8_t last_in_batch;   // 1: tables of groups up to and including this one are built together
-    uint8_t pad[3];
+    uint8_t n_ex;            // table mode: entries of ex[] = 1 + loop bits
+    uint8_t pad[2];
     URun uruns[3];
+    uint8_t ex[8];           // ascending local bit positions that are NOT thread bits: the pivot and the loop bits
+    uint8_t lp[8];           // the loop bits (n_ex - 1 of them): local positions outside the table index bits, so
+                             // that W is constant over a thread's pairs
 };
 
 struct DPass {               // one read-only sweep over the state

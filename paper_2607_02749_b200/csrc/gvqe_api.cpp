@@ -503,6 +503,14 @@ size_t gvqe_dump_schedule(const gvqe_ctx *c, char *buf, size_t cap)
             s += line;
             for (int r = 0; r < dp.n_runs; ++r) { snprintf(line, sizeof line, "%d:%d+%d ", dp.runs[r].lpos, dp.runs[r].gpos, dp.runs[r].len); s += line; }
             s += "\n";
+            int nd = 0, hist[16] = {0}; size_t nt_d = 0, nt_t = 0;
+            for (uint32_t gi = dp.group_begin; gi < dp.group_end; ++gi) {
+                const DGroup &dg = c->plan.groups[gi];
+                if (dg.direct) { ++nd; nt_d += dg.term_end - dg.term_begin; } else { ++hist[dg.ubits & 15]; nt_t += dg.term_end - dg.term_begin; }
+            }
+            snprintf(line, sizeof line, "grp  direct=%d (terms %zu) table terms=%zu ubits hist:", nd, nt_d, nt_t); s += line;
+            for (int u = 0; u < 16; ++u) if (hist[u]) { snprintf(line, sizeof line, " %d:%d", u, hist[u]); s += line; }
+            s += "\n";
         }
     }
     if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }

@@ -178,41 +178,70 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
         dp.n_runs = (uint8_t)nr;
         dp.group_begin = (uint32_t)plan.groups.size();
         uint32_t tab_used = 0;
+        const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // log2(threads) of the expectation kernel
+        const int L = k - 1 - TB;                                   // loop bits: 2^L pairs per thread and group
+        const int umax_eff = umax < TB ? umax : TB;
         for (int g : passG[p]) {
-            DGroup dg; memset(&dg, 0, sizeof dg);
-            dg.m_loc = compress(gm[g], T);
-            dg.pivot = (uint8_t)(31 - __builtin_clz(dg.m_loc));
-            uint64_t U = 0;
-            for (int t : gterms[g]) U |= H.terms[t].z;
-            U &= T;
-            const uint32_t Uloc = compress(U, T);
-            Run ur[4];
-            const int nur = runs_of(Uloc, ur, 4);
-            const int ubits = __builtin_popcount(Uloc);
-            const bool table = (ubits <= umax) && (nur <= 3) && ((1u << ubits) <= tab_cap);
-            dg.direct = table ? 0 : 1;
-            dg.term_begin = (uint32_t)plan.terms.size();
-            if (table) {
-                dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)nur;
-                for (int r = 0; r < nur; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
-                if (tab_used + (1u << ubits) > tab_cap) {   // close the batch before this group
-                    if (!plan.groups.empty() && plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
-                    tab_used = 0;
-                }
-                dg.tab_off = tab_used; tab_used += 1u << ubits;
-            }
+            // slice the group's terms so that every slice's table index (in-tile z bits) stays small  (Eq. 12)
+            std::vector<std::vector<int>> slices;
+            std::vector<uint32_t> sliceU;
             for (int t : gterms[g]) {
-                const HostTerm &ht = H.terms[t];
-                DTerm dt; memset(&dt, 0, sizeof dt);
-                static const double pr[4] = {1, 0, -1, 0}, pim[4] = {0, 1, 0, -1};
-                dt.cr = ht.c * pr[ht.ny & 3]; dt.ci = ht.c * pim[ht.ny & 3];
-                dt.zout = ht.z & ~T;
-                const uint32_t zloc = compress(ht.z & T, T);
-                dt.zu = table ? compress(zloc, Uloc) : zloc;
-                plan.terms.push_back(dt);
+                const uint32_t zl = compress(H.terms[t].z & T, T);
+                Run ur[4];
+                bool placed = false;
+                if (!slices.empty()) {
+                    const uint32_t U2 = sliceU.back() | zl;
+                    if (__builtin_popcount(U2) <= umax_eff && runs_of(U2, ur, 4) <= 3) {
+                        slices.back().push_back(t); sliceU.back() = U2; placed = true;
+                    }
+                }
+                if (!placed) { slices.emplace_back(1, t); sliceU.push_back(zl); }
             }
-            dg.term_end = (uint32_t)plan.terms.size();
-            plan.groups.push_back(dg);
+            for (size_t sl = 0; sl < slices.size(); ++sl) {
+                DGroup dg; memset(&dg, 0, sizeof dg);
+                dg.m_loc = compress(gm[g], T);
+                dg.pivot = (uint8_t)(31 - __builtin_clz(dg.m_loc));
+                const uint32_t Uloc = sliceU[sl];
+                Run ur[4];
+                const int nur = runs_of(Uloc, ur, 4);
+                const int ubits = __builtin_popcount(Uloc);
+                const bool table = (ubits <= umax_eff) && (nur <= 3) && ((1u << ubits) <= tab_cap);
+                dg.direct = table ? 0 : 1;
+                dg.term_begin = (uint32_t)plan.terms.size();
+                if (table) {
+                    dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)nur;
+                    for (int r = 0; r < nur; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
+                    if (tab_used + (1u << ubits) > tab_cap) {   // close the batch before this group
+                        if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
+                        tab_used = 0;
+                    }
+                    dg.tab_off = tab_used; tab_used += 1u << ubits;
+                    // loop bits: the L highest local bits outside the table index bits and the pivot
+                    uint32_t excl = 1u << dg.pivot;
+                    int nl = 0;
+                    for (int b = k - 1; b >= 0 && nl < L; --b)
+                        if (!((Uloc | (1u << dg.pivot)) >> b & 1)) { excl |= 1u << b; ++nl; }
+                    if (nl < L) { err = "hamiltonian: no room for loop bits (internal)"; return false; }
+                    int ne = 0, nlp = 0;
+                    for (int b = 0; b < k; ++b) if (excl >> b & 1) {
+                        dg.ex[ne++] = (uint8_t)b;
+                        if (b != dg.pivot) dg.lp[nlp++] = (uint8_t)b;
+                    }
+                    dg.n_ex = (uint8_t)ne;
+                }
+                for (int t : slices[sl]) {
+                    const HostTerm &ht = H.terms[t];
+                    DTerm dt; memset(&dt, 0, sizeof dt);
+                    static const double pr[4] = {1, 0, -1, 0}, pim[4] = {0, 1, 0, -1};
+                    dt.cr = ht.c * pr[ht.ny & 3]; dt.ci = ht.c * pim[ht.ny & 3];
+                    dt.zout = ht.z & ~T;
+                    const uint32_t zloc = compress(ht.z & T, T);
+                    dt.zu = table ? compress(zloc, Uloc) : zloc;
+                    plan.terms.push_back(dt);
+                }
+                dg.term_end = (uint32_t)plan.terms.size();
+                plan.groups.push_back(dg);
+            }
         }
         if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
         dp.group_end = (uint32_t)plan.groups.size();

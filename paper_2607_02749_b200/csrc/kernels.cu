@@ -39,13 +39,17 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
     const int k = sb->k, n_runs = sb->n_runs;
     const uint64_t xbase = tile_base(blockIdx.x, sb->runs, n_runs);
     const bool zero = sb->source_zero != 0;
+    constexpr int NLD = (1 << R) / (16 / (int)sizeof(cx<T>));   // 16-byte vectors per thread
+    uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
+    if (tid < NLD) hi[tid] = scatter_runs(tid * nthr * (16 / (uint32_t)sizeof(cx<T>)), sb->runs, n_runs);
     if (zero && xbase != 0) {   // |0...0> has no weight in this tile and gates act inside tiles: stays zero
         tile_zero_store<T>(state, xbase, sb->runs, n_runs, k, tid, nthr);
         return;
     }
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
-    else tile_load<T>(tile, state, xbase, sb->runs, n_runs, k, tid, nthr);
+    __syncthreads();   // hi[] visible
+    if (!zero) tile_load_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
     __syncthreads();
     if (zero) {
         if (tid == 0) tile[0] = cx<T>{T(1), T(0)};
@@ -56,7 +60,7 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
         gate_stage<T, R>(pv, pv.stages[s], tile, tid, xbase, sb->runs, n_runs);
         __syncthreads();
     }
-    tile_store<T>(tile, state, xbase, sb->runs, n_runs, k, tid, nthr);
+    tile_store_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
 }
 
 // ---- expectation pass: read-only sweep, diagonal table + every flip-mask group of the pass --
@@ -71,7 +75,7 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return s;   // valid on thread 0
 }
 
-template <typename T, typename TT>
+template <typename T, typename TT, int L>
 __global__ void __launch_bounds__(256, 2)
 expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
                    const cx<T> *states, uint64_t stride, const TT *__restrict__ table, double *partial,
@@ -80,20 +84,25 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ double red[32];
     DPass *sp = reinterpret_cast<DPass *>(smem);
-    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;   // nthr = 2^(k-1-L)
     {
         const uint32_t *src = reinterpret_cast<const uint32_t *>(passes + pi);
         uint32_t *dst = reinterpret_cast<uint32_t *>(sp);
         for (uint32_t i = tid; i < sizeof(DPass) / 4; i += nthr) dst[i] = src[i];
     }
     __syncthreads();
+    constexpr int V = 16 / (int)sizeof(cx<T>);
+    constexpr int NLD = (2 << L) / V;
+    uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
     cx<T> *tab = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);
     cx<T> *tile = tab + EXPECT_TAB_CAP;
     const uint32_t b = blockIdx.y;
     const cx<T> *state = states + (uint64_t)b * stride;
     const int k = sp->k, n_runs = sp->n_runs;
     const uint64_t xbase = tile_base(blockIdx.x, sp->runs, n_runs);
-    double acc = expect_load<T, TT>(tile, state, table, sp->with_diag != 0, xbase, sp->runs, n_runs, k, tid, nthr);
+    if (tid < NLD) hi[tid] = scatter_runs(tid * nthr * V, sp->runs, n_runs);
+    __syncthreads();
+    double acc = expect_load_u<T, TT, NLD>(tile, state, table, sp->with_diag != 0, xbase, sp->runs, n_runs, tid, nthr, hi);
     __syncthreads();
     uint32_t g = sp->group_begin;
     const uint32_t gend = sp->group_end;
@@ -109,7 +118,8 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {
             const DGroup dg = groups[gi];
-            acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
+            if (dg.direct) acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
+            else acc += group_accumulate_fast<T, L>(dg, tile, tab, tid);
         }
         __syncthreads();
         g = ge + 1;
@@ -193,8 +203,14 @@ int kernels_init(void)
     e |= set_smem(gate_block_kernel<double, 3, 256>, big);
     e |= set_smem(gate_block_kernel<double, 3, 512>, big);
     e |= set_smem(gate_block_kernel<double, 5, 256>, big);
-    e |= set_smem(expect_pass_kernel<float, float>, big);
-    e |= set_smem(expect_pass_kernel<double, double>, big);
+    e |= set_smem(expect_pass_kernel<float, float, 2>, big);
+    e |= set_smem(expect_pass_kernel<float, float, 3>, big);
+    e |= set_smem(expect_pass_kernel<float, float, 4>, big);
+    e |= set_smem(expect_pass_kernel<float, float, 5>, big);
+    e |= set_smem(expect_pass_kernel<double, double, 2>, big);
+    e |= set_smem(expect_pass_kernel<double, double, 3>, big);
+    e |= set_smem(expect_pass_kernel<double, double, 4>, big);
+    e |= set_smem(expect_pass_kernel<double, double, 5>, big);
     e |= set_smem(fwht_pass_kernel<float>, big);
     e |= set_smem(fwht_pass_kernel<double>, big);
     return e;
@@ -232,23 +248,40 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, int bi, int k, uint3
     return (int)cudaErrorInvalidConfiguration;
 }
 
+template <typename T, typename TT>
+static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
+                           const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                           uint32_t slot_off, int batch, cudaStream_t st)
+{
+    dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
+    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + (sizeof(cx<T>) << k);
+    const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
+    const int L = k - 1 - TB;
+#define GV_EXPECT(LL)                                                                                                  \
+    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)states, stride, \
+                                                               (const TT *)table, partial, slots_per_b, slot_off)
+    switch (L) {
+    case 2: GV_EXPECT(2); break;
+    case 3: GV_EXPECT(3); break;
+    case 4: GV_EXPECT(4); break;
+    case 5: GV_EXPECT(5); break;
+    default: return (int)cudaErrorInvalidConfiguration;
+    }
+#undef GV_EXPECT
+    return (int)cudaGetLastError();
+}
+
 int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
                        const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                        uint32_t slot_off, int batch, void *stream, uint64_t *launches)
 {
     cudaStream_t st = (cudaStream_t)stream;
-    dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
-    const size_t esz = prec == 0 ? sizeof(cx<float>) : sizeof(cx<double>);
-    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * esz + (esz << k);
-    const int thr = (1 << k) >= 2048 ? 256 : ((1 << k) / 8 < 32 ? 32 : (1 << k) / 8);
-    if (prec == 0)
-        expect_pass_kernel<float, float><<<grid, thr, smem, st>>>(passes, pi, groups, terms, (const cx<float> *)states, stride,
-                                                                  (const float *)table, partial, slots_per_b, slot_off);
-    else
-        expect_pass_kernel<double, double><<<grid, thr, smem, st>>>(passes, pi, groups, terms, (const cx<double> *)states,
-                                                                    stride, (const double *)table, partial, slots_per_b, slot_off);
     ++*launches;
-    return (int)cudaGetLastError();
+    if (prec == 0)
+        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, states, stride, table, partial, slots_per_b,
+                                             slot_off, batch, st);
+    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, states, stride, table, partial, slots_per_b,
+                                           slot_off, batch, st);
 }
 
 int launch_reduce(const double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches)

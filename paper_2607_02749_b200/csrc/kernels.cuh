@@ -134,6 +134,45 @@ GV_DEV void tile_store(const cx<T> *tile, cx<T> *state, uint64_t xbase, const Ru
     }
 }
 
+// Unrolled variants: every thread moves NLD 16-byte vectors; vector i of thread tid is chunk tid + i*nthr, whose
+// local index splits into disjoint bit fields (tid part | i part), so the global offset is x0 | hi[i] with
+// hi[i] = scatter(i * nthr * V) precomputed once per thread block (shared memory).  All NLD loads are in flight
+// before the first shared-memory store.
+template <typename T, int NLD>
+GV_DEV void tile_load_u(cx<T> *tile, const cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, uint32_t tid,
+                        uint32_t nthr, const uint64_t *hi)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint64_t x0 = xbase | scatter_runs(tid * V, runs, n_runs);
+    const uint32_t p0 = phys<T>(tid * V);
+    vec16<T> v[NLD];
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) v[i] = *reinterpret_cast<const vec16<T> *>(state + (x0 | hi[i]));
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) {
+        const uint32_t p = p0 ^ phys<T>((uint32_t)i * nthr * V);
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v[i].v[e];
+    }
+}
+
+template <typename T, int NLD>
+GV_DEV void tile_store_u(const cx<T> *tile, cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, uint32_t tid,
+                         uint32_t nthr, const uint64_t *hi)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint64_t x0 = xbase | scatter_runs(tid * V, runs, n_runs);
+    const uint32_t p0 = phys<T>(tid * V);
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) {
+        const uint32_t p = p0 ^ phys<T>((uint32_t)i * nthr * V);
+        vec16<T> v;
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) v.v[e] = tile[p ^ e];
+        *reinterpret_cast<vec16<T> *>(state + (x0 | hi[i])) = v;
+    }
+}
+
 template <typename T>
 GV_DEV void tile_zero_store(cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k, uint32_t tid, uint32_t nthr)
 {
@@ -328,6 +367,65 @@ GV_DEV double expect_load(cx<T> *tile, const cx<T> *state, const TT *table, bool
         }
     }
     return acc;
+}
+
+// Unrolled variant of expect_load: NLD 16-byte vectors per thread, all loads in flight (see tile_load_u).
+template <typename T, typename TT, int NLD>
+GV_DEV double expect_load_u(cx<T> *tile, const cx<T> *state, const TT *table, bool with_diag, uint64_t xbase,
+                            const Run *runs, int n_runs, uint32_t tid, uint32_t nthr, const uint64_t *hi)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    struct alignas(V * sizeof(TT)) tvec { TT t[V]; };
+    const uint64_t x0 = xbase | scatter_runs(tid * V, runs, n_runs);
+    const uint32_t p0 = phys<T>(tid * V);
+    vec16<T> v[NLD];
+    tvec tv[NLD];
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) v[i] = *reinterpret_cast<const vec16<T> *>(state + (x0 | hi[i]));
+    if (with_diag) {
+        GV_UNROLL
+        for (int i = 0; i < NLD; ++i) tv[i] = *reinterpret_cast<const tvec *>(table + (x0 | hi[i]));
+    }
+    T acc = T(0);
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) {
+        const uint32_t p = p0 ^ phys<T>((uint32_t)i * nthr * V);
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) {
+            tile[p ^ e] = v[i].v[e];
+            if (with_diag) acc += (v[i].v[e].x * v[i].v[e].x + v[i].v[e].y * v[i].v[e].y) * (T)tv[i].t[e];
+        }
+    }
+    return (double)acc;
+}
+
+// Table-mode group with thread-constant W: the thread's 2^L pairs differ only in the loop bits, which lie outside
+// the table index bits, so  sum_pairs Re(conj(b) W a) = Re(W * sum_pairs conj(b) a).
+template <typename T, int L>
+GV_DEV double group_accumulate_fast(const DGroup &g, const cx<T> *tile, const cx<T> *tab, uint32_t tid)
+{
+    uint32_t j = tid;
+    GV_UNROLL
+    for (int e = 0; e < L + 1; ++e) j = insert_zero(j, g.ex[e]);
+    uint32_t u = 0;
+    for (int r = 0; r < g.n_uruns; ++r)
+        u |= ((j >> g.uruns[r].lpos) & ((1u << g.uruns[r].len) - 1u)) << g.uruns[r].shift;
+    const cx<T> w = tab[g.tab_off + u];
+    const uint32_t pj = phys<T>(j), pm = phys<T>(g.m_loc);
+    uint32_t po[L];
+    GV_UNROLL
+    for (int s = 0; s < L; ++s) po[s] = phys<T>(1u << g.lp[s]);
+    T tr = T(0), ti = T(0);
+    GV_UNROLL
+    for (int i = 0; i < (1 << L); ++i) {
+        uint32_t o = pj;
+        GV_UNROLL
+        for (int s = 0; s < L; ++s) if (i & (1 << s)) o ^= po[s];
+        const cx<T> a = tile[o], b = tile[o ^ pm];
+        tr += b.x * a.x + b.y * a.y;   // conj(b) * a
+        ti += b.x * a.y - b.y * a.x;
+    }
+    return 2.0 * (double)(w.x * tr - w.y * ti);
 }
 
 // W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the

@@ -17,7 +17,7 @@ struct GateLaunch {
 
 constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area
 constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
-constexpr uint32_t HDR_BYTES = 128;         // shared-memory header holding the DBlock / DPass copy
+constexpr uint32_t HDR_BYTES = 384;         // shared-memory header holding the DBlock / DPass copy
 
 // prec: 0 = complex64 (float), 1 = complex128 (double)
 int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches);
