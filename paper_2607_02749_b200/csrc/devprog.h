@@ -64,7 +64,7 @@ struct DTerm {               // one Pauli term of an off-diagonal group, 32 byte
 
 struct URun { uint8_t lpos, len, shift, pad; };   // table index bits: ((j >> lpos) & ((1<<len)-1)) << shift
 
-struct DGroup {              // one flip mask (or a slice of its terms) inside a pass, 52 bytes
+struct DGroup {              // one flip mask (or a slice of its terms) inside a pass, 64 bytes
     uint32_t m_loc;          // flip mask in local tile coordinates (non-zero)
     uint32_t term_begin, term_end;
     uint32_t tab_off;        // offset of the group's W table in the shared-memory table area
@@ -75,6 +75,10 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
     uint8_t last_in_batch;   // 1: tables of groups up to and including this one are built together
     uint8_t n_ex;            // table mode: entries of ex[] = 1 + loop bits
     uint8_t pad[2];
+    uint32_t dyn_end;        // terms [term_begin, dyn_end) have z bits outside the tile (sign depends on the tile) and
+                             // are added per thread block; terms [dyn_end, term_end) are folded into the static table
+    uint32_t gtab_off;       // offset of the group's static W table in the global table array (= batch base + tab_off)
+    uint32_t batch_entries;  // table entries of the whole batch this group belongs to
     URun uruns[3];
     uint8_t ex[8];           // ascending local bit positions that are NOT thread bits: the pivot and the loop bits
     uint8_t lp[8];           // the loop bits (n_ex - 1 of them): local positions outside the table index bits, so

@@ -49,7 +49,8 @@ struct gvqe_ctx {
     // carved device pointers
     GateLaunch gl{};
     DPass *d_passes = nullptr; DGroup *d_groups = nullptr; DTerm *d_terms = nullptr;
-    uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr;
+    uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr; void *d_wstat = nullptr;
+    std::vector<float> wstat_f;
     void *d_table = nullptr; void *d_states = nullptr; void *d_cs = nullptr;
     double *d_params = nullptr, *d_partial = nullptr, *d_E = nullptr;
     uint32_t slots_per_b = 0;
@@ -227,7 +228,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, passes, groups, terms, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, passes, groups, terms, wstat, dz, dc, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -247,6 +248,7 @@ Layout layout_of(const gvqe_ctx *c)
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
     L.groups = cv.take(c->plan.groups.size() * sizeof(DGroup));
     L.terms = cv.take(c->plan.terms.size() * sizeof(DTerm));
+    L.wstat = cv.take(c->plan.wstat.size() / 2 * c->amp_bytes());
     L.dz = cv.take(c->H.diag_z.size() * 8);
     L.dc = cv.take(c->H.diag_c.size() * 8);
     L.table = cv.take(c->tab_bytes() << c->n_store);
@@ -299,6 +301,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.trzs = (const DTrz *)(w + L.trzs); c->gl.tczs = (const uint64_t *)(w + L.tczs);
     c->gl.csidx = (const int32_t *)(w + L.csidx);
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
+    c->d_wstat = w + L.wstat;
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
     c->d_table = w + L.table;
     char *p = w + L.fixed_end;
@@ -313,6 +316,10 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     UP(c->gl.blocks, d.blocks); UP(c->gl.stages, d.stages); UP(c->gl.ops, d.ops); UP(c->gl.segs, d.segs);
     UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx);
     UP(c->d_passes, c->plan.passes); UP(c->d_groups, c->plan.groups); UP(c->d_terms, c->plan.terms);
+    if (c->prec == GVQE_C64) {
+        c->wstat_f.assign(c->plan.wstat.begin(), c->plan.wstat.end());
+        UP(c->d_wstat, c->wstat_f);
+    } else UP(c->d_wstat, c->plan.wstat);
     UP(c->d_diag_z, c->H.diag_z); UP(c->d_diag_c, c->H.diag_c);
 #undef UP
     // diagonal energy table: E(x) = sum_{Z-only k} c_k (-1)^{popcount(x & z_k)} = WHT of the scattered coefficients
@@ -356,7 +363,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     if (c->profiling) cudaEventRecord(e4[1], st);
     const uint32_t tiles = 1u << (c->n_store - c->plan.k);
     for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
-        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_states,
+        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat, c->d_states,
                                 stride, c->d_table, c->d_partial, c->slots_per_b, (uint32_t)pi * tiles, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "expectation pass");
     }

@@ -229,8 +229,13 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                     }
                     dg.n_ex = (uint8_t)ne;
                 }
+                long dyn_end = -1;
+                for (int phase = 0; phase < 2; ++phase)
                 for (int t : slices[sl]) {
                     const HostTerm &ht = H.terms[t];
+                    const bool dyn = (ht.z & ~T) != 0 || !table;
+                    if (dyn != (phase == 0)) continue;   // dynamic terms first
+                    if (phase == 1 && dyn_end < 0) dyn_end = (long)plan.terms.size();
                     DTerm dt; memset(&dt, 0, sizeof dt);
                     static const double pr[4] = {1, 0, -1, 0}, pim[4] = {0, 1, 0, -1};
                     dt.cr = ht.c * pr[ht.ny & 3]; dt.ci = ht.c * pim[ht.ny & 3];
@@ -240,11 +245,39 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                     plan.terms.push_back(dt);
                 }
                 dg.term_end = (uint32_t)plan.terms.size();
+                dg.dyn_end = dyn_end < 0 ? dg.term_end : (uint32_t)dyn_end;
                 plan.groups.push_back(dg);
             }
         }
         if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
         dp.group_end = (uint32_t)plan.groups.size();
+        // static tables, batch by batch, in the layout of the shared-memory table area
+        for (uint32_t g0 = dp.group_begin; g0 < dp.group_end;) {
+            uint32_t g1 = g0;
+            while (!plan.groups[g1].last_in_batch) ++g1;
+            uint32_t entries = 0;
+            for (uint32_t gi = g0; gi <= g1; ++gi)
+                if (!plan.groups[gi].direct) entries = plan.groups[gi].tab_off + (1u << plan.groups[gi].ubits);
+            const size_t base = plan.wstat.size() / 2;
+            plan.wstat.resize(plan.wstat.size() + 2 * (size_t)entries, 0.0);
+            for (uint32_t gi = g0; gi <= g1; ++gi) {
+                DGroup &dg = plan.groups[gi];
+                dg.batch_entries = entries;
+                dg.gtab_off = (uint32_t)base + dg.tab_off;
+                if (dg.direct) { dg.gtab_off = (uint32_t)base; continue; }
+                for (uint32_t u = 0; u < (1u << dg.ubits); ++u) {
+                    double wr = 0.0, wi = 0.0;
+                    for (uint32_t t = dg.dyn_end; t < dg.term_end; ++t) {
+                        const DTerm &tm = plan.terms[t];
+                        const int par = __builtin_popcount(u & tm.zu) & 1;
+                        wr += par ? -tm.cr : tm.cr; wi += par ? -tm.ci : tm.ci;
+                    }
+                    plan.wstat[2 * (base + dg.tab_off + u)] = wr;
+                    plan.wstat[2 * (base + dg.tab_off + u) + 1] = wi;
+                }
+            }
+            g0 = g1 + 1;
+        }
         plan.passes.push_back(dp);
     }
     return true;

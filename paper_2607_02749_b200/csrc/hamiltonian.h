@@ -33,6 +33,7 @@ struct ExpectPlan {
     std::vector<DPass> passes;
     std::vector<DGroup> groups;
     std::vector<DTerm> terms;
+    std::vector<double> wstat;   // static W tables (re, im interleaved), laid out batch by batch like the smem area
 };
 
 // n_store: qubits of the stored state; k/f: tile bits / fixed low tile bits; umax: largest table (bits);

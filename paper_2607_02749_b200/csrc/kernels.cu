@@ -78,8 +78,8 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 template <typename T, typename TT, int L>
 __global__ void __launch_bounds__(256, 2)
 expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
-                   const cx<T> *states, uint64_t stride, const TT *__restrict__ table, double *partial,
-                   uint32_t slots_per_b, uint32_t slot_off)
+                   const cx<T> *__restrict__ wstat, const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
+                   double *partial, uint32_t slots_per_b, uint32_t slot_off)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ double red[32];
@@ -109,11 +109,17 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     while (g < gend) {
         uint32_t ge = g;
         while (!groups[ge].last_in_batch) ++ge;
-        for (uint32_t gi = g; gi <= ge; ++gi) {
+        {   // static tables of the whole batch: one flat coalesced copy
+            const uint32_t ne = groups[g].batch_entries;
+            const cx<T> *src = wstat + (groups[g].gtab_off - groups[g].tab_off);
+            for (uint32_t e = tid; e < ne; e += nthr) tab[e] = src[e];
+        }
+        __syncthreads();
+        for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
             const DGroup dg = groups[gi];
-            if (dg.direct) continue;
+            if (dg.direct || dg.dyn_end == dg.term_begin) continue;
             for (uint32_t u = tid; u < (1u << dg.ubits); u += nthr)
-                tab[dg.tab_off + u] = group_table_entry<T>(dg, terms, xbase, u);
+                tab[dg.tab_off + u] = group_table_entry<T>(dg, terms, xbase, u, tab[dg.tab_off + u]);
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {
@@ -250,7 +256,7 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, int bi, int k, uint3
 
 template <typename T, typename TT>
 static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                           const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                           const void *wstat, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                            uint32_t slot_off, int batch, cudaStream_t st)
 {
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
@@ -258,7 +264,7 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
     const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
     const int L = k - 1 - TB;
 #define GV_EXPECT(LL)                                                                                                  \
-    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)states, stride, \
+    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, (const cx<T> *)states, stride, \
                                                                (const TT *)table, partial, slots_per_b, slot_off)
     switch (L) {
     case 2: GV_EXPECT(2); break;
@@ -272,15 +278,15 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
 }
 
 int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                       const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                       const void *wstat, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                        uint32_t slot_off, int batch, void *stream, uint64_t *launches)
 {
     cudaStream_t st = (cudaStream_t)stream;
     ++*launches;
     if (prec == 0)
-        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, states, stride, table, partial, slots_per_b,
+        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, wstat, states, stride, table, partial, slots_per_b,
                                              slot_off, batch, st);
-    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, states, stride, table, partial, slots_per_b,
+    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, wstat, states, stride, table, partial, slots_per_b,
                                            slot_off, batch, st);
 }
 

@@ -205,16 +205,42 @@ template <typename T, int R, int S> GV_DEV void ry_slot(cx<T> *a, T c, T s)
     }
 }
 
-// CNOT with target slot S: swap the pair when the control bit is set.
-template <typename T, int R, int S> GV_DEV void cx_slot(cx<T> *a, bool fixed, bool fixed_bit, uint32_t ctl_mask)
+// CNOT with target slot S.  Control in register slot C: a fixed permutation of the thread's
+// registers.  Control outside the registers: the whole thread swaps or not (bit of the thread's index).
+template <typename T, int R, int S, int C> GV_DEV void cx_rr(cx<T> *a)
 {
     GV_UNROLL
     for (int r = 0; r < (1 << R); ++r) {
-        if (r & (1 << S)) continue;
-        const bool on = fixed ? fixed_bit : ((r & ctl_mask) != 0);
-        const cx<T> u = a[r], v = a[r | (1 << S)];
-        a[r] = on ? v : u;
-        a[r | (1 << S)] = on ? u : v;
+        if ((r & (1 << S)) || !(r & (1 << C))) continue;
+        const cx<T> u = a[r];
+        a[r] = a[r | (1 << S)];
+        a[r | (1 << S)] = u;
+    }
+}
+
+template <typename T, int R, int S> GV_DEV void cx_rr_c(cx<T> *a, int c)
+{
+    switch (c) {
+    case 0: if constexpr (R > 0 && S != 0) cx_rr<T, R, S, 0>(a); break;
+    case 1: if constexpr (R > 1 && S != 1) cx_rr<T, R, S, 1>(a); break;
+    case 2: if constexpr (R > 2 && S != 2) cx_rr<T, R, S, 2>(a); break;
+    case 3: if constexpr (R > 3 && S != 3) cx_rr<T, R, S, 3>(a); break;
+    case 4: if constexpr (R > 4 && S != 4) cx_rr<T, R, S, 4>(a); break;
+    default: break;
+    }
+}
+
+template <typename T, int R, int S> GV_DEV void cx_slot(cx<T> *a, bool fixed, bool fixed_bit, int ctl_slot)
+{
+    if (!fixed) { cx_rr_c<T, R, S>(a, ctl_slot); return; }
+    if (fixed_bit) {
+        GV_UNROLL
+        for (int r = 0; r < (1 << R); ++r) {
+            if (r & (1 << S)) continue;
+            const cx<T> u = a[r];
+            a[r] = a[r | (1 << S)];
+            a[r | (1 << S)] = u;
+        }
     }
 }
 
@@ -230,7 +256,7 @@ template <typename T, int R> GV_DEV void ry_dispatch(cx<T> *a, int slot, T c, T 
     }
 }
 
-template <typename T, int R> GV_DEV void cx_dispatch(cx<T> *a, int slot, bool fixed, bool fixed_bit, uint32_t ctl_mask)
+template <typename T, int R> GV_DEV void cx_dispatch(cx<T> *a, int slot, bool fixed, bool fixed_bit, int ctl_mask)
 {
     switch (slot) {
     case 0: cx_slot<T, R, 0>(a, fixed, fixed_bit, ctl_mask); break;
@@ -328,7 +354,7 @@ GV_DEV void gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
         } else if (o.kind == MOP_CX) {
             const bool fixed = (o.c == CTL_FIXED);
             const bool fb = fixed ? (((x >> o.b) & 1ull) != 0) : false;
-            cx_dispatch<T, R>(a, o.a, fixed, fb, fixed ? 0u : (1u << o.b));
+            cx_dispatch<T, R>(a, o.a, fixed, fb, (int)o.b);
         } else {
             diag_apply<T, R>(a, pv, pv.segs[o.idx], x);
         }
@@ -431,10 +457,10 @@ GV_DEV double group_accumulate_fast(const DGroup &g, const cx<T> *tile, const cx
 // W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the
 // sign from the bits outside the tile).  One entry per call.
 template <typename T>
-GV_DEV cx<T> group_table_entry(const DGroup &g, const DTerm *terms, uint64_t xbase, uint32_t u)
+GV_DEV cx<T> group_table_entry(const DGroup &g, const DTerm *terms, uint64_t xbase, uint32_t u, cx<T> w0)
 {
-    double wr = 0.0, wi = 0.0;
-    for (uint32_t t = g.term_begin; t < g.term_end; ++t) {
+    double wr = (double)w0.x, wi = (double)w0.y;   // static part (terms with no z bit outside the tile)
+    for (uint32_t t = g.term_begin; t < g.dyn_end; ++t) {
         const DTerm tm = terms[t];
         const int par = (gv_popcll(xbase & tm.zout) + gv_popc(u & tm.zu)) & 1;
         wr += par ? -tm.cr : tm.cr;
