@@ -10,14 +10,15 @@
 namespace gv {
 
 constexpr int DEV_MAX_R = 5;
+enum : uint8_t { MOP_RYL = 3 };   // device-only micro-op: RY on every register slot that has one (ryl[slot] >= 0)
 
 // ---- gate engine ------------------------------------------------------------------------------------------
 struct DOp {                 // 8 bytes; one register-level micro-op of a stage
-    uint8_t kind;            // MOP_RY, MOP_CX, MOP_DIAG
+    uint8_t kind;            // MOP_RYL (a layer of RY on distinct register slots) or MOP_DIAG
     uint8_t a;               // RY: register slot; CX: target slot
     uint8_t b;               // CX: control register slot (CTL_REG) or global qubit (CTL_FIXED)
     uint8_t c;               // CX: CTL_REG / CTL_FIXED
-    int32_t idx;             // RY: block-local (cos,sin) index; DIAG: block-local segment index
+    int32_t idx;             // RYL: offset into the block's ryl array (DEV_MAX_R entries); DIAG: segment index
 };
 
 struct DTrz {                // RZ on a qubit that is not a register bit of the stage (thread- or tile-constant)
@@ -36,11 +37,20 @@ struct DSeg {                // one merged diagonal segment (all its RZ and CZ, 
     uint64_t nbr[DEV_MAX_R];            // per slot: global qubits CZ-coupled to it that are not register bits
 };
 
-struct DStage {              // 16 bytes
+struct DStage {              // 28 bytes
     uint8_t regbit[DEV_MAX_R];          // local bit position (inside the tile) of each register slot, ascending
-    uint8_t pad[3];
+    uint8_t has_cx;                     // the stage ends with a CNOT run
     uint16_t op_begin, op_end;          // DOp entries (block-local)
-    uint32_t pad2;
+    uint16_t cx_begin, cx_end;          // DCx entries (block-local): the trailing CNOT run
+    uint16_t postbit[DEV_MAX_R];        // image of the unit vector of each register bit under the CNOT run (linear part)
+    uint16_t pad;
+};
+
+struct DCx {                 // one CNOT of a trailing run, as an update of the LOCAL index: j ^= ctl_bit << tl
+    uint8_t tl;              // target: local bit position
+    uint8_t cl;              // control: local bit position, or 255 when the control qubit is outside the tile
+    uint8_t cq;              // control: global qubit (used when cl == 255: bit of the tile base)
+    uint8_t pad;
 };
 
 struct DBlock {              // one HBM round trip over every statevector in flight
@@ -49,8 +59,8 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint8_t source_zero;     // 1: tile starts as |0...0> restricted to the tile (no global read)
     uint8_t n_stages;
     Run runs[MAX_RUNS];      // local bits [lpos,lpos+len) <-> global qubits [gpos,gpos+len)
-    uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off;   // offsets into the device arrays
-    uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs;
+    uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off, ryl_off, cx_off;   // offsets into the device arrays
+    uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs, n_ryl, n_cx;
     uint32_t smem_prog_bytes;                                         // shared memory the slice needs
 };
 

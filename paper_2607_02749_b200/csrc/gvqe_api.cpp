@@ -228,7 +228,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, passes, groups, terms, wstat, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, passes, groups, terms, wstat, dz, dc, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -245,6 +245,8 @@ Layout layout_of(const gvqe_ctx *c)
     L.trzs = cv.take(d.trzs.size() * sizeof(DTrz));
     L.tczs = cv.take(d.tczs.size() * 8);
     L.csidx = cv.take(d.csidx.size() * 4);
+    L.ryl = cv.take(d.ryl.size() * 2);
+    L.cxs = cv.take(d.cxs.size() * sizeof(DCx));
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
     L.groups = cv.take(c->plan.groups.size() * sizeof(DGroup));
     L.terms = cv.take(c->plan.terms.size() * sizeof(DTerm));
@@ -300,6 +302,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.ops = (const DOp *)(w + L.ops); c->gl.segs = (const DSeg *)(w + L.segs);
     c->gl.trzs = (const DTrz *)(w + L.trzs); c->gl.tczs = (const uint64_t *)(w + L.tczs);
     c->gl.csidx = (const int32_t *)(w + L.csidx);
+    c->gl.ryl = (const int16_t *)(w + L.ryl); c->gl.cxs = (const DCx *)(w + L.cxs);
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
     c->d_wstat = w + L.wstat;
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
@@ -314,7 +317,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     gvqe_status s;
 #define UP(dst, vec) if ((s = upload(c, (void *)(dst), (vec).data(), (vec).size() * sizeof((vec)[0]), st)) != GVQE_OK) return s
     UP(c->gl.blocks, d.blocks); UP(c->gl.stages, d.stages); UP(c->gl.ops, d.ops); UP(c->gl.segs, d.segs);
-    UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx);
+    UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx); UP(c->gl.ryl, d.ryl); UP(c->gl.cxs, d.cxs);
     UP(c->d_passes, c->plan.passes); UP(c->d_groups, c->plan.groups); UP(c->d_terms, c->plan.terms);
     if (c->prec == GVQE_C64) {
         c->wstat_f.assign(c->plan.wstat.begin(), c->plan.wstat.end());

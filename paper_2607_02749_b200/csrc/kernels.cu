@@ -56,8 +56,13 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
         __syncthreads();
     }
     const int ns = sb->n_stages;
+    cx<T> amp[1 << R];
+    uint32_t po[R], pj2 = 0;
     for (int s = 0; s < ns; ++s) {
-        gate_stage<T, R>(pv, pv.stages[s], tile, tid, xbase, sb->runs, n_runs);
+        if (gate_stage<T, R>(pv, pv.stages[s], tile, tid, xbase, sb->runs, n_runs, amp, po, pj2)) {
+            __syncthreads();   // all reads of the stage done before the permuted writes
+            gate_stage_store<T, R>(pv.stages[s], tile, pj2, po, amp);
+        }
         __syncthreads();
     }
     tile_store_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
@@ -183,7 +188,7 @@ template <typename T, int R, int MAXT>
 int gate_launch_t(const GateLaunch &g, int bi, int k, uint32_t smem_prog, int n, void *states, uint64_t stride,
                   const void *cs, int P, int batch, cudaStream_t st)
 {
-    DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx};
+    DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx, g.ryl, g.cxs};
     const size_t smem = HDR_BYTES + smem_prog + ((size_t)sizeof(cx<T>) << k);
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
     gate_block_kernel<T, R, MAXT><<<grid, 1u << (k - R), smem, st>>>(da, bi, (cx<T> *)states, stride, (const cx<T> *)cs, P);

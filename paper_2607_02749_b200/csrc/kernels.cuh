@@ -67,13 +67,13 @@ GV_DEV uint32_t insert_zero(uint32_t i, uint32_t pos) { return ((i >> pos) << (p
 
 struct DevArrays {
     const DBlock *blocks; const DStage *stages; const DOp *ops; const DSeg *segs; const DTrz *trzs;
-    const uint64_t *tczs; const int32_t *csidx;
+    const uint64_t *tczs; const int32_t *csidx; const int16_t *ryl; const DCx *cxs;
 };
 
 GV_DEV uint32_t al16u(uint32_t v) { return (v + 15u) & ~15u; }
 
 template <typename T> struct ProgView {
-    cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz;
+    cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz; DCx *cxs; int16_t *ryl;
     GV_DEV void bind(unsigned char *p, const DBlock &b)
     {
         cs = (cx<T> *)p;        p += al16u(b.n_cs * (uint32_t)sizeof(cx<T>));
@@ -81,7 +81,9 @@ template <typename T> struct ProgView {
         segs = (DSeg *)p;       p += al16u(b.n_segs * (uint32_t)sizeof(DSeg));
         stages = (DStage *)p;   p += al16u(b.n_stages * (uint32_t)sizeof(DStage));
         ops = (DOp *)p;         p += al16u(b.n_ops * (uint32_t)sizeof(DOp));
-        trz = (DTrz *)p;
+        trz = (DTrz *)p;        p += al16u(b.n_trz * (uint32_t)sizeof(DTrz));
+        cxs = (DCx *)p;         p += al16u(b.n_cx * (uint32_t)sizeof(DCx));
+        ryl = (int16_t *)p;
     }
 };
 
@@ -96,6 +98,8 @@ GV_DEV void gate_prologue(ProgView<T> &pv, const DBlock &b, const DevArrays &da,
     for (uint32_t i = tid; i < b.n_stages; i += nthr) pv.stages[i] = da.stages[b.stage_off + i];
     for (uint32_t i = tid; i < b.n_ops; i += nthr) pv.ops[i] = da.ops[b.op_off + i];
     for (uint32_t i = tid; i < b.n_trz; i += nthr) pv.trz[i] = da.trzs[b.trz_off + i];
+    for (uint32_t i = tid; i < b.n_cx; i += nthr) pv.cxs[i] = da.cxs[b.cx_off + i];
+    for (uint32_t i = tid; i < b.n_ryl; i += nthr) pv.ryl[i] = da.ryl[b.ryl_off + i];
 }
 
 // ---- tile <-> global -------------------------------------------------------------------------------------
@@ -205,66 +209,20 @@ template <typename T, int R, int S> GV_DEV void ry_slot(cx<T> *a, T c, T s)
     }
 }
 
-// CNOT with target slot S.  Control in register slot C: a fixed permutation of the thread's
-// registers.  Control outside the registers: the whole thread swaps or not (bit of the thread's index).
-template <typename T, int R, int S, int C> GV_DEV void cx_rr(cx<T> *a)
+// A layer of R_y gates on distinct register slots: slot s is rotated when ryl[s] >= 0 (uniform branch, static slots).
+template <typename T, int R> GV_DEV void ry_layer(cx<T> *a, const int16_t *ryl, const cx<T> *cs)
 {
     GV_UNROLL
-    for (int r = 0; r < (1 << R); ++r) {
-        if ((r & (1 << S)) || !(r & (1 << C))) continue;
-        const cx<T> u = a[r];
-        a[r] = a[r | (1 << S)];
-        a[r | (1 << S)] = u;
-    }
-}
-
-template <typename T, int R, int S> GV_DEV void cx_rr_c(cx<T> *a, int c)
-{
-    switch (c) {
-    case 0: if constexpr (R > 0 && S != 0) cx_rr<T, R, S, 0>(a); break;
-    case 1: if constexpr (R > 1 && S != 1) cx_rr<T, R, S, 1>(a); break;
-    case 2: if constexpr (R > 2 && S != 2) cx_rr<T, R, S, 2>(a); break;
-    case 3: if constexpr (R > 3 && S != 3) cx_rr<T, R, S, 3>(a); break;
-    case 4: if constexpr (R > 4 && S != 4) cx_rr<T, R, S, 4>(a); break;
-    default: break;
-    }
-}
-
-template <typename T, int R, int S> GV_DEV void cx_slot(cx<T> *a, bool fixed, bool fixed_bit, int ctl_slot)
-{
-    if (!fixed) { cx_rr_c<T, R, S>(a, ctl_slot); return; }
-    if (fixed_bit) {
-        GV_UNROLL
-        for (int r = 0; r < (1 << R); ++r) {
-            if (r & (1 << S)) continue;
-            const cx<T> u = a[r];
-            a[r] = a[r | (1 << S)];
-            a[r | (1 << S)] = u;
+    for (int s = 0; s < R; ++s) {
+        const int i = ryl[s];
+        if (i >= 0) {
+            const cx<T> v = cs[i];
+            if (s == 0) ry_slot<T, R, 0>(a, v.x, v.y);
+            if (s == 1) ry_slot<T, R, (R > 1 ? 1 : 0)>(a, v.x, v.y);
+            if (s == 2) ry_slot<T, R, (R > 2 ? 2 : 0)>(a, v.x, v.y);
+            if (s == 3) ry_slot<T, R, (R > 3 ? 3 : 0)>(a, v.x, v.y);
+            if (s == 4) ry_slot<T, R, (R > 4 ? 4 : 0)>(a, v.x, v.y);
         }
-    }
-}
-
-template <typename T, int R> GV_DEV void ry_dispatch(cx<T> *a, int slot, T c, T s)
-{
-    switch (slot) {
-    case 0: ry_slot<T, R, 0>(a, c, s); break;
-    case 1: if constexpr (R > 1) ry_slot<T, R, 1>(a, c, s); break;
-    case 2: if constexpr (R > 2) ry_slot<T, R, 2>(a, c, s); break;
-    case 3: if constexpr (R > 3) ry_slot<T, R, 3>(a, c, s); break;
-    case 4: if constexpr (R > 4) ry_slot<T, R, 4>(a, c, s); break;
-    default: break;
-    }
-}
-
-template <typename T, int R> GV_DEV void cx_dispatch(cx<T> *a, int slot, bool fixed, bool fixed_bit, int ctl_mask)
-{
-    switch (slot) {
-    case 0: cx_slot<T, R, 0>(a, fixed, fixed_bit, ctl_mask); break;
-    case 1: if constexpr (R > 1) cx_slot<T, R, 1>(a, fixed, fixed_bit, ctl_mask); break;
-    case 2: if constexpr (R > 2) cx_slot<T, R, 2>(a, fixed, fixed_bit, ctl_mask); break;
-    case 3: if constexpr (R > 3) cx_slot<T, R, 3>(a, fixed, fixed_bit, ctl_mask); break;
-    case 4: if constexpr (R > 4) cx_slot<T, R, 4>(a, fixed, fixed_bit, ctl_mask); break;
-    default: break;
     }
 }
 
@@ -323,13 +281,14 @@ template <typename T, int R> GV_DEV void diag_apply(cx<T> *a, const ProgView<T> 
 }
 
 // One stage: 2^R amplitudes per thread in registers, all micro-ops of the stage, back to shared memory.
+// Returns true when the stage ends with a CNOT run: the amplitudes are then left in keep[] and must be written by
+// gate_stage_store after a barrier.
 template <typename T, int R>
-GV_DEV void gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uint32_t tid, uint64_t xbase,
-                       const Run *runs, int n_runs)
+GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uint32_t tid, uint64_t xbase,
+                       const Run *runs, int n_runs, cx<T> *keep, uint32_t *po, uint32_t &pj2)
 {
     constexpr int NR = 1 << R;
     uint32_t j = tid;
-    uint32_t po[R];
     GV_UNROLL
     for (int s = 0; s < R; ++s) {
         const uint32_t pos = st.regbit[s];
@@ -337,7 +296,7 @@ GV_DEV void gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
         po[s] = phys<T>(1u << pos);
     }
     const uint32_t pj = phys<T>(j);
-    cx<T> a[NR];
+    cx<T> *a = keep;
     GV_UNROLL
     for (int r = 0; r < NR; ++r) {
         uint32_t o = 0;
@@ -348,23 +307,45 @@ GV_DEV void gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
     const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
     for (uint32_t oi = st.op_begin; oi < st.op_end; ++oi) {
         const DOp o = pv.ops[oi];
-        if (o.kind == MOP_RY) {
-            const cx<T> cs = pv.cs[o.idx];
-            ry_dispatch<T, R>(a, o.a, cs.x, cs.y);
-        } else if (o.kind == MOP_CX) {
-            const bool fixed = (o.c == CTL_FIXED);
-            const bool fb = fixed ? (((x >> o.b) & 1ull) != 0) : false;
-            cx_dispatch<T, R>(a, o.a, fixed, fb, (int)o.b);
-        } else {
-            diag_apply<T, R>(a, pv, pv.segs[o.idx], x);
-        }
+        if (o.kind == MOP_RYL) ry_layer<T, R>(a, pv.ryl + o.idx, pv.cs);
+        else diag_apply<T, R>(a, pv, pv.segs[o.idx], x);
     }
+    if (!st.has_cx) {
+        GV_UNROLL
+        for (int r = 0; r < NR; ++r) {
+            uint32_t o = 0;
+            GV_UNROLL
+            for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
+            tile[pj ^ o] = a[r];
+        }
+        return false;
+    }
+    // Trailing CNOT run: |j> -> |A j ^ c>, A linear over GF(2).  The amplitude of logical index
+    // j_thread ^ j_r is written to  A j_thread ^ c  ^  A j_r : the thread part is updated CNOT by CNOT, the register
+    // part comes from the precomputed images of the register unit vectors.  No register work at all.
+    uint32_t jj = j;
+    for (uint32_t ci = st.cx_begin; ci < st.cx_end; ++ci) {
+        const DCx c = pv.cxs[ci];
+        const uint32_t bit = (c.cl != 255) ? ((jj >> c.cl) & 1u) : (uint32_t)((xbase >> c.cq) & 1ull);
+        jj ^= bit << c.tl;
+    }
+    pj2 = phys<T>(jj);
     GV_UNROLL
-    for (int r = 0; r < NR; ++r) {
+    for (int s = 0; s < R; ++s) po[s] = phys<T>((uint32_t)st.postbit[s]);
+    return true;
+}
+
+// Second half of a stage that ends with a CNOT run; called after a block-wide barrier (every thread has read its
+// amplitudes before any thread overwrites another thread's locations).
+template <typename T, int R>
+GV_DEV void gate_stage_store(const DStage &st, cx<T> *tile, uint32_t pj2, const uint32_t *po, const cx<T> *a)
+{
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
         uint32_t o = 0;
         GV_UNROLL
         for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
-        tile[pj ^ o] = a[r];
+        tile[pj2 ^ o] = a[r];
     }
 }
 

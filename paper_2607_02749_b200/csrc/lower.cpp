@@ -12,11 +12,11 @@ inline uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
 }  // namespace
 
 uint32_t prog_slice_bytes(uint32_t n_stages, uint32_t n_ops, uint32_t n_segs, uint32_t n_trz, uint32_t n_tcz,
-                          uint32_t n_cs, int scs_bytes)
+                          uint32_t n_cs, uint32_t n_ryl, uint32_t n_cx, int scs_bytes)
 {
     return al16(n_cs * (uint32_t)scs_bytes) + al16(n_tcz * 8u) + al16(n_segs * (uint32_t)sizeof(DSeg)) +
            al16(n_stages * (uint32_t)sizeof(DStage)) + al16(n_ops * (uint32_t)sizeof(DOp)) +
-           al16(n_trz * (uint32_t)sizeof(DTrz));
+           al16(n_trz * (uint32_t)sizeof(DTrz)) + al16(n_cx * (uint32_t)sizeof(DCx)) + al16(n_ryl * 2u);
 }
 
 bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &err)
@@ -34,6 +34,12 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
             db.stage_off = (uint32_t)D.stages.size(); db.op_off = (uint32_t)D.ops.size();
             db.seg_off = (uint32_t)D.segs.size(); db.trz_off = (uint32_t)D.trzs.size();
             db.tcz_off = (uint32_t)D.tczs.size(); db.cs_off = (uint32_t)D.csidx.size();
+            db.ryl_off = (uint32_t)D.ryl.size(); db.cx_off = (uint32_t)D.cxs.size();
+            auto lpos_of = [&](int q) -> int {   // local bit position of global qubit q in this block's tile, or 255
+                for (int r = 0; r < B.n_runs; ++r)
+                    if (q >= B.runs[r].gpos && q < B.runs[r].gpos + B.runs[r].len) return B.runs[r].lpos + (q - B.runs[r].gpos);
+                return 255;
+            };
             std::vector<int32_t> cs_local;   // parameter index per local slot (deduplicated)
             auto cs_slot = [&](int32_t param) -> uint32_t {
                 for (size_t i = 0; i < cs_local.size(); ++i) if (cs_local[i] == param) return (uint32_t)i;
@@ -45,6 +51,7 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                 const Stage &S = p.stages[si];
                 // size of this stage's contribution
                 uint32_t add_ops = S.op_end - S.op_begin, add_segs = 0, add_trz = 0, add_tcz = 0, add_cs = 0;
+                const uint32_t add_cx = S.cx_end - S.cx_begin, add_ryl = DEV_MAX_R * add_ops;   // upper bounds
                 for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
                     const MicroOp &m = p.mops[oi];
                     if (m.kind == MOP_RY) ++add_cs;
@@ -58,18 +65,28 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                                                       (uint32_t)(D.segs.size() - db.seg_off) + add_segs,
                                                       (uint32_t)(D.trzs.size() - db.trz_off) + add_trz,
                                                       (uint32_t)(D.tczs.size() - db.tcz_off) + add_tcz,
-                                                      (uint32_t)cs_local.size() + add_cs, scs_bytes);
+                                                      (uint32_t)cs_local.size() + add_cs,
+                                                      (uint32_t)(D.ryl.size() - db.ryl_off) + add_ryl,
+                                                      (uint32_t)(D.cxs.size() - db.cx_off) + add_cx, scs_bytes);
                 if (n_stages > 0 && (tot > SLICE_BUDGET || n_stages >= 250)) break;
                 if (tot > 4 * SLICE_BUDGET) { err = "lower: a single stage exceeds the program budget (internal)"; return false; }
                 // ---- emit the stage
                 DStage ds; memset(&ds, 0, sizeof ds);
                 for (int s = 0; s < p.R; ++s) ds.regbit[s] = S.regbit[s];
                 ds.op_begin = (uint16_t)(D.ops.size() - db.op_off);
+                long open_ryl = -1;   // offset (block-local) of the RY layer being filled, -1 = none
                 for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
                     const MicroOp &m = p.mops[oi];
                     DOp o; o.kind = m.kind; o.a = m.a; o.b = m.b; o.c = m.c; o.idx = -1;
-                    if (m.kind == MOP_RY) o.idx = (int32_t)cs_slot(m.param);
-                    else if (m.kind == MOP_DIAG) {
+                    if (m.kind == MOP_RY) {   // consecutive RYs on distinct slots commute: one layer micro-op
+                        const int16_t slot = (int16_t)cs_slot(m.param);
+                        if (open_ryl >= 0 && D.ryl[db.ryl_off + open_ryl + m.a] < 0) { D.ryl[db.ryl_off + open_ryl + m.a] = slot; continue; }
+                        open_ryl = (long)(D.ryl.size() - db.ryl_off);
+                        for (int s2 = 0; s2 < DEV_MAX_R; ++s2) D.ryl.push_back(-1);
+                        D.ryl[db.ryl_off + open_ryl + m.a] = slot;
+                        o.kind = MOP_RYL; o.idx = (int32_t)open_ryl;
+                    } else if (m.kind == MOP_DIAG) {
+                        open_ryl = -1;
                         const DiagSeg &g = p.segs[m.param];
                         DSeg sg; memset(&sg, 0, sizeof sg);
                         for (int s = 0; s < DEV_MAX_R; ++s) sg.reg_rz[s] = -1;
@@ -101,6 +118,18 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                     D.ops.push_back(o);
                 }
                 ds.op_end = (uint16_t)(D.ops.size() - db.op_off);
+                // trailing CNOT run as an update of the local index; postbit = image of each register unit vector
+                ds.cx_begin = (uint16_t)(D.cxs.size() - db.cx_off);
+                for (int s2 = 0; s2 < p.R; ++s2) ds.postbit[s2] = (uint16_t)(1u << S.regbit[s2]);
+                for (uint32_t ci = S.cx_begin; ci < S.cx_end; ++ci) {
+                    DCx c; c.tl = (uint8_t)lpos_of(p.cxs[ci].tq); c.cl = (uint8_t)lpos_of(p.cxs[ci].cq); c.cq = p.cxs[ci].cq; c.pad = 0;
+                    if (c.tl == 255) { err = "lower: CNOT target outside the tile (internal)"; return false; }
+                    D.cxs.push_back(c);
+                    if (c.cl != 255)
+                        for (int s2 = 0; s2 < p.R; ++s2) ds.postbit[s2] ^= (uint16_t)(((ds.postbit[s2] >> c.cl) & 1u) << c.tl);
+                }
+                ds.cx_end = (uint16_t)(D.cxs.size() - db.cx_off);
+                ds.has_cx = ds.cx_end > ds.cx_begin ? 1 : 0;
                 D.stages.push_back(ds);
                 ++n_stages; ++si;
             }
@@ -110,8 +139,9 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
             db.n_trz = (uint32_t)(D.trzs.size() - db.trz_off);
             db.n_tcz = (uint32_t)(D.tczs.size() - db.tcz_off);
             db.n_cs = (uint32_t)cs_local.size();
+            db.n_ryl = (uint32_t)(D.ryl.size() - db.ryl_off); db.n_cx = (uint32_t)(D.cxs.size() - db.cx_off);
             for (int32_t v : cs_local) D.csidx.push_back(v);
-            db.smem_prog_bytes = prog_slice_bytes(db.n_stages, db.n_ops, db.n_segs, db.n_trz, db.n_tcz, db.n_cs, scs_bytes);
+            db.smem_prog_bytes = prog_slice_bytes(db.n_stages, db.n_ops, db.n_segs, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes);
             if (db.smem_prog_bytes > D.max_smem_prog) D.max_smem_prog = db.smem_prog_bytes;
             if (db.n_ops > 65535 || db.n_trz > 65535 || db.n_tcz > 65535 || db.n_cs > 65535) {
                 err = "lower: block too large (internal)"; return false;

@@ -17,6 +17,8 @@ struct DevProgram {
     std::vector<DTrz> trzs;
     std::vector<uint64_t> tczs;
     std::vector<int32_t> csidx;   // block-local (cos,sin) slot -> parameter index
+    std::vector<int16_t> ryl;     // RY layers: DEV_MAX_R block-local (cos,sin) slots each, -1 = no gate on the slot
+    std::vector<DCx> cxs;         // trailing CNOT runs
     uint32_t max_smem_prog = 0;   // largest per-block program slice (bytes)
 };
 
@@ -25,6 +27,6 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &out, std::string
 
 // Bytes of the shared-memory program slice for given counts (layout used by the kernels, 16-byte aligned parts).
 uint32_t prog_slice_bytes(uint32_t n_stages, uint32_t n_ops, uint32_t n_segs, uint32_t n_trz, uint32_t n_tcz,
-                          uint32_t n_cs, int scs_bytes);
+                          uint32_t n_cs, uint32_t n_ryl, uint32_t n_cx, int scs_bytes);
 
 }  // namespace gv

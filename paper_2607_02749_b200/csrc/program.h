@@ -50,8 +50,11 @@ struct Stage {        // 32 bytes
     uint8_t pad;
     uint32_t op_begin, op_end;  // into the MicroOp array
     uint32_t seg_begin;         // first diagonal segment of this stage (its R-tables are built per stage)
-    uint32_t pad2[2];
+    uint32_t cx_begin, cx_end;  // trailing CNOT run of the stage (into the StageCx array): applied as an index
+                                // permutation when the stage writes its amplitudes back (no register work)
 };
+
+struct StageCx { uint8_t tq, cq; };   // CNOT: target qubit, control qubit (global numbering)
 
 // T as runs of consecutive qubits: local bits [lpos, lpos+len) <-> global qubits [gpos, gpos+len)
 struct Run { uint8_t lpos, gpos, len, pad; };

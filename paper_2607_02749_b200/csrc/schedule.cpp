@@ -123,6 +123,7 @@ struct StageTake {
     std::vector<int> carry;      // diagonal ops taken but not yet flushed
     std::vector<int> rest;       // ops left for later stages (block-list positions)
     int n_nondiag = 0, n_seg = 0;
+    bool has_cx = false;         // the stage ends with a CNOT run (nothing but CNOTs may follow the first one)
 };
 
 // bops: the block's ops in execution order; L: positions (into bops) still to run; carry: pending diagonals.
@@ -130,7 +131,7 @@ struct StageTake {
 void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, const std::vector<int> &carry_in,
                 uint64_t Rset, bool flush_anywhere, StageTake &out)
 {
-    out.items.clear(); out.rest.clear(); out.n_nondiag = 0; out.n_seg = 0;
+    out.items.clear(); out.rest.clear(); out.n_nondiag = 0; out.n_seg = 0; out.has_cx = false;
     std::vector<int> pend = carry_in;
     uint64_t pend_touch = 0;
     for (int p : pend) { const Acts a = acts_of(bops[p]); for (int i = 0; i < a.nq; ++i) pend_touch |= 1ull << a.q[i]; }
@@ -143,9 +144,12 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
         for (int i = 0; i < a.nq; ++i) {
             const uint64_t b = 1ull << a.q[i];
             if (full & b) ok = false;
-            if (!a.diag[i]) { ndq |= b; if ((nd & b) || !(Rset & b)) ok = false; }
+            // RY needs its qubit in a register slot; a CNOT target only has to be a tile bit (block level)
+            if (!a.diag[i]) { ndq |= b; if ((nd & b) || (o.kind == 0 && !(Rset & b))) ok = false; }
         }
         if (ok && !is_diag(o) && (pend_touch & ndq) && !flush_anywhere && out.n_nondiag > 0) ok = false;
+        if (ok && o.kind == 0 && out.has_cx) ok = false;                          // no rotation after the CNOT run began
+        if (ok && o.kind == 3 && out.has_cx && (pend_touch & ndq)) ok = false;    // no diagonal flush inside the run
         // size caps (shared-memory slice of the program): an op that does not fit waits for the next stage
         if (ok && is_diag(o) && (int)pend.size() >= MAX_SEG_OPS) ok = false;
         if (ok && !is_diag(o) && out.n_nondiag >= MAX_STAGE_ND) ok = false;
@@ -162,6 +166,7 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
                 }
                 StageItem it; it.is_seg = false; it.op = pos;
                 out.items.push_back(std::move(it)); ++out.n_nondiag;
+                if (o.kind == 3) out.has_cx = true;
             }
         } else {
             out.rest.push_back(pos);
@@ -199,7 +204,7 @@ void stage_candidates(const std::vector<HostOp> &bops, const std::vector<int> &L
     for (int pos : L) {
         const Acts a = acts_of(bops[pos]);
         for (int i = 0; i < a.nq && cnt < R; ++i)
-            if (!a.diag[i] && !(s >> a.q[i] & 1)) { s |= 1ull << a.q[i]; ++cnt; }
+            if (!a.diag[i] && bops[pos].kind == 0 && !(s >> a.q[i] & 1)) { s |= 1ull << a.q[i]; ++cnt; }
         if (cnt >= R) break;
     }
     for (int p = 0; p < k && cnt < R; ++p) if (!(s >> tq[p] & 1)) { s |= 1ull << tq[p]; ++cnt; }
@@ -304,7 +309,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                     if (score > bscore) { bscore = score; sbest = st; Rset = rs; }
                 }
                 if (bscore < -1e29) { err = "schedule: stage made no progress (internal)"; return false; }
-                if (sbest.rest.empty() && !sbest.carry.empty()) {  // last stage of the block: flush what is pending
+                if (sbest.rest.empty() && !sbest.carry.empty() && !sbest.has_cx) {  // last stage of the block: flush what is pending
                     StageItem s; s.is_seg = true; s.op = -1; s.seg_ops = sbest.carry;
                     sbest.items.push_back(s); sbest.carry.clear();
                 }
@@ -320,6 +325,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
             auto slot_of = [&](int q) -> int { for (int s = 0; s < R; ++s) if (S.regq[s] == q) return s; return 255; };
             S.op_begin = (uint32_t)P.mops.size();
             S.seg_begin = (uint32_t)P.segs.size();
+            S.cx_begin = (uint32_t)P.cxs.size();
             uint32_t nseg = 0;
             for (const StageItem &it : sbest.items) {
                 MicroOp m; memset(&m, 0, sizeof m);
@@ -344,16 +350,12 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                     const HostOp &o = bops[it.op];
                     P.exec_order.push_back(best.taken[it.op]);
                     if (o.kind == 0) { m.kind = MOP_RY; m.a = (uint8_t)slot_of(o.q0); m.param = o.param; }
-                    else {
-                        m.kind = MOP_CX; m.a = (uint8_t)slot_of(o.q0);
-                        const int cs = slot_of(o.q1);
-                        if (cs != 255) { m.b = (uint8_t)cs; m.c = CTL_REG; } else { m.b = (uint8_t)o.q1; m.c = CTL_FIXED; }
-                        m.param = -1;
-                    }
+                    else { P.cxs.push_back(StageCx{(uint8_t)o.q0, (uint8_t)o.q1}); continue; }
                 }
                 P.mops.push_back(m);
             }
             S.op_end = (uint32_t)P.mops.size();
+            S.cx_end = (uint32_t)P.cxs.size();
             S.n_seg = (uint8_t)nseg;
             if (nseg > 255) { err = "schedule: too many diagonal segments in a stage"; return false; }
             max_seg = std::max(max_seg, nseg);
@@ -397,12 +399,14 @@ std::string dump_program(const Program &p)
             for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
                 const MicroOp &m = p.mops[oi];
                 if (m.kind == MOP_RY) snprintf(buf, sizeof buf, " RY(s%d,p%d)", m.a, m.param);
-                else if (m.kind == MOP_CX) snprintf(buf, sizeof buf, " CX(t=s%d,c=%s%d)", m.a, m.c == CTL_REG ? "s" : "q", m.b);
                 else {
                     const DiagSeg &g = p.segs[m.param];
                     snprintf(buf, sizeof buf, " DIAG(#%d rz=%u cz=%u)", m.param, g.rz_end - g.rz_begin, g.cz_end - g.cz_begin);
                 }
                 s += buf;
+            }
+            for (uint32_t ci = S.cx_begin; ci < S.cx_end; ++ci) {
+                snprintf(buf, sizeof buf, " CX(t=q%d,c=q%d)", p.cxs[ci].tq, p.cxs[ci].cq); s += buf;
             }
             s += "\n";
         }

@@ -23,6 +23,7 @@ struct Program {
     std::vector<DiagSeg> segs;
     std::vector<DiagRZ> rzs;
     std::vector<DiagCZ> czs;
+    std::vector<StageCx> cxs;
     // bookkeeping for tests: for every block the ops (indices into the input list) in execution order
     std::vector<std::vector<int>> block_ops;
     // every input op exactly once, in the order the device executes them (stages flattened, segments expanded)
