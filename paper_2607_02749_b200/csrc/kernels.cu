@@ -19,7 +19,7 @@ __global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *_
 
 // ---- fused gate block: one HBM round trip, all stages of the block in shared memory ---------
 template <typename T, int R, int MAXT>
-__global__ void __launch_bounds__(MAXT, (MAXT <= 256 ? 2 : 1))
+__global__ void __launch_bounds__(MAXT, (MAXT <= 256 || R <= 4 ? 2 : 1))
 gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
 {
     extern __shared__ __align__(16) unsigned char smem[];
