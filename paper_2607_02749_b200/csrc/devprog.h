@@ -61,7 +61,7 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     Run runs[MAX_RUNS];      // local bits [lpos,lpos+len) <-> global qubits [gpos,gpos+len)
     uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off, ryl_off, cx_off;   // offsets into the device arrays
     uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs, n_ryl, n_cx;
-    uint32_t smem_prog_bytes;                                         // shared memory the slice needs
+    uint32_t smem_prog_bytes;                                         // shared memory the slice needs (program + phase tables)
 };
 
 // ---- Hamiltonian engine -----------------------------------------------------------------------------------
@@ -89,6 +89,9 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
                              // are added per thread block; terms [dyn_end, term_end) are folded into the static table
     uint32_t gtab_off;       // offset of the group's static W table in the global table array (= batch base + tab_off)
     uint32_t batch_entries;  // table entries of the whole batch this group belongs to
+    uint32_t ex_pack;        // ex[] packed 4 bits each (entry e at bits 4e)
+    uint32_t lp_pack;        // lp[] packed 4 bits each
+    uint64_t urun_pack;      // uruns packed 12 bits each: lpos | len << 4 | shift << 8
     URun uruns[3];
     uint8_t ex[8];           // ascending local bit positions that are NOT thread bits: the pivot and the loop bits
     uint8_t lp[8];           // the loop bits (n_ex - 1 of them): local positions outside the table index bits, so

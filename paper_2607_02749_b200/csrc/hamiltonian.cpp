@@ -228,6 +228,10 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                         if (b != dg.pivot) dg.lp[nlp++] = (uint8_t)b;
                     }
                     dg.n_ex = (uint8_t)ne;
+                    for (int e = 0; e < ne; ++e) dg.ex_pack |= (uint32_t)dg.ex[e] << (4 * e);
+                    for (int e = 0; e < nlp; ++e) dg.lp_pack |= (uint32_t)dg.lp[e] << (4 * e);
+                    for (int r = 0; r < nur; ++r)
+                        dg.urun_pack |= (uint64_t)(dg.uruns[r].lpos | (dg.uruns[r].len << 4) | (dg.uruns[r].shift << 8)) << (12 * r);
                 }
                 long dyn_end = -1;
                 for (int phase = 0; phase < 2; ++phase)

@@ -128,9 +128,14 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {
-            const DGroup dg = groups[gi];
-            if (dg.direct) acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
-            else acc += group_accumulate_fast<T, L>(dg, tile, tab, tid);
+            const DGroup *pg = groups + gi;
+            if (pg->direct) {
+                const DGroup dg = *pg;
+                acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
+            } else {
+                const GroupFast gf{pg->m_loc, pg->tab_off, pg->ex_pack, pg->lp_pack, pg->n_uruns, pg->urun_pack};
+                acc += group_accumulate_fast<T, L>(gf, tile, tab, tid);
+            }
         }
         __syncthreads();
         g = ge + 1;

@@ -425,29 +425,38 @@ GV_DEV double expect_load_u(cx<T> *tile, const cx<T> *state, const TT *table, bo
 
 // Table-mode group with thread-constant W: the thread's 2^L pairs differ only in the loop bits, which lie outside
 // the table index bits, so  sum_pairs Re(conj(b) W a) = Re(W * sum_pairs conj(b) a).
+// Scalars of a table-mode group that the pair loop needs, read once (uniform loads) instead of copying the struct.
+struct GroupFast { uint32_t m_loc, tab_off, ex_pack, lp_pack, n_uruns; uint64_t urun_pack; };
+
 template <typename T, int L>
-GV_DEV double group_accumulate_fast(const DGroup &g, const cx<T> *tile, const cx<T> *tab, uint32_t tid)
+GV_DEV double group_accumulate_fast(const GroupFast g, const cx<T> *tile, const cx<T> *tab, uint32_t tid)
 {
     uint32_t j = tid;
     GV_UNROLL
-    for (int e = 0; e < L + 1; ++e) j = insert_zero(j, g.ex[e]);
+    for (int e = 0; e < L + 1; ++e) j = insert_zero(j, (g.ex_pack >> (4 * e)) & 15u);
     uint32_t u = 0;
-    for (int r = 0; r < g.n_uruns; ++r)
-        u |= ((j >> g.uruns[r].lpos) & ((1u << g.uruns[r].len) - 1u)) << g.uruns[r].shift;
+    for (uint32_t r = 0; r < g.n_uruns; ++r) {
+        const uint32_t f = (uint32_t)(g.urun_pack >> (12 * r));
+        u |= ((j >> (f & 15u)) & ((1u << ((f >> 4) & 15u)) - 1u)) << ((f >> 8) & 15u);
+    }
     const cx<T> w = tab[g.tab_off + u];
     const uint32_t pj = phys<T>(j), pm = phys<T>(g.m_loc);
     uint32_t po[L];
     GV_UNROLL
-    for (int s = 0; s < L; ++s) po[s] = phys<T>(1u << g.lp[s]);
+    for (int s = 0; s < L; ++s) po[s] = phys<T>(1u << ((g.lp_pack >> (4 * s)) & 15u));
+    uint32_t off[1 << L];   // all XOR combinations of the loop-bit offsets (built incrementally)
+    off[0] = pj;
+    GV_UNROLL
+    for (int s = 0; s < L; ++s) {
+        GV_UNROLL
+        for (int e = 0; e < (1 << s); ++e) off[e | (1 << s)] = off[e] ^ po[s];
+    }
     T tr = T(0), ti = T(0);
     GV_UNROLL
     for (int i = 0; i < (1 << L); ++i) {
-        uint32_t o = pj;
-        GV_UNROLL
-        for (int s = 0; s < L; ++s) if (i & (1 << s)) o ^= po[s];
-        const cx<T> a = tile[o], b = tile[o ^ pm];
-        tr += b.x * a.x + b.y * a.y;   // conj(b) * a
-        ti += b.x * a.y - b.y * a.x;
+        const cx<T> a = tile[off[i]], b = tile[off[i] ^ pm];
+        tr = b.x * a.x + tr; tr = b.y * a.y + tr;     // Re conj(b) a
+        ti = b.x * a.y + ti; ti = -b.y * a.x + ti;    // Im conj(b) a
     }
     return 2.0 * (double)(w.x * tr - w.y * ti);
 }
