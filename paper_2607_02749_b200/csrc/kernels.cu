@@ -121,10 +121,11 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
-            const DGroup dg = groups[gi];
-            if (dg.direct || dg.dyn_end == dg.term_begin) continue;
-            for (uint32_t u = tid; u < (1u << dg.ubits); u += nthr)
-                tab[dg.tab_off + u] = group_table_entry<T>(dg, terms, xbase, u, tab[dg.tab_off + u]);
+            const DGroup *pg = groups + gi;
+            const uint32_t tb = pg->term_begin, de = pg->dyn_end, to = pg->tab_off, ne = 1u << pg->ubits;
+            if (pg->direct || de == tb) continue;
+            for (uint32_t u = tid; u < ne; u += nthr)
+                tab[to + u] = group_table_entry<T>(tb, de, terms, xbase, u, tab[to + u]);
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {

@@ -464,10 +464,11 @@ GV_DEV double group_accumulate_fast(const GroupFast g, const cx<T> *tile, const 
 // W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the
 // sign from the bits outside the tile).  One entry per call.
 template <typename T>
-GV_DEV cx<T> group_table_entry(const DGroup &g, const DTerm *terms, uint64_t xbase, uint32_t u, cx<T> w0)
+GV_DEV cx<T> group_table_entry(uint32_t term_begin, uint32_t dyn_end, const DTerm *terms, uint64_t xbase, uint32_t u,
+                               cx<T> w0)
 {
     double wr = (double)w0.x, wi = (double)w0.y;   // static part (terms with no z bit outside the tile)
-    for (uint32_t t = g.term_begin; t < g.dyn_end; ++t) {
+    for (uint32_t t = term_begin; t < dyn_end; ++t) {
         const DTerm tm = terms[t];
         const int par = (gv_popcll(xbase & tm.zout) + gv_popc(u & tm.zu)) & 1;
         wr += par ? -tm.cr : tm.cr;
