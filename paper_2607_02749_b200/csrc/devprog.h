@@ -92,11 +92,20 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
     uint32_t ex_pack;        // ex[] packed 4 bits each (entry e at bits 4e)
     uint32_t lp_pack;        // lp[] packed 4 bits each
     uint64_t urun_pack;      // uruns packed 12 bits each: lpos | len << 4 | shift << 8
+    uint32_t pm_bytes;       // swizzled byte offset of the flip mask: phys(m_loc) * sizeof(amplitude)
+    uint32_t gt_index;       // index of the group's lookup block (GT_WORDS uint32) in the group-table array
     URun uruns[3];
     uint8_t ex[8];           // ascending local bit positions that are NOT thread bits: the pivot and the loop bits
     uint8_t lp[8];           // the loop bits (n_ex - 1 of them): local positions outside the table index bits, so
                              // that W is constant over a thread's pairs
 };
+
+// Per-group lookup block (host-built, tile-independent), GT_WORDS uint32:
+//   [0,16)  low table : thread-index bits 0..3 -> swizzled byte offset of the thread's local index | table index << 20
+//   [16,32) high table: thread-index bits 4..  -> same; the thread's word is low ^ high (both maps are GF(2)-linear)
+//   [32,64) swizzled byte offsets of the 2^L loop-bit combinations
+constexpr int GT_WORDS = 64;
+constexpr int GT_BATCH_MAX = 32;   // groups per table batch (shared-memory copy of their lookup blocks)
 
 struct DPass {               // one read-only sweep over the state
     uint8_t k, n_runs, with_diag, pad;

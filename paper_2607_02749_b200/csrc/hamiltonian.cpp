@@ -111,9 +111,11 @@ bool hamiltonian_from_masks(int n, int M, const uint64_t *xm, const uint64_t *zm
     return finish(H, err);
 }
 
-bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint32_t tab_cap, ExpectPlan &plan,
-                      std::string &err)
+bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint32_t tab_cap, int amp_bytes,
+                      ExpectPlan &plan, std::string &err)
 {
+    const int FB = amp_bytes == 8 ? 4 : 3;   // same fold as phys<T>() in kernels.cuh
+    auto hphys = [FB](uint32_t j) { uint32_t p = j; for (int sh = FB; sh < 16; sh += FB) p ^= (j >> sh) & ((1u << FB) - 1u); return p; };
     plan = ExpectPlan();
     if (k > n) k = n;
     if (f > k) f = k;
@@ -178,6 +180,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
         dp.n_runs = (uint8_t)nr;
         dp.group_begin = (uint32_t)plan.groups.size();
         uint32_t tab_used = 0;
+        int batch_groups = 0;
         const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // log2(threads) of the expectation kernel
         const int L = k - 1 - TB;                                   // loop bits: 2^L pairs per thread and group
         const int umax_eff = umax < TB ? umax : TB;
@@ -208,13 +211,14 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 const bool table = (ubits <= umax_eff) && (nur <= 3) && ((1u << ubits) <= tab_cap);
                 dg.direct = table ? 0 : 1;
                 dg.term_begin = (uint32_t)plan.terms.size();
+                if (batch_groups >= GT_BATCH_MAX || (table && tab_used + (1u << ubits) > tab_cap)) {   // close the batch
+                    if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
+                    tab_used = 0; batch_groups = 0;
+                }
+                ++batch_groups;
                 if (table) {
                     dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)nur;
                     for (int r = 0; r < nur; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
-                    if (tab_used + (1u << ubits) > tab_cap) {   // close the batch before this group
-                        if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
-                        tab_used = 0;
-                    }
                     dg.tab_off = tab_used; tab_used += 1u << ubits;
                     // loop bits: the L highest local bits outside the table index bits and the pivot
                     uint32_t excl = 1u << dg.pivot;
@@ -228,6 +232,28 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                         if (b != dg.pivot) dg.lp[nlp++] = (uint8_t)b;
                     }
                     dg.n_ex = (uint8_t)ne;
+                    {   // lookup block
+                        dg.pm_bytes = hphys(dg.m_loc) * (uint32_t)amp_bytes;
+                        dg.gt_index = (uint32_t)(plan.gtabs.size() / GT_WORDS);
+                        int tpos[16], nt = 0;
+                        for (int b = 0; b < k; ++b) if (!(excl >> b & 1)) tpos[nt++] = b;
+                        auto word_of = [&](uint32_t j) {
+                            uint32_t u = 0;
+                            for (int r = 0; r < nur; ++r) u |= ((j >> ur[r].gpos) & ((1u << ur[r].len) - 1u)) << ur[r].lpos;
+                            return (hphys(j) * (uint32_t)amp_bytes) | (u << 20);
+                        };
+                        for (int half = 0; half < 2; ++half)
+                            for (uint32_t e = 0; e < 16; ++e) {
+                                uint32_t j = 0;
+                                for (int b = 0; b < 4; ++b) { const int tb = 4 * half + b; if (tb < nt && (e >> b & 1)) j |= 1u << tpos[tb]; }
+                                plan.gtabs.push_back(word_of(j));
+                            }
+                        for (uint32_t i = 0; i < 32; ++i) {
+                            uint32_t j = 0;
+                            for (int s2 = 0; s2 < nlp; ++s2) if (i >> s2 & 1) j |= 1u << dg.lp[s2];
+                            plan.gtabs.push_back(hphys(j) * (uint32_t)amp_bytes);
+                        }
+                    }
                     for (int e = 0; e < ne; ++e) dg.ex_pack |= (uint32_t)dg.ex[e] << (4 * e);
                     for (int e = 0; e < nlp; ++e) dg.lp_pack |= (uint32_t)dg.lp[e] << (4 * e);
                     for (int r = 0; r < nur; ++r)

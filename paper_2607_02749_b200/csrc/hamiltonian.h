@@ -33,12 +33,14 @@ struct ExpectPlan {
     std::vector<DPass> passes;
     std::vector<DGroup> groups;
     std::vector<DTerm> terms;
+    std::vector<uint32_t> gtabs; // GT_WORDS words per table-mode group (see devprog.h)
     std::vector<double> wstat;   // static W tables (re, im interleaved), laid out batch by batch like the smem area
 };
 
 // n_store: qubits of the stored state; k/f: tile bits / fixed low tile bits; umax: largest table (bits);
 // tab_cap: complex entries of the shared-memory table area.
-bool plan_expectation(const Hamiltonian &H, int n_store, int k, int f, int umax, uint32_t tab_cap, ExpectPlan &plan,
-                      std::string &err);
+// amp_bytes: 8 (complex64) or 16 (complex128): fixes the shared-memory swizzle and the byte offsets of the lookups.
+bool plan_expectation(const Hamiltonian &H, int n_store, int k, int f, int umax, uint32_t tab_cap, int amp_bytes,
+                      ExpectPlan &plan, std::string &err);
 
 }  // namespace gv

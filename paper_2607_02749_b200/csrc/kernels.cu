@@ -83,7 +83,7 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 template <typename T, typename TT, int L>
 __global__ void __launch_bounds__(256, 2)
 expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
-                   const cx<T> *__restrict__ wstat, const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
+                   const cx<T> *__restrict__ wstat, const uint32_t *__restrict__ gtabs, const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
                    double *partial, uint32_t slots_per_b, uint32_t slot_off)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -100,7 +100,8 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     constexpr int NLD = (2 << L) / V;
     uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
     cx<T> *tab = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);
-    cx<T> *tile = tab + EXPECT_TAB_CAP;
+    uint32_t *gts = reinterpret_cast<uint32_t *>(tab + EXPECT_TAB_CAP);
+    cx<T> *tile = reinterpret_cast<cx<T> *>(gts + GT_BATCH_MAX * GT_WORDS);
     const uint32_t b = blockIdx.y;
     const cx<T> *state = states + (uint64_t)b * stride;
     const int k = sp->k, n_runs = sp->n_runs;
@@ -118,6 +119,11 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
             const uint32_t ne = groups[g].batch_entries;
             const cx<T> *src = wstat + (groups[g].gtab_off - groups[g].tab_off);
             for (uint32_t e = tid; e < ne; e += nthr) tab[e] = src[e];
+            const uint32_t ng = ge - g + 1;   // lookup blocks of the batch's table-mode groups
+            for (uint32_t e = tid; e < ng * GT_WORDS; e += nthr) {
+                const DGroup *pg = groups + g + e / GT_WORDS;
+                if (!pg->direct) gts[e] = gtabs[(uint64_t)pg->gt_index * GT_WORDS + (e % GT_WORDS)];
+            }
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
@@ -134,8 +140,8 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
                 const DGroup dg = *pg;
                 acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
             } else {
-                const GroupFast gf{pg->m_loc, pg->tab_off, pg->ex_pack, pg->lp_pack, pg->n_uruns, pg->urun_pack};
-                acc += group_accumulate_fast<T, L>(gf, tile, tab, tid);
+                acc += group_accumulate_lut<T, L>(gts + (gi - g) * GT_WORDS, pg->pm_bytes, pg->tab_off,
+                                                  reinterpret_cast<const unsigned char *>(tile), tab, tid);
             }
         }
         __syncthreads();
@@ -267,15 +273,15 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, int bi, int k, uint3
 
 template <typename T, typename TT>
 static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                           const void *wstat, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                           const void *wstat, const uint32_t *gtabs, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                            uint32_t slot_off, int batch, cudaStream_t st)
 {
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
-    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + (sizeof(cx<T>) << k);
+    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + (sizeof(cx<T>) << k);
     const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
     const int L = k - 1 - TB;
 #define GV_EXPECT(LL)                                                                                                  \
-    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, (const cx<T> *)states, stride, \
+    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, gtabs, (const cx<T> *)states, stride, \
                                                                (const TT *)table, partial, slots_per_b, slot_off)
     switch (L) {
     case 2: GV_EXPECT(2); break;
@@ -289,15 +295,15 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
 }
 
 int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                       const void *wstat, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                       const void *wstat, const uint32_t *gtabs, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                        uint32_t slot_off, int batch, void *stream, uint64_t *launches)
 {
     cudaStream_t st = (cudaStream_t)stream;
     ++*launches;
     if (prec == 0)
-        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, wstat, states, stride, table, partial, slots_per_b,
+        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, wstat, gtabs, states, stride, table, partial, slots_per_b,
                                              slot_off, batch, st);
-    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, wstat, states, stride, table, partial, slots_per_b,
+    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, wstat, gtabs, states, stride, table, partial, slots_per_b,
                                            slot_off, batch, st);
 }
 

@@ -461,6 +461,27 @@ GV_DEV double group_accumulate_fast(const GroupFast g, const cx<T> *tile, const 
     return 2.0 * (double)(w.x * tr - w.y * ti);
 }
 
+// Same sum with every index taken from the group's host-built lookup block (devprog.h GT_WORDS): two table reads
+// give the thread's swizzled byte offset and its W index, the loop-bit combinations are broadcast reads.
+template <typename T, int L>
+GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32_t tab_off, const unsigned char *tile_bytes,
+                                   const cx<T> *tab, uint32_t tid)
+{
+    const uint32_t w0 = gt[tid & 15u] ^ gt[16u + (tid >> 4)];
+    const uint32_t pjb = w0 & 0xFFFFFu;
+    const cx<T> w = tab[tab_off + (w0 >> 20)];
+    T tr = T(0), ti = T(0);
+    GV_UNROLL
+    for (int i = 0; i < (1 << L); ++i) {
+        const uint32_t ob = pjb ^ gt[32 + i];
+        const cx<T> a = *reinterpret_cast<const cx<T> *>(tile_bytes + ob);
+        const cx<T> b = *reinterpret_cast<const cx<T> *>(tile_bytes + (ob ^ pm_bytes));
+        tr = b.x * a.x + tr; tr = b.y * a.y + tr;     // Re conj(b) a
+        ti = b.x * a.y + ti; ti = -b.y * a.x + ti;    // Im conj(b) a
+    }
+    return 2.0 * (double)(w.x * tr - w.y * ti);
+}
+
 // W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the
 // sign from the bits outside the tile).  One entry per call.
 template <typename T>
