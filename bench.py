@@ -31,6 +31,12 @@ PREC_OF = {1: "c128", 2: "c128", 3: "c64", 4: "c64", 5: "c64", 6: "c128"}
 ROWS_PER_STEP = {1: 141, 2: 73, 3: 64, 4: 8, 5: 1, 6: 1}
 
 
+def rows_for_step(n_rows_total, rows, world, rank, step):
+    """Row indices (into the workload's parameter batch) that `rank` evaluates in step `step`: consecutive blocks of
+    `rows` rows, rank-shifted so that the ranks of one step work on different rows, wrapping around the batch."""
+    return (np.arange(rows) + (step * world + rank) * rows) % n_rows_total
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -168,8 +174,7 @@ def run_ours(args):
     total = args.warmup + args.steps
 
     def step_rows(i):   # each step takes the next `rows` rows of the sweep (rank-shifted), wrapping around
-        idx = (np.arange(rows) + (i * world + rank) * rows) % w.B
-        return w.params[idx]
+        return w.params[rows_for_step(w.B, rows, world, rank, i)]
 
     host_in = [torch.from_numpy(np.ascontiguousarray(step_rows(i))).pin_memory() for i in range(total)]
     host_out = torch.zeros(rows, dtype=torch.float64).pin_memory()
