@@ -220,6 +220,11 @@ def run_ours(args):
     if rank != 0:
         return
     peak, peak_src = peaks()
+    traffic = None   # measured DRAM bytes per gate-block launch from the committed ncu capture (null when none)
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json"))).get(str(cfg), {}).get("gate_block_kernel")
+    except Exception:
+        pass
     gate_gbs = prof["gate_bytes"] / (prof["gate_ms"] * 1e-3) / 1e9 if prof["gate_ms"] > 0 else 0.0
     exp_gbs = prof["expect_bytes"] / (prof["expect_ms"] * 1e-3) / 1e9 if prof["expect_ms"] > 0 else 0.0
     value = rows * world * args.steps / (ms_dev * 1e-3)
@@ -232,7 +237,7 @@ def run_ours(args):
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": rows * w.P * 8, "d2h_bytes_per_step": rows * 8},
         "gpu_launches": int(launches), "clocks": clocks,
         "roofline": {"bound": "hbm", "kernel": "gate_block_kernel", "achieved": gate_gbs, "peak": peak, "unit": "GB/s",
-                     "frac": gate_gbs / peak, "frac_of_8TBs": gate_gbs / 8000.0, "traffic": None, "peak_source": peak_src,
+                     "frac": gate_gbs / peak, "frac_of_8TBs": gate_gbs / 8000.0, "traffic": traffic, "peak_source": peak_src,
                      "launches_per_step": n_gate_blocks,
                      "avg_launch_ms": prof["gate_ms"] / max(prof["gate_launches"], 1),
                      "share_of_step": prof["gate_ms"] / max(prof["gate_ms"] + prof["expect_ms"] + prof["other_ms"], 1e-9)},
