@@ -21,19 +21,27 @@ struct DOp {                 // 8 bytes; one register-level micro-op of a stage
     int32_t idx;             // RYL: offset into the block's ryl array (DEV_MAX_R entries); DIAG: segment index
 };
 
+constexpr int TPH_ENTRIES = 16 + 32;   // thread-phase tables of a segment: [0,16) over thread-index bits 0..3 (and all
+                                       // tile-constant factors), [16,48) over thread-index bits 4..8
+enum : uint8_t { TB_CONST = 254, TB_XREG = 200 };   // DTrz.tb: tile-constant qubit / TB_XREG + s: further RZ on slot s
+enum : int { TCZ_LO = 0, TCZ_HI = 1, TCZ_CROSS = 2, TCZ_CLASS_SHIFT = 62 };   // class of a thread-level CZ pair
+
 struct DTrz {                // RZ on a qubit that is not a register bit of the stage (thread- or tile-constant)
     uint8_t qubit;           // global qubit
-    uint8_t pad;             // 0: thread/tile-constant; s+1: a further RZ on register slot s of the same segment
+    uint8_t tb;              // thread-index bit the qubit maps to in the segment's stage, TB_CONST, or TB_XREG + slot
     uint16_t cs;             // block-local (cos,sin) index
 };
 
 struct DSeg {                // one merged diagonal segment (all its RZ and CZ, Eq. 7 phases and CZ signs)
-    uint16_t trz_begin, trz_end;        // DTrz entries (block-local)
-    uint16_t tcz_begin, tcz_end;        // CZ pairs with no register bit: 64-bit masks with two bits set
+    uint16_t trz_begin, trz_end;        // DTrz entries (block-local); the TB_XREG entries come first
+    uint16_t tcz_begin, tcz_end;        // CZ pairs with no register bit: two qubit bits + class in bits 62-63;
+                                        // the TCZ_CROSS pairs come first
     int16_t reg_rz[DEV_MAX_R];          // per register slot: block-local (cos,sin) index of its RZ, or -1
-    uint16_t pad;
+    uint8_t stage;                      // block-local stage of the segment (fixes the thread-bit layout)
+    uint8_t n_xreg;                     // TB_XREG entries
     uint32_t regreg_neg;                // bit r set: amplitude with register index r changes sign (reg-reg CZ)
-    uint32_t pad2;
+    uint16_t n_cross;                   // TCZ_CROSS pairs
+    uint16_t pad2;
     uint64_t nbr[DEV_MAX_R];            // per slot: global qubits CZ-coupled to it that are not register bits
 };
 
@@ -62,6 +70,7 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off, ryl_off, cx_off;   // offsets into the device arrays
     uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs, n_ryl, n_cx;
     uint32_t smem_prog_bytes;                                         // shared memory the slice needs (program + phase tables)
+    uint32_t tph_off;                                                 // byte offset of the thread-phase tables in the slice (program + phase tables)
 };
 
 // ---- Hamiltonian engine -----------------------------------------------------------------------------------

@@ -48,7 +48,9 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
     }
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
-    __syncthreads();   // hi[] visible
+    __syncthreads();   // hi[] and the program slice visible
+    for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)
+        tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
     if (!zero) tile_load_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
     __syncthreads();
     if (zero) {

@@ -73,9 +73,10 @@ struct DevArrays {
 GV_DEV uint32_t al16u(uint32_t v) { return (v + 15u) & ~15u; }
 
 template <typename T> struct ProgView {
-    cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz; DCx *cxs; int16_t *ryl;
+    cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz; DCx *cxs; int16_t *ryl; cx<T> *tph;
     GV_DEV void bind(unsigned char *p, const DBlock &b)
     {
+        unsigned char *p0 = p;
         cs = (cx<T> *)p;        p += al16u(b.n_cs * (uint32_t)sizeof(cx<T>));
         tcz = (uint64_t *)p;    p += al16u(b.n_tcz * 8u);
         segs = (DSeg *)p;       p += al16u(b.n_segs * (uint32_t)sizeof(DSeg));
@@ -84,6 +85,7 @@ template <typename T> struct ProgView {
         trz = (DTrz *)p;        p += al16u(b.n_trz * (uint32_t)sizeof(DTrz));
         cxs = (DCx *)p;         p += al16u(b.n_cx * (uint32_t)sizeof(DCx));
         ryl = (int16_t *)p;
+        tph = (cx<T> *)(p0 + b.tph_off);
     }
 };
 
@@ -243,13 +245,58 @@ template <typename T, int R> GV_DEV void ry_layer(cx<T> *a, const int16_t *ryl, 
     }
 }
 
-// Merged diagonal segment: every R_z phase (Eq. 7: e^{-i phi/2} on bit 0, e^{+i phi/2} on bit 1) and every CZ sign
-// of the segment as ONE complex factor per amplitude.  The factor of amplitude (thread index x, register index r)
-// splits into a thread part, a table over the low register slots and a table over the high register slots.
-template <typename T, int R> GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint64_t x)
+// Complex multiply a * w; for complex64 with the packed f32x2 pipe: a.x * (w.x, w.y) + a.y * (-w.y, w.x).
+template <typename T> GV_DEV cx<T> cmul_w(cx<T> a, cx<T> w, cx<T> wsw) { (void)wsw; return cmul(a, w); }
+#ifndef GVQE_EMU
+template <> GV_DEV cx<float> cmul_w<float>(cx<float> a, cx<float> w, cx<float> wsw)
+{
+    const float2 r = __ffma2_rn(make_float2(a.y, a.y), make_float2(wsw.x, wsw.y),
+                                __fmul2_rn(make_float2(a.x, a.x), make_float2(w.x, w.y)));
+    return cx<float>{r.x, r.y};
+}
+#endif
+
+// Thread-phase tables of the block's diagonal segments (one entry per call): the factor that is constant over a
+// thread's registers splits into (tile-constant x thread-index bits 0..3) and (thread-index bits 4..).  Built once
+// per thread block in the prologue, so a stage needs two table reads instead of one multiply per RZ and thread.
+template <typename T, int R>
+GV_DEV void tph_build_entry(const ProgView<T> &pv, uint32_t item, uint64_t xbase, const Run *runs, int n_runs, int k)
+{
+    const uint32_t sgi = item / TPH_ENTRIES, e = item % TPH_ENTRIES;
+    const DSeg &sg = pv.segs[sgi];
+    const DStage &st = pv.stages[sg.stage];
+    const bool high = e >= 16;
+    uint32_t j = high ? ((e - 16u) << 4) : e;
+    if (j >> (k - R)) return;                       // no such thread
+    GV_UNROLL
+    for (int s = 0; s < R; ++s) j = insert_zero(j, st.regbit[s]);
+    const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
+    cx<T> ph{T(1), T(0)};
+    for (uint32_t t = sg.trz_begin + sg.n_xreg; t < sg.trz_end; ++t) {
+        const DTrz z = pv.trz[t];
+        const bool mine = high ? (z.tb >= 4 && z.tb < TB_XREG) : (z.tb < 4 || z.tb == TB_CONST);
+        if (!mine) continue;
+        const cx<T> cs = pv.cs[z.cs];
+        const bool bit = (x >> z.qubit) & 1ull;
+        ph = cmul(ph, cx<T>{cs.x, bit ? cs.y : -cs.y});     // Eq. 7: e^{-i phi/2} on bit 0, e^{+i phi/2} on bit 1
+    }
+    uint32_t par = 0;
+    for (uint32_t t = sg.tcz_begin + sg.n_cross; t < sg.tcz_end; ++t) {
+        const uint64_t m = pv.tcz[t];
+        if ((int)(m >> TCZ_CLASS_SHIFT) != (high ? TCZ_HI : TCZ_LO)) continue;
+        const uint64_t mm = m & ((1ull << TCZ_CLASS_SHIFT) - 1ull);
+        par ^= ((x & mm) == mm) ? 1u : 0u;
+    }
+    pv.tph[item] = par ? cneg(ph) : ph;
+}
+
+// Merged diagonal segment: every R_z phase (Eq. 7) and every CZ sign of the segment as ONE complex factor per
+// amplitude = thread factor (two table reads) x table over the low register slots x table over the high slots.
+template <typename T, int R>
+GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint32_t sgi, uint64_t x, uint32_t tid)
 {
     constexpr int RL = R / 2, RH = R - RL;
-    cx<T> ph{T(1), T(0)};
+    cx<T> ph = cmul(pv.tph[sgi * TPH_ENTRIES + (tid & 15u)], pv.tph[sgi * TPH_ENTRIES + 16u + (tid >> 4)]);
     cx<T> F0[R], F1[R];
     GV_UNROLL
     for (int s = 0; s < R; ++s) {
@@ -257,20 +304,18 @@ template <typename T, int R> GV_DEV void diag_apply(cx<T> *a, const ProgView<T> 
         if (i >= 0) { const cx<T> cs = pv.cs[i]; F0[s] = cx<T>{cs.x, -cs.y}; F1[s] = cs; }
         else { F0[s] = cx<T>{T(1), T(0)}; F1[s] = F0[s]; }
     }
-    for (uint32_t e = sg.trz_begin; e < sg.trz_end; ++e) {
+    for (uint32_t e = sg.trz_begin; e < sg.trz_begin + sg.n_xreg; ++e) {   // rare: a further R_z on a register slot
         const DTrz t = pv.trz[e];
         const cx<T> cs = pv.cs[t.cs];
-        if (t.pad == 0) {
-            const bool bit = (x >> t.qubit) & 1ull;
-            ph = cmul(ph, cx<T>{cs.x, bit ? cs.y : -cs.y});
-        } else {   // a further R_z on a register slot that already has one in this segment
-            GV_UNROLL
-            for (int s = 0; s < R; ++s)
-                if (t.pad - 1 == s) { F0[s] = cmul(F0[s], cx<T>{cs.x, -cs.y}); F1[s] = cmul(F1[s], cs); }
-        }
+        GV_UNROLL
+        for (int s = 0; s < R; ++s)
+            if (t.tb - TB_XREG == s) { F0[s] = cmul(F0[s], cx<T>{cs.x, -cs.y}); F1[s] = cmul(F1[s], cs); }
     }
     uint32_t par = 0;
-    for (uint32_t e = sg.tcz_begin; e < sg.tcz_end; ++e) { const uint64_t m = pv.tcz[e]; par ^= ((x & m) == m) ? 1u : 0u; }
+    for (uint32_t e = sg.tcz_begin; e < sg.tcz_begin + sg.n_cross; ++e) {
+        const uint64_t m = pv.tcz[e] & ((1ull << TCZ_CLASS_SHIFT) - 1ull);
+        par ^= ((x & m) == m) ? 1u : 0u;
+    }
     if (par) ph = cneg(ph);
     GV_UNROLL
     for (int s = 0; s < R; ++s)
@@ -288,12 +333,22 @@ template <typename T, int R> GV_DEV void diag_apply(cx<T> *a, const ProgView<T> 
         GV_UNROLL
         for (int e = 0; e < (1 << s); ++e) { thi[e | (1 << s)] = cmul(thi[e], F1[RL + s]); thi[e] = cmul(thi[e], F0[RL + s]); }
     }
+    cx<T> tlosw[1 << RL], thisw[1 << RH];
+    GV_UNROLL
+    for (int e = 0; e < (1 << RL); ++e) tlosw[e] = cx<T>{-tlo[e].y, tlo[e].x};
+    GV_UNROLL
+    for (int e = 0; e < (1 << RH); ++e) thisw[e] = cx<T>{-thi[e].y, thi[e].x};
     const uint32_t neg = sg.regreg_neg;
     GV_UNROLL
     for (int r = 0; r < (1 << R); ++r) {
-        cx<T> w = cmul(tlo[r & ((1 << RL) - 1)], thi[r >> RL]);
-        if ((neg >> r) & 1u) w = cneg(w);
-        a[r] = cmul(a[r], w);
+        cx<T> v = cmul_w<T>(a[r], tlo[r & ((1 << RL) - 1)], tlosw[r & ((1 << RL) - 1)]);
+        v = cmul_w<T>(v, thi[r >> RL], thisw[r >> RL]);
+        a[r] = v;
+    }
+    if (neg) {
+        GV_UNROLL
+        for (int r = 0; r < (1 << R); ++r)
+            if ((neg >> r) & 1u) a[r] = cneg(a[r]);
     }
 }
 
@@ -325,7 +380,7 @@ GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
     for (uint32_t oi = st.op_begin; oi < st.op_end; ++oi) {
         const DOp o = pv.ops[oi];
         if (o.kind == MOP_RYL) ry_layer<T, R>(a, pv.ryl + o.idx, pv.cs);
-        else diag_apply<T, R>(a, pv, pv.segs[o.idx], x);
+        else diag_apply<T, R>(a, pv, pv.segs[o.idx], (uint32_t)o.idx, x, tid);
     }
     if (!st.has_cx) {
         GV_UNROLL

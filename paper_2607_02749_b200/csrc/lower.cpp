@@ -16,7 +16,8 @@ uint32_t prog_slice_bytes(uint32_t n_stages, uint32_t n_ops, uint32_t n_segs, ui
 {
     return al16(n_cs * (uint32_t)scs_bytes) + al16(n_tcz * 8u) + al16(n_segs * (uint32_t)sizeof(DSeg)) +
            al16(n_stages * (uint32_t)sizeof(DStage)) + al16(n_ops * (uint32_t)sizeof(DOp)) +
-           al16(n_trz * (uint32_t)sizeof(DTrz)) + al16(n_cx * (uint32_t)sizeof(DCx)) + al16(n_ryl * 2u);
+           al16(n_trz * (uint32_t)sizeof(DTrz)) + al16(n_cx * (uint32_t)sizeof(DCx)) + al16(n_ryl * 2u) +
+           n_segs * (uint32_t)TPH_ENTRIES * (uint32_t)scs_bytes;
 }
 
 bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &err)
@@ -92,15 +93,31 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                         for (int s = 0; s < DEV_MAX_R; ++s) sg.reg_rz[s] = -1;
                         sg.trz_begin = (uint16_t)(D.trzs.size() - db.trz_off);
                         sg.tcz_begin = (uint16_t)(D.tczs.size() - db.tcz_off);
+                        // thread-bit layout of this stage: local bits that are not register bits, ascending
+                        auto tb_of = [&](int q) -> int {
+                            const int lp = lpos_of(q);
+                            if (lp == 255) return (int)TB_CONST;
+                            int rank = 0;
+                            for (int s2 = 0; s2 < p.R; ++s2) {
+                                if (S.regbit[s2] == lp) return (int)TB_XREG + s2;
+                                if (S.regbit[s2] < lp) ++rank;
+                            }
+                            return lp - rank;
+                        };
+                        std::vector<DTrz> thr_rz, xreg_rz;
                         for (uint32_t r = g.rz_begin; r < g.rz_end; ++r) {
                             const DiagRZ &z = p.rzs[r];
                             const uint32_t slot = cs_slot(z.param);
                             if (z.slot != 255 && sg.reg_rz[z.slot] < 0) sg.reg_rz[z.slot] = (int16_t)slot;
-                            else {   // not a register bit (or a second RZ on the same slot): per-thread factor.
-                                DTrz t; t.qubit = z.qubit; t.pad = (uint8_t)(z.slot != 255 ? z.slot + 1 : 0); t.cs = (uint16_t)slot;
-                                D.trzs.push_back(t);
+                            else {   // not a register bit (or a second RZ on the same slot)
+                                DTrz t; t.qubit = z.qubit; t.tb = (uint8_t)tb_of(z.qubit); t.cs = (uint16_t)slot;
+                                (t.tb >= TB_XREG && t.tb != TB_CONST ? xreg_rz : thr_rz).push_back(t);
                             }
                         }
+                        sg.n_xreg = (uint8_t)xreg_rz.size();
+                        for (const DTrz &t : xreg_rz) D.trzs.push_back(t);
+                        for (const DTrz &t : thr_rz) D.trzs.push_back(t);
+                        std::vector<uint64_t> cross, sameh;
                         for (uint32_t c = g.cz_begin; c < g.cz_end; ++c) {
                             const DiagCZ &z = p.czs[c];
                             if (z.s0 != 255 && z.s1 != 255) {
@@ -108,8 +125,20 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                                 sg.regreg_neg ^= A[z.s0] & A[z.s1];
                             } else if (z.s0 != 255) sg.nbr[z.s0] ^= 1ull << z.q1;
                             else if (z.s1 != 255) sg.nbr[z.s1] ^= 1ull << z.q0;
-                            else D.tczs.push_back((1ull << z.q0) | (1ull << z.q1));
+                            else {
+                                const int t0 = tb_of(z.q0), t1 = tb_of(z.q1);
+                                auto kind = [](int t) { return t == (int)TB_CONST ? 0 : (t < 4 ? 1 : 2); };   // const / low / high
+                                const int k0 = kind(t0), k1 = kind(t1);
+                                const uint64_t m = (1ull << z.q0) | (1ull << z.q1);
+                                if ((k0 == 2 && k1 == 1) || (k0 == 1 && k1 == 2)) cross.push_back(m | ((uint64_t)TCZ_CROSS << TCZ_CLASS_SHIFT));
+                                else if (k0 == 2 || k1 == 2) sameh.push_back(m | ((uint64_t)TCZ_HI << TCZ_CLASS_SHIFT));
+                                else sameh.push_back(m | ((uint64_t)TCZ_LO << TCZ_CLASS_SHIFT));
+                            }
                         }
+                        sg.n_cross = (uint16_t)cross.size();
+                        for (uint64_t m : cross) D.tczs.push_back(m);
+                        for (uint64_t m : sameh) D.tczs.push_back(m);
+                        sg.stage = (uint8_t)n_stages;
                         sg.trz_end = (uint16_t)(D.trzs.size() - db.trz_off);
                         sg.tcz_end = (uint16_t)(D.tczs.size() - db.tcz_off);
                         o.idx = (int32_t)(D.segs.size() - db.seg_off);
@@ -141,6 +170,7 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
             db.n_cs = (uint32_t)cs_local.size();
             db.n_ryl = (uint32_t)(D.ryl.size() - db.ryl_off); db.n_cx = (uint32_t)(D.cxs.size() - db.cx_off);
             for (int32_t v : cs_local) D.csidx.push_back(v);
+            db.tph_off = prog_slice_bytes(db.n_stages, db.n_ops, 0, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes) + ((db.n_segs * (uint32_t)sizeof(DSeg) + 15u) & ~15u);
             db.smem_prog_bytes = prog_slice_bytes(db.n_stages, db.n_ops, db.n_segs, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes);
             if (db.smem_prog_bytes > D.max_smem_prog) D.max_smem_prog = db.smem_prog_bytes;
             if (db.n_ops > 65535 || db.n_trz > 65535 || db.n_tcz > 65535 || db.n_cs > 65535) {
