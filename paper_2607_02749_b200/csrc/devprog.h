@@ -70,7 +70,10 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t stage_off, op_off, seg_off, trz_off, tcz_off, cs_off, ryl_off, cx_off;   // offsets into the device arrays
     uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs, n_ryl, n_cx;
     uint32_t smem_prog_bytes;                                         // shared memory the slice needs (program + phase tables)
-    uint32_t tph_off;                                                 // byte offset of the thread-phase tables in the slice (program + phase tables)
+    uint32_t tph_off;                                                 // byte offset of the thread-phase tables in the slice
+    uint32_t pad3;
+    uint64_t hi[16];         // global offsets of the 16-byte vectors a thread moves: hi[i] = scatter(i * threads * V)
+    uint32_t hip[16];        // their swizzled shared-memory element offsets: phys(i * threads * V) (program + phase tables)
 };
 
 // ---- Hamiltonian engine -----------------------------------------------------------------------------------
@@ -121,6 +124,7 @@ struct DPass {               // one read-only sweep over the state
     Run runs[MAX_RUNS];
     uint32_t group_begin, group_end;
     uint32_t pad2[2];
+    uint64_t hi[64];         // as DBlock::hi for the expectation kernel's thread count
 };
 
 }  // namespace gv

@@ -361,7 +361,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->profiling) cudaEventRecord(e4[0], st);
     for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
-        ke = launch_gate_block(c->prec, c->R, c->gl, (int)bi, c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
+        ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[bi], c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
                                c->n_store, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "gate block");
     }

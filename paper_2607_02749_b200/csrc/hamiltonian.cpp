@@ -178,6 +178,16 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
         const int nr = runs_of(T, dp.runs, MAX_RUNS);
         if (nr > MAX_RUNS) { err = "hamiltonian: too many tile runs (internal)"; return false; }
         dp.n_runs = (uint8_t)nr;
+        {   // vector offsets of the tile load (kernels.cuh expect_load_u)
+            const int TBh = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);
+            const uint32_t V = 16u / (uint32_t)amp_bytes, nthr = 1u << TBh, nld = (1u << k) / V / nthr;
+            for (uint32_t i = 0; i < nld && i < 64; ++i) {
+                const uint32_t j = i * nthr * V;
+                uint64_t x = 0;
+                for (int r = 0; r < nr; ++r) x |= (uint64_t)((j >> dp.runs[r].lpos) & ((1u << dp.runs[r].len) - 1u)) << dp.runs[r].gpos;
+                dp.hi[i] = x;
+            }
+        }
         dp.group_begin = (uint32_t)plan.groups.size();
         uint32_t tab_used = 0;
         int batch_groups = 0;

@@ -20,17 +20,12 @@ __global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *_
 // ---- fused gate block: one HBM round trip, all stages of the block in shared memory ---------
 template <typename T, int R, int MAXT>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 || R <= 4 ? 2 : 1))
-gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
+gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> *states, uint64_t stride,
+                  const cx<T> *cs_table, int P)
 {
     extern __shared__ __align__(16) unsigned char smem[];
-    DBlock *sb = reinterpret_cast<DBlock *>(smem);
+    const DBlock *sb = &blk;   // kernel parameter (constant bank): no load latency before the tile loads start
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
-    {
-        const uint32_t *src = reinterpret_cast<const uint32_t *>(da.blocks + bi);
-        uint32_t *dst = reinterpret_cast<uint32_t *>(sb);
-        for (uint32_t i = tid; i < sizeof(DBlock) / 4; i += nthr) dst[i] = src[i];
-    }
-    __syncthreads();
     ProgView<T> pv;
     pv.bind(smem + HDR_BYTES, *sb);
     cx<T> *tile = reinterpret_cast<cx<T> *>(smem + HDR_BYTES + sb->smem_prog_bytes);
@@ -40,23 +35,26 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
     const uint64_t xbase = tile_base(blockIdx.x, sb->runs, n_runs);
     const bool zero = sb->source_zero != 0;
     constexpr int NLD = (1 << R) / (16 / (int)sizeof(cx<T>));   // 16-byte vectors per thread
-    uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
-    if (tid < NLD) hi[tid] = scatter_runs(tid * nthr * (16 / (uint32_t)sizeof(cx<T>)), sb->runs, n_runs);
+    const uint64_t *hi = sb->hi;
     if (zero && xbase != 0) {   // |0...0> has no weight in this tile and gates act inside tiles: stays zero
         tile_zero_store<T>(state, xbase, sb->runs, n_runs, k, tid, nthr);
         return;
     }
+    // tile loads first (they need nothing but the kernel parameters) so that the program slice is fetched under them
+    vec16<T> ld[NLD];
+    const uint64_t x0 = xbase | scatter_runs(tid * (16 / (uint32_t)sizeof(cx<T>)), sb->runs, n_runs);
+    if (!zero) {
+#pragma unroll
+        for (int i = 0; i < NLD; ++i) ld[i] = *reinterpret_cast<const vec16<T> *>(state + (x0 | hi[i]));
+    }
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
-    __syncthreads();   // hi[] and the program slice visible
+    else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
+    __syncthreads();   // program slice and tile visible
     for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)
         tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
-    if (!zero) tile_load_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
+    if (zero && tid == 0) tile[0] = cx<T>{T(1), T(0)};
     __syncthreads();
-    if (zero) {
-        if (tid == 0) tile[0] = cx<T>{T(1), T(0)};
-        __syncthreads();
-    }
     const int ns = sb->n_stages;
     cx<T> amp[1 << R];
     uint32_t po[R], pj2 = 0;
@@ -67,7 +65,7 @@ gate_block_kernel(DevArrays da, int bi, cx<T> *states, uint64_t stride, const cx
         }
         __syncthreads();
     }
-    tile_store_u<T, NLD>(tile, state, xbase, sb->runs, n_runs, tid, nthr, hi);
+    tile_store_u<T, NLD>(tile, state, x0, tid, hi, sb->hip);
 }
 
 // ---- expectation pass: read-only sweep, diagonal table + every flip-mask group of the pass --
@@ -199,13 +197,13 @@ __global__ void __launch_bounds__(256) fwht_pass_kernel(TT *table, TileDesc td, 
 namespace {
 
 template <typename T, int R, int MAXT>
-int gate_launch_t(const GateLaunch &g, int bi, int k, uint32_t smem_prog, int n, void *states, uint64_t stride,
+int gate_launch_t(const GateLaunch &g, const DBlock &blk, int k, uint32_t smem_prog, int n, void *states, uint64_t stride,
                   const void *cs, int P, int batch, cudaStream_t st)
 {
     DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx, g.ryl, g.cxs};
     const size_t smem = HDR_BYTES + smem_prog + ((size_t)sizeof(cx<T>) << k);
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
-    gate_block_kernel<T, R, MAXT><<<grid, 1u << (k - R), smem, st>>>(da, bi, (cx<T> *)states, stride, (const cx<T> *)cs, P);
+    gate_block_kernel<T, R, MAXT><<<grid, 1u << (k - R), smem, st>>>(da, blk, (cx<T> *)states, stride, (const cx<T> *)cs, P);
     return (int)cudaGetLastError();
 }
 
@@ -252,7 +250,7 @@ int launch_expand_params(int prec, const double *params, void *cs, uint64_t coun
     return (int)cudaGetLastError();
 }
 
-int launch_gate_block(int prec, int R, const GateLaunch &g, int bi, int k, uint32_t smem_prog, int n, void *states,
+int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &bi, int k, uint32_t smem_prog, int n, void *states,
                       uint64_t stride, const void *cs, int P, int batch, void *stream, uint64_t *launches)
 {
     cudaStream_t st = (cudaStream_t)stream;

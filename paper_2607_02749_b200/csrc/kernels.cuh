@@ -162,16 +162,29 @@ GV_DEV void tile_load_u(cx<T> *tile, const cx<T> *state, uint64_t xbase, const R
     }
 }
 
+// Second half of tile_load_u when the loads were issued by the caller: registers -> swizzled shared memory.
 template <typename T, int NLD>
-GV_DEV void tile_store_u(const cx<T> *tile, cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, uint32_t tid,
-                         uint32_t nthr, const uint64_t *hi)
+GV_DEV void tile_commit(cx<T> *tile, const vec16<T> *v, uint32_t tid, const uint32_t *hip)
 {
     constexpr uint32_t V = 16 / sizeof(cx<T>);
-    const uint64_t x0 = xbase | scatter_runs(tid * V, runs, n_runs);
     const uint32_t p0 = phys<T>(tid * V);
     GV_UNROLL
     for (int i = 0; i < NLD; ++i) {
-        const uint32_t p = p0 ^ phys<T>((uint32_t)i * nthr * V);
+        const uint32_t p = p0 ^ hip[i];
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v[i].v[e];
+    }
+}
+
+template <typename T, int NLD>
+GV_DEV void tile_store_u(const cx<T> *tile, cx<T> *state, uint64_t x0, uint32_t tid, const uint64_t *hi,
+                         const uint32_t *hip)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t p0 = phys<T>(tid * V);
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) {
+        const uint32_t p = p0 ^ hip[i];
         vec16<T> v;
         GV_UNROLL
         for (uint32_t e = 0; e < V; ++e) v.v[e] = tile[p ^ e];

@@ -21,7 +21,7 @@ constexpr uint32_t HDR_BYTES = 384;         // shared-memory header holding the 
 
 // prec: 0 = complex64 (float), 1 = complex128 (double)
 int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches);
-int launch_gate_block(int prec, int R, const GateLaunch &g, int block_index, int k, uint32_t smem_prog_bytes, int n,
+int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &block, int k, uint32_t smem_prog_bytes, int n,
                       void *states, uint64_t stride_amps, const void *cs, int P, int batch, void *stream,
                       uint64_t *launches);
 int launch_expect_pass(int prec, const DPass *passes, int pass_index, int k, int n, const DGroup *groups,

@@ -163,6 +163,19 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                 ++n_stages; ++si;
             }
             db.n_stages = (uint8_t)n_stages;
+            {   // vector offsets of the tile load/store (kernels.cuh tile_load_u)
+                const uint32_t V = 16u / (uint32_t)scs_bytes, nthr = 1u << (B.k - p.R), nld = (1u << p.R) / V;
+                for (uint32_t i = 0; i < nld && i < 16; ++i) {
+                    const uint32_t j = i * nthr * V;
+                    uint64_t x = 0;
+                    for (int r = 0; r < B.n_runs; ++r) x |= (uint64_t)((j >> B.runs[r].lpos) & ((1u << B.runs[r].len) - 1u)) << B.runs[r].gpos;
+                    db.hi[i] = x;
+                    const int FB = scs_bytes == 8 ? 4 : 3;   // phys<T>() of kernels.cuh
+                    uint32_t ph = j;
+                    for (int sh = FB; sh < 16; sh += FB) ph ^= (j >> sh) & ((1u << FB) - 1u);
+                    db.hip[i] = ph;
+                }
+            }
             db.n_ops = (uint32_t)(D.ops.size() - db.op_off);
             db.n_segs = (uint32_t)(D.segs.size() - db.seg_off);
             db.n_trz = (uint32_t)(D.trzs.size() - db.trz_off);
