@@ -45,13 +45,17 @@ struct DSeg {                // one merged diagonal segment (all its RZ and CZ, 
     uint64_t nbr[DEV_MAX_R];            // per slot: global qubits CZ-coupled to it that are not register bits
 };
 
-struct DStage {              // 28 bytes
+constexpr int SLUT_ENTRIES = 16 + 32;   // per-stage thread lookup: [0,16) thread-index bits 0..3, [16,48) bits 4..8
+
+struct DStage {              // 68 bytes
     uint8_t regbit[DEV_MAX_R];          // local bit position (inside the tile) of each register slot, ascending
     uint8_t has_cx;                     // the stage ends with a CNOT run
     uint16_t op_begin, op_end;          // DOp entries (block-local)
     uint16_t cx_begin, cx_end;          // DCx entries (block-local): the trailing CNOT run
     uint16_t postbit[DEV_MAX_R];        // image of the unit vector of each register bit under the CNOT run (linear part)
     uint16_t pad;
+    uint32_t po_bytes[DEV_MAX_R];       // swizzled BYTE offset of each register bit: phys(1 << regbit) * sizeof(amplitude)
+    uint32_t post_bytes[DEV_MAX_R];     // the same for postbit (write-back of a stage with a CNOT run)
 };
 
 struct DCx {                 // one CNOT of a trailing run, as an update of the LOCAL index: j ^= ctl_bit << tl
@@ -71,6 +75,8 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t n_ops, n_segs, n_trz, n_tcz, n_cs, n_ryl, n_cx;
     uint32_t smem_prog_bytes;                                         // shared memory the slice needs (program + phase tables)
     uint32_t tph_off;                                                 // byte offset of the thread-phase tables in the slice
+    uint32_t slut_off;       // byte offset of the per-stage thread lookups (SLUT_ENTRIES x (u32 + u64) per stage)
+    uint32_t off_tcz, off_segs, off_stages, off_ops, off_trz, off_cxs, off_ryl;   // byte offsets of the slice parts (cs = 0)
     uint32_t pad3;
     uint64_t hi[16];         // global offsets of the 16-byte vectors a thread moves: hi[i] = scatter(i * threads * V)
     uint32_t hip[16];        // their swizzled shared-memory element offsets: phys(i * threads * V) (program + phase tables)

@@ -27,8 +27,8 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     const DBlock *sb = &blk;   // kernel parameter (constant bank): no load latency before the tile loads start
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
     ProgView<T> pv;
-    pv.bind(smem + HDR_BYTES, *sb);
-    cx<T> *tile = reinterpret_cast<cx<T> *>(smem + HDR_BYTES + sb->smem_prog_bytes);
+    cx<T> *tile = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);   // fixed offset: LDS/STS take it as an immediate
+    pv.bind(smem + HDR_BYTES + ((size_t)sizeof(cx<T>) << sb->k), *sb);
     const uint32_t b = blockIdx.y;
     cx<T> *state = states + (uint64_t)b * stride;
     const int k = sb->k, n_runs = sb->n_runs;
@@ -53,15 +53,17 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     __syncthreads();   // program slice and tile visible
     for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)
         tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
+    for (uint32_t item = tid; item < (uint32_t)sb->n_stages * SLUT_ENTRIES; item += nthr)
+        slut_build_entry<T, R>(pv, item, sb->runs, n_runs, k);
     if (zero && tid == 0) tile[0] = cx<T>{T(1), T(0)};
     __syncthreads();
     const int ns = sb->n_stages;
     cx<T> amp[1 << R];
     uint32_t po[R], pj2 = 0;
     for (int s = 0; s < ns; ++s) {
-        if (gate_stage<T, R>(pv, pv.stages[s], tile, tid, xbase, sb->runs, n_runs, amp, po, pj2)) {
+        if (gate_stage<T, R>(pv, pv.stages[s], (uint32_t)s, reinterpret_cast<unsigned char *>(tile), tid, xbase, amp, po, pj2)) {
             __syncthreads();   // all reads of the stage done before the permuted writes
-            gate_stage_store<T, R>(pv.stages[s], tile, pj2, po, amp);
+            gate_stage_store<T, R>(reinterpret_cast<unsigned char *>(tile), pj2, po, amp);
         }
         __syncthreads();
     }

@@ -74,18 +74,19 @@ GV_DEV uint32_t al16u(uint32_t v) { return (v + 15u) & ~15u; }
 
 template <typename T> struct ProgView {
     cx<T> *cs; uint64_t *tcz; DSeg *segs; DStage *stages; DOp *ops; DTrz *trz; DCx *cxs; int16_t *ryl; cx<T> *tph;
+    unsigned char *slut;   // per stage: SLUT_ENTRIES x u32 (j | swizzled byte offset... see slut_build_entry) then x u64
     GV_DEV void bind(unsigned char *p, const DBlock &b)
     {
-        unsigned char *p0 = p;
-        cs = (cx<T> *)p;        p += al16u(b.n_cs * (uint32_t)sizeof(cx<T>));
-        tcz = (uint64_t *)p;    p += al16u(b.n_tcz * 8u);
-        segs = (DSeg *)p;       p += al16u(b.n_segs * (uint32_t)sizeof(DSeg));
-        stages = (DStage *)p;   p += al16u(b.n_stages * (uint32_t)sizeof(DStage));
-        ops = (DOp *)p;         p += al16u(b.n_ops * (uint32_t)sizeof(DOp));
-        trz = (DTrz *)p;        p += al16u(b.n_trz * (uint32_t)sizeof(DTrz));
-        cxs = (DCx *)p;         p += al16u(b.n_cx * (uint32_t)sizeof(DCx));
-        ryl = (int16_t *)p;
-        tph = (cx<T> *)(p0 + b.tph_off);
+        cs = (cx<T> *)p;
+        tcz = (uint64_t *)(p + b.off_tcz);
+        segs = (DSeg *)(p + b.off_segs);
+        stages = (DStage *)(p + b.off_stages);
+        ops = (DOp *)(p + b.off_ops);
+        trz = (DTrz *)(p + b.off_trz);
+        cxs = (DCx *)(p + b.off_cxs);
+        ryl = (int16_t *)(p + b.off_ryl);
+        tph = (cx<T> *)(p + b.tph_off);
+        slut = p + b.slut_off;
     }
 };
 
@@ -365,31 +366,47 @@ GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint32_t
     }
 }
 
-// One stage: 2^R amplitudes per thread in registers, all micro-ops of the stage, back to shared memory.
-// Returns true when the stage ends with a CNOT run: the amplitudes are then left in keep[] and must be written by
-// gate_stage_store after a barrier.
+// Per-stage thread lookups (one entry per call; built once per thread block): the thread's local index j (register
+// bits zero), its swizzled byte offset and its global index are GF(2)-linear in the thread index, so each is the XOR / OR
+// of a low-bits entry and a high-bits entry.  u32 entry = j | swizzled element offset << 16; u64 entry = scatter(j).
 template <typename T, int R>
-GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uint32_t tid, uint64_t xbase,
-                       const Run *runs, int n_runs, cx<T> *keep, uint32_t *po, uint32_t &pj2)
+GV_DEV void slut_build_entry(const ProgView<T> &pv, uint32_t item, const Run *runs, int n_runs, int k)
+{
+    const uint32_t si = item / SLUT_ENTRIES, e = item % SLUT_ENTRIES;
+    const DStage &st = pv.stages[si];
+    uint32_t j = e >= 16 ? ((e - 16u) << 4) : e;
+    if (j >> (k - R)) return;
+    GV_UNROLL
+    for (int s = 0; s < R; ++s) j = insert_zero(j, st.regbit[s]);
+    uint32_t *w32 = reinterpret_cast<uint32_t *>(pv.slut + (size_t)si * SLUT_ENTRIES * 12u);
+    uint64_t *w64 = reinterpret_cast<uint64_t *>(w32 + SLUT_ENTRIES);
+    w32[e] = j | (phys<T>(j) << 16);
+    w64[e] = scatter_runs(j, runs, n_runs);
+}
+
+// One stage: 2^R amplitudes per thread in registers, all micro-ops of the stage, back to shared memory.
+// Returns true when the stage ends with a CNOT run: the amplitudes then stay in a[] and must be written by
+// gate_stage_store after a barrier.  All shared-memory addressing is in swizzled BYTE offsets (XOR only).
+template <typename T, int R>
+GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, uint32_t si, unsigned char *tile, uint32_t tid,
+                       uint64_t xbase, cx<T> *a, uint32_t *po, uint32_t &pj2)
 {
     constexpr int NR = 1 << R;
-    uint32_t j = tid;
+    const uint32_t *w32 = reinterpret_cast<const uint32_t *>(pv.slut + (size_t)si * SLUT_ENTRIES * 12u);
+    const uint64_t *w64 = reinterpret_cast<const uint64_t *>(w32 + SLUT_ENTRIES);
+    const uint32_t lo = tid & 15u, hi = 16u + (tid >> 4);
+    const uint32_t w = w32[lo] ^ w32[hi];
+    const uint32_t j = w & 0xFFFFu, pjb = (w >> 16) * (uint32_t)sizeof(cx<T>);
+    const uint64_t x = xbase | w64[lo] | w64[hi];
     GV_UNROLL
-    for (int s = 0; s < R; ++s) {
-        const uint32_t pos = st.regbit[s];
-        j = insert_zero(j, pos);
-        po[s] = phys<T>(1u << pos);
-    }
-    const uint32_t pj = phys<T>(j);
-    cx<T> *a = keep;
+    for (int s = 0; s < R; ++s) po[s] = st.po_bytes[s];
     GV_UNROLL
     for (int r = 0; r < NR; ++r) {
-        uint32_t o = 0;
+        uint32_t o = pjb;
         GV_UNROLL
         for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
-        a[r] = tile[pj ^ o];
+        a[r] = *reinterpret_cast<const cx<T> *>(tile + o);
     }
-    const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
     for (uint32_t oi = st.op_begin; oi < st.op_end; ++oi) {
         const DOp o = pv.ops[oi];
         if (o.kind == MOP_RYL) ry_layer<T, R>(a, pv.ryl + o.idx, pv.cs);
@@ -398,10 +415,10 @@ GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
     if (!st.has_cx) {
         GV_UNROLL
         for (int r = 0; r < NR; ++r) {
-            uint32_t o = 0;
+            uint32_t o = pjb;
             GV_UNROLL
             for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
-            tile[pj ^ o] = a[r];
+            *reinterpret_cast<cx<T> *>(tile + o) = a[r];
         }
         return false;
     }
@@ -414,23 +431,23 @@ GV_DEV bool gate_stage(const ProgView<T> &pv, const DStage &st, cx<T> *tile, uin
         const uint32_t bit = (c.cl != 255) ? ((jj >> c.cl) & 1u) : (uint32_t)((xbase >> c.cq) & 1ull);
         jj ^= bit << c.tl;
     }
-    pj2 = phys<T>(jj);
+    pj2 = phys<T>(jj) * (uint32_t)sizeof(cx<T>);
     GV_UNROLL
-    for (int s = 0; s < R; ++s) po[s] = phys<T>((uint32_t)st.postbit[s]);
+    for (int s = 0; s < R; ++s) po[s] = st.post_bytes[s];
     return true;
 }
 
 // Second half of a stage that ends with a CNOT run; called after a block-wide barrier (every thread has read its
 // amplitudes before any thread overwrites another thread's locations).
 template <typename T, int R>
-GV_DEV void gate_stage_store(const DStage &st, cx<T> *tile, uint32_t pj2, const uint32_t *po, const cx<T> *a)
+GV_DEV void gate_stage_store(unsigned char *tile, uint32_t pj2, const uint32_t *po, const cx<T> *a)
 {
     GV_UNROLL
     for (int r = 0; r < (1 << R); ++r) {
-        uint32_t o = 0;
+        uint32_t o = pj2;
         GV_UNROLL
         for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= po[s];
-        tile[pj2 ^ o] = a[r];
+        *reinterpret_cast<cx<T> *>(tile + o) = a[r];
     }
 }
 

@@ -17,7 +17,7 @@ uint32_t prog_slice_bytes(uint32_t n_stages, uint32_t n_ops, uint32_t n_segs, ui
     return al16(n_cs * (uint32_t)scs_bytes) + al16(n_tcz * 8u) + al16(n_segs * (uint32_t)sizeof(DSeg)) +
            al16(n_stages * (uint32_t)sizeof(DStage)) + al16(n_ops * (uint32_t)sizeof(DOp)) +
            al16(n_trz * (uint32_t)sizeof(DTrz)) + al16(n_cx * (uint32_t)sizeof(DCx)) + al16(n_ryl * 2u) +
-           n_segs * (uint32_t)TPH_ENTRIES * (uint32_t)scs_bytes;
+           n_segs * (uint32_t)TPH_ENTRIES * (uint32_t)scs_bytes + n_stages * (uint32_t)SLUT_ENTRIES * 12u;
 }
 
 bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &err)
@@ -159,6 +159,14 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                 }
                 ds.cx_end = (uint16_t)(D.cxs.size() - db.cx_off);
                 ds.has_cx = ds.cx_end > ds.cx_begin ? 1 : 0;
+                {
+                    const int FB = scs_bytes == 8 ? 4 : 3;
+                    auto hphys = [FB](uint32_t j) { uint32_t ph = j; for (int sh = FB; sh < 16; sh += FB) ph ^= (j >> sh) & ((1u << FB) - 1u); return ph; };
+                    for (int s2 = 0; s2 < p.R; ++s2) {
+                        ds.po_bytes[s2] = hphys(1u << S.regbit[s2]) * (uint32_t)scs_bytes;
+                        ds.post_bytes[s2] = hphys(ds.postbit[s2]) * (uint32_t)scs_bytes;
+                    }
+                }
                 D.stages.push_back(ds);
                 ++n_stages; ++si;
             }
@@ -183,7 +191,18 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
             db.n_cs = (uint32_t)cs_local.size();
             db.n_ryl = (uint32_t)(D.ryl.size() - db.ryl_off); db.n_cx = (uint32_t)(D.cxs.size() - db.cx_off);
             for (int32_t v : cs_local) D.csidx.push_back(v);
-            db.tph_off = prog_slice_bytes(db.n_stages, db.n_ops, 0, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes) + ((db.n_segs * (uint32_t)sizeof(DSeg) + 15u) & ~15u);
+            {
+                uint32_t o = al16(db.n_cs * (uint32_t)scs_bytes);
+                db.off_tcz = o; o += al16(db.n_tcz * 8u);
+                db.off_segs = o; o += al16(db.n_segs * (uint32_t)sizeof(DSeg));
+                db.off_stages = o; o += al16(db.n_stages * (uint32_t)sizeof(DStage));
+                db.off_ops = o; o += al16(db.n_ops * (uint32_t)sizeof(DOp));
+                db.off_trz = o; o += al16(db.n_trz * (uint32_t)sizeof(DTrz));
+                db.off_cxs = o; o += al16(db.n_cx * (uint32_t)sizeof(DCx));
+                db.off_ryl = o; o += al16(db.n_ryl * 2u);
+                db.slut_off = o + db.n_segs * (uint32_t)TPH_ENTRIES * (uint32_t)scs_bytes;
+            }
+            db.tph_off = prog_slice_bytes(0, db.n_ops, 0, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes) + ((db.n_segs * (uint32_t)sizeof(DSeg) + 15u) & ~15u) + ((db.n_stages * (uint32_t)sizeof(DStage) + 15u) & ~15u);
             db.smem_prog_bytes = prog_slice_bytes(db.n_stages, db.n_ops, db.n_segs, db.n_trz, db.n_tcz, db.n_cs, db.n_ryl, db.n_cx, scs_bytes);
             if (db.smem_prog_bytes > D.max_smem_prog) D.max_smem_prog = db.smem_prog_bytes;
             if (db.n_ops > 65535 || db.n_trz > 65535 || db.n_tcz > 65535 || db.n_cs > 65535) {
