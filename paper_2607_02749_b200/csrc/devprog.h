@@ -53,7 +53,8 @@ struct DStage {              // 68 bytes
     uint16_t op_begin, op_end;          // DOp entries (block-local)
     uint16_t cx_begin, cx_end;          // DCx entries (block-local): the trailing CNOT run
     uint16_t postbit[DEV_MAX_R];        // image of the unit vector of each register bit under the CNOT run (linear part)
-    uint16_t pad;
+    uint8_t warp_sync_after;            // 1: the next stage's warps read only what the same warp wrote: __syncwarp suffices
+    uint8_t warp_sync_cx;               // 1: the CNOT-run write-back stays inside each warp's own footprint
     uint32_t po_bytes[DEV_MAX_R];       // swizzled BYTE offset of each register bit: phys(1 << regbit) * sizeof(amplitude)
     uint32_t post_bytes[DEV_MAX_R];     // the same for postbit (write-back of a stage with a CNOT run)
 };
@@ -79,7 +80,11 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t off_tcz, off_segs, off_stages, off_ops, off_trz, off_cxs, off_ryl;   // byte offsets of the slice parts (cs = 0)
     uint32_t pad3;
     uint64_t hi[16];         // global offsets of the 16-byte vectors a thread moves: hi[i] = scatter(i * threads * V)
-    uint32_t hip[16];        // their swizzled shared-memory element offsets: phys(i * threads * V) (program + phase tables)
+    uint32_t hip[16];        // their swizzled shared-memory element offsets: phys(i * threads * V)
+    uint32_t lead_cx;        // 1: stage 0 is nothing but a CNOT run; it is applied while the tile is written to shared
+                             // memory after the load (permuted addresses) and skipped in the stage loop
+    uint32_t e1_cx;          // swizzled image of local index 1 under that run (second amplitude of a 16-byte vector)
+    uint32_t hip_cx[16];     // swizzled images of i * threads * V under that run (linear part) (program + phase tables)
 };
 
 // ---- Hamiltonian engine -----------------------------------------------------------------------------------

@@ -49,7 +49,11 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     }
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
-    else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
+    else if (sb->lead_cx) {
+        const DStage *s0 = da.stages + sb->stage_off;   // read from global: the shared-memory copy is not visible yet
+        tile_commit_cx<T, NLD>(tile, ld, tid, xbase, da.cxs + sb->cx_off + s0->cx_begin, (uint32_t)(s0->cx_end - s0->cx_begin),
+                               sb->hip_cx, sb->e1_cx);
+    } else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
     __syncthreads();   // program slice and tile visible
     for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)
         tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
@@ -60,12 +64,12 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     const int ns = sb->n_stages;
     cx<T> amp[1 << R];
     uint32_t po[R], pj2 = 0;
-    for (int s = 0; s < ns; ++s) {
+    for (int s = (int)sb->lead_cx; s < ns; ++s) {
         if (gate_stage<T, R>(pv, pv.stages[s], (uint32_t)s, reinterpret_cast<unsigned char *>(tile), tid, xbase, amp, po, pj2)) {
-            __syncthreads();   // all reads of the stage done before the permuted writes
+            if (pv.stages[s].warp_sync_cx) __syncwarp(); else __syncthreads();   // reads done before the permuted writes
             gate_stage_store<T, R>(reinterpret_cast<unsigned char *>(tile), pj2, po, amp);
         }
-        __syncthreads();
+        if (pv.stages[s].warp_sync_after) __syncwarp(); else __syncthreads();
     }
     tile_store_u<T, NLD>(tile, state, x0, tid, hi, sb->hip);
 }

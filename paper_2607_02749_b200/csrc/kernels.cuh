@@ -177,6 +177,27 @@ GV_DEV void tile_commit(cx<T> *tile, const vec16<T> *v, uint32_t tid, const uint
     }
 }
 
+// tile_commit for a block whose first stage is only a CNOT run: element j goes to the swizzled image of A j ^ c.
+template <typename T, int NLD>
+GV_DEV void tile_commit_cx(cx<T> *tile, const vec16<T> *v, uint32_t tid, uint64_t xbase, const DCx *cxs, uint32_t n_cx,
+                           const uint32_t *hip_cx, uint32_t e1_cx)
+{
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    uint32_t jj = tid * V;
+    for (uint32_t ci = 0; ci < n_cx; ++ci) {
+        const DCx c = cxs[ci];
+        const uint32_t bit = (c.cl != 255) ? ((jj >> c.cl) & 1u) : (uint32_t)((xbase >> c.cq) & 1ull);
+        jj ^= bit << c.tl;
+    }
+    const uint32_t p0 = phys<T>(jj);
+    GV_UNROLL
+    for (int i = 0; i < NLD; ++i) {
+        const uint32_t p = p0 ^ hip_cx[i];
+        GV_UNROLL
+        for (uint32_t e = 0; e < V; ++e) tile[p ^ (e ? e1_cx : 0u)] = v[i].v[e];
+    }
+}
+
 template <typename T, int NLD>
 GV_DEV void tile_store_u(const cx<T> *tile, cx<T> *state, uint64_t x0, uint32_t tid, const uint64_t *hi,
                          const uint32_t *hip)

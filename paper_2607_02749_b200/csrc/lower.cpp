@@ -171,6 +171,43 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                 ++n_stages; ++si;
             }
             db.n_stages = (uint8_t)n_stages;
+            if (n_stages > 1) {   // a leading stage that is only a CNOT run is folded into the tile load
+                const DStage &s0 = D.stages[db.stage_off];
+                if (s0.op_begin == s0.op_end && s0.has_cx && !db.source_zero) {
+                    const int FB = scs_bytes == 8 ? 4 : 3;
+                    auto hphys = [FB](uint32_t j) { uint32_t ph = j; for (int sh = FB; sh < 16; sh += FB) ph ^= (j >> sh) & ((1u << FB) - 1u); return ph; };
+                    auto alin = [&](uint32_t j) {
+                        for (uint32_t ci = s0.cx_begin; ci < s0.cx_end; ++ci) {
+                            const DCx &c = D.cxs[db.cx_off + ci];
+                            if (c.cl != 255) j ^= ((j >> c.cl) & 1u) << c.tl;
+                        }
+                        return j;
+                    };
+                    const uint32_t V = 16u / (uint32_t)scs_bytes, nthr = 1u << (B.k - p.R), nld = (1u << p.R) / V;
+                    db.lead_cx = 1;
+                    db.e1_cx = hphys(alin(1u));
+                    for (uint32_t i = 0; i < nld && i < 16; ++i) db.hip_cx[i] = hphys(alin(i * nthr * V));
+                }
+            }
+            {   // which stage boundaries need only a warp-level barrier: a warp's footprint in the tile is fixed by the
+                // local positions of its warp-index bits = the highest non-register local bits of the stage
+                const int nwb = B.k - p.R - 5;
+                auto warp_bits = [&](const DStage &st) {
+                    uint32_t regs = 0, wb = 0; int cnt = 0;
+                    for (int s2 = 0; s2 < p.R; ++s2) regs |= 1u << st.regbit[s2];
+                    for (int b2 = B.k - 1; b2 >= 0 && cnt < nwb; --b2) if (!(regs >> b2 & 1)) { wb |= 1u << b2; ++cnt; }
+                    return wb;
+                };
+                for (uint32_t si2 = 0; si2 < n_stages; ++si2) {
+                    DStage &st = D.stages[db.stage_off + si2];
+                    const uint32_t wb = warp_bits(st);
+                    bool cx_inside = true;
+                    for (uint32_t ci = st.cx_begin; ci < st.cx_end; ++ci) if (wb >> D.cxs[db.cx_off + ci].tl & 1) cx_inside = false;
+                    st.warp_sync_cx = (uint8_t)(cx_inside ? 1 : 0);
+                    st.warp_sync_after = 0;
+                    if (si2 + 1 < n_stages && cx_inside && warp_bits(D.stages[db.stage_off + si2 + 1]) == wb) st.warp_sync_after = 1;
+                }
+            }
             {   // vector offsets of the tile load/store (kernels.cuh tile_load_u)
                 const uint32_t V = 16u / (uint32_t)scs_bytes, nthr = 1u << (B.k - p.R), nld = (1u << p.R) / V;
                 for (uint32_t i = 0; i < nld && i < 16; ++i) {
