@@ -35,6 +35,8 @@ struct gvqe_ctx {
     std::vector<HostOp> ops;
     Program prog;
     DevProgram dev;
+    Prefix px;               // product-state prefix of the op list (written, not simulated)
+    PrefixDev pxd{};
     bool have_h = false;
     Hamiltonian H;
     ExpectPlan plan;
@@ -95,10 +97,29 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
     if (c->K > c->n_store) c->K = c->n_store;
     if (c->K < c->R + 5 || c->K > 14 || c->F < 1 || c->F >= c->K || c->K - c->R > 9) { delete c; return GVQE_ERR_INVALID_ARG; }
     std::string err;
-    if (!compile_program(c->n_store, c->ops, c->K, c->F, c->R, c->prog, err) ||
+    // Two candidate schedules: everything through the fused blocks (first block write-only), or the product-state
+    // prefix written by its own kernel and the rest through the blocks.  Fewer HBM passes wins (ties: no prefix).
+    if (!compile_program(c->n_store, c->ops, c->K, c->F, c->R, c->prog, err, true) ||
         !lower_program(c->prog, (int)c->amp_bytes(), c->dev, err)) {
         delete c;
         return GVQE_ERR_UNSUPPORTED;
+    }
+    const char *pf = getenv("GVQE_PREFIX");   // "0" = never, "1" = always when there is one, unset = by pass count
+    Prefix px = (pf && pf[0] == '0') || getenv("GVQE_NO_PREFIX") ? Prefix() : find_prefix(c->n_store, c->ops);
+    if (px.n_ops > 0) {
+        Program prog2; DevProgram dev2;
+        const std::vector<HostOp> rest(c->ops.begin() + px.n_ops, c->ops.end());
+        if (compile_program(c->n_store, rest, c->K, c->F, c->R, prog2, err, false) &&
+            lower_program(prog2, (int)c->amp_bytes(), dev2, err)) {
+            const size_t passes_plain = 2 * c->dev.blocks.size() - 1, passes_px = 1 + 2 * dev2.blocks.size();
+            if (passes_px < passes_plain || (pf && pf[0] == '1')) { c->px = px; c->prog = prog2; c->dev = dev2; }
+        }
+    }
+    if (c->px.n_ops > 0) {   // execution order in terms of the caller's op list: prefix first, then the compiled rest
+        std::vector<int> eo;
+        for (int i = 0; i < c->px.n_ops; ++i) eo.push_back(i);
+        for (int e : c->prog.exec_order) eo.push_back(e + c->px.n_ops);
+        c->prog.exec_order.swap(eo);
     }
     *out = c;
     return GVQE_OK;
@@ -228,7 +249,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, passes, groups, terms, wstat, gtabs, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, dz, dc, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -247,6 +268,8 @@ Layout layout_of(const gvqe_ctx *c)
     L.csidx = cv.take(d.csidx.size() * 4);
     L.ryl = cv.take(d.ryl.size() * 2);
     L.cxs = cv.take(d.cxs.size() * sizeof(DCx));
+    L.px_begin = cv.take(c->px.rot_begin.size() * 4); L.px_kind = cv.take(c->px.rot_kind.size());
+    L.px_param = cv.take(c->px.rot_param.size() * 4); L.px_t = cv.take(c->px.cx_t.size()); L.px_c = cv.take(c->px.cx_c.size());
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
     L.groups = cv.take(c->plan.groups.size() * sizeof(DGroup));
     L.terms = cv.take(c->plan.terms.size() * sizeof(DTerm));
@@ -304,6 +327,10 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.trzs = (const DTrz *)(w + L.trzs); c->gl.tczs = (const uint64_t *)(w + L.tczs);
     c->gl.csidx = (const int32_t *)(w + L.csidx);
     c->gl.ryl = (const int16_t *)(w + L.ryl); c->gl.cxs = (const DCx *)(w + L.cxs);
+    c->pxd.rot_begin = (const int32_t *)(w + L.px_begin); c->pxd.rot_kind = (const uint8_t *)(w + L.px_kind);
+    c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
+    c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
+    for (int i = 0; i < 4; ++i) { c->pxd.cz_d[i] = c->px.cz_d[i]; c->pxd.cz_m[i] = c->px.cz_m[i]; }
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
     c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs);
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
@@ -319,6 +346,8 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
 #define UP(dst, vec) if ((s = upload(c, (void *)(dst), (vec).data(), (vec).size() * sizeof((vec)[0]), st)) != GVQE_OK) return s
     UP(c->gl.blocks, d.blocks); UP(c->gl.stages, d.stages); UP(c->gl.ops, d.ops); UP(c->gl.segs, d.segs);
     UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx); UP(c->gl.ryl, d.ryl); UP(c->gl.cxs, d.cxs);
+    UP(c->pxd.rot_begin, c->px.rot_begin); UP(c->pxd.rot_kind, c->px.rot_kind); UP(c->pxd.rot_param, c->px.rot_param);
+    UP(c->pxd.cx_t, c->px.cx_t); UP(c->pxd.cx_c, c->px.cx_c);
     UP(c->d_passes, c->plan.passes); UP(c->d_groups, c->plan.groups); UP(c->d_terms, c->plan.terms);
     if (c->prec == GVQE_C64) {
         c->wstat_f.assign(c->plan.wstat.begin(), c->plan.wstat.end());
@@ -360,6 +389,10 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     int ke = launch_expand_params(c->prec, params_dev, c->d_cs, (uint64_t)nb * c->P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->profiling) cudaEventRecord(e4[0], st);
+    if (c->px.n_ops > 0) {
+        ke = launch_init_product(c->prec, c->pxd, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
+        if (ke) return cuda_fail(c, ke, "product-state init");
+    }
     for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
         ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[bi], c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
                                c->n_store, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
@@ -381,7 +414,8 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
         const double S = (double)(c->amp_bytes() << c->n_store);
         double gb = 0;
         for (const DBlock &b : c->dev.blocks) gb += (b.source_zero ? 1.0 : 2.0) * S * nb;
-        c->prof_acc[1] += (double)c->dev.blocks.size(); c->prof_acc[2] += gb;
+        if (c->px.n_ops > 0) gb += S * nb;   // write-only product-state kernel
+        c->prof_acc[1] += (double)c->dev.blocks.size() + (c->px.n_ops > 0 ? 1.0 : 0.0); c->prof_acc[2] += gb;
         c->prof_acc[4] += (double)c->plan.passes.size();
         c->prof_acc[5] += (double)c->plan.passes.size() * S * nb + (double)(c->tab_bytes() << c->n_store);
         c->prof_acc[7] += 1.0;
@@ -495,7 +529,7 @@ gvqe_status gvqe_get_state(gvqe_ctx *c, int slot, void *host_out)
 gvqe_status gvqe_schedule_info(const gvqe_ctx *c, int32_t *nb, int32_t *np, int32_t *inflight)
 {
     if (!c) return GVQE_ERR_INVALID_ARG;
-    if (nb) *nb = (int32_t)c->dev.blocks.size();
+    if (nb) *nb = (int32_t)c->dev.blocks.size() + (c->px.n_ops > 0 ? 1 : 0);   // + the write-only product-state kernel
     if (np) *np = c->have_h ? (int32_t)c->plan.passes.size() : 0;
     if (inflight) *inflight = c->in_flight;
     return GVQE_OK;
@@ -505,6 +539,11 @@ size_t gvqe_dump_schedule(const gvqe_ctx *c, char *buf, size_t cap)
 {
     if (!c) return 0;
     std::string s = dump_program(c->prog);
+    {
+        char pl[160];
+        snprintf(pl, sizeof pl, "prefix ops=%d rotations=%zu cnots=%zu cz_distances=%d\n", c->px.n_ops, c->px.rot_kind.size(), c->px.cx_t.size(), c->px.n_cz);
+        s += pl;
+    }
     char line[256];
     snprintf(line, sizeof line, "device blocks=%zu max_prog_smem=%u\n", c->dev.blocks.size(), c->dev.max_smem_prog);
     s += line;

@@ -17,6 +17,70 @@ __global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *_
     cs[i] = cx<T>{(T)c, (T)s};
 }
 
+// ---- product-state prefix, write-only --------------------------------------------------------------
+// psi[y] = sign(y) * prod_q f_q[x_q],  x = A^-1 y  (A = the prefix's CNOT run, linear over GF(2); sign = its CZ run),
+// f_q = (rotations of qubit q)|0>.  The product comes from tables over 7-qubit groups; A^-1 y is split into the
+// thread's part, the vector's part and the lane-in-vector part (linearity), so nothing per amplitude depends on
+// the number of CNOTs.  Each thread block writes 2^kk contiguous amplitudes with 16-byte stores.
+__device__ __forceinline__ uint64_t prefix_ainv(const PrefixDev &pd, uint64_t y)
+{
+    for (int i = pd.n_cx - 1; i >= 0; --i) y ^= ((y >> pd.cx_c[i]) & 1ull) << pd.cx_t[i];
+    return y;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256, 2)
+init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
+{
+    __shared__ cx<T> f[40][2];
+    __shared__ cx<T> tab[5][128];
+    __shared__ uint64_t xi[64];
+    constexpr uint32_t V = 16 / sizeof(cx<T>);
+    const uint32_t tid = threadIdx.x, nthr = blockDim.x;
+    const cx<T> *cs = cs_table + (uint64_t)blockIdx.y * P;
+    cx<T> *state = states + (uint64_t)blockIdx.y * stride;
+    const int n = pd.n;
+    if ((int)tid < n) {   // f_q = U_m ... U_1 |0>, Eq. 7
+        cx<T> a{T(1), T(0)}, b{T(0), T(0)};
+        for (int r = pd.rot_begin[tid]; r < pd.rot_begin[tid + 1]; ++r) {
+            const cx<T> v = cs[pd.rot_param[r]];   // (cos, sin) of theta / 2
+            if (pd.rot_kind[r] == 0) {
+                const cx<T> a2{v.x * a.x - v.y * b.x, v.x * a.y - v.y * b.y}, b2{v.y * a.x + v.x * b.x, v.y * a.y + v.x * b.y};
+                a = a2; b = b2;
+            } else { a = cmul(a, cx<T>{v.x, -v.y}); b = cmul(b, v); }
+        }
+        f[tid][0] = a; f[tid][1] = b;
+    }
+    const uint32_t nvec = (1u << pd.kk) / V / nthr;   // vectors per thread
+    if (tid < nvec) xi[tid] = prefix_ainv(pd, (uint64_t)tid * nthr * V);
+    __syncthreads();
+    const int ngrp = (n + 6) / 7;
+    for (uint32_t e = tid; e < (uint32_t)ngrp * 128u; e += nthr) {
+        const uint32_t g = e >> 7, v = e & 127u;
+        cx<T> p{T(1), T(0)};
+        for (int j = 0; j < 7 && (int)(7 * g) + j < n; ++j) p = cmul(p, f[7 * g + j][(v >> j) & 1u]);
+        tab[g][v] = p;
+    }
+    __syncthreads();
+    const uint64_t ybase = ((uint64_t)blockIdx.x << pd.kk) | (uint64_t)(tid * V);
+    const uint64_t xthr = prefix_ainv(pd, ybase);
+    const uint64_t xe1 = prefix_ainv(pd, 1ull);
+    for (uint32_t i = 0; i < nvec; ++i) {
+        vec16<T> out;
+#pragma unroll
+        for (uint32_t e = 0; e < V; ++e) {
+            const uint64_t y = ybase | ((uint64_t)i * nthr * V) | e;
+            const uint64_t x = xthr ^ xi[i] ^ (e ? xe1 : 0ull);
+            cx<T> p = tab[0][x & 127ull];
+            for (int g = 1; g < ngrp; ++g) p = cmul(p, tab[g][(x >> (7 * g)) & 127ull]);
+            int par = 0;
+            for (int c = 0; c < pd.n_cz; ++c) par += __popcll(y & (y >> pd.cz_d[c]) & pd.cz_m[c]);
+            out.v[e] = (par & 1) ? cneg(p) : p;
+        }
+        *reinterpret_cast<vec16<T> *>(state + (ybase | ((uint64_t)i * nthr * V))) = out;
+    }
+}
+
 // ---- fused gate block: one HBM round trip, all stages of the block in shared memory ---------
 template <typename T, int R, int MAXT>
 __global__ void __launch_bounds__(MAXT, (MAXT <= 256 || R <= 4 ? 2 : 1))
@@ -252,6 +316,17 @@ int launch_expand_params(int prec, const double *params, void *cs, uint64_t coun
     cudaStream_t st = (cudaStream_t)stream;
     if (prec == 0) expand_params_kernel<float><<<nb, 256, 0, st>>>(params, (cx<float> *)cs, count);
     else expand_params_kernel<double><<<nb, 256, 0, st>>>(params, (cx<double> *)cs, count);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
+int launch_init_product(int prec, const PrefixDev &pd, void *states, uint64_t stride, const void *cs, int P, int batch,
+                        void *stream, uint64_t *launches)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    dim3 grid((unsigned)(1ull << (pd.n - pd.kk)), (unsigned)batch);
+    if (prec == 0) init_product_kernel<float><<<grid, 256, 0, st>>>(pd, (cx<float> *)states, stride, (const cx<float> *)cs, P);
+    else init_product_kernel<double><<<grid, 256, 0, st>>>(pd, (cx<double> *)states, stride, (const cx<double> *)cs, P);
     ++*launches;
     return (int)cudaGetLastError();
 }

@@ -19,8 +19,18 @@ constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-mem
 constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
 constexpr uint32_t HDR_BYTES = 384;         // shared-memory header holding the DBlock / DPass copy
 
+struct PrefixDev {   // device view of schedule.h Prefix
+    const int32_t *rot_begin; const uint8_t *rot_kind; const int32_t *rot_param;
+    const uint8_t *cx_t, *cx_c;
+    int n_cx, n_cz, n, kk;   // kk: log2 of the amplitudes one thread block writes (contiguous)
+    int cz_d[4];
+    uint64_t cz_m[4];
+};
+
 // prec: 0 = complex64 (float), 1 = complex128 (double)
 int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches);
+int launch_init_product(int prec, const PrefixDev &pd, void *states, uint64_t stride_amps, const void *cs, int P, int batch,
+                        void *stream, uint64_t *launches);
 int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &block, int k, uint32_t smem_prog_bytes, int n,
                       void *states, uint64_t stride_amps, const void *cs, int P, int batch, void *stream,
                       uint64_t *launches);

@@ -229,7 +229,41 @@ int conflict_penalty(uint64_t T, uint64_t Rset, int k)
 
 }  // namespace
 
-bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &P, std::string &err)
+Prefix find_prefix(int n, const std::vector<HostOp> &ops)
+{
+    Prefix px;
+    size_t i = 0;
+    std::vector<std::vector<std::pair<uint8_t, int32_t>>> rot((size_t)n);
+    while (i < ops.size() && ops[i].kind <= 1) { rot[ops[i].q0].push_back({(uint8_t)ops[i].kind, ops[i].param}); ++i; }
+    if (i == 0) return px;
+    size_t j = i;
+    const int ekind = j < ops.size() ? ops[j].kind : -1;
+    std::vector<std::pair<int, uint64_t>> dist;   // CZ pairs grouped by distance
+    while (j < ops.size() && ops[j].kind >= 2 && ops[j].kind == ekind) {
+        if (ekind == 3) { px.cx_t.push_back((uint8_t)ops[j].q0); px.cx_c.push_back((uint8_t)ops[j].q1); }
+        else {
+            const int lo = ops[j].q0 < ops[j].q1 ? ops[j].q0 : ops[j].q1, d = ops[j].q0 + ops[j].q1 - 2 * lo;
+            size_t e = 0;
+            while (e < dist.size() && dist[e].first != d) ++e;
+            if (e == dist.size()) { if (dist.size() == 4) break; dist.push_back({d, 0}); }
+            dist[e].second ^= 1ull << lo;   // a repeated pair cancels
+        }
+        ++j;
+    }
+    px.n_ops = (int)j;
+    px.n_cz = (int)dist.size();
+    for (size_t e = 0; e < dist.size(); ++e) { px.cz_d[e] = dist[e].first; px.cz_m[e] = dist[e].second; }
+    px.rot_begin.assign((size_t)n + 1, 0);
+    for (int q = 0; q < n; ++q) {
+        px.rot_begin[q] = (int32_t)px.rot_kind.size();
+        for (auto &r : rot[q]) { px.rot_kind.push_back(r.first); px.rot_param.push_back(r.second); }
+    }
+    px.rot_begin[n] = (int32_t)px.rot_kind.size();
+    return px;
+}
+
+bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &P, std::string &err,
+                     bool from_zero)
 {
     P = Program();
     if (n < 1 || n > 40) { err = "schedule: bad qubit count"; return false; }
@@ -250,6 +284,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
     std::vector<uint64_t> cand;
     BlockTake bt, best;
     bool first = true;
+    const bool zero_first = from_zero;
     while (!pending.empty() || first) {
         // ---- choose T
         block_candidates(ops, pending, n, k, f, cand);
@@ -266,7 +301,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
         const uint64_t T = bestT;
         // ---- block header
         Block B; memset(&B, 0, sizeof B);
-        B.k = (uint8_t)k; B.source_zero = first ? 1 : 0;
+        B.k = (uint8_t)k; B.source_zero = (first && zero_first) ? 1 : 0;
         {
             int lp = 0, nr = 0;
             for (int q = 0; q < n;) {

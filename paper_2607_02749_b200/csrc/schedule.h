@@ -31,7 +31,24 @@ struct Program {
 };
 
 // Compile.  Returns false and sets err on failure (never throws).
-bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &out, std::string &err);
+// from_zero: the first block starts from |0...0> without reading (false when a product-state prefix wrote the state).
+bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &out, std::string &err,
+                     bool from_zero = true);
+
+// Product-state prefix: the leading run of single-qubit rotations followed by the run of entanglers
+// that comes before the next rotation.  RZ RY |0> on every qubit is a product state, CZ multiplies it by a sign, a
+// CNOT permutes indices, so  psi[y] = sign(y) * prod_q f_q[(A^-1 y)_q]  can be WRITTEN without reading anything.
+struct Prefix {
+    int n_ops = 0;                         // ops [0, n_ops) of the list are covered (0 = no prefix)
+    std::vector<int32_t> rot_begin;        // per qubit: range into rot_kind / rot_param (n + 1 entries)
+    std::vector<uint8_t> rot_kind;         // 0 RY, 1 RZ, in application order
+    std::vector<int32_t> rot_param;
+    std::vector<uint8_t> cx_t, cx_c;       // CNOTs in list order (target, control); empty when the run is CZ
+    int n_cz = 0;                          // CZ run as sum over distances d: popcount(y & (y >> d) & mask_d)
+    int cz_d[4] = {0, 0, 0, 0};
+    uint64_t cz_m[4] = {0, 0, 0, 0};
+};
+Prefix find_prefix(int n, const std::vector<HostOp> &ops);
 
 std::string dump_program(const Program &p);
 

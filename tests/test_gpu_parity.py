@@ -308,3 +308,25 @@ def test_c64_vs_c128_at_28_qubits():
         E[prec] = g.energy_batch(w.params[:1])
         del g
     assert_close("c64", E["c64"], E["c128"], w.coeffs, "c64 vs c128")
+
+
+@pytest.mark.parametrize("n,D,ent,topo,prec", [(14, 2, "cz", "ring", "c64"), (15, 2, "cnot", "ring", "c128"), (12, 1, "cnot", "linear", "c64")])
+def test_without_product_state_prefix(orc, n, D, ent, topo, prec, monkeypatch):
+    """The first layer is normally WRITTEN as a product state; with GVQE_NO_PREFIX the same circuit runs
+    through the generic blocks from |0...0>.  Both must match the oracle (and so each other)."""
+    ops = np.array(layout_ops(n, D, ent, topo, 1), dtype=np.int32)
+    P = num_params(n, D, 1)
+    paulis, coeffs = random_paulis(500 + n, n, 100, 5)
+    th = np.random.default_rng(n).uniform(-math.pi, math.pi, (3, P))
+    ref = orc.energy_batch(n, ops, th, paulis, coeffs)
+    for no_prefix in (False, True):
+        monkeypatch.setenv("GVQE_PREFIX", "1")
+        if no_prefix:
+            monkeypatch.setenv("GVQE_PREFIX", "0")
+        monkeypatch.setenv("GVQE_K", "10")
+        g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo), precision=prec)
+        assert ("prefix ops=0" in g.dump_schedule()) == no_prefix
+        g.set_hamiltonian(paulis, coeffs)
+        g.alloc_workspace(3)
+        assert_close(prec, g.energy_batch(th), ref, coeffs, f"no_prefix={no_prefix}")
+        assert np.max(np.abs(g.get_state(2) - orc.state(n, ops, th[2]))) < (1e-12 if prec == "c128" else 2e-5)
