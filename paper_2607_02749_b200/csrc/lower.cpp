@@ -7,7 +7,7 @@
 namespace gv {
 
 namespace {
-constexpr uint32_t SLICE_BUDGET = 12 * 1024;   // bytes of shared memory for the program slice of one block
+constexpr uint32_t SLICE_BUDGET = 40 * 1024;   // bytes of shared memory for the program slice of one block
 inline uint32_t al16(uint32_t v) { return (v + 15u) & ~15u; }
 }  // namespace
 
@@ -70,7 +70,7 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                                                       (uint32_t)(D.ryl.size() - db.ryl_off) + add_ryl,
                                                       (uint32_t)(D.cxs.size() - db.cx_off) + add_cx, scs_bytes);
                 if (n_stages > 0 && (tot > SLICE_BUDGET || n_stages >= 250)) break;
-                if (tot > 4 * SLICE_BUDGET) { err = "lower: a single stage exceeds the program budget (internal)"; return false; }
+                if (tot > SLICE_BUDGET + 4096) { err = "lower: a single stage exceeds the program budget (internal)"; return false; }
                 // ---- emit the stage
                 DStage ds; memset(&ds, 0, sizeof ds);
                 for (int s = 0; s < p.R; ++s) ds.regbit[s] = S.regbit[s];

@@ -340,7 +340,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                 for (uint64_t rs : rc) for (int fa = 0; fa < 2; ++fa) {
                     stage_take(bops, L, carry, rs, fa != 0, st);
                     if (st.n_nondiag == 0) continue;
-                    const double score = st.n_nondiag - 2.0 * st.n_seg - 0.01 * conflict_penalty(T, rs, k);
+                    const double score = st.n_nondiag - 0.1 * st.n_seg - 0.01 * conflict_penalty(T, rs, k);
                     if (score > bscore) { bscore = score; sbest = st; Rset = rs; }
                 }
                 if (bscore < -1e29) { err = "schedule: stage made no progress (internal)"; return false; }
