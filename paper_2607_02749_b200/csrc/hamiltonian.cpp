@@ -247,6 +247,17 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                         dg.gt_index = (uint32_t)(plan.gtabs.size() / GT_WORDS);
                         int tpos[16], nt = 0;
                         for (int b = 0; b < k; ++b) if (!(excl >> b & 1)) tpos[nt++] = b;
+                        {   // lanes 0..15 (thread-index bits 0..3) must hit 16 distinct bank pairs: give them local bit
+                            // positions with distinct residues modulo the swizzle fold width (see phys<T>())
+                            int pick[16], np = 0; bool used[16] = {false};
+                            for (int r = 0; r < FB && np < 4; ++r)
+                                for (int t = 0; t < nt; ++t) if (!used[t] && tpos[t] % FB == r) { pick[np++] = t; used[t] = true; break; }
+                            for (int t = 0; t < nt && np < 4; ++t) if (!used[t]) { pick[np++] = t; used[t] = true; }
+                            int ord[16], no = 0;
+                            for (int i2 = 0; i2 < np; ++i2) ord[no++] = tpos[pick[i2]];
+                            for (int t = 0; t < nt; ++t) if (!used[t]) ord[no++] = tpos[t];
+                            for (int t = 0; t < nt; ++t) tpos[t] = ord[t];
+                        }
                         auto word_of = [&](uint32_t j) {
                             uint32_t u = 0;
                             for (int r = 0; r < nur; ++r) u |= ((j >> ur[r].gpos) & ((1u << ur[r].len) - 1u)) << ur[r].lpos;

@@ -576,10 +576,17 @@ GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32
     const uint32_t w0 = gt[tid & 15u] ^ gt[16u + (tid >> 4)];
     const uint32_t pjb = w0 & 0xFFFFFu;
     const cx<T> w = tab[tab_off + (w0 >> 20)];
+    uint32_t cmb[1 << L];   // loop-bit combinations: broadcast reads, four words at a time
+    GV_UNROLL
+    for (int i = 0; i < (1 << L); i += 4) {
+        struct alignas(16) u4 { uint32_t a, b, c, d; };
+        const u4 q = *reinterpret_cast<const u4 *>(gt + 32 + i);
+        cmb[i] = q.a; cmb[i + 1] = q.b; cmb[i + 2] = q.c; cmb[i + 3] = q.d;
+    }
     T tr = T(0), ti = T(0);
     GV_UNROLL
     for (int i = 0; i < (1 << L); ++i) {
-        const uint32_t ob = pjb ^ gt[32 + i];
+        const uint32_t ob = pjb ^ cmb[i];
         const cx<T> a = *reinterpret_cast<const cx<T> *>(tile_bytes + ob);
         const cx<T> b = *reinterpret_cast<const cx<T> *>(tile_bytes + (ob ^ pm_bytes));
         tr = b.x * a.x + tr; tr = b.y * a.y + tr;     // Re conj(b) a
