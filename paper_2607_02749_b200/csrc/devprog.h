@@ -112,9 +112,13 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
                              // are added per thread block; terms [dyn_end, term_end) are folded into the static table
     uint32_t gtab_off;       // offset of the group's static W table in the global table array (= batch base + tab_off)
     uint32_t batch_entries;  // table entries of the whole batch this group belongs to
+    uint32_t batch_last;     // index of the last group of that batch
     uint32_t ex_pack;        // ex[] packed 4 bits each (entry e at bits 4e)
     uint32_t lp_pack;        // lp[] packed 4 bits each
     uint64_t urun_pack;      // uruns packed 12 bits each: lpos | len << 4 | shift << 8
+    uint8_t rs;              // 1: register-stage group: flip mask and table index live in the register bits of stage rs_id
+    uint8_t m_r;             // its flip mask over the register slots
+    uint16_t rs_id;          // index into the DRs array
     uint32_t pm_bytes;       // swizzled byte offset of the flip mask: phys(m_loc) * sizeof(amplitude)
     uint32_t gt_index;       // index of the group's lookup block (GT_WORDS uint32) in the group-table array
     URun uruns[3];
@@ -129,6 +133,14 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
 //   [32,64) swizzled byte offsets of the 2^L loop-bit combinations
 constexpr int GT_WORDS = 64;
 constexpr int GT_BATCH_MAX = 32;   // groups per table batch (shared-memory copy of their lookup blocks)
+
+// Register stage of the expectation kernel: every thread holds the 2^R amplitudes that differ in these local bits; all
+// groups whose flip mask and z bits lie inside them are evaluated from registers (partner = another register).
+struct DRs {
+    uint8_t regbit[DEV_MAX_R];     // local bit positions, ascending
+    uint8_t pad[3];
+    uint32_t po_bytes[DEV_MAX_R];  // swizzled byte offset of each register bit
+};
 
 struct DPass {               // one read-only sweep over the state
     uint8_t k, n_runs, with_diag, pad;

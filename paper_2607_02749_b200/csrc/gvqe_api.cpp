@@ -51,7 +51,7 @@ struct gvqe_ctx {
     // carved device pointers
     GateLaunch gl{};
     DPass *d_passes = nullptr; DGroup *d_groups = nullptr; DTerm *d_terms = nullptr;
-    uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr; void *d_wstat = nullptr; uint32_t *d_gtabs = nullptr;
+    uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr; void *d_wstat = nullptr; uint32_t *d_gtabs = nullptr; DRs *d_rss = nullptr;
     std::vector<float> wstat_f;
     void *d_table = nullptr; void *d_states = nullptr; void *d_cs = nullptr;
     double *d_params = nullptr, *d_partial = nullptr, *d_E = nullptr;
@@ -249,7 +249,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -275,6 +275,7 @@ Layout layout_of(const gvqe_ctx *c)
     L.terms = cv.take(c->plan.terms.size() * sizeof(DTerm));
     L.wstat = cv.take(c->plan.wstat.size() / 2 * c->amp_bytes());
     L.gtabs = cv.take(c->plan.gtabs.size() * 4);
+    L.rss = cv.take(c->plan.rss.size() * sizeof(DRs));
     L.dz = cv.take(c->H.diag_z.size() * 8);
     L.dc = cv.take(c->H.diag_c.size() * 8);
     L.table = cv.take(c->tab_bytes() << c->n_store);
@@ -332,7 +333,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
     for (int i = 0; i < 4; ++i) { c->pxd.cz_d[i] = c->px.cz_d[i]; c->pxd.cz_m[i] = c->px.cz_m[i]; }
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
-    c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs);
+    c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs); c->d_rss = (DRs *)(w + L.rss);
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
     c->d_table = w + L.table;
     char *p = w + L.fixed_end;
@@ -353,7 +354,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
         c->wstat_f.assign(c->plan.wstat.begin(), c->plan.wstat.end());
         UP(c->d_wstat, c->wstat_f);
     } else UP(c->d_wstat, c->plan.wstat);
-    UP(c->d_gtabs, c->plan.gtabs);
+    UP(c->d_gtabs, c->plan.gtabs); UP(c->d_rss, c->plan.rss);
     UP(c->d_diag_z, c->H.diag_z); UP(c->d_diag_c, c->H.diag_c);
 #undef UP
     // diagonal energy table: E(x) = sum_{Z-only k} c_k (-1)^{popcount(x & z_k)} = WHT of the scattered coefficients
@@ -401,7 +402,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     if (c->profiling) cudaEventRecord(e4[1], st);
     const uint32_t tiles = 1u << (c->n_store - c->plan.k);
     for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
-        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat, c->d_gtabs, c->d_states,
+        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat, c->d_gtabs, c->d_rss, c->d_states,
                                 stride, c->d_table, c->d_partial, c->slots_per_b, (uint32_t)pi * tiles, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "expectation pass");
     }

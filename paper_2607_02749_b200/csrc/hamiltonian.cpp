@@ -3,6 +3,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 
@@ -194,7 +195,70 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
         const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // log2(threads) of the expectation kernel
         const int L = k - 1 - TB;                                   // loop bits: 2^L pairs per thread and group
         const int umax_eff = umax < TB ? umax : TB;
+        // ---- register stages: groups whose flip mask and in-tile z bits fit RSB local bits are clustered; a cluster is
+        // evaluated with those bits as register bits (amplitudes and partners in registers, W broadcast)
+        const int RSB = k - TB;
+        std::vector<char> in_rs(gm.size(), 0);
+        if (RSB >= 2 && RSB <= DEV_MAX_R && !getenv("GVQE_NO_RS")) {
+            std::vector<uint32_t> sets; std::vector<std::vector<int>> members;
+            std::vector<std::pair<uint32_t, int>> cand;
+            for (int g : passG[p]) {
+                uint32_t S = compress(gm[g], T);
+                for (int t : gterms[g]) S |= compress(H.terms[t].z & T, T);
+                if (__builtin_popcount(S) <= RSB) cand.push_back({S, g});
+            }
+            std::sort(cand.begin(), cand.end());
+            for (auto &cg : cand) {
+                size_t si = 0;
+                while (si < sets.size() && __builtin_popcount(sets[si] | cg.first) > RSB) ++si;
+                if (si == sets.size()) { sets.push_back(0); members.emplace_back(); }
+                sets[si] |= cg.first; members[si].push_back(cg.second);
+            }
+            for (size_t si = 0; si < sets.size(); ++si) {
+                uint32_t regs = sets[si];
+                for (int b = 0; b < k && __builtin_popcount(regs) < RSB; ++b) regs |= 1u << b;   // pad with low bits
+                DRs rs; memset(&rs, 0, sizeof rs);
+                int nrb = 0;
+                for (int b = 0; b < k; ++b) if (regs >> b & 1) { rs.regbit[nrb] = (uint8_t)b; rs.po_bytes[nrb] = hphys(1u << b) * (uint32_t)amp_bytes; ++nrb; }
+                const uint32_t rs_id = (uint32_t)plan.rss.size();
+                plan.rss.push_back(rs);
+                std::sort(members[si].begin(), members[si].end());
+                for (int g : members[si]) {
+                    in_rs[g] = 1;
+                    DGroup dg; memset(&dg, 0, sizeof dg);
+                    dg.m_loc = compress(gm[g], T);
+                    dg.pivot = (uint8_t)(31 - __builtin_clz(dg.m_loc));
+                    dg.rs = 1; dg.rs_id = (uint16_t)rs_id; dg.m_r = (uint8_t)compress(dg.m_loc, regs);
+                    dg.ubits = (uint8_t)RSB;
+                    dg.term_begin = (uint32_t)plan.terms.size();
+                    if (batch_groups >= GT_BATCH_MAX || tab_used + (1u << RSB) > tab_cap) {
+                        if (plan.groups.size() > dp.group_begin) plan.groups.back().last_in_batch = 1;
+                        tab_used = 0; batch_groups = 0;
+                    }
+                    ++batch_groups;
+                    dg.tab_off = tab_used; tab_used += 1u << RSB;
+                    long dyn_end = -1;
+                    for (int phase = 0; phase < 2; ++phase)
+                        for (int t : gterms[g]) {
+                            const HostTerm &ht = H.terms[t];
+                            const bool dyn = (ht.z & ~T) != 0;
+                            if (dyn != (phase == 0)) continue;
+                            if (phase == 1 && dyn_end < 0) dyn_end = (long)plan.terms.size();
+                            DTerm dt; memset(&dt, 0, sizeof dt);
+                            static const double pr[4] = {1, 0, -1, 0}, pim[4] = {0, 1, 0, -1};
+                            dt.cr = ht.c * pr[ht.ny & 3]; dt.ci = ht.c * pim[ht.ny & 3];
+                            dt.zout = ht.z & ~T;
+                            dt.zu = compress(compress(ht.z & T, T), regs);
+                            plan.terms.push_back(dt);
+                        }
+                    dg.term_end = (uint32_t)plan.terms.size();
+                    dg.dyn_end = dyn_end < 0 ? dg.term_end : (uint32_t)dyn_end;
+                    plan.groups.push_back(dg);
+                }
+            }
+        }
         for (int g : passG[p]) {
+            if (in_rs[g]) continue;
             // slice the group's terms so that every slice's table index (in-tile z bits) stays small  (Eq. 12)
             std::vector<std::vector<int>> slices;
             std::vector<uint32_t> sliceU;
@@ -313,7 +377,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
             plan.wstat.resize(plan.wstat.size() + 2 * (size_t)entries, 0.0);
             for (uint32_t gi = g0; gi <= g1; ++gi) {
                 DGroup &dg = plan.groups[gi];
-                dg.batch_entries = entries;
+                dg.batch_entries = entries; dg.batch_last = g1;
                 dg.gtab_off = (uint32_t)base + dg.tab_off;
                 if (dg.direct) { dg.gtab_off = (uint32_t)base; continue; }
                 for (uint32_t u = 0; u < (1u << dg.ubits); ++u) {

@@ -33,6 +33,7 @@ struct ExpectPlan {
     std::vector<DPass> passes;
     std::vector<DGroup> groups;
     std::vector<DTerm> terms;
+    std::vector<DRs> rss;        // register stages
     std::vector<uint32_t> gtabs; // GT_WORDS words per table-mode group (see devprog.h)
     std::vector<double> wstat;   // static W tables (re, im interleaved), laid out batch by batch like the smem area
 };

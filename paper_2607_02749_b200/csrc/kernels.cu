@@ -138,6 +138,8 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     tile_store_u<T, NLD>(tile, state, x0, tid, hi, sb->hip);
 }
 
+constexpr uint32_t SGR_STRIDE = (uint32_t)((sizeof(DGroup) + 15) / 16 * 16);   // == sizeof(DGroup): shared-memory copy of a batch's groups
+
 // ---- expectation pass: read-only sweep, diagonal table + every flip-mask group of the pass --
 __device__ __forceinline__ double block_sum(double v, double *red)
 {
@@ -153,7 +155,8 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 template <typename T, typename TT, int L>
 __global__ void __launch_bounds__(256, 2)
 expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
-                   const cx<T> *__restrict__ wstat, const uint32_t *__restrict__ gtabs, const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
+                   const cx<T> *__restrict__ wstat, const uint32_t *__restrict__ gtabs, const DRs *__restrict__ rss,
+                   const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
                    double *partial, uint32_t slots_per_b, uint32_t slot_off)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -171,7 +174,8 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
     cx<T> *tab = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);
     uint32_t *gts = reinterpret_cast<uint32_t *>(tab + EXPECT_TAB_CAP);
-    cx<T> *tile = reinterpret_cast<cx<T> *>(gts + GT_BATCH_MAX * GT_WORDS);
+    DGroup *sgr = reinterpret_cast<DGroup *>(gts + GT_BATCH_MAX * GT_WORDS);
+    cx<T> *tile = reinterpret_cast<cx<T> *>(reinterpret_cast<unsigned char *>(sgr) + GT_BATCH_MAX * SGR_STRIDE);
     const uint32_t b = blockIdx.y;
     const cx<T> *state = states + (uint64_t)b * stride;
     const int k = sp->k, n_runs = sp->n_runs;
@@ -183,30 +187,41 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     uint32_t g = sp->group_begin;
     const uint32_t gend = sp->group_end;
     while (g < gend) {
-        uint32_t ge = g;
-        while (!groups[ge].last_in_batch) ++ge;
-        {   // static tables of the whole batch: one flat coalesced copy
+        const uint32_t ge = groups[g].batch_last;
+        {   // the batch's group descriptors, static W tables and lookup blocks: flat coalesced copies into shared memory
+            const uint32_t ng = ge - g + 1;
+            const uint32_t *gsrc = reinterpret_cast<const uint32_t *>(groups + g);
+            uint32_t *gdst = reinterpret_cast<uint32_t *>(sgr);
+            for (uint32_t e = tid; e < ng * (uint32_t)(sizeof(DGroup) / 4); e += nthr) gdst[e] = gsrc[e];
             const uint32_t ne = groups[g].batch_entries;
             const cx<T> *src = wstat + (groups[g].gtab_off - groups[g].tab_off);
             for (uint32_t e = tid; e < ne; e += nthr) tab[e] = src[e];
-            const uint32_t ng = ge - g + 1;   // lookup blocks of the batch's table-mode groups
             for (uint32_t e = tid; e < ng * GT_WORDS; e += nthr) {
                 const DGroup *pg = groups + g + e / GT_WORDS;
-                if (!pg->direct) gts[e] = gtabs[(uint64_t)pg->gt_index * GT_WORDS + (e % GT_WORDS)];
+                if (!pg->direct && !pg->rs) gts[e] = gtabs[(uint64_t)pg->gt_index * GT_WORDS + (e % GT_WORDS)];
             }
         }
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
-            const DGroup *pg = groups + gi;
+            const DGroup *pg = sgr + (gi - g);
             const uint32_t tb = pg->term_begin, de = pg->dyn_end, to = pg->tab_off, ne = 1u << pg->ubits;
             if (pg->direct || de == tb) continue;
             for (uint32_t u = tid; u < ne; u += nthr)
                 tab[to + u] = group_table_entry<T>(tb, de, terms, xbase, u, tab[to + u]);
         }
         __syncthreads();
+        int cur_rs = -1;
+        constexpr int RSR = (L + 1 <= DEV_MAX_R) ? L + 1 : 1;   // the planner makes register stages only when L + 1 <= DEV_MAX_R
+        cx<T> ra[1 << RSR];   // register stage: 2^(L+1) amplitudes per thread
         for (uint32_t gi = g; gi <= ge; ++gi) {
-            const DGroup *pg = groups + gi;
-            if (pg->direct) {
+            const DGroup *pg = sgr + (gi - g);
+            if (pg->rs) {
+                if ((int)pg->rs_id != cur_rs) {
+                    cur_rs = pg->rs_id;
+                    rs_load<T, RSR>(ra, rss[cur_rs], reinterpret_cast<const unsigned char *>(tile), tid);
+                }
+                acc += 2.0 * (double)RsDispatch<T, RSR, (1 << RSR) - 1>::run(pg->m_r, ra, tab + pg->tab_off);
+            } else if (pg->direct) {
                 const DGroup dg = *pg;
                 acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
             } else {
@@ -354,15 +369,15 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &bi, in
 
 template <typename T, typename TT>
 static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                           const void *wstat, const uint32_t *gtabs, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                           const void *wstat, const uint32_t *gtabs, const DRs *rss, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                            uint32_t slot_off, int batch, cudaStream_t st)
 {
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
-    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + (sizeof(cx<T>) << k);
+    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + GT_BATCH_MAX * SGR_STRIDE + (sizeof(cx<T>) << k);
     const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
     const int L = k - 1 - TB;
 #define GV_EXPECT(LL)                                                                                                  \
-    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, gtabs, (const cx<T> *)states, stride, \
+    expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, gtabs, rss, (const cx<T> *)states, stride, \
                                                                (const TT *)table, partial, slots_per_b, slot_off)
     switch (L) {
     case 2: GV_EXPECT(2); break;
@@ -376,15 +391,15 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
 }
 
 int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, const DGroup *groups, const DTerm *terms,
-                       const void *wstat, const uint32_t *gtabs, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
+                       const void *wstat, const uint32_t *gtabs, const DRs *rss, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                        uint32_t slot_off, int batch, void *stream, uint64_t *launches)
 {
     cudaStream_t st = (cudaStream_t)stream;
     ++*launches;
     if (prec == 0)
-        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, wstat, gtabs, states, stride, table, partial, slots_per_b,
+        return expect_launch_t<float, float>(passes, pi, k, n, groups, terms, wstat, gtabs, rss, states, stride, table, partial, slots_per_b,
                                              slot_off, batch, st);
-    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, wstat, gtabs, states, stride, table, partial, slots_per_b,
+    return expect_launch_t<double, double>(passes, pi, k, n, groups, terms, wstat, gtabs, rss, states, stride, table, partial, slots_per_b,
                                            slot_off, batch, st);
 }
 

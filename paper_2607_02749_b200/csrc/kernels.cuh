@@ -595,6 +595,53 @@ GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32
     return 2.0 * (double)(w.x * tr - w.y * ti);
 }
 
+// ---- register-stage groups: amplitudes and partners in registers, W (indexed by the register index) broadcast ------
+template <int M> struct TopBit { static constexpr int value = 1 + TopBit<(M >> 1)>::value; };
+template <> struct TopBit<1> { static constexpr int value = 0; };
+template <> struct TopBit<0> { static constexpr int value = 0; };
+
+template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T> *w)
+{
+    constexpr int PV = TopBit<M>::value;
+    T acc = T(0);
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
+        if (r & (1 << PV)) continue;
+        const cx<T> ww = w[r], u = a[r], v = a[r ^ M];
+        T tr = v.x * u.x; tr = v.y * u.y + tr;      // Re conj(v) u
+        T ti = v.x * u.y; ti = -v.y * u.x + ti;     // Im conj(v) u
+        acc = ww.x * tr + acc; acc = -ww.y * ti + acc;
+    }
+    return acc;
+}
+
+template <typename T, int R, int M> struct RsDispatch {
+    static GV_DEV T run(int m, const cx<T> *a, const cx<T> *w)
+    {
+        if (m == M) return rs_pairs<T, R, M>(a, w);
+        return RsDispatch<T, R, M - 1>::run(m, a, w);
+    }
+};
+template <typename T, int R> struct RsDispatch<T, R, 0> {
+    static GV_DEV T run(int, const cx<T> *, const cx<T> *) { return T(0); }
+};
+
+template <typename T, int R>
+GV_DEV void rs_load(cx<T> *a, const DRs &rs, const unsigned char *tile_bytes, uint32_t tid)
+{
+    uint32_t j = tid;
+    GV_UNROLL
+    for (int s = 0; s < R; ++s) j = insert_zero(j, rs.regbit[s]);
+    const uint32_t pjb = phys<T>(j) * (uint32_t)sizeof(cx<T>);
+    GV_UNROLL
+    for (int r = 0; r < (1 << R); ++r) {
+        uint32_t o = pjb;
+        GV_UNROLL
+        for (int s = 0; s < R; ++s) if (r & (1 << s)) o ^= rs.po_bytes[s];
+        a[r] = *reinterpret_cast<const cx<T> *>(tile_bytes + o);
+    }
+}
+
 // W_g(u) = sum_k c_k i^{nY_k} (-1)^{popcount(x & z_k)} for the table index u of group g (tile-constant part of the
 // sign from the bits outside the tile).  One entry per call.
 template <typename T>
