@@ -220,7 +220,7 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
                     cur_rs = pg->rs_id;
                     rs_load<T, RSR>(ra, rss[cur_rs], reinterpret_cast<const unsigned char *>(tile), tid);
                 }
-                acc += 2.0 * (double)RsDispatch<T, RSR, (1 << RSR) - 1>::run(pg->m_r, ra, tab + pg->tab_off);
+                acc += 2.0 * (double)RsDispatch<T, RSR, 1, (1 << RSR) - 1>::run(pg->m_r, ra, tab + pg->tab_off);
             } else if (pg->direct) {
                 const DGroup dg = *pg;
                 acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);

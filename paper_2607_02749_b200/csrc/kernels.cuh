@@ -603,27 +603,32 @@ template <> struct TopBit<0> { static constexpr int value = 0; };
 template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T> *w)
 {
     constexpr int PV = TopBit<M>::value;
-    T acc = T(0);
+    T acc[4] = {T(0), T(0), T(0), T(0)};   // independent chains
+    int n = 0;
     GV_UNROLL
     for (int r = 0; r < (1 << R); ++r) {
         if (r & (1 << PV)) continue;
         const cx<T> ww = w[r], u = a[r], v = a[r ^ M];
         T tr = v.x * u.x; tr = v.y * u.y + tr;      // Re conj(v) u
         T ti = v.x * u.y; ti = -v.y * u.x + ti;     // Im conj(v) u
-        acc = ww.x * tr + acc; acc = -ww.y * ti + acc;
+        acc[n & 3] = ww.x * tr + acc[n & 3];
+        acc[(n + 2) & 3] = -ww.y * ti + acc[(n + 2) & 3];
+        ++n;
     }
-    return acc;
+    return (acc[0] + acc[1]) + (acc[2] + acc[3]);
 }
 
-template <typename T, int R, int M> struct RsDispatch {
+// binary search over the flip mask (uniform branches): masks LO..HI
+template <typename T, int R, int LO, int HI> struct RsDispatch {
     static GV_DEV T run(int m, const cx<T> *a, const cx<T> *w)
     {
-        if (m == M) return rs_pairs<T, R, M>(a, w);
-        return RsDispatch<T, R, M - 1>::run(m, a, w);
+        if constexpr (LO == HI) return rs_pairs<T, R, LO>(a, w);
+        else {
+            constexpr int MID = (LO + HI) / 2;
+            if (m <= MID) return RsDispatch<T, R, LO, MID>::run(m, a, w);
+            return RsDispatch<T, R, MID + 1, HI>::run(m, a, w);
+        }
     }
-};
-template <typename T, int R> struct RsDispatch<T, R, 0> {
-    static GV_DEV T run(int, const cx<T> *, const cx<T> *) { return T(0); }
 };
 
 template <typename T, int R>
