@@ -330,3 +330,17 @@ def test_without_product_state_prefix(orc, n, D, ent, topo, prec, monkeypatch):
         g.alloc_workspace(3)
         assert_close(prec, g.energy_batch(th), ref, coeffs, f"no_prefix={no_prefix}")
         assert np.max(np.abs(g.get_state(2) - orc.state(n, ops, th[2]))) < (1e-12 if prec == "c128" else 2e-5)
+
+
+@pytest.mark.parametrize("prec", ["c64", "c128"])
+def test_expectation_modes_agree(orc, prec, monkeypatch):
+    """The planner evaluates most community-local groups as register stages; GVQE_NO_RS sends every group through the
+    lookup / direct modes instead.  Both plans must match the oracle on the config-4 recipe (pooled flip masks)."""
+    w = make_workload(4, n=15, M=1500, D=2, batch=3)
+    ref = orc.energy_batch(w.n, w.ops, w.params, w.paulis, w.coeffs)
+    for no_rs in (False, True):
+        if no_rs:
+            monkeypatch.setenv("GVQE_NO_RS", "1")
+        monkeypatch.setenv("GVQE_K", "11")
+        g = ctx_for(w, prec, 3)
+        assert_close(prec, g.energy_batch(w.params), ref, w.coeffs, f"no_rs={no_rs}")
