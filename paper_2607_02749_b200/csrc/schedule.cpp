@@ -135,7 +135,7 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
     std::vector<int> pend = carry_in;
     uint64_t pend_touch = 0;
     for (int p : pend) { const Acts a = acts_of(bops[p]); for (int i = 0; i < a.nq; ++i) pend_touch |= 1ull << a.q[i]; }
-    uint64_t full = 0, nd = 0;
+    uint64_t full = 0, nd = 0, cx_touch = 0;
     for (int pos : L) {
         const HostOp &o = bops[pos];
         const Acts a = acts_of(o);
@@ -148,7 +148,9 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
             if (!a.diag[i]) { ndq |= b; if ((nd & b) || (o.kind == 0 && !(Rset & b))) ok = false; }
         }
         if (ok && !is_diag(o) && (pend_touch & ndq) && !flush_anywhere && out.n_nondiag > 0) ok = false;
-        if (ok && o.kind == 0 && out.has_cx) ok = false;                          // no rotation after the CNOT run began
+        // after the CNOT run began, a rotation is taken only if it commutes with the whole run (its qubit is neither a
+        // target nor a control of it) and needs no diagonal flush: it then executes before the run
+        if (ok && o.kind == 0 && out.has_cx && ((cx_touch | pend_touch) & ndq)) ok = false;
         if (ok && o.kind == 3 && out.has_cx && (pend_touch & ndq)) ok = false;    // no diagonal flush inside the run
         // size caps (shared-memory slice of the program): an op that does not fit waits for the next stage
         if (ok && is_diag(o) && (int)pend.size() >= MAX_SEG_OPS) ok = false;
@@ -166,7 +168,7 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
                 }
                 StageItem it; it.is_seg = false; it.op = pos;
                 out.items.push_back(std::move(it)); ++out.n_nondiag;
-                if (o.kind == 3) out.has_cx = true;
+                if (o.kind == 3) { out.has_cx = true; cx_touch |= (1ull << o.q0) | (1ull << o.q1); }
             }
         } else {
             out.rest.push_back(pos);
