@@ -344,3 +344,19 @@ def test_expectation_modes_agree(orc, prec, monkeypatch):
         monkeypatch.setenv("GVQE_K", "11")
         g = ctx_for(w, prec, 3)
         assert_close(prec, g.energy_batch(w.params), ref, w.coeffs, f"no_rs={no_rs}")
+
+
+def test_long_op_list_splits_blocks(orc):
+    """1 500 random ops on 12 qubits: the program slice of a block outgrows its shared-memory budget and the block is
+    cut into several device blocks at stage boundaries; results unchanged."""
+    n = 12
+    ops, P = random_ops(4242, n, 1500)
+    paulis, coeffs = random_paulis(4243, n, 60, 5)
+    th = np.random.default_rng(7).uniform(-math.pi, math.pi, (2, P))
+    for prec in ("c128", "c64"):
+        g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec)
+        g.set_hamiltonian(paulis, coeffs)
+        g.alloc_workspace(2)
+        assert g.schedule_info()[0] >= 2
+        assert_close(prec, g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, "long op list")
+        assert np.max(np.abs(g.get_state(0) - orc.state(n, ops, th[0]))) < (1e-11 if prec == "c128" else 1e-4)
