@@ -378,6 +378,8 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
             for (uint32_t gi = g0; gi <= g1; ++gi) {
                 DGroup &dg = plan.groups[gi];
                 dg.batch_entries = entries; dg.batch_last = g1;
+                dg.hot = (uint64_t)(dg.rs ? 1 : (dg.direct ? 2 : 0)) | ((uint64_t)dg.m_r << 2) | ((uint64_t)dg.rs_id << 8) |
+                         ((uint64_t)dg.tab_off << 24) | ((uint64_t)((!dg.direct && dg.dyn_end != dg.term_begin) ? 1 : 0) << 63);
                 dg.gtab_off = (uint32_t)base + dg.tab_off;
                 if (dg.direct) { dg.gtab_off = (uint32_t)base; continue; }
                 for (uint32_t u = 0; u < (1u << dg.ubits); ++u) {

@@ -204,8 +204,8 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         __syncthreads();
         for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
             const DGroup *pg = sgr + (gi - g);
+            if (!(pg->hot >> 63)) continue;
             const uint32_t tb = pg->term_begin, de = pg->dyn_end, to = pg->tab_off, ne = 1u << pg->ubits;
-            if (pg->direct || de == tb) continue;
             for (uint32_t u = tid; u < ne; u += nthr)
                 tab[to + u] = group_table_entry<T>(tb, de, terms, xbase, u, tab[to + u]);
         }
@@ -215,17 +215,20 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         cx<T> ra[1 << RSR];   // register stage: 2^(L+1) amplitudes per thread
         for (uint32_t gi = g; gi <= ge; ++gi) {
             const DGroup *pg = sgr + (gi - g);
-            if (pg->rs) {
-                if ((int)pg->rs_id != cur_rs) {
-                    cur_rs = pg->rs_id;
+            const uint64_t hot = pg->hot;
+            const uint32_t mode = (uint32_t)hot & 3u, tab_off = (uint32_t)(hot >> 24) & 0xFFFFFFu;
+            if (mode == 1u) {
+                const int rs_id = (int)((hot >> 8) & 0xFFFFu);
+                if (rs_id != cur_rs) {
+                    cur_rs = rs_id;
                     rs_load<T, RSR>(ra, rss[cur_rs], reinterpret_cast<const unsigned char *>(tile), tid);
                 }
-                acc += 2.0 * (double)RsDispatch<T, RSR, 1, (1 << RSR) - 1>::run(pg->m_r, ra, tab + pg->tab_off);
-            } else if (pg->direct) {
+                acc += 2.0 * (double)RsDispatch<T, RSR, 1, (1 << RSR) - 1>::run((int)((hot >> 2) & 63u), ra, tab + tab_off);
+            } else if (mode == 2u) {
                 const DGroup dg = *pg;
                 acc += group_accumulate<T>(dg, terms, tile, tab, xbase, k, tid, nthr);
             } else {
-                acc += group_accumulate_lut<T, L>(gts + (gi - g) * GT_WORDS, pg->pm_bytes, pg->tab_off,
+                acc += group_accumulate_lut<T, L>(gts + (gi - g) * GT_WORDS, pg->pm_bytes, tab_off,
                                                   reinterpret_cast<const unsigned char *>(tile), tab, tid);
             }
         }
