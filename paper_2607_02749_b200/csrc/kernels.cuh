@@ -108,62 +108,11 @@ GV_DEV void gate_prologue(ProgView<T> &pv, const DBlock &b, const DevArrays &da,
 // ---- tile <-> global -------------------------------------------------------------------------------------
 template <typename T> struct alignas(16) vec16 { cx<T> v[16 / sizeof(cx<T>)]; };
 
-template <typename T>
-GV_DEV void tile_load(cx<T> *tile, const cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k,
-                      uint32_t tid, uint32_t nthr)
-{
-    constexpr uint32_t V = 16 / sizeof(cx<T>);
-    const uint32_t nchunk = (1u << k) / V;
-    for (uint32_t c = tid; c < nchunk; c += nthr) {
-        const uint32_t j = c * V;
-        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
-        const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + x);
-        const uint32_t p = phys<T>(j);
-        GV_UNROLL
-        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v.v[e];
-    }
-}
-
-template <typename T>
-GV_DEV void tile_store(const cx<T> *tile, cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, int k,
-                       uint32_t tid, uint32_t nthr)
-{
-    constexpr uint32_t V = 16 / sizeof(cx<T>);
-    const uint32_t nchunk = (1u << k) / V;
-    for (uint32_t c = tid; c < nchunk; c += nthr) {
-        const uint32_t j = c * V;
-        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
-        const uint32_t p = phys<T>(j);
-        vec16<T> v;
-        GV_UNROLL
-        for (uint32_t e = 0; e < V; ++e) v.v[e] = tile[p ^ e];
-        *reinterpret_cast<vec16<T> *>(state + x) = v;
-    }
-}
-
 // Unrolled variants: every thread moves NLD 16-byte vectors; vector i of thread tid is chunk tid + i*nthr, whose
 // local index splits into disjoint bit fields (tid part | i part), so the global offset is x0 | hi[i] with
-// hi[i] = scatter(i * nthr * V) precomputed once per thread block (shared memory).  All NLD loads are in flight
+// hi[i] = scatter(i * nthr * V) precomputed on the host (DBlock::hi, DPass::hi).  All NLD loads are in flight
 // before the first shared-memory store.
-template <typename T, int NLD>
-GV_DEV void tile_load_u(cx<T> *tile, const cx<T> *state, uint64_t xbase, const Run *runs, int n_runs, uint32_t tid,
-                        uint32_t nthr, const uint64_t *hi)
-{
-    constexpr uint32_t V = 16 / sizeof(cx<T>);
-    const uint64_t x0 = xbase | scatter_runs(tid * V, runs, n_runs);
-    const uint32_t p0 = phys<T>(tid * V);
-    vec16<T> v[NLD];
-    GV_UNROLL
-    for (int i = 0; i < NLD; ++i) v[i] = *reinterpret_cast<const vec16<T> *>(state + (x0 | hi[i]));
-    GV_UNROLL
-    for (int i = 0; i < NLD; ++i) {
-        const uint32_t p = p0 ^ phys<T>((uint32_t)i * nthr * V);
-        GV_UNROLL
-        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v[i].v[e];
-    }
-}
-
-// Second half of tile_load_u when the loads were issued by the caller: registers -> swizzled shared memory.
+// The caller issues the NLD loads (vec16 registers); this writes them to swizzled shared memory.
 template <typename T, int NLD>
 GV_DEV void tile_commit(cx<T> *tile, const vec16<T> *v, uint32_t tid, const uint32_t *hip)
 {
@@ -473,33 +422,8 @@ GV_DEV void gate_stage_store(unsigned char *tile, uint32_t pj2, const uint32_t *
 }
 
 // ---- Hamiltonian engine ----------------------------------------------------------------------------------
-// Diagonal part while the tile is loaded: sum_x |psi[x]|^2 E(x), E = diagonal energy table.
-template <typename T, typename TT>
-GV_DEV double expect_load(cx<T> *tile, const cx<T> *state, const TT *table, bool with_diag, uint64_t xbase,
-                          const Run *runs, int n_runs, int k, uint32_t tid, uint32_t nthr)
-{
-    constexpr uint32_t V = 16 / sizeof(cx<T>);
-    const uint32_t nchunk = (1u << k) / V;
-    double acc = 0.0;
-    for (uint32_t c = tid; c < nchunk; c += nthr) {
-        const uint32_t j = c * V;
-        const uint64_t x = xbase | scatter_runs(j, runs, n_runs);
-        const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + x);
-        const uint32_t p = phys<T>(j);
-        GV_UNROLL
-        for (uint32_t e = 0; e < V; ++e) tile[p ^ e] = v.v[e];
-        if (with_diag) {
-            GV_UNROLL
-            for (uint32_t e = 0; e < V; ++e) {
-                const T pr = v.v[e].x * v.v[e].x + v.v[e].y * v.v[e].y;
-                acc += (double)(pr * (T)table[x + e]);
-            }
-        }
-    }
-    return acc;
-}
-
-// Unrolled variant of expect_load: NLD 16-byte vectors per thread, all loads in flight (see tile_load_u).
+// Tile load of the expectation kernel, NLD 16-byte vectors per thread, all loads in flight; the diagonal part
+// sum_x |psi[x]|^2 E(x) (E = diagonal energy table) is accumulated on the way.
 template <typename T, typename TT, int NLD>
 GV_DEV double expect_load_u(cx<T> *tile, const cx<T> *state, const TT *table, bool with_diag, uint64_t xbase,
                             const Run *runs, int n_runs, uint32_t tid, uint32_t nthr, const uint64_t *hi)
@@ -531,43 +455,9 @@ GV_DEV double expect_load_u(cx<T> *tile, const cx<T> *state, const TT *table, bo
 
 // Table-mode group with thread-constant W: the thread's 2^L pairs differ only in the loop bits, which lie outside
 // the table index bits, so  sum_pairs Re(conj(b) W a) = Re(W * sum_pairs conj(b) a).
-// Scalars of a table-mode group that the pair loop needs, read once (uniform loads) instead of copying the struct.
-struct GroupFast { uint32_t m_loc, tab_off, ex_pack, lp_pack, n_uruns; uint64_t urun_pack; };
-
-template <typename T, int L>
-GV_DEV double group_accumulate_fast(const GroupFast g, const cx<T> *tile, const cx<T> *tab, uint32_t tid)
-{
-    uint32_t j = tid;
-    GV_UNROLL
-    for (int e = 0; e < L + 1; ++e) j = insert_zero(j, (g.ex_pack >> (4 * e)) & 15u);
-    uint32_t u = 0;
-    for (uint32_t r = 0; r < g.n_uruns; ++r) {
-        const uint32_t f = (uint32_t)(g.urun_pack >> (12 * r));
-        u |= ((j >> (f & 15u)) & ((1u << ((f >> 4) & 15u)) - 1u)) << ((f >> 8) & 15u);
-    }
-    const cx<T> w = tab[g.tab_off + u];
-    const uint32_t pj = phys<T>(j), pm = phys<T>(g.m_loc);
-    uint32_t po[L];
-    GV_UNROLL
-    for (int s = 0; s < L; ++s) po[s] = phys<T>(1u << ((g.lp_pack >> (4 * s)) & 15u));
-    uint32_t off[1 << L];   // all XOR combinations of the loop-bit offsets (built incrementally)
-    off[0] = pj;
-    GV_UNROLL
-    for (int s = 0; s < L; ++s) {
-        GV_UNROLL
-        for (int e = 0; e < (1 << s); ++e) off[e | (1 << s)] = off[e] ^ po[s];
-    }
-    T tr = T(0), ti = T(0);
-    GV_UNROLL
-    for (int i = 0; i < (1 << L); ++i) {
-        const cx<T> a = tile[off[i]], b = tile[off[i] ^ pm];
-        tr = b.x * a.x + tr; tr = b.y * a.y + tr;     // Re conj(b) a
-        ti = b.x * a.y + ti; ti = -b.y * a.x + ti;    // Im conj(b) a
-    }
-    return 2.0 * (double)(w.x * tr - w.y * ti);
-}
-
-// Same sum with every index taken from the group's host-built lookup block (devprog.h GT_WORDS): two table reads
+// Table-mode group with thread-constant W: the thread's 2^L pairs differ only in the loop bits, which lie outside the
+// table index bits, so  sum_pairs Re(conj(b) W a) = Re(W * sum_pairs conj(b) a).  Every index comes from the group's
+// host-built lookup block (devprog.h GT_WORDS): two table reads
 // give the thread's swizzled byte offset and its W index, the loop-bit combinations are broadcast reads.
 template <typename T, int L>
 GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32_t tab_off, const unsigned char *tile_bytes,
