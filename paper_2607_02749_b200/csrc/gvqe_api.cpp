@@ -555,12 +555,14 @@ size_t gvqe_dump_schedule(const gvqe_ctx *c, char *buf, size_t cap)
             s += line;
             for (int r = 0; r < dp.n_runs; ++r) { snprintf(line, sizeof line, "%d:%d+%d ", dp.runs[r].lpos, dp.runs[r].gpos, dp.runs[r].len); s += line; }
             s += "\n";
-            int nd = 0, hist[16] = {0}; size_t nt_d = 0, nt_t = 0;
+            int nd = 0, nrs = 0, hist[16] = {0}; size_t nt_d = 0, nt_t = 0, nt_rs = 0;
             for (uint32_t gi = dp.group_begin; gi < dp.group_end; ++gi) {
                 const DGroup &dg = c->plan.groups[gi];
-                if (dg.direct) { ++nd; nt_d += dg.term_end - dg.term_begin; } else { ++hist[dg.ubits & 15]; nt_t += dg.term_end - dg.term_begin; }
+                if (dg.rs) { ++nrs; nt_rs += dg.term_end - dg.term_begin; }
+                else if (dg.direct) { ++nd; nt_d += dg.term_end - dg.term_begin; }
+                else { ++hist[dg.ubits & 15]; nt_t += dg.term_end - dg.term_begin; }
             }
-            snprintf(line, sizeof line, "grp  direct=%d (terms %zu) table terms=%zu ubits hist:", nd, nt_d, nt_t); s += line;
+            snprintf(line, sizeof line, "grp  register-stage=%d (terms %zu) direct=%d (terms %zu) lookup terms=%zu ubits hist:", nrs, nt_rs, nd, nt_d, nt_t); s += line;
             for (int u = 0; u < 16; ++u) if (hist[u]) { snprintf(line, sizeof line, " %d:%d", u, hist[u]); s += line; }
             s += "\n";
         }

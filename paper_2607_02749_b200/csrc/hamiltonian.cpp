@@ -264,11 +264,10 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
             std::vector<uint32_t> sliceU;
             for (int t : gterms[g]) {
                 const uint32_t zl = compress(H.terms[t].z & T, T);
-                Run ur[4];
                 bool placed = false;
                 if (!slices.empty()) {
                     const uint32_t U2 = sliceU.back() | zl;
-                    if (__builtin_popcount(U2) <= umax_eff && runs_of(U2, ur, 4) <= 3) {
+                    if (__builtin_popcount(U2) <= umax_eff) {
                         slices.back().push_back(t); sliceU.back() = U2; placed = true;
                     }
                 }
@@ -282,7 +281,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 Run ur[4];
                 const int nur = runs_of(Uloc, ur, 4);
                 const int ubits = __builtin_popcount(Uloc);
-                const bool table = (ubits <= umax_eff) && (nur <= 3) && ((1u << ubits) <= tab_cap);
+                const bool table = (ubits <= umax_eff) && ((1u << ubits) <= tab_cap);   // any bit pattern: the index comes from the lookup block
                 dg.direct = table ? 0 : 1;
                 dg.term_begin = (uint32_t)plan.terms.size();
                 if (batch_groups >= GT_BATCH_MAX || (table && tab_used + (1u << ubits) > tab_cap)) {   // close the batch
@@ -291,8 +290,8 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 }
                 ++batch_groups;
                 if (table) {
-                    dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)nur;
-                    for (int r = 0; r < nur; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
+                    dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)(nur < 3 ? nur : 3);
+                    for (int r = 0; r < nur && r < 3; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
                     dg.tab_off = tab_used; tab_used += 1u << ubits;
                     // loop bits: the L highest local bits outside the table index bits and the pivot
                     uint32_t excl = 1u << dg.pivot;
@@ -323,8 +322,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                             for (int t = 0; t < nt; ++t) tpos[t] = ord[t];
                         }
                         auto word_of = [&](uint32_t j) {
-                            uint32_t u = 0;
-                            for (int r = 0; r < nur; ++r) u |= ((j >> ur[r].gpos) & ((1u << ur[r].len) - 1u)) << ur[r].lpos;
+                            const uint32_t u = compress(j, Uloc);
                             return (hphys(j) * (uint32_t)amp_bytes) | (u << 20);
                         };
                         for (int half = 0; half < 2; ++half)
@@ -341,7 +339,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                     }
                     for (int e = 0; e < ne; ++e) dg.ex_pack |= (uint32_t)dg.ex[e] << (4 * e);
                     for (int e = 0; e < nlp; ++e) dg.lp_pack |= (uint32_t)dg.lp[e] << (4 * e);
-                    for (int r = 0; r < nur; ++r)
+                    for (int r = 0; r < nur && r < 3; ++r)
                         dg.urun_pack |= (uint64_t)(dg.uruns[r].lpos | (dg.uruns[r].len << 4) | (dg.uruns[r].shift << 8)) << (12 * r);
                 }
                 long dyn_end = -1;
