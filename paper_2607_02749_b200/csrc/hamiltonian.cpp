@@ -167,6 +167,22 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 return false;
             }
             std::sort(mine.begin(), mine.end());
+            {   // spare tile bits: prefer the qubits the pass's terms act on with Z (their sign then is part of the
+                // tile-independent table instead of a per-tile correction), most frequent first
+                std::vector<std::pair<long, int>> freq;
+                for (int q = f; q < n; ++q) {
+                    if (Thi >> q & 1) continue;
+                    long cnt = 0;
+                    for (int g : mine) for (int t : gterms[g]) cnt += (long)(H.terms[t].z >> q & 1);
+                    if (cnt) freq.push_back({-cnt, q});
+                }
+                std::sort(freq.begin(), freq.end());
+                for (auto &fq : freq) {
+                    if (__builtin_popcountll(Thi) >= h) break;
+                    const uint64_t cand = Thi | (1ull << fq.second);
+                    if (runs_of(fill_bits(cand, n, f, h) | low, tmp, MAX_RUNS) <= MAX_RUNS) Thi = cand;
+                }
+            }
             passT.push_back(fill_bits(Thi, n, f, h) | low);
             passG.push_back(mine);
         }

@@ -240,12 +240,26 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
 }
 
 // ---- second-stage deterministic reduction ------------------------------------------------------
-__global__ void __launch_bounds__(256) reduce_kernel(const double *__restrict__ partial, uint32_t slots_per_b, double *E)
+// Large slot counts (one statevector of 2^32 amplitudes has 2^19 tiles per pass) are summed in two steps: slice c of a
+// row is reduced into the first element of that slice, then the slice heads are summed.  Fixed order: deterministic.
+__global__ void __launch_bounds__(256) reduce_slices_kernel(double *partial, uint32_t slots_per_b, uint32_t slice_len)
+{
+    __shared__ double red[32];
+    double *p = partial + (uint64_t)blockIdx.y * slots_per_b + (uint64_t)blockIdx.x * slice_len;
+    const uint32_t n = min(slice_len, slots_per_b - blockIdx.x * slice_len);
+    double v = 0.0;
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) v += p[i];
+    const double s = block_sum(v, red);   // contains the barrier that orders every read before the write below
+    if (threadIdx.x == 0) p[0] = s;
+}
+
+__global__ void __launch_bounds__(256) reduce_kernel(const double *__restrict__ partial, uint32_t slots_per_b, uint32_t stride,
+                                                     double *E)
 {
     __shared__ double red[32];
     const double *p = partial + (uint64_t)blockIdx.x * slots_per_b;
     double v = 0.0;
-    for (uint32_t i = threadIdx.x; i < slots_per_b; i += blockDim.x) v += p[i];
+    for (uint32_t i = threadIdx.x * stride; i < slots_per_b; i += blockDim.x * stride) v += p[i];
     const double s = block_sum(v, red);
     if (threadIdx.x == 0) E[blockIdx.x] = s;
 }
@@ -406,9 +420,16 @@ int launch_expect_pass(int prec, const DPass *passes, int pi, int k, int n, cons
                                            slot_off, batch, st);
 }
 
-int launch_reduce(const double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches)
+int launch_reduce(double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches)
 {
-    reduce_kernel<<<batch, 256, 0, (cudaStream_t)stream>>>(partial, slots_per_b, E);
+    uint32_t stride = 1;
+    if (slots_per_b > (1u << 16)) {   // two steps
+        stride = 4096;
+        dim3 grid((slots_per_b + stride - 1) / stride, (unsigned)batch);
+        reduce_slices_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(partial, slots_per_b, stride);
+        ++*launches;
+    }
+    reduce_kernel<<<batch, 256, 0, (cudaStream_t)stream>>>(partial, slots_per_b, stride, E);
     ++*launches;
     return (int)cudaGetLastError();
 }

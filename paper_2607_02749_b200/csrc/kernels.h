@@ -37,7 +37,7 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &block,
 int launch_expect_pass(int prec, const DPass *passes, int pass_index, int k, int n, const DGroup *groups,
                        const DTerm *terms, const void *wstat, const uint32_t *gtabs, const DRs *rss, const void *states, uint64_t stride_amps, const void *table, double *partial,
                        uint32_t slots_per_b, uint32_t slot_off, int batch, void *stream, uint64_t *launches);
-int launch_reduce(const double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches);
+int launch_reduce(double *partial, uint32_t slots_per_b, double *E, int batch, void *stream, uint64_t *launches);
 int launch_table_scatter(int prec, void *table, const uint64_t *z, const double *c, uint32_t count, void *stream,
                          uint64_t *launches);
 int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches);
