@@ -202,9 +202,18 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
             }
         }
         __syncthreads();
-        for (uint32_t gi = g; gi <= ge; ++gi) {   // tile-dependent terms (z bits outside the tile) on top
+        // tile-dependent terms (z bits outside the tile) on top: small tables one warp per group (different groups
+        // concurrently), large tables with the whole block
+        for (uint32_t gi = g + (tid >> 5); gi <= ge; gi += (nthr >> 5)) {
             const DGroup *pg = sgr + (gi - g);
-            if (!(pg->hot >> 63)) continue;
+            if (!(pg->hot >> 63) || pg->ubits > 6) continue;
+            const uint32_t tb = pg->term_begin, de = pg->dyn_end, to = pg->tab_off, ne = 1u << pg->ubits;
+            for (uint32_t u = tid & 31u; u < ne; u += 32u)
+                tab[to + u] = group_table_entry<T>(tb, de, terms, xbase, u, tab[to + u]);
+        }
+        for (uint32_t gi = g; gi <= ge; ++gi) {
+            const DGroup *pg = sgr + (gi - g);
+            if (!(pg->hot >> 63) || pg->ubits <= 6) continue;
             const uint32_t tb = pg->term_begin, de = pg->dyn_end, to = pg->tab_off, ne = 1u << pg->ubits;
             for (uint32_t u = tid; u < ne; u += nthr)
                 tab[to + u] = group_table_entry<T>(tb, de, terms, xbase, u, tab[to + u]);
