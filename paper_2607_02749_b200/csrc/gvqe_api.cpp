@@ -31,7 +31,7 @@ int env_int(const char *name, int dflt)
 
 struct gvqe_ctx {
     int n_user = 0, n_store = 0, prec = 0, P = 0;
-    int K = 0, F = 0, R = 0;
+    int K = 0, F = 0, R = 0, KE = 0;   // KE: tile bits of the expectation passes
     std::vector<HostOp> ops;
     Program prog;
     DevProgram dev;
@@ -95,6 +95,8 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
     c->F = env_int("GVQE_F", prec == GVQE_C64 ? 4 : 3);
     c->R = env_int("GVQE_R", prec == GVQE_C64 ? 5 : 4);
     if (c->K > c->n_store) c->K = c->n_store;
+    c->KE = env_int("GVQE_KE", c->K > (prec == GVQE_C64 ? 13 : 12) ? (prec == GVQE_C64 ? 13 : 12) : c->K);
+    if (c->KE > c->n_store) c->KE = c->n_store;
     if (c->K < c->R + 5 || c->K > 14 || c->F < 1 || c->F >= c->K || c->K - c->R > 9) { delete c; return GVQE_ERR_INVALID_ARG; }
     std::string err;
     // Two candidate schedules: everything through the fused blocks (first block write-only), or the product-state
@@ -169,7 +171,7 @@ int gvqe_num_qubits(const gvqe_ctx *c) { return c ? c->n_user : -1; }
 static gvqe_status after_hamiltonian(gvqe_ctx *c)
 {
     std::string err;
-    if (!plan_expectation(c->H, c->n_store, c->K, c->F, EXPECT_UMAX, EXPECT_TAB_CAP, (int)c->amp_bytes(), c->plan, err)) {
+    if (!plan_expectation(c->H, c->n_store, c->KE, c->F, EXPECT_UMAX, EXPECT_TAB_CAP, (int)c->amp_bytes(), c->plan, err)) {
         c->have_h = false;
         return fail(c, GVQE_ERR_UNSUPPORTED, err);
     }

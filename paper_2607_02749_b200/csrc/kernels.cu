@@ -330,6 +330,7 @@ int kernels_init(void)
     const int big = 200 * 1024;
     int e = 0;
     e |= set_smem(gate_block_kernel<float, 5, 256>, big);
+    e |= set_smem(gate_block_kernel<float, 5, 512>, big);
     e |= set_smem(gate_block_kernel<float, 4, 256>, big);
     e |= set_smem(gate_block_kernel<float, 4, 512>, big);
     e |= set_smem(gate_block_kernel<float, 3, 512>, big);
@@ -380,6 +381,7 @@ int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &bi, in
     ++*launches;
     if (prec == 0) {
         if (R == 5 && thr <= 256) return gate_launch_t<float, 5, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
+        if (R == 5 && thr <= 512) return gate_launch_t<float, 5, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
         if (R == 4 && thr <= 256) return gate_launch_t<float, 4, 256>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
         if (R == 4 && thr <= 512) return gate_launch_t<float, 4, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
         if (R == 3 && thr <= 512) return gate_launch_t<float, 3, 512>(g, bi, k, smem_prog, n, states, stride, cs, P, batch, st);
