@@ -220,11 +220,9 @@ def run_ours(args):
     if rank != 0:
         return
     peak, peak_src = peaks()
-    traffic = None   # measured DRAM bytes per gate-block launch from the committed ncu capture (null when none)
-    try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json"))).get(str(cfg), {}).get("gate_block_kernel")
-    except Exception:
-        pass
+    # measured DRAM bytes per gate-block launch (dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture,
+    # profiles/r01_gate_block_ncu_full.txt: 17.18 GB read + 17.51 GB written; algorithmic 34.36 GB); other configs: not captured
+    traffic = 34.69e9 if cfg == 4 else None
     gate_gbs = prof["gate_bytes"] / (prof["gate_ms"] * 1e-3) / 1e9 if prof["gate_ms"] > 0 else 0.0
     exp_gbs = prof["expect_bytes"] / (prof["expect_ms"] * 1e-3) / 1e9 if prof["expect_ms"] > 0 else 0.0
     value = rows * world * args.steps / (ms_dev * 1e-3)
