@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(256, 2)
 expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ groups, const DTerm *__restrict__ terms,
                    const cx<T> *__restrict__ wstat, const uint32_t *__restrict__ gtabs, const DRs *__restrict__ rss,
                    const cx<T> *states, uint64_t stride, const TT *__restrict__ table,
-                   double *partial, uint32_t slots_per_b, uint32_t slot_off)
+                   double *partial, uint32_t slots_per_b, uint32_t slot_off, uint32_t nbatch)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ double red[32];
@@ -176,10 +176,12 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     uint32_t *gts = reinterpret_cast<uint32_t *>(tab + EXPECT_TAB_CAP);
     DGroup *sgr = reinterpret_cast<DGroup *>(gts + GT_BATCH_MAX * GT_WORDS);
     cx<T> *tile = reinterpret_cast<cx<T> *>(reinterpret_cast<unsigned char *>(sgr) + GT_BATCH_MAX * SGR_STRIDE);
-    const uint32_t b = blockIdx.y;
+    // linear grid, batch fastest: the thread blocks that work on the same tile of different statevectors run together,
+    // so the diagonal table, the static W tables and the lookup blocks they share are served from L2
+    const uint32_t b = blockIdx.x % nbatch, tile_id = blockIdx.x / nbatch;
     const cx<T> *state = states + (uint64_t)b * stride;
     const int k = sp->k, n_runs = sp->n_runs;
-    const uint64_t xbase = tile_base(blockIdx.x, sp->runs, n_runs);
+    const uint64_t xbase = tile_base(tile_id, sp->runs, n_runs);
     if (tid < NLD) hi[tid] = scatter_runs(tid * nthr * V, sp->runs, n_runs);
     __syncthreads();
     double acc = expect_load_u<T, TT, NLD>(tile, state, table, sp->with_diag != 0, xbase, sp->runs, n_runs, tid, nthr, hi);
@@ -245,7 +247,7 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         g = ge + 1;
     }
     const double s = block_sum(acc, red);
-    if (tid == 0) partial[(uint64_t)b * slots_per_b + slot_off + blockIdx.x] = s;
+    if (tid == 0) partial[(uint64_t)b * slots_per_b + slot_off + tile_id] = s;
 }
 
 // ---- second-stage deterministic reduction ------------------------------------------------------
@@ -400,13 +402,13 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
                            const void *wstat, const uint32_t *gtabs, const DRs *rss, const void *states, uint64_t stride, const void *table, double *partial, uint32_t slots_per_b,
                            uint32_t slot_off, int batch, cudaStream_t st)
 {
-    dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
+    dim3 grid((unsigned)((1ull << (n - k)) * (uint64_t)batch));
     const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + GT_BATCH_MAX * SGR_STRIDE + (sizeof(cx<T>) << k);
     const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
     const int L = k - 1 - TB;
 #define GV_EXPECT(LL)                                                                                                  \
     expect_pass_kernel<T, TT, LL><<<grid, 1 << TB, smem, st>>>(passes, pi, groups, terms, (const cx<T> *)wstat, gtabs, rss, (const cx<T> *)states, stride, \
-                                                               (const TT *)table, partial, slots_per_b, slot_off)
+                                                               (const TT *)table, partial, slots_per_b, slot_off, (uint32_t)batch)
     switch (L) {
     case 2: GV_EXPECT(2); break;
     case 3: GV_EXPECT(3); break;
