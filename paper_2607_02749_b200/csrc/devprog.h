@@ -84,7 +84,11 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t lead_cx;        // 1: stage 0 is nothing but a CNOT run; it is applied while the tile is written to shared
                              // memory after the load (permuted addresses) and skipped in the stage loop
     uint32_t e1_cx;          // swizzled image of local index 1 under that run (second amplitude of a 16-byte vector)
-    uint32_t hip_cx[16];     // swizzled images of i * threads * V under that run (linear part) (program + phase tables)
+    uint32_t hip_cx[16];     // swizzled images of i * threads * V under that run (linear part)
+    uint32_t n_lead_cx;      // entries of lead_cxs (0 when the run is longer than the inline array: read from global)
+    DCx lead_cxs[32];        // the leading CNOT run inline: as a kernel parameter it costs no global-load latency
+    uint32_t n_cs_inline;    // entries of cs_inline (0: too many, read csidx from global)
+    int32_t cs_inline[64];   // parameter index of each (cos,sin) slot, inline for the same reason (program + phase tables)
 };
 
 // ---- Hamiltonian engine -----------------------------------------------------------------------------------

@@ -114,9 +114,12 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
     else if (sb->lead_cx) {
-        const DStage *s0 = da.stages + sb->stage_off;   // read from global: the shared-memory copy is not visible yet
-        tile_commit_cx<T, NLD>(tile, ld, tid, xbase, da.cxs + sb->cx_off + s0->cx_begin, (uint32_t)(s0->cx_end - s0->cx_begin),
-                               sb->hip_cx, sb->e1_cx);
+        if (sb->n_lead_cx) tile_commit_cx<T, NLD>(tile, ld, tid, xbase, sb->lead_cxs, sb->n_lead_cx, sb->hip_cx, sb->e1_cx);
+        else {
+            const DStage *s0 = da.stages + sb->stage_off;   // read from global: the shared-memory copy is not visible yet
+            tile_commit_cx<T, NLD>(tile, ld, tid, xbase, da.cxs + sb->cx_off + s0->cx_begin,
+                                   (uint32_t)(s0->cx_end - s0->cx_begin), sb->hip_cx, sb->e1_cx);
+        }
     } else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
     __syncthreads();   // program slice and tile visible
     for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)

@@ -95,7 +95,11 @@ template <typename T>
 GV_DEV void gate_prologue(ProgView<T> &pv, const DBlock &b, const DevArrays &da, const cx<T> *cs_row, uint32_t tid,
                           uint32_t nthr)
 {
-    for (uint32_t i = tid; i < b.n_cs; i += nthr) pv.cs[i] = cs_row[da.csidx[b.cs_off + i]];
+    if (b.n_cs_inline == b.n_cs) {   // indices from the kernel parameter: one global-load latency instead of two
+        for (uint32_t i = tid; i < b.n_cs; i += nthr) pv.cs[i] = cs_row[b.cs_inline[i]];
+    } else {
+        for (uint32_t i = tid; i < b.n_cs; i += nthr) pv.cs[i] = cs_row[da.csidx[b.cs_off + i]];
+    }
     for (uint32_t i = tid; i < b.n_tcz; i += nthr) pv.tcz[i] = da.tczs[b.tcz_off + i];
     for (uint32_t i = tid; i < b.n_segs; i += nthr) pv.segs[i] = da.segs[b.seg_off + i];
     for (uint32_t i = tid; i < b.n_stages; i += nthr) pv.stages[i] = da.stages[b.stage_off + i];

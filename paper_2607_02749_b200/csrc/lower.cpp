@@ -186,6 +186,10 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                     };
                     const uint32_t V = 16u / (uint32_t)scs_bytes, nthr = 1u << (B.k - p.R), nld = (1u << p.R) / V;
                     db.lead_cx = 1;
+                    if (s0.cx_end - s0.cx_begin <= 32) {
+                        db.n_lead_cx = s0.cx_end - s0.cx_begin;
+                        for (uint32_t ci = 0; ci < db.n_lead_cx; ++ci) db.lead_cxs[ci] = D.cxs[db.cx_off + s0.cx_begin + ci];
+                    }
                     db.e1_cx = hphys(alin(1u));
                     for (uint32_t i = 0; i < nld && i < 16; ++i) db.hip_cx[i] = hphys(alin(i * nthr * V));
                 }
@@ -231,6 +235,10 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
             db.n_cs = (uint32_t)cs_local.size();
             db.n_ryl = (uint32_t)(D.ryl.size() - db.ryl_off); db.n_cx = (uint32_t)(D.cxs.size() - db.cx_off);
             for (int32_t v : cs_local) D.csidx.push_back(v);
+            if (cs_local.size() <= 64) {
+                db.n_cs_inline = (uint32_t)cs_local.size();
+                for (size_t ci = 0; ci < cs_local.size(); ++ci) db.cs_inline[ci] = cs_local[ci];
+            }
             {
                 uint32_t o = al16(db.n_cs * (uint32_t)scs_bytes);
                 db.off_tcz = o; o += al16(db.n_tcz * 8u);
