@@ -21,7 +21,8 @@ struct DOp {                 // 8 bytes; one register-level micro-op of a stage
     int32_t idx;             // RYL: offset into the block's ryl array (DEV_MAX_R entries); DIAG: segment index
 };
 
-constexpr int TPH_ENTRIES = 16 + 32;   // thread-phase tables of a segment: [0,16) over thread-index bits 0..3 (and all
+constexpr int TPH_CONST = 48;           // entry holding the product of the tile-constant RZ factors
+constexpr int TPH_ENTRIES = 16 + 32 + 16;   // thread-phase tables of a segment: [0,16) over thread-index bits 0..3 (and all
                                        // tile-constant factors), [16,48) over thread-index bits 4..8
 enum : uint8_t { TB_CONST = 254, TB_XREG = 200 };   // DTrz.tb: tile-constant qubit / TB_XREG + s: further RZ on slot s
 enum : int { TCZ_LO = 0, TCZ_HI = 1, TCZ_CROSS = 2, TCZ_CLASS_SHIFT = 62 };   // class of a thread-level CZ pair
@@ -77,6 +78,7 @@ struct DBlock {              // one HBM round trip over every statevector in fli
     uint32_t smem_prog_bytes;                                         // shared memory the slice needs (program + phase tables)
     uint32_t tph_off;                                                 // byte offset of the thread-phase tables in the slice
     uint32_t slut_off;       // byte offset of the per-stage thread lookups (SLUT_ENTRIES x (u32 + u64) per stage)
+    uint32_t slut_goff;      // byte offset of their host-built image in the device slut array
     uint32_t off_tcz, off_segs, off_stages, off_ops, off_trz, off_cxs, off_ryl;   // byte offsets of the slice parts (cs = 0)
     uint32_t pad3;
     uint64_t hi[16];         // global offsets of the 16-byte vectors a thread moves: hi[i] = scatter(i * threads * V)

@@ -251,7 +251,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -270,6 +270,7 @@ Layout layout_of(const gvqe_ctx *c)
     L.csidx = cv.take(d.csidx.size() * 4);
     L.ryl = cv.take(d.ryl.size() * 2);
     L.cxs = cv.take(d.cxs.size() * sizeof(DCx));
+    L.slut = cv.take(d.slut.size() * 4);
     L.px_begin = cv.take(c->px.rot_begin.size() * 4); L.px_kind = cv.take(c->px.rot_kind.size());
     L.px_param = cv.take(c->px.rot_param.size() * 4); L.px_t = cv.take(c->px.cx_t.size()); L.px_c = cv.take(c->px.cx_c.size());
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
@@ -330,6 +331,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.trzs = (const DTrz *)(w + L.trzs); c->gl.tczs = (const uint64_t *)(w + L.tczs);
     c->gl.csidx = (const int32_t *)(w + L.csidx);
     c->gl.ryl = (const int16_t *)(w + L.ryl); c->gl.cxs = (const DCx *)(w + L.cxs);
+    c->gl.slut = (const uint32_t *)(w + L.slut);
     c->pxd.rot_begin = (const int32_t *)(w + L.px_begin); c->pxd.rot_kind = (const uint8_t *)(w + L.px_kind);
     c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
     c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
@@ -348,7 +350,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     gvqe_status s;
 #define UP(dst, vec) if ((s = upload(c, (void *)(dst), (vec).data(), (vec).size() * sizeof((vec)[0]), st)) != GVQE_OK) return s
     UP(c->gl.blocks, d.blocks); UP(c->gl.stages, d.stages); UP(c->gl.ops, d.ops); UP(c->gl.segs, d.segs);
-    UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx); UP(c->gl.ryl, d.ryl); UP(c->gl.cxs, d.cxs);
+    UP(c->gl.trzs, d.trzs); UP(c->gl.tczs, d.tczs); UP(c->gl.csidx, d.csidx); UP(c->gl.ryl, d.ryl); UP(c->gl.cxs, d.cxs); UP(c->gl.slut, d.slut);
     UP(c->pxd.rot_begin, c->px.rot_begin); UP(c->pxd.rot_kind, c->px.rot_kind); UP(c->pxd.rot_param, c->px.rot_param);
     UP(c->pxd.cx_t, c->px.cx_t); UP(c->pxd.cx_c, c->px.cx_c);
     UP(c->d_passes, c->plan.passes); UP(c->d_groups, c->plan.groups); UP(c->d_terms, c->plan.terms);

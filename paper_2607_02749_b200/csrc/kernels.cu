@@ -122,10 +122,20 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
         }
     } else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
     __syncthreads();   // program slice and tile visible
-    for (uint32_t item = tid; item < sb->n_segs * TPH_ENTRIES; item += nthr)
+    for (uint32_t item = tid; item < sb->n_segs * TPH_CONST; item += nthr)
         tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
-    for (uint32_t item = tid; item < (uint32_t)sb->n_stages * SLUT_ENTRIES; item += nthr)
-        slut_build_entry<T, R>(pv, item, sb->runs, n_runs, k);
+    for (uint32_t sgi = tid >> 5; sgi < sb->n_segs; sgi += nthr >> 5) {   // tile-constant factors: one warp per segment
+        const DSeg &sg = pv.segs[sgi];
+        cx<T> pr{T(1), T(0)};
+        for (uint32_t t = sg.trz_begin + sg.n_xreg + (tid & 31u); t < sg.trz_end; t += 32u) pr = cmul(pr, tph_const_factor<T>(pv, t, xbase));
+        for (int o = 16; o > 0; o >>= 1) {
+            cx<T> other;
+            other.x = __shfl_xor_sync(0xffffffffu, pr.x, o);
+            other.y = __shfl_xor_sync(0xffffffffu, pr.y, o);
+            pr = cmul(pr, other);
+        }
+        if ((tid & 31u) == 0) pv.tph[sgi * TPH_ENTRIES + TPH_CONST] = pr;
+    }
     if (zero && tid == 0) tile[0] = cx<T>{T(1), T(0)};
     __syncthreads();
     const int ns = sb->n_stages;
@@ -316,7 +326,7 @@ template <typename T, int R, int MAXT>
 int gate_launch_t(const GateLaunch &g, const DBlock &blk, int k, uint32_t smem_prog, int n, void *states, uint64_t stride,
                   const void *cs, int P, int batch, cudaStream_t st)
 {
-    DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx, g.ryl, g.cxs};
+    DevArrays da{g.blocks, g.stages, g.ops, g.segs, g.trzs, g.tczs, g.csidx, g.ryl, g.cxs, g.slut};
     const size_t smem = HDR_BYTES + smem_prog + ((size_t)sizeof(cx<T>) << k);
     dim3 grid((unsigned)(1ull << (n - k)), (unsigned)batch);
     gate_block_kernel<T, R, MAXT><<<grid, 1u << (k - R), smem, st>>>(da, blk, (cx<T> *)states, stride, (const cx<T> *)cs, P);

@@ -67,7 +67,7 @@ GV_DEV uint32_t insert_zero(uint32_t i, uint32_t pos) { return ((i >> pos) << (p
 
 struct DevArrays {
     const DBlock *blocks; const DStage *stages; const DOp *ops; const DSeg *segs; const DTrz *trzs;
-    const uint64_t *tczs; const int32_t *csidx; const int16_t *ryl; const DCx *cxs;
+    const uint64_t *tczs; const int32_t *csidx; const int16_t *ryl; const DCx *cxs; const uint32_t *slut;
 };
 
 GV_DEV uint32_t al16u(uint32_t v) { return (v + 15u) & ~15u; }
@@ -107,6 +107,11 @@ GV_DEV void gate_prologue(ProgView<T> &pv, const DBlock &b, const DevArrays &da,
     for (uint32_t i = tid; i < b.n_trz; i += nthr) pv.trz[i] = da.trzs[b.trz_off + i];
     for (uint32_t i = tid; i < b.n_cx; i += nthr) pv.cxs[i] = da.cxs[b.cx_off + i];
     for (uint32_t i = tid; i < b.n_ryl; i += nthr) pv.ryl[i] = da.ryl[b.ryl_off + i];
+    {   // host-built per-stage thread lookups
+        uint32_t *dst = reinterpret_cast<uint32_t *>(pv.slut);
+        const uint32_t *src = da.slut + b.slut_goff / 4;
+        for (uint32_t i = tid; i < (uint32_t)b.n_stages * SLUT_ENTRIES * 3u; i += nthr) dst[i] = src[i];
+    }
 }
 
 // ---- tile <-> global -------------------------------------------------------------------------------------
@@ -250,7 +255,7 @@ template <> GV_DEV cx<float> cmul_w<float>(cx<float> a, cx<float> w, cx<float> w
 template <typename T, int R>
 GV_DEV void tph_build_entry(const ProgView<T> &pv, uint32_t item, uint64_t xbase, const Run *runs, int n_runs, int k)
 {
-    const uint32_t sgi = item / TPH_ENTRIES, e = item % TPH_ENTRIES;
+    const uint32_t sgi = item / TPH_CONST, e = item % TPH_CONST;   // items cover the 48 thread entries of every segment
     const DSeg &sg = pv.segs[sgi];
     const DStage &st = pv.stages[sg.stage];
     const bool high = e >= 16;
@@ -262,7 +267,7 @@ GV_DEV void tph_build_entry(const ProgView<T> &pv, uint32_t item, uint64_t xbase
     cx<T> ph{T(1), T(0)};
     for (uint32_t t = sg.trz_begin + sg.n_xreg; t < sg.trz_end; ++t) {
         const DTrz z = pv.trz[t];
-        const bool mine = high ? (z.tb >= 4 && z.tb < TB_XREG) : (z.tb < 4 || z.tb == TB_CONST);
+        const bool mine = high ? (z.tb >= 4 && z.tb < TB_XREG) : (z.tb < 4);   // tile-constant factors: tph_const_factor
         if (!mine) continue;
         const cx<T> cs = pv.cs[z.cs];
         const bool bit = (x >> z.qubit) & 1ull;
@@ -275,7 +280,18 @@ GV_DEV void tph_build_entry(const ProgView<T> &pv, uint32_t item, uint64_t xbase
         const uint64_t mm = m & ((1ull << TCZ_CLASS_SHIFT) - 1ull);
         par ^= ((x & mm) == mm) ? 1u : 0u;
     }
-    pv.tph[item] = par ? cneg(ph) : ph;
+    pv.tph[sgi * TPH_ENTRIES + e] = par ? cneg(ph) : ph;
+}
+
+// Factor of one tile-constant R_z of a segment (identity for the others); their product goes to entry TPH_CONST.
+template <typename T>
+GV_DEV cx<T> tph_const_factor(const ProgView<T> &pv, uint32_t trz_index, uint64_t xbase)
+{
+    const DTrz z = pv.trz[trz_index];
+    if (z.tb != TB_CONST) return cx<T>{T(1), T(0)};
+    const cx<T> cs = pv.cs[z.cs];
+    const bool bit = (xbase >> z.qubit) & 1ull;
+    return cx<T>{cs.x, bit ? cs.y : -cs.y};
 }
 
 // Merged diagonal segment: every R_z phase (Eq. 7) and every CZ sign of the segment as ONE complex factor per
@@ -284,7 +300,8 @@ template <typename T, int R>
 GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint32_t sgi, uint64_t x, uint32_t tid)
 {
     constexpr int RL = R / 2, RH = R - RL;
-    cx<T> ph = cmul(pv.tph[sgi * TPH_ENTRIES + (tid & 15u)], pv.tph[sgi * TPH_ENTRIES + 16u + (tid >> 4)]);
+    cx<T> ph = cmul(cmul(pv.tph[sgi * TPH_ENTRIES + (tid & 15u)], pv.tph[sgi * TPH_ENTRIES + 16u + (tid >> 4)]),
+                    pv.tph[sgi * TPH_ENTRIES + TPH_CONST]);
     cx<T> F0[R], F1[R];
     GV_UNROLL
     for (int s = 0; s < R; ++s) {
@@ -340,23 +357,9 @@ GV_DEV void diag_apply(cx<T> *a, const ProgView<T> &pv, const DSeg &sg, uint32_t
     }
 }
 
-// Per-stage thread lookups (one entry per call; built once per thread block): the thread's local index j (register
-// bits zero), its swizzled byte offset and its global index are GF(2)-linear in the thread index, so each is the XOR / OR
-// of a low-bits entry and a high-bits entry.  u32 entry = j | swizzled element offset << 16; u64 entry = scatter(j).
-template <typename T, int R>
-GV_DEV void slut_build_entry(const ProgView<T> &pv, uint32_t item, const Run *runs, int n_runs, int k)
-{
-    const uint32_t si = item / SLUT_ENTRIES, e = item % SLUT_ENTRIES;
-    const DStage &st = pv.stages[si];
-    uint32_t j = e >= 16 ? ((e - 16u) << 4) : e;
-    if (j >> (k - R)) return;
-    GV_UNROLL
-    for (int s = 0; s < R; ++s) j = insert_zero(j, st.regbit[s]);
-    uint32_t *w32 = reinterpret_cast<uint32_t *>(pv.slut + (size_t)si * SLUT_ENTRIES * 12u);
-    uint64_t *w64 = reinterpret_cast<uint64_t *>(w32 + SLUT_ENTRIES);
-    w32[e] = j | (phys<T>(j) << 16);
-    w64[e] = scatter_runs(j, runs, n_runs);
-}
+// Per-stage thread lookups (host-built, lower.cpp): the thread's local index j (register bits zero), its swizzled
+// offset and its global index are GF(2)-linear in the thread index, so each is the XOR / OR of a low-bits entry and a
+// high-bits entry.  u32 entry = j | swizzled element offset << 16; u64 entry = scatter(j).
 
 // One stage: 2^R amplitudes per thread in registers, all micro-ops of the stage, back to shared memory.
 // Returns true when the stage ends with a CNOT run: the amplitudes then stay in a[] and must be written by

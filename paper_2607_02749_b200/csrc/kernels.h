@@ -12,7 +12,7 @@ struct TileDesc { uint8_t k, n_runs, pad[2]; Run runs[MAX_RUNS]; };
 
 struct GateLaunch {
     const DBlock *blocks; const DStage *stages; const DOp *ops; const DSeg *segs; const DTrz *trzs;
-    const uint64_t *tczs; const int32_t *csidx; const int16_t *ryl; const DCx *cxs;
+    const uint64_t *tczs; const int32_t *csidx; const int16_t *ryl; const DCx *cxs; const uint32_t *slut;
 };
 
 constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area

@@ -172,6 +172,27 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                 ++n_stages; ++si;
             }
             db.n_stages = (uint8_t)n_stages;
+            {   // per-stage thread lookups: thread index -> local index j (register bits zero) | swizzled element offset << 16,
+                // and -> global index; each GF(2)-linear in the thread index, stored for its low 4 bits and its high bits
+                const int FB = scs_bytes == 8 ? 4 : 3;
+                auto hphys = [FB](uint32_t j) { uint32_t ph = j; for (int sh = FB; sh < 16; sh += FB) ph ^= (j >> sh) & ((1u << FB) - 1u); return ph; };
+                db.slut_goff = (uint32_t)(D.slut.size() * 4);
+                for (uint32_t si2 = 0; si2 < n_stages; ++si2) {
+                    const DStage &st = D.stages[db.stage_off + si2];
+                    uint32_t w32[SLUT_ENTRIES]; uint64_t w64[SLUT_ENTRIES];
+                    for (int e = 0; e < SLUT_ENTRIES; ++e) {
+                        uint32_t j = e >= 16 ? ((uint32_t)(e - 16) << 4) : (uint32_t)e;
+                        w32[e] = 0; w64[e] = 0;
+                        if (j >> (B.k - p.R)) continue;
+                        for (int s2 = 0; s2 < p.R; ++s2) { const uint32_t pos = st.regbit[s2]; j = ((j >> pos) << (pos + 1)) | (j & ((1u << pos) - 1u)); }
+                        uint64_t x = 0;
+                        for (int r = 0; r < B.n_runs; ++r) x |= (uint64_t)((j >> B.runs[r].lpos) & ((1u << B.runs[r].len) - 1u)) << B.runs[r].gpos;
+                        w32[e] = j | (hphys(j) << 16); w64[e] = x;
+                    }
+                    for (int e = 0; e < SLUT_ENTRIES; ++e) D.slut.push_back(w32[e]);
+                    for (int e = 0; e < SLUT_ENTRIES; ++e) { D.slut.push_back((uint32_t)w64[e]); D.slut.push_back((uint32_t)(w64[e] >> 32)); }
+                }
+            }
             if (n_stages > 1) {   // a leading stage that is only a CNOT run is folded into the tile load
                 const DStage &s0 = D.stages[db.stage_off];
                 if (s0.op_begin == s0.op_end && s0.has_cx && !db.source_zero) {

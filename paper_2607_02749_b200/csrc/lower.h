@@ -19,6 +19,7 @@ struct DevProgram {
     std::vector<int32_t> csidx;   // block-local (cos,sin) slot -> parameter index
     std::vector<int16_t> ryl;     // RY layers: DEV_MAX_R block-local (cos,sin) slots each, -1 = no gate on the slot
     std::vector<DCx> cxs;         // trailing CNOT runs
+    std::vector<uint32_t> slut;   // per-stage thread lookups (devprog.h SLUT_ENTRIES): 48 u32 then 48 u64 per stage
     uint32_t max_smem_prog = 0;   // largest per-block program slice (bytes)
 };
 
