@@ -221,8 +221,8 @@ def run_ours(args):
         return
     peak, peak_src = peaks()
     # measured DRAM bytes per gate-block launch (dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture,
-    # profiles/r01_gate_block_ncu_full.txt: 17.18 GB read + 17.51 GB written; algorithmic 34.36 GB); other configs: not captured
-    traffic = 34.69e9 if cfg == 4 else None
+    # profiles/r01_gate_block_ncu_full.txt: 17.18 GB read + 17.18 GB written; algorithmic 34.36 GB); other configs: not captured
+    traffic = 34.37e9 if cfg == 4 else None
     gate_gbs = prof["gate_bytes"] / (prof["gate_ms"] * 1e-3) / 1e9 if prof["gate_ms"] > 0 else 0.0
     exp_gbs = prof["expect_bytes"] / (prof["expect_ms"] * 1e-3) / 1e9 if prof["expect_ms"] > 0 else 0.0
     value = rows * world * args.steps / (ms_dev * 1e-3)
