@@ -155,8 +155,12 @@ struct DPass {               // one read-only sweep over the state
     uint8_t k, n_runs, with_diag, pad;
     Run runs[MAX_RUNS];
     uint32_t group_begin, group_end;
-    uint32_t pad2[2];
+    uint32_t n_batches;      // <= PASS_MAX_BATCHES (longer passes are cut into several with the same tile bits)
+    uint32_t pad2;
     uint64_t hi[64];         // as DBlock::hi for the expectation kernel's thread count
+    struct Batch { uint32_t g_first, g_last, entries, wbase; } batch[12];   // groups [g_first, g_last], their table entries,
+                                                                            // offset of their static tables in the wstat array
 };
+constexpr int PASS_MAX_BATCHES = 12;
 
 }  // namespace gv

@@ -407,9 +407,29 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                     plan.wstat[2 * (base + dg.tab_off + u) + 1] = wi;
                 }
             }
+            if (dp.n_batches == PASS_MAX_BATCHES) {   // cut the pass: same tile bits, the groups so far
+                DPass done = dp;
+                done.group_end = g0;
+                plan.passes.push_back(done);
+                dp.group_begin = g0; dp.with_diag = 0; dp.n_batches = 0;
+            }
+            dp.batch[dp.n_batches].g_first = g0; dp.batch[dp.n_batches].g_last = g1;
+            dp.batch[dp.n_batches].entries = entries; dp.batch[dp.n_batches].wbase = (uint32_t)base;
+            ++dp.n_batches;
             g0 = g1 + 1;
         }
         plan.passes.push_back(dp);
+    }
+    {   // lookup blocks re-laid by group index (zero blocks for register-stage / direct groups): a batch's blocks are
+        // then one contiguous range, copied together with its descriptors and static tables
+        std::vector<uint32_t> gt2(plan.groups.size() * (size_t)GT_WORDS, 0u);
+        for (size_t gi = 0; gi < plan.groups.size(); ++gi) {
+            DGroup &dg = plan.groups[gi];
+            if (!dg.rs && !dg.direct)
+                memcpy(&gt2[gi * GT_WORDS], &plan.gtabs[(size_t)dg.gt_index * GT_WORDS], GT_WORDS * sizeof(uint32_t));
+            dg.gt_index = (uint32_t)gi;
+        }
+        plan.gtabs.swap(gt2);
     }
     return true;
 }

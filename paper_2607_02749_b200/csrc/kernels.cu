@@ -184,8 +184,9 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     __syncthreads();
     constexpr int V = 16 / (int)sizeof(cx<T>);
     constexpr int NLD = (2 << L) / V;
-    uint64_t *hi = reinterpret_cast<uint64_t *>(smem + 128);
-    cx<T> *tab = reinterpret_cast<cx<T> *>(smem + HDR_BYTES);
+    static_assert(sizeof(DPass) <= EXPECT_HDR_BYTES, "DPass must fit the shared-memory header");
+    const uint64_t *hi = sp->hi;   // host-built vector offsets
+    cx<T> *tab = reinterpret_cast<cx<T> *>(smem + EXPECT_HDR_BYTES);
     uint32_t *gts = reinterpret_cast<uint32_t *>(tab + EXPECT_TAB_CAP);
     DGroup *sgr = reinterpret_cast<DGroup *>(gts + GT_BATCH_MAX * GT_WORDS);
     cx<T> *tile = reinterpret_cast<cx<T> *>(reinterpret_cast<unsigned char *>(sgr) + GT_BATCH_MAX * SGR_STRIDE);
@@ -195,25 +196,24 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
     const cx<T> *state = states + (uint64_t)b * stride;
     const int k = sp->k, n_runs = sp->n_runs;
     const uint64_t xbase = tile_base(tile_id, sp->runs, n_runs);
-    if (tid < NLD) hi[tid] = scatter_runs(tid * nthr * V, sp->runs, n_runs);
-    __syncthreads();
     double acc = expect_load_u<T, TT, NLD>(tile, state, table, sp->with_diag != 0, xbase, sp->runs, n_runs, tid, nthr, hi);
     __syncthreads();
-    uint32_t g = sp->group_begin;
-    const uint32_t gend = sp->group_end;
-    while (g < gend) {
-        const uint32_t ge = groups[g].batch_last;
-        {   // the batch's group descriptors, static W tables and lookup blocks: flat coalesced copies into shared memory
+    for (uint32_t bi = 0; bi < sp->n_batches; ++bi) {
+        const uint32_t g = sp->batch[bi].g_first, ge = sp->batch[bi].g_last;
+        {   // the batch's group descriptors, static W tables and lookup blocks: three contiguous global ranges copied by
+            // ONE loop of independent 8-byte loads (a single round of L2 latency)
+            struct alignas(8) u2 { uint32_t a, b; };
             const uint32_t ng = ge - g + 1;
-            const uint32_t *gsrc = reinterpret_cast<const uint32_t *>(groups + g);
-            uint32_t *gdst = reinterpret_cast<uint32_t *>(sgr);
-            for (uint32_t e = tid; e < ng * (uint32_t)(sizeof(DGroup) / 4); e += nthr) gdst[e] = gsrc[e];
-            const uint32_t ne = groups[g].batch_entries;
-            const cx<T> *src = wstat + (groups[g].gtab_off - groups[g].tab_off);
-            for (uint32_t e = tid; e < ne; e += nthr) tab[e] = src[e];
-            for (uint32_t e = tid; e < ng * GT_WORDS; e += nthr) {
-                const DGroup *pg = groups + g + e / GT_WORDS;
-                if (!pg->direct && !pg->rs) gts[e] = gtabs[(uint64_t)pg->gt_index * GT_WORDS + (e % GT_WORDS)];
+            const uint32_t nd = ng * (uint32_t)(sizeof(DGroup) / 8), nt = sp->batch[bi].entries * (uint32_t)(sizeof(cx<T>) / 8),
+                           nl = ng * (GT_WORDS / 2);
+            const u2 *s_d = reinterpret_cast<const u2 *>(groups + g);
+            const u2 *s_t = reinterpret_cast<const u2 *>(wstat + sp->batch[bi].wbase);
+            const u2 *s_l = reinterpret_cast<const u2 *>(gtabs + (uint64_t)g * GT_WORDS);
+            u2 *d_d = reinterpret_cast<u2 *>(sgr), *d_t = reinterpret_cast<u2 *>(tab), *d_l = reinterpret_cast<u2 *>(gts);
+            for (uint32_t i = tid; i < nd + nt + nl; i += nthr) {
+                if (i < nd) d_d[i] = s_d[i];
+                else if (i < nd + nt) d_t[i - nd] = s_t[i - nd];
+                else d_l[i - nd - nt] = s_l[i - nd - nt];
             }
         }
         __syncthreads();
@@ -257,7 +257,6 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
             }
         }
         __syncthreads();
-        g = ge + 1;
     }
     const double s = block_sum(acc, red);
     if (tid == 0) partial[(uint64_t)b * slots_per_b + slot_off + tile_id] = s;
@@ -416,7 +415,7 @@ static int expect_launch_t(const DPass *passes, int pi, int k, int n, const DGro
                            uint32_t slot_off, int batch, cudaStream_t st)
 {
     dim3 grid((unsigned)((1ull << (n - k)) * (uint64_t)batch));
-    const size_t smem = HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + GT_BATCH_MAX * SGR_STRIDE + (sizeof(cx<T>) << k);
+    const size_t smem = EXPECT_HDR_BYTES + EXPECT_TAB_CAP * sizeof(cx<T>) + GT_BATCH_MAX * GT_WORDS * 4 + GT_BATCH_MAX * SGR_STRIDE + (sizeof(cx<T>) << k);
     const int TB = (k >= 11) ? 8 : (k - 3 < 5 ? 5 : k - 3);   // must match plan_expectation
     const int L = k - 1 - TB;
 #define GV_EXPECT(LL)                                                                                                  \

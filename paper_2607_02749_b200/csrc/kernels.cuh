@@ -551,7 +551,19 @@ GV_DEV cx<T> group_table_entry(uint32_t term_begin, uint32_t dyn_end, const DTer
                                cx<T> w0)
 {
     double wr = (double)w0.x, wi = (double)w0.y;   // static part (terms with no z bit outside the tile)
-    for (uint32_t t = term_begin; t < dyn_end; ++t) {
+    uint32_t t = term_begin;
+    for (; t + 4 <= dyn_end; t += 4) {   // four independent loads in flight
+        DTerm tm[4];
+        GV_UNROLL
+        for (int q = 0; q < 4; ++q) tm[q] = terms[t + q];
+        GV_UNROLL
+        for (int q = 0; q < 4; ++q) {
+            const int par = (gv_popcll(xbase & tm[q].zout) + gv_popc(u & tm[q].zu)) & 1;
+            wr += par ? -tm[q].cr : tm[q].cr;
+            wi += par ? -tm[q].ci : tm[q].ci;
+        }
+    }
+    for (; t < dyn_end; ++t) {
         const DTerm tm = terms[t];
         const int par = (gv_popcll(xbase & tm.zout) + gv_popc(u & tm.zu)) & 1;
         wr += par ? -tm.cr : tm.cr;

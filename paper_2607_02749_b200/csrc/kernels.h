@@ -17,7 +17,8 @@ struct GateLaunch {
 
 constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area
 constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
-constexpr uint32_t HDR_BYTES = 384;         // shared-memory header holding the DBlock / DPass copy
+constexpr uint32_t HDR_BYTES = 384;         // shared-memory header of the gate kernel
+constexpr uint32_t EXPECT_HDR_BYTES = 1024; // shared-memory header of the expectation kernel: holds the DPass copy
 
 struct PrefixDev {   // device view of schedule.h Prefix
     const int32_t *rot_begin; const uint8_t *rot_kind; const int32_t *rot_param;
