@@ -237,9 +237,11 @@ expect_pass_kernel(const DPass *passes, int pi, const DGroup *__restrict__ group
         int cur_rs = -1;
         constexpr int RSR = (L + 1 <= DEV_MAX_R) ? L + 1 : 1;   // the planner makes register stages only when L + 1 <= DEV_MAX_R
         cx<T> ra[1 << RSR];   // register stage: 2^(L+1) amplitudes per thread
+        uint64_t hot_next = sgr[0].hot;   // one group ahead: the shared-memory read overlaps the previous group's pairs
         for (uint32_t gi = g; gi <= ge; ++gi) {
             const DGroup *pg = sgr + (gi - g);
-            const uint64_t hot = pg->hot;
+            const uint64_t hot = hot_next;
+            if (gi < ge) hot_next = pg[1].hot;
             const uint32_t mode = (uint32_t)hot & 3u, tab_off = (uint32_t)(hot >> 24) & 0xFFFFFFu;
             if (mode == 1u) {
                 const int rs_id = (int)((hot >> 8) & 0xFFFFu);

@@ -481,6 +481,23 @@ GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32
         cmb[i] = q.a; cmb[i + 1] = q.b; cmb[i + 2] = q.c; cmb[i + 3] = q.d;
     }
     T tr = T(0), ti = T(0);
+#ifndef GVQE_EMU
+    if constexpr (sizeof(T) == 4) {
+        // packed: accA += b.x * (a.x, a.y), accB += b.y * (a.y, a.x); Re = accA.x + accB.x, Im = accA.y - accB.y
+        float2 accA = make_float2(0.f, 0.f), accB = make_float2(0.f, 0.f);
+        GV_UNROLL
+        for (int i = 0; i < (1 << L); ++i) {
+            const uint32_t ob = pjb ^ cmb[i];
+            const float2 a = *reinterpret_cast<const float2 *>(tile_bytes + ob);
+            const float2 b = *reinterpret_cast<const float2 *>(tile_bytes + (ob ^ pm_bytes));
+            accA = __ffma2_rn(make_float2(b.x, b.x), a, accA);
+            accB = __ffma2_rn(make_float2(b.y, b.y), make_float2(a.y, a.x), accB);
+        }
+        tr = accA.x + accB.x;
+        ti = accA.y - accB.y;
+        return 2.0 * (double)(w.x * tr - w.y * ti);
+    }
+#endif
     GV_UNROLL
     for (int i = 0; i < (1 << L); ++i) {
         const uint32_t ob = pjb ^ cmb[i];
@@ -500,6 +517,28 @@ template <> struct TopBit<0> { static constexpr int value = 0; };
 template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T> *w)
 {
     constexpr int PV = TopBit<M>::value;
+#ifndef GVQE_EMU
+    if constexpr (sizeof(T) == 4) {
+        // packed: accA += v.x * (w.x u.x, w.y u.y), accB += v.y * (w.x u.y, w.y u.x);
+        // Re(w conj(v) u) summed = (accA.x - accA.y) + (accB.x + accB.y).  Two chains each.
+        float2 accA[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        float2 accB[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
+        int n = 0;
+        GV_UNROLL
+        for (int r = 0; r < (1 << R); ++r) {
+            if (r & (1 << PV)) continue;
+            const float2 ww = make_float2(w[r].x, w[r].y), u = make_float2(a[r].x, a[r].y);
+            const cx<T> v = a[r ^ M];
+            const float2 g = __fmul2_rn(ww, u);
+            const float2 h = __fmul2_rn(ww, make_float2(u.y, u.x));
+            accA[n & 1] = __ffma2_rn(make_float2(v.x, v.x), g, accA[n & 1]);
+            accB[n & 1] = __ffma2_rn(make_float2(v.y, v.y), h, accB[n & 1]);
+            ++n;
+        }
+        const float2 sa = __fadd2_rn(accA[0], accA[1]), sb = __fadd2_rn(accB[0], accB[1]);
+        return (sa.x - sa.y) + (sb.x + sb.y);
+    }
+#endif
     T acc[4] = {T(0), T(0), T(0), T(0)};   // independent chains
     int n = 0;
     GV_UNROLL
@@ -515,7 +554,7 @@ template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T
     return (acc[0] + acc[1]) + (acc[2] + acc[3]);
 }
 
-// binary search over the flip mask (uniform branches): masks LO..HI
+// binary search over the flip mask (uniform branches): masks LO..HI  (an indexed branch measured slower)
 template <typename T, int R, int LO, int HI> struct RsDispatch {
     static GV_DEV T run(int m, const cx<T> *a, const cx<T> *w)
     {
