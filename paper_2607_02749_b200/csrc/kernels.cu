@@ -113,15 +113,7 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     }
     gate_prologue<T>(pv, *sb, da, cs_table + (uint64_t)b * P, tid, nthr);
     if (zero) tile_init_zero_state<T>(tile, k, tid, nthr);
-    else if (sb->lead_cx) {
-        if (sb->n_lead_cx) tile_commit_cx<T, NLD>(tile, ld, tid, xbase, sb->lead_cxs, sb->n_lead_cx, sb->hip_cx, sb->e1_cx);
-        else {
-            const DStage *s0 = da.stages + sb->stage_off;   // read from global: the shared-memory copy is not visible yet
-            tile_commit_cx<T, NLD>(tile, ld, tid, xbase, da.cxs + sb->cx_off + s0->cx_begin,
-                                   (uint32_t)(s0->cx_end - s0->cx_begin), sb->hip_cx, sb->e1_cx);
-        }
-    } else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
-    __syncthreads();   // program slice and tile visible
+    __syncthreads();   // program slice visible; the tile loads are still in flight and the phase tables are built under them
     for (uint32_t item = tid; item < sb->n_segs * TPH_CONST; item += nthr)
         tph_build_entry<T, R>(pv, item, xbase, sb->runs, n_runs, k);
     for (uint32_t sgi = tid >> 5; sgi < sb->n_segs; sgi += nthr >> 5) {   // tile-constant factors: one warp per segment
@@ -136,8 +128,17 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
         }
         if ((tid & 31u) == 0) pv.tph[sgi * TPH_ENTRIES + TPH_CONST] = pr;
     }
-    if (zero && tid == 0) tile[0] = cx<T>{T(1), T(0)};
-    __syncthreads();
+    if (zero) {
+        if (tid == 0) tile[0] = cx<T>{T(1), T(0)};
+    } else if (sb->lead_cx) {
+        if (sb->n_lead_cx) tile_commit_cx<T, NLD>(tile, ld, tid, xbase, sb->lead_cxs, sb->n_lead_cx, sb->hip_cx, sb->e1_cx);
+        else {
+            const DStage *s0 = da.stages + sb->stage_off;
+            tile_commit_cx<T, NLD>(tile, ld, tid, xbase, da.cxs + sb->cx_off + s0->cx_begin,
+                                   (uint32_t)(s0->cx_end - s0->cx_begin), sb->hip_cx, sb->e1_cx);
+        }
+    } else tile_commit<T, NLD>(tile, ld, tid, sb->hip);
+    __syncthreads();   // tile and phase tables visible
     const int ns = sb->n_stages;
     cx<T> amp[1 << R];
     uint32_t po[R], pj2 = 0;
