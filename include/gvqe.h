@@ -126,6 +126,58 @@ uint64_t gvqe_launch_count(const gvqe_ctx *ctx);
 gvqe_status gvqe_profile_enable(gvqe_ctx *ctx, int on);
 gvqe_status gvqe_profile_read(gvqe_ctx *ctx, double *out);
 
+/* ---- Host-side Graph-VQE driver (north_star item 3: partitioning and the optimiser loop stay on the host as plain
+ * C++).  These calls do no GPU work of their own; gvqe_graph_vqe_minimize obtains every energy and gradient through
+ * gvqe_energy_batch / gvqe_param_shift_grad above.  All pointers are HOST memory owned by the caller. ---------------- */
+
+/* Eq. 9: w[i*n+j] = sum of |c_k| over the terms that act non-trivially on both qubit i and
+ * qubit j (i != j); symmetric, zero diagonal.  w: n*n doubles (n = gvqe_num_qubits).  Needs a Hamiltonian. */
+gvqe_status gvqe_interaction_graph(const gvqe_ctx *ctx, double *w);
+/* Eq. 10 with a resolution factor gamma on the null-model term (gamma = 1: the paper's Q):
+ * Q = 1/(2m) sum_ij [w_ij - gamma k_i k_j / (2m)] delta(c_i, c_j).  community: n labels >= 0.  Q = 0 if m = 0. */
+gvqe_status gvqe_modularity(int n, const double *w, const int32_t *community, double gamma, double *Q);
+/* Louvain community detection on w: local moving in ascending qubit order (a qubit moves to the
+ * neighbouring community of largest modularity gain; ties: stay, else the lowest label), then aggregation,
+ * repeated until a level moves nothing.  community: n labels out, 0..K-1 in order of first appearance by ascending
+ * qubit; *n_communities = K; *Q (optional) = Eq. 10 of the result.  Deterministic. */
+gvqe_status gvqe_louvain(int n, const double *w, double gamma, int32_t *community, int32_t *n_communities, double *Q);
+/* PAPER.md:197 ("blocks smaller than S_min are iteratively merged with neighbors"): while a block has fewer than
+ * s_min qubits, the smallest such block (ties: lowest label) joins the block it shares the largest total weight
+ * with (ties: lowest label).  community: in/out, relabelled by first appearance; *n_communities = new K. */
+gvqe_status gvqe_merge_small_blocks(int n, const double *w, int s_min, int32_t *community, int32_t *n_communities);
+/* theta_{B_i} (reading A11): mask[p] = 1 when parameter p drives a rotation on a qubit q with
+ * community[q] == block, else 0.  mask: P bytes. */
+gvqe_status gvqe_block_param_mask(const gvqe_ctx *ctx, const int32_t *community, int32_t block, uint8_t *mask);
+
+typedef struct {
+    int32_t max_epochs;     /* >= 1 */
+    int32_t block_iters;    /* L-BFGS iterations per block and epoch (0 = skip the block phase) */
+    int32_t global_iters;   /* iterations of the global refinement per epoch (0 = the paper's no_Global ablation) */
+    int32_t window;         /* W of Eq. 14 (paper: 40) */
+    int32_t patience;       /* p_block = p_global of Eq. 14 (paper: 12) */
+    int32_t epoch_patience; /* p_epoch (paper: 3) */
+    int32_t lbfgs_memory;   /* correction pairs kept (>= 1) */
+    int32_t reserved;
+    double tol;             /* eps_tol of Eq. 14 and the epoch-level improvement threshold (paper: 1e-4) */
+    double f_tol;           /* L-BFGS relative decrease tolerance; g_tol = 0.1 f_tol */
+} gvqe_opt_options;
+
+typedef struct {
+    double E_best;          /* best energy found; params holds the matching vector */
+    int64_t energy_evals;   /* circuit-energy evaluations issued (rows of all batches) */
+    int32_t epochs, n_blocks, steps /* accepted L-BFGS steps */, stop_reason /* 0 max_epochs, 1 epoch patience */;
+} gvqe_opt_result;
+
+/* Graph-VQE epochs: from theta*_best, every block minimises Eq. 11 over its own parameters
+ * (L-BFGS, parameter-shift gradients, Eq. 13) starting from the same vector, the block solutions are fused, a
+ * global refinement over all parameters follows, the best vector is kept, and the run stops after epoch_patience
+ * epochs without an improvement larger than tol.  Blocks run one after another on this GPU (the paper's worker
+ * pool is out of scope).  params: P doubles in/out; history (optional): energy before the first epoch and after
+ * every epoch, at most history_cap entries, *history_len written. */
+gvqe_status gvqe_graph_vqe_minimize(gvqe_ctx *ctx, const gvqe_opt_options *opt, const int32_t *community,
+                                    double *params, gvqe_opt_result *result, double *history, int32_t history_cap,
+                                    int32_t *history_len, void *cuda_stream);
+
 const char *gvqe_last_error(const gvqe_ctx *ctx);
 void gvqe_destroy(gvqe_ctx *ctx);
 

@@ -23,11 +23,23 @@ EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
-           "gvqe_profile_enable", "gvqe_profile_read", "gvqe_last_error", "gvqe_destroy"]
+           "gvqe_profile_enable", "gvqe_profile_read", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
+           "gvqe_merge_small_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
 
 class GvqeLayout(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("entangler", C.c_int32), ("topology", C.c_int32), ("final_rot", C.c_int32)]
+
+
+class GvqeOptOptions(C.Structure):
+    _fields_ = [("max_epochs", C.c_int32), ("block_iters", C.c_int32), ("global_iters", C.c_int32),
+                ("window", C.c_int32), ("patience", C.c_int32), ("epoch_patience", C.c_int32),
+                ("lbfgs_memory", C.c_int32), ("reserved", C.c_int32), ("tol", C.c_double), ("f_tol", C.c_double)]
+
+
+class GvqeOptResult(C.Structure):
+    _fields_ = [("E_best", C.c_double), ("energy_evals", C.c_int64), ("epochs", C.c_int32), ("n_blocks", C.c_int32),
+                ("steps", C.c_int32), ("stop_reason", C.c_int32)]
 
 
 class GvqeError(RuntimeError):
@@ -75,6 +87,12 @@ def load():
     L.gvqe_launch_count.restype = u64
     L.gvqe_profile_enable.argtypes = [vp, i32]
     L.gvqe_profile_read.argtypes = [vp, vp]
+    L.gvqe_interaction_graph.argtypes = [vp, vp]
+    L.gvqe_modularity.argtypes = [i32, vp, vp, C.c_double, vp]
+    L.gvqe_louvain.argtypes = [i32, vp, C.c_double, vp, vp, vp]
+    L.gvqe_merge_small_blocks.argtypes = [i32, vp, i32, vp, vp]
+    L.gvqe_block_param_mask.argtypes = [vp, vp, i32, vp]
+    L.gvqe_graph_vqe_minimize.argtypes = [vp, C.POINTER(GvqeOptOptions), vp, vp, C.POINTER(GvqeOptResult), vp, i32, vp, vp]
     L.gvqe_last_error.argtypes = [vp]
     L.gvqe_last_error.restype = C.c_char_p
     L.gvqe_destroy.argtypes = [vp]
@@ -233,3 +251,63 @@ class Gvqe:
 
     def launch_count(self) -> int:
         return int(self._L.gvqe_launch_count(self._h))
+
+    # -- host-side Graph-VQE driver
+    def interaction_graph(self) -> np.ndarray:
+        w = np.zeros((self.n, self.n), dtype=np.float64)
+        self._check(self._L.gvqe_interaction_graph(self._h, w.ctypes.data))
+        return w
+
+    def block_param_mask(self, community, block: int) -> np.ndarray:
+        c = np.ascontiguousarray(community, dtype=np.int32)
+        if len(c) != self.n:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, f"community must have {self.n} entries")
+        m = np.zeros(max(self.P, 1), dtype=np.uint8)
+        self._check(self._L.gvqe_block_param_mask(self._h, c.ctypes.data, int(block), m.ctypes.data))
+        return m[:self.P]
+
+    def graph_vqe_minimize(self, params, community, *, max_epochs=10, block_iters=50, global_iters=50, window=40,
+                           patience=12, epoch_patience=3, lbfgs_memory=8, tol=1e-4, f_tol=1e-9, stream: int = 0):
+        """Returns (params_best, result dict, history array).  Defaults are the paper's settings."""
+        p = np.array(params, dtype=np.float64).reshape(-1)
+        c = np.ascontiguousarray(community, dtype=np.int32)
+        if len(p) != self.P or len(c) != self.n:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, "params / community size")
+        opt = GvqeOptOptions(max_epochs, block_iters, global_iters, window, patience, epoch_patience, lbfgs_memory, 0,
+                             tol, f_tol)
+        res = GvqeOptResult()
+        hist = np.zeros(max_epochs + 1, dtype=np.float64)
+        hl = C.c_int32(0)
+        self._check(self._L.gvqe_graph_vqe_minimize(self._h, C.byref(opt), c.ctypes.data, p.ctypes.data, C.byref(res),
+                                                    hist.ctypes.data, len(hist), C.addressof(hl), C.c_void_p(stream)))
+        return p, {f: getattr(res, f) for f, _ in GvqeOptResult._fields_}, hist[:hl.value]
+
+
+def _graph_check(st: int, what: str):
+    if st != GVQE_OK:
+        raise GvqeError(st, what)
+
+
+def modularity(w, community, gamma: float = 1.0) -> float:
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    c = np.ascontiguousarray(community, dtype=np.int32)
+    q = C.c_double(0.0)
+    _graph_check(load().gvqe_modularity(w.shape[0], w.ctypes.data, c.ctypes.data, float(gamma), C.addressof(q)), "gvqe_modularity")
+    return q.value
+
+
+def louvain(w, gamma: float = 1.0):
+    """(community[n], K, Q) of gvqe_louvain."""
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    c = np.zeros(w.shape[0], dtype=np.int32)
+    k, q = C.c_int32(0), C.c_double(0.0)
+    _graph_check(load().gvqe_louvain(w.shape[0], w.ctypes.data, float(gamma), c.ctypes.data, C.addressof(k), C.addressof(q)), "gvqe_louvain")
+    return c, k.value, q.value
+
+
+def merge_small_blocks(w, community, s_min: int):
+    w = np.ascontiguousarray(w, dtype=np.float64)
+    c = np.array(community, dtype=np.int32)
+    k = C.c_int32(0)
+    _graph_check(load().gvqe_merge_small_blocks(w.shape[0], w.ctypes.data, int(s_min), c.ctypes.data, C.addressof(k)), "gvqe_merge_small_blocks")
+    return c, k.value

@@ -8,8 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libgvqe.so")
-SOURCES = ["schedule.cpp", "lower.cpp", "hamiltonian.cpp", "gvqe_api.cpp", "kernels.cu"]
-HEADERS = ["program.h", "devprog.h", "schedule.h", "lower.h", "hamiltonian.h", "kernels.h", "kernels.cuh",
+SOURCES = ["schedule.cpp", "lower.cpp", "hamiltonian.cpp", "graph.cpp", "driver.cpp", "gvqe_api.cpp", "kernels.cu"]
+HEADERS = ["program.h", "devprog.h", "schedule.h", "lower.h", "hamiltonian.h", "graph.h", "kernels.h", "kernels.cuh",
            os.path.join("..", "..", "include", "gvqe.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",

@@ -11,6 +11,7 @@
 #include <vector>
 
 #include "../../include/gvqe.h"
+#include "graph.h"
 #include "hamiltonian.h"
 #include "kernels.h"
 #include "lower.h"
@@ -614,6 +615,72 @@ gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out)
 }
 
 uint64_t gvqe_launch_count(const gvqe_ctx *c) { return c ? c->launches : 0; }
+// ---- host-side Graph-VQE driver: graph construction and partitioning (graph.cpp), parameter masks ----------------
+gvqe_status gvqe_interaction_graph(const gvqe_ctx *c, double *w)
+{
+    if (!c || !w) return GVQE_ERR_INVALID_ARG;
+    if (!c->have_h) return GVQE_ERR_NO_HAMILTONIAN;
+    const int n = c->n_user;
+    for (size_t t = 0; t < (size_t)n * n; ++t) w[t] = 0.0;
+    for (const HostTerm &t : c->H.terms) {   // Eq. 9: non-identity on qubit i <=> bit i of x | z
+        const uint64_t s = t.x | t.z;
+        const double a = std::fabs(t.c);
+        for (int i = 0; i < n; ++i) {
+            if (!((s >> i) & 1)) continue;
+            for (int j = i + 1; j < n; ++j)
+                if ((s >> j) & 1) { w[(size_t)i * n + j] += a; w[(size_t)j * n + i] += a; }
+        }
+    }
+    return GVQE_OK;
+}
+
+static bool graph_args_ok(int n, const double *w)
+{
+    if (n < 1 || !w) return false;
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) {
+            const double v = w[(size_t)i * n + j];
+            if (!(v >= 0.0) || !std::isfinite(v) || v != w[(size_t)j * n + i]) return false;
+        }
+    return true;
+}
+
+gvqe_status gvqe_modularity(int n, const double *w, const int32_t *community, double gamma, double *Q)
+{
+    if (!graph_args_ok(n, w) || !community || !Q || !std::isfinite(gamma)) return GVQE_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) if (community[i] < 0) return GVQE_ERR_INVALID_ARG;
+    *Q = modularity(n, w, community, gamma);
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_louvain(int n, const double *w, double gamma, int32_t *community, int32_t *n_communities, double *Q)
+{
+    if (!graph_args_ok(n, w) || !community || !std::isfinite(gamma) || gamma < 0.0) return GVQE_ERR_INVALID_ARG;
+    const int K = louvain(n, w, gamma, community);
+    if (n_communities) *n_communities = K;
+    if (Q) *Q = modularity(n, w, community, gamma);
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_merge_small_blocks(int n, const double *w, int s_min, int32_t *community, int32_t *n_communities)
+{
+    if (!graph_args_ok(n, w) || !community) return GVQE_ERR_INVALID_ARG;
+    for (int i = 0; i < n; ++i) if (community[i] < 0 || community[i] > (1 << 20)) return GVQE_ERR_INVALID_ARG;
+    const int K = merge_small_blocks(n, w, s_min, community);
+    if (n_communities) *n_communities = K;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_block_param_mask(const gvqe_ctx *c, const int32_t *community, int32_t block, uint8_t *mask)
+{
+    if (!c || !community || (c->P > 0 && !mask)) return GVQE_ERR_INVALID_ARG;
+    for (int p = 0; p < c->P; ++p) mask[p] = 0;
+    for (const HostOp &o : c->ops)
+        if ((o.kind == GVQE_OP_RY || o.kind == GVQE_OP_RZ) && o.param >= 0 && o.q0 < c->n_user && community[o.q0] == block)
+            mask[o.param] = 1;
+    return GVQE_OK;
+}
+
 const char *gvqe_last_error(const gvqe_ctx *c) { return c ? c->err.c_str() : "null context"; }
 void gvqe_destroy(gvqe_ctx *c)
 {

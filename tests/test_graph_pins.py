@@ -1,0 +1,194 @@
+"""CPU tests of the Hamiltonian-aware partitioning (Eq. 9 and 10).
+
+First the oracle (oracle/graph_oracle.py) is pinned to things other than itself: a hand-computed Eq. 9 example,
+closed forms of Eq. 10, brute force over all set partitions of tiny graphs, planted communities.  Then the library's
+host C++ (gvqe_interaction_graph / gvqe_modularity / gvqe_louvain / gvqe_merge_small_blocks / gvqe_block_param_mask)
+is compared with the oracle: weights and Q to rounding, partitions and masks exactly."""
+import numpy as np
+import pytest
+
+import paper_2607_02749_b200 as gv
+from paper_2607_02749_b200 import binding as gb
+from oracle import graph_oracle as go
+from workload import make_workload, CONFIGS
+from workload.generator import SplitMix64, community_param_mask
+
+
+def set_partitions(n):
+    """All set partitions of range(n) as restricted-growth label lists."""
+    def rec(prefix, k):
+        if len(prefix) == n:
+            yield list(prefix)
+            return
+        for l in range(k + 1):
+            prefix.append(l)
+            yield from rec(prefix, max(k, l + 1))
+            prefix.pop()
+    yield from rec([], 0)
+
+
+def cliques(sizes, w_in=1.0, w_out=0.0):
+    n = sum(sizes)
+    lab = [c for c, s in enumerate(sizes) for _ in range(s)]
+    w = np.zeros((n, n))
+    for i in range(n):
+        for j in range(n):
+            if i != j:
+                w[i, j] = w_in if lab[i] == lab[j] else w_out
+    return w, lab
+
+
+def random_graph(seed, n, density=0.6):
+    r = SplitMix64(seed)
+    w = np.zeros((n, n))
+    for i in range(n):
+        for j in range(i + 1, n):
+            if r.uniform() < density:
+                w[i, j] = w[j, i] = 0.1 + r.uniform()
+    return w
+
+
+# ---- pins of the oracle ---------------------------------------------------------------------------------------
+def test_eq9_hand_example():
+    """Three terms on 4 qubits, weights added by hand from Eq. 9."""
+    paulis = ["XZII", "IZYI", "ZIIX", "IIII", "IXII"]      # character j acts on qubit j
+    coeffs = [-2.0, 0.5, 3.0, 7.0, -1.0]                    # identity and weight-1 terms make no edge
+    w = go.interaction_graph(4, paulis, coeffs)
+    expect = np.zeros((4, 4))
+    expect[0, 1] = expect[1, 0] = 2.0
+    expect[1, 2] = expect[2, 1] = 0.5
+    expect[0, 3] = expect[3, 0] = 3.0
+    assert np.array_equal(w, expect)
+
+
+def test_eq10_closed_forms():
+    """r disjoint equal cliques, each its own block: Q = 1 - 1/r.  One block: Q = 1 - gamma.  Singletons:
+    Q = -sum k_i^2 / (2m)^2.  Two triangles joined by one edge, split at the bridge: Q = 5/14 (textbook value:
+    2 * (6/14 - (7/14)^2))."""
+    for r in (2, 3, 5):
+        w, lab = cliques([4] * r)
+        assert abs(go.modularity(w, lab) - (1.0 - 1.0 / r)) < 1e-14
+    w = random_graph(3, 9)
+    assert abs(go.modularity(w, [0] * 9)) < 1e-14
+    assert abs(go.modularity(w, [0] * 9, gamma=0.3) - 0.7) < 1e-14
+    k, two_m = w.sum(axis=1), w.sum()
+    assert abs(go.modularity(w, list(range(9))) + np.sum(k * k) / two_m ** 2) < 1e-14
+    w = np.zeros((6, 6))
+    for a, b in [(0, 1), (1, 2), (0, 2), (3, 4), (4, 5), (3, 5), (2, 3)]:
+        w[a, b] = w[b, a] = 1.0
+    assert abs(go.modularity(w, [0, 0, 0, 1, 1, 1]) - 5.0 / 14.0) < 1e-14
+    assert go.modularity(np.zeros((3, 3)), [0, 1, 2]) == 0.0
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_louvain_vs_brute_force(seed):
+    """n = 7: Q of every one of the 877 set partitions; Louvain's Q can never exceed the maximum, and no single-node
+    move improves its result (local optimality of phase 1 on the final partition's aggregate is implied by stopping)."""
+    w = random_graph(100 + seed, 7)
+    q_best = max(go.modularity(w, p) for p in set_partitions(7))
+    lab, K = go.louvain(w)
+    q = go.modularity(w, lab)
+    assert q <= q_best + 1e-12
+    assert q >= 0.0 and K == max(lab) + 1 and lab[0] == 0
+    assert q >= 0.75 * q_best      # heuristic, but on 7 nodes it is never far off
+
+
+def test_louvain_planted_is_optimal():
+    """Cliques with weak links between them: brute force says the planted partition is the optimum, Louvain finds it."""
+    w, planted = cliques([3, 2, 2], w_in=1.0, w_out=0.05)
+    q_all = {tuple(p): go.modularity(w, p) for p in set_partitions(7)}
+    best = max(q_all, key=q_all.get)
+    assert list(best) == planted
+    lab, K = go.louvain(w)
+    assert lab == planted and K == 3
+    lab, K = go.louvain(np.zeros((5, 5)))
+    assert lab == [0, 1, 2, 3, 4] and K == 5
+    # resolution: gamma -> 0 puts every connected node into one block
+    lab, K = go.louvain(w, gamma=0.0)
+    assert K == 1
+
+
+def test_merge_small_blocks_rules():
+    w = np.zeros((6, 6))
+    def e(a, b, v):
+        w[a, b] = w[b, a] = v
+    e(0, 1, 1.0); e(2, 3, 1.0); e(4, 0, 0.2); e(4, 2, 0.7); e(5, 1, 0.1)
+    lab, K = go.merge_small_blocks(w, [0, 0, 1, 1, 2, 3], 2)
+    # blocks 2 = {4} and 3 = {5} are too small: {4} (lowest label first) joins {2,3} (0.7 > 0.2), then {5} joins {0,1}
+    assert lab == [0, 0, 1, 1, 1, 0] and K == 2
+    lab, K = go.merge_small_blocks(w, [0, 0, 1, 1, 2, 3], 1)
+    assert lab == [0, 0, 1, 1, 2, 3] and K == 4
+    lab, K = go.merge_small_blocks(w, [0, 0, 1, 1, 2, 3], 7)     # nothing can reach 7: everything ends in one block
+    assert K == 1 and lab == [0] * 6
+    # sizes are conserved, labels are contiguous
+    lab, K = go.merge_small_blocks(random_graph(5, 9), [0, 1, 2, 3, 4, 5, 6, 7, 8], 3)
+    assert sorted(set(lab)) == list(range(K)) and min(lab.count(c) for c in range(K)) >= 3
+
+
+def test_block_param_mask_counts():
+    """cfg 2: one community of 4 qubits owns 4 * (2*4 + 1) = 36 parameters; masks of all blocks
+    partition the parameter set; equals the workload module's own mask."""
+    w = make_workload(2, M=10)
+    comm = [c for c, qs in enumerate(w.communities) for _ in qs]
+    masks = [go.block_param_mask(w.ops, w.P, comm, b) for b in range(4)]
+    assert all(int(m.sum()) == 36 for m in masks)
+    assert np.array_equal(np.sum(masks, axis=0), np.ones(w.P))
+    assert np.array_equal(masks[0], community_param_mask(w.n, w.D, w.final_rot, w.communities[0]))
+
+
+# ---- the library against the oracle -----------------------------------------------------------------------------
+def lib_ctx(w):
+    g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
+                precision="c128")
+    g.set_hamiltonian(w.paulis, w.coeffs)
+    return g
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_library_graph_and_louvain_recover_planted_communities(cfg):
+    """Eq. 9 weights of the BASELINE Hamiltonians (full term count, 1-layer circuit): library = oracle to rounding;
+    Louvain (library and oracle) returns the same partition, and it is the planted one (SURVEY 8(f) check)."""
+    w = make_workload(cfg, D=1, batch=1)
+    g = lib_ctx(w)
+    W = g.interaction_graph()
+    Wo = go.interaction_graph(w.n, w.pauli_list(), w.coeffs)
+    assert np.allclose(W, Wo, rtol=1e-13, atol=0.0) and np.array_equal(W, W.T) and not W.diagonal().any()
+    lab, K, Q = gb.louvain(W)
+    lab_o, K_o = go.louvain(Wo)
+    assert list(lab) == lab_o and K == K_o
+    assert abs(Q - go.modularity(Wo, lab_o)) < 1e-12
+    planted = [c for c, qs in enumerate(w.communities) for _ in qs]
+    assert list(lab) == planted
+    for b in range(K):
+        assert np.array_equal(g.block_param_mask(lab, b), go.block_param_mask(w.ops, w.P, lab_o, b))
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_library_louvain_random_graphs(seed):
+    n = 5 + 3 * seed
+    W = random_graph(500 + seed, n, density=0.35)
+    for gamma in (1.0, 0.5, 1.7):
+        lab, K, Q = gb.louvain(W, gamma)
+        lab_o, K_o = go.louvain(W, gamma)
+        assert list(lab) == lab_o and K == K_o
+        assert abs(Q - go.modularity(W, lab_o, gamma)) < 1e-12
+        assert abs(gb.modularity(W, lab, gamma) - Q) < 1e-15
+    for s_min in (1, 2, 4, n + 1):
+        start = [i // 2 if i % 3 else i for i in range(n)]
+        m, Km = gb.merge_small_blocks(W, start, s_min)
+        m_o, Km_o = go.merge_small_blocks(W, start, s_min)
+        assert list(m) == m_o and Km == Km_o
+
+
+def test_library_graph_argument_checks():
+    W = random_graph(1, 4)
+    bad = W.copy(); bad[0, 1] += 1.0
+    with pytest.raises(gv.GvqeError):
+        gb.louvain(bad)                      # not symmetric
+    with pytest.raises(gv.GvqeError):
+        gb.louvain(-W)                       # negative weights
+    with pytest.raises(gv.GvqeError):
+        gb.modularity(W, [0, -1, 0, 0])
+    g = gv.Gvqe(4, layout=dict(n_layers=1, entangler="cz", topology="linear"), precision="c128")
+    with pytest.raises(gv.GvqeError):
+        g.interaction_graph()                # no Hamiltonian yet
