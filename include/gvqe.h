@@ -47,10 +47,19 @@ typedef struct { int32_t kind, q0, q1, param; } gvqe_op;
 /* Layered ansatz: for l in 0..n_layers-1: RY(theta[2Nl+q]) all q, RZ(theta[2Nl+N+q]) all q,
  * entanglers (q,q+1) ascending (CNOT: control q, target q+1), then (N-1 -> 0) if topology == 1;
  * finally RY(theta[2ND+q]) (and RZ(theta[2ND+N+q]) if final_rot == 2, which gives Eq. 8's P = 2N(D+1)). */
+/* Entanglement maps (PAPER.md:260 evaluates Circular, Full, Linear, Reverse Linear, Pairwise and SCA); pairs are
+ * (control, target), CZ ignores the roles.  n <= 2: every map with a wrap pair degenerates to the chain.
+ *   LINEAR (q,q+1) q ascending | RING = LINEAR then (N-1,0) | FULL (i,j) all i<j, i then j ascending |
+ *   REVERSE_LINEAR (q,q+1) q descending | PAIRWISE (q,q+1) even q ascending, then odd q ascending |
+ *   CIRCULAR (N-1,0) then LINEAR | SCA: layer l uses the circular list C = [(N-1,0),(0,1),...,(N-2,N-1)] shifted
+ *   by l places (entry j = C[(j-l) mod N]) with control and target swapped on odd l. */
+typedef enum { GVQE_TOPO_LINEAR = 0, GVQE_TOPO_RING = 1, GVQE_TOPO_FULL = 2, GVQE_TOPO_REVERSE_LINEAR = 3,
+               GVQE_TOPO_PAIRWISE = 4, GVQE_TOPO_CIRCULAR = 5, GVQE_TOPO_SCA = 6 } gvqe_topology;
+
 typedef struct {
     int32_t n_layers;  /* D >= 0 */
     int32_t entangler; /* GVQE_OP_CZ or GVQE_OP_CNOT */
-    int32_t topology;  /* 0 linear chain, 1 ring */
+    int32_t topology;  /* gvqe_topology: 0 linear chain, 1 ring (chain, then the wrap pair), 2..6 see below */
     int32_t final_rot; /* 1 = RY only, 2 = RY then RZ */
 } gvqe_layout;
 

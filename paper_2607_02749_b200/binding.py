@@ -102,7 +102,7 @@ def load():
 
 
 _ENT = {"cz": 2, "cnot": 3}
-_TOPO = {"linear": 0, "ring": 1}
+_TOPO = {"linear": 0, "ring": 1, "full": 2, "reverse_linear": 3, "pairwise": 4, "circular": 5, "sca": 6}
 
 
 class Gvqe:

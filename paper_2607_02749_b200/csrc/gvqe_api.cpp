@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/gvqe.h"
@@ -136,7 +137,7 @@ gvqe_status gvqe_create(int n, const gvqe_layout *L, gvqe_precision prec, gvqe_c
 {
     if (!L || !out || n < 1 || n > N_MAX) return GVQE_ERR_INVALID_ARG;
     if (L->n_layers < 0 || L->n_layers > 4096 || (L->entangler != GVQE_OP_CZ && L->entangler != GVQE_OP_CNOT) ||
-        (L->topology != 0 && L->topology != 1) || (L->final_rot != 1 && L->final_rot != 2))
+        (L->topology < 0 || L->topology > 6) || (L->final_rot != 1 && L->final_rot != 2))
         return GVQE_ERR_INVALID_ARG;
     // D x (RY layer, RZ layer, entanglers), then the final rotation layer.
     std::vector<HostOp> ops;
@@ -144,13 +145,40 @@ gvqe_status gvqe_create(int n, const gvqe_layout *L, gvqe_precision prec, gvqe_c
     for (int l = 0; l < D; ++l) {
         for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RY, q, -1, 2 * n * l + q});
         for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RZ, q, -1, 2 * n * l + n + q});
-        for (int q = 0; q + 1 < n; ++q) {
-            if (L->entangler == GVQE_OP_CZ) ops.push_back({GVQE_OP_CZ, q, q + 1, -1});
-            else ops.push_back({GVQE_OP_CNOT, q + 1, q, -1});
+        // (control, target) pairs of the layer's entanglement map (reading A17)
+        std::vector<std::pair<int, int>> pr;
+        const bool wrap = n > 2;
+        switch (L->topology) {
+        case 0: case 1:
+            for (int q = 0; q + 1 < n; ++q) pr.push_back({q, q + 1});
+            if (L->topology == 1 && wrap) pr.push_back({n - 1, 0});
+            break;
+        case 2:
+            for (int i = 0; i < n; ++i) for (int j = i + 1; j < n; ++j) pr.push_back({i, j});
+            break;
+        case 3:
+            for (int q = n - 2; q >= 0; --q) pr.push_back({q, q + 1});
+            break;
+        case 4:
+            for (int par = 0; par < 2; ++par) for (int q = par; q + 1 < n; q += 2) pr.push_back({q, q + 1});
+            break;
+        case 5:
+            if (wrap) pr.push_back({n - 1, 0});
+            for (int q = 0; q + 1 < n; ++q) pr.push_back({q, q + 1});
+            break;
+        default: {   // 6, shifted-circular-alternating
+            if (!wrap) { for (int q = 0; q + 1 < n; ++q) pr.push_back({q, q + 1}); break; }
+            for (int j = 0; j < n; ++j) {
+                const int e = ((j - l) % n + n) % n;          // entry e of the circular list: (e-1, e), e = 0: (n-1, 0)
+                std::pair<int, int> p = e == 0 ? std::make_pair(n - 1, 0) : std::make_pair(e - 1, e);
+                if (l & 1) std::swap(p.first, p.second);
+                pr.push_back(p);
+            }
         }
-        if (L->topology == 1 && n > 2) {
-            if (L->entangler == GVQE_OP_CZ) ops.push_back({GVQE_OP_CZ, n - 1, 0, -1});
-            else ops.push_back({GVQE_OP_CNOT, 0, n - 1, -1});
+        }
+        for (const auto &p : pr) {
+            if (L->entangler == GVQE_OP_CZ) ops.push_back({GVQE_OP_CZ, p.first, p.second, -1});
+            else ops.push_back({GVQE_OP_CNOT, p.second, p.first, -1});
         }
     }
     for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RY, q, -1, 2 * n * D + q});

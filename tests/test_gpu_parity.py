@@ -172,7 +172,12 @@ def test_random_circuits_and_paulis(orc, seed, monkeypatch):
 
 @pytest.mark.parametrize("n,D,ent,topo,fr,prec", [(13, 3, "cz", "linear", 1, "c64"), (15, 2, "cnot", "ring", 1, "c64"),
                                                    (14, 2, "cnot", "linear", 2, "c128"), (16, 3, "cz", "ring", 2, "c128"),
-                                                   (17, 2, "cnot", "ring", 1, "c128"), (18, 2, "cz", "linear", 2, "c64")])
+                                                   (17, 2, "cnot", "ring", 1, "c128"), (18, 2, "cz", "linear", 2, "c64"),
+                                                   # the paper's other entanglement maps (reading A17)
+                                                   (12, 2, "cnot", "full", 1, "c128"), (15, 3, "cnot", "reverse_linear", 1, "c64"),
+                                                   (14, 3, "cnot", "pairwise", 2, "c128"), (13, 2, "cnot", "circular", 1, "c128"),
+                                                   (15, 4, "cnot", "sca", 1, "c128"), (16, 3, "cz", "full", 1, "c64"),
+                                                   (17, 3, "cnot", "sca", 2, "c64")])
 def test_layered_ansatz_variants(orc, n, D, ent, topo, fr, prec):
     ops = np.array(layout_ops(n, D, ent, topo, fr), dtype=np.int32)
     P = num_params(n, D, fr)

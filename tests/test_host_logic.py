@@ -90,11 +90,28 @@ def test_schedule_order_is_equivalent_layered(orc, n, D, ent, topo, fr, prec, mo
 def test_layout_expansion_matches_generator():
     """gvqe_create(layout) builds the same op list as workload.layout_ops (readings A1-A5)."""
     from workload import layout_ops, num_params
-    for n, D, ent, topo, fr in [(6, 2, "cz", "linear", 1), (7, 3, "cnot", "ring", 2), (2, 1, "cnot", "ring", 1)]:
+    cases = [(6, 2, "cz", "linear", 1), (7, 3, "cnot", "ring", 2), (2, 1, "cnot", "ring", 1)]
+    cases += [(n, 3, ent, topo, 1) for topo in ("full", "reverse_linear", "pairwise", "circular", "sca")
+              for n, ent in ((5, "cnot"), (6, "cz"), (2, "cnot"))]
+    for n, D, ent, topo, fr in cases:
         a = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo, final_rot=fr))
         b = gv.Gvqe(n, ops=np.array(layout_ops(n, D, ent, topo, fr), dtype=np.int32), n_params=num_params(n, D, fr))
         assert a.P == b.P == num_params(n, D, fr)
         assert a.dump_schedule() == b.dump_schedule()
+
+
+def test_entangler_maps_by_hand():
+    """Reading A17 written out for n = 4 (control, target)."""
+    from workload.generator import entangler_pairs as ep
+    assert ep(4, "full", 0) == [(0, 1), (0, 2), (0, 3), (1, 2), (1, 3), (2, 3)]
+    assert ep(4, "reverse_linear", 0) == [(2, 3), (1, 2), (0, 1)]
+    assert ep(5, "pairwise", 0) == [(0, 1), (2, 3), (1, 2), (3, 4)]
+    assert ep(4, "circular", 1) == [(3, 0), (0, 1), (1, 2), (2, 3)]
+    assert ep(4, "ring", 1) == [(0, 1), (1, 2), (2, 3), (3, 0)]
+    assert ep(4, "sca", 0) == [(3, 0), (0, 1), (1, 2), (2, 3)]
+    assert ep(4, "sca", 1) == [(3, 2), (0, 3), (1, 0), (2, 1)]      # shifted by one, roles swapped
+    assert ep(4, "sca", 2) == [(1, 2), (2, 3), (3, 0), (0, 1)]
+    assert ep(2, "sca", 1) == [(0, 1)]
 
 
 def test_large_configs_compile_and_plan():

@@ -102,6 +102,28 @@ def num_params(n: int, D: int, final_rot: int) -> int:
     return 2 * n * D + n * final_rot
 
 
+def entangler_pairs(n: int, topology: str, layer: int) -> List[Tuple[int, int]]:
+    """(control, target) pairs of one entangling layer (reading A17; PAPER.md:260 lists the maps)."""
+    chain = [(q, q + 1) for q in range(n - 1)]
+    if topology == "linear" or n <= 2 and topology in ("ring", "circular", "sca"):
+        return chain
+    if topology == "ring":
+        return chain + [(n - 1, 0)]
+    if topology == "circular":
+        return [(n - 1, 0)] + chain
+    if topology == "full":
+        return [(i, j) for i in range(n) for j in range(i + 1, n)]
+    if topology == "reverse_linear":
+        return chain[::-1]
+    if topology == "pairwise":
+        return [p for p in chain if p[0] % 2 == 0] + [p for p in chain if p[0] % 2 == 1]
+    if topology == "sca":
+        circ = [(n - 1, 0)] + chain
+        shifted = [circ[(j - layer) % n] for j in range(n)]
+        return [(t, c) for (c, t) in shifted] if layer % 2 else shifted
+    raise ValueError(topology)
+
+
 def layout_ops(n: int, D: int, entangler: str, topology: str, final_rot: int) -> List[Tuple[int, int, int, int]]:
     """Ansatz layout -> explicit op list [(kind, q0, q1, param)] (readings A1-A5).
 
@@ -115,9 +137,7 @@ def layout_ops(n: int, D: int, entangler: str, topology: str, final_rot: int) ->
             ops.append((OP_RY, q, -1, 2 * n * l + q))
         for q in range(n):
             ops.append((OP_RZ, q, -1, 2 * n * l + n + q))
-        pairs = [(q, q + 1) for q in range(n - 1)]
-        if topology == "ring" and n > 2:
-            pairs.append((n - 1, 0))
+        pairs = entangler_pairs(n, topology, l)
         for (c, t) in pairs:
             if entangler == "cz":
                 ops.append((OP_CZ, c, t, -1))
