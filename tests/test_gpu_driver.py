@@ -94,3 +94,27 @@ def test_minimize_argument_checks():
         g.graph_vqe_minimize(w.theta, [0, 0, 0, 0, 0, -1])
     with pytest.raises(gv.GvqeError):
         g.graph_vqe_minimize(w.theta, [0] * 6, tol=0.0)
+
+
+@pytest.mark.parametrize("n,D,budget", [(6, 1, (3, 4, 5)), (8, 2, (2, 3, 3))])
+def test_loop_follows_the_step_by_step_oracle(orc, n, D, budget):
+    """Same start vector, same blocks, same budgets: the library's epoch loop (energies from the kernels, c128) and
+    oracle/driver_oracle.py (energies from oracle T0) take the same steps -- same epoch count, step count and stop
+    reason, histories and final parameters equal up to the amplification of the 1e-13 energy differences."""
+    from oracle import driver_oracle as do
+    epochs, bi, gi = budget
+    w = make_workload(2, n=n, M=50, D=D, batch=1)
+    g = ctx(w)
+    W = g.interaction_graph()
+    lab, K, _ = gb.louvain(W)
+    lab, K = gb.merge_small_blocks(W, lab, 2)
+    theta, res, hist = g.graph_vqe_minimize(w.theta, lab, max_epochs=epochs, block_iters=bi, global_iters=gi, f_tol=1e-12)
+    energy = lambda rows: orc.energy_batch(w.n, w.ops, np.ascontiguousarray(rows), w.paulis, w.coeffs)
+    masks = [g.block_param_mask(lab, b) for b in range(K)]
+    th_o, E_o, hist_o, ep_o, steps_o, reason_o = do.graph_vqe_minimize(
+        energy, w.theta, masks, max_epochs=epochs, block_iters=bi, global_iters=gi, f_tol=1e-12)
+    assert (res["epochs"], res["steps"], res["stop_reason"], res["n_blocks"]) == (ep_o, steps_o, reason_o, K)
+    scale = np.sum(np.abs(w.coeffs))
+    assert np.max(np.abs(hist - hist_o)) < 1e-8 * scale
+    assert abs(res["E_best"] - E_o) < 1e-8 * scale
+    assert np.max(np.abs(theta - th_o)) < 1e-6

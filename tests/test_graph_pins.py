@@ -192,3 +192,44 @@ def test_library_graph_argument_checks():
     g = gv.Gvqe(4, layout=dict(n_layers=1, entangler="cz", topology="linear"), precision="c128")
     with pytest.raises(gv.GvqeError):
         g.interaction_graph()                # no Hamiltonian yet
+
+
+# ---- pins of the epoch-loop oracle (oracle/driver_oracle.py) ----------------------------------------------------------
+def test_driver_oracle_eq14_by_hand():
+    from oracle import driver_oracle as do
+    hist = [5.0, 3.0, 2.5, 2.4, 2.4, 2.39]
+    assert do.delta_max(hist, 40) == 2.0                       # whole history
+    assert abs(do.delta_max(hist, 3) - 0.1) < 1e-15            # last three differences: 0.1, 0.0, 0.01
+    assert abs(do.delta_max(hist, 1) - 0.01) < 1e-15
+    assert do.delta_max([1.0], 40) == 0.0
+
+
+def test_driver_oracle_parameter_shift_is_exact_for_sinusoids():
+    """Eq. 13 is exact for E = a cos(theta - b) + c in every coordinate (what a rotation gate gives)."""
+    from oracle import driver_oracle as do
+    a, b = np.array([1.0, -2.0, 0.5]), np.array([0.3, -1.0, 2.0])
+    energy = lambda rows: np.sum(a * np.cos(rows - b), axis=1) + 4.0
+    th = np.array([0.7, -0.2, 1.9])
+    E, g = do.param_shift_grad(energy, th, [0, 2])
+    assert abs(E - energy(th.reshape(1, -1))[0]) < 1e-15
+    assert np.allclose(g, (-a * np.sin(th - b))[[0, 2]], atol=1e-14)
+
+
+def test_driver_oracle_separable_minimum_and_frozen_coordinates():
+    """min of sum a_q cos(theta_q) is -sum |a_q|; with one block left out its coordinates never move (Eq. 11)."""
+    from oracle import driver_oracle as do
+    a = np.array([1.0, -0.5, 2.0, 0.25])
+    energy = lambda rows: np.sum(a * np.cos(rows), axis=1)
+    th0 = np.array([0.4, 1.1, -2.0, 0.9])
+    masks = [np.array([1, 1, 0, 0], np.uint8), np.array([0, 0, 1, 0], np.uint8)]
+    th, E, hist, epochs, steps, reason = do.graph_vqe_minimize(energy, th0, masks, max_epochs=5, global_iters=0, f_tol=1e-14)
+    assert th[3] == th0[3]
+    assert abs(E - (-1.0 - 0.5 - 2.0 + 0.25 * np.cos(0.9))) < 1e-9
+    assert hist[0] == energy(th0.reshape(1, -1))[0] and abs(min(hist) - E) < 1e-15
+    assert all(hist[i + 1] <= hist[i] + 1e-12 for i in range(len(hist) - 1))
+    th, E, *_ = do.graph_vqe_minimize(energy, th0, masks, max_epochs=3, global_iters=30, f_tol=1e-14)
+    assert abs(E + np.sum(np.abs(a))) < 1e-9                   # the global phase reaches the frozen coordinate too
+    # nothing to do: zero budgets stop by epoch patience after exactly epoch_patience epochs
+    th, E, hist, epochs, steps, reason = do.graph_vqe_minimize(energy, th0, masks, max_epochs=9, block_iters=0,
+                                                               global_iters=0, epoch_patience=2)
+    assert np.array_equal(th, th0) and epochs == 2 and reason == 1 and steps == 0
