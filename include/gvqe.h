@@ -111,6 +111,12 @@ gvqe_status gvqe_param_shift_grad(gvqe_ctx *ctx, const double *params, const uin
  * as left by the last energy call, copied to host_out (HOST). */
 gvqe_status gvqe_get_state(gvqe_ctx *ctx, int slot, void *host_out);
 
+/* Read-out, PAPER.md:245 ("the bitstring with the highest probability is identified as the optimal turn sequence"):
+ * *x = argmax_x |psi_x|^2 over the statevector in in-flight slot `slot` as left by the last energy call (bit q of
+ * x = qubit q), ties to the lowest x; *prob (HOST, optional) = that probability.  |psi_x|^2 = re*re + im*im in the
+ * context's precision, each operation rounded separately.  One read-only sweep of the state on the GPU. */
+gvqe_status gvqe_argmax(gvqe_ctx *ctx, int slot, uint64_t *x, double *prob, void *cuda_stream);
+
 /* Introspection of the compiled schedule (host; for tests and traffic accounting).
  * gvqe_schedule_info: number of fused gate blocks, number of off-diagonal passes, statevectors in flight.
  * gvqe_dump_schedule: writes a text description of every block/stage/op into buf (NUL-terminated, truncated to

@@ -22,7 +22,7 @@ STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "G
 EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
-           "gvqe_get_state", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
+           "gvqe_get_state", "gvqe_argmax", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
            "gvqe_merge_small_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
@@ -79,6 +79,7 @@ def load():
     L.gvqe_energy_batch_device.argtypes = [vp, vp, i32, vp, vp]
     L.gvqe_param_shift_grad.argtypes = [vp, vp, vp, vp, vp, vp]
     L.gvqe_get_state.argtypes = [vp, i32, vp]
+    L.gvqe_argmax.argtypes = [vp, i32, vp, vp, vp]
     L.gvqe_schedule_info.argtypes = [vp, vp, vp, vp]
     L.gvqe_dump_schedule.argtypes = [vp, C.c_char_p, sz]
     L.gvqe_dump_schedule.restype = sz
@@ -222,6 +223,12 @@ class Gvqe:
         out = np.empty(1 << self.n, dtype=dt)
         self._check(self._L.gvqe_get_state(self._h, slot, out.ctypes.data))
         return out
+
+    def argmax(self, slot: int = 0, stream: int = 0):
+        """(x, |psi_x|^2) of the most probable basis state of in-flight slot `slot` (ties: lowest x)."""
+        x, p = C.c_uint64(0), C.c_double(0.0)
+        self._check(self._L.gvqe_argmax(self._h, int(slot), C.addressof(x), C.addressof(p), C.c_void_p(stream)))
+        return int(x.value), p.value
 
     def schedule_info(self):
         a, b, c = C.c_int32(0), C.c_int32(0), C.c_int32(0)

@@ -55,7 +55,7 @@ struct gvqe_ctx {
     DPass *d_passes = nullptr; DGroup *d_groups = nullptr; DTerm *d_terms = nullptr;
     uint64_t *d_diag_z = nullptr; double *d_diag_c = nullptr; void *d_wstat = nullptr; uint32_t *d_gtabs = nullptr; DRs *d_rss = nullptr;
     std::vector<float> wstat_f;
-    void *d_table = nullptr; void *d_states = nullptr; void *d_cs = nullptr;
+    void *d_table = nullptr; void *d_states = nullptr; void *d_cs = nullptr; void *d_readout = nullptr;
     double *d_params = nullptr, *d_partial = nullptr, *d_E = nullptr;
     uint32_t slots_per_b = 0;
     uint64_t launches = 0;
@@ -280,7 +280,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -310,6 +310,7 @@ Layout layout_of(const gvqe_ctx *c)
     L.rss = cv.take(c->plan.rss.size() * sizeof(DRs));
     L.dz = cv.take(c->H.diag_z.size() * 8);
     L.dc = cv.take(c->H.diag_c.size() * 8);
+    L.readout = cv.take((size_t)(READOUT_BLOCKS + 1) * 16);
     L.table = cv.take(c->tab_bytes() << c->n_store);
     L.fixed_end = cv.off;
     const uint64_t tiles = 1ull << (c->n_store - c->plan.k);
@@ -369,6 +370,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs); c->d_rss = (DRs *)(w + L.rss);
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);
     c->d_table = w + L.table;
+    c->d_readout = w + L.readout;
     char *p = w + L.fixed_end;
     c->d_states = p; p += L.state_b * fit;
     c->d_cs = p; p += L.cs_b * fit;
@@ -558,6 +560,26 @@ gvqe_status gvqe_get_state(gvqe_ctx *c, int slot, void *host_out)
     if (e == cudaSuccess)
         e = cudaMemcpy(host_out, (char *)c->d_states + L.state_b * (size_t)slot, c->amp_bytes() << c->n_user, cudaMemcpyDeviceToHost);
     return e == cudaSuccess ? GVQE_OK : cuda_fail(c, e, "get_state");
+}
+
+gvqe_status gvqe_argmax(gvqe_ctx *c, int slot, uint64_t *x, double *prob, void *stream)
+{
+    if (!c || !x) return GVQE_ERR_INVALID_ARG;
+    if (c->dirty || !c->ws) return fail(c, GVQE_ERR_WORKSPACE, "argmax: no energy call has run on this workspace");
+    if (slot < 0 || slot >= c->in_flight) return fail(c, GVQE_ERR_INVALID_ARG, "argmax: slot out of range");
+    const Layout L = layout_of(c);
+    cudaStream_t st = (cudaStream_t)stream;
+    // idle padding qubits stay |0>: the user's amplitudes are the first 2^n_user of the stored state
+    const int ke = launch_argmax(c->prec, (char *)c->d_states + L.state_b * (size_t)slot, 1ull << c->n_user, c->d_readout, st,
+                                 &c->launches);
+    if (ke) return cuda_fail(c, ke, "argmax launch");
+    struct { double p; uint64_t x; } r;
+    cudaError_t e = cudaMemcpyAsync(&r, c->d_readout, sizeof r, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "argmax D2H");
+    *x = r.x;
+    if (prob) *prob = r.p;
+    return GVQE_OK;
 }
 
 gvqe_status gvqe_schedule_info(const gvqe_ctx *c, int32_t *nb, int32_t *np, int32_t *inflight)

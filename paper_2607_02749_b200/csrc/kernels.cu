@@ -1,6 +1,8 @@
 // kernels.cu -- __global__ wrappers and launchers (see kernels.cuh for the per-thread code).  sm_100a only.
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "kernels.cuh"
 #include "kernels.h"
 
@@ -288,6 +290,74 @@ __global__ void __launch_bounds__(256) reduce_kernel(const double *__restrict__ 
     for (uint32_t i = threadIdx.x * stride; i < slots_per_b; i += blockDim.x * stride) v += p[i];
     const double s = block_sum(v, red);
     if (threadIdx.x == 0) E[blockIdx.x] = s;
+}
+
+// ---- read-out ("the bitstring with the highest probability") -------------------
+// One read-only sweep: every thread keeps the best (|psi_x|^2, x) of its 16-byte vectors, ties to the lowest x; warp
+// shuffles, one entry per block, then a single block picks the winner.  max / lowest-index are order independent, so
+// the result does not depend on the grid.  |psi|^2 = re*re + im*im in the working precision, each operation rounded
+// separately (no FMA contraction) so that the decision is reproducible outside the kernel.
+struct ProbIdx { double p; uint64_t x; };
+__device__ __forceinline__ float prob_of(cx<float> a) { return __fadd_rn(__fmul_rn(a.x, a.x), __fmul_rn(a.y, a.y)); }
+__device__ __forceinline__ double prob_of(cx<double> a) { return __dadd_rn(__dmul_rn(a.x, a.x), __dmul_rn(a.y, a.y)); }
+__device__ __forceinline__ void take_better(double &p, uint64_t &x, double q, uint64_t y)
+{
+    if (q > p || (q == p && y < x)) { p = q; x = y; }
+}
+__device__ __forceinline__ void block_best(double &p, uint64_t &x, ProbIdx *red)
+{
+    for (int o = 16; o > 0; o >>= 1) {
+        const double q = __shfl_down_sync(0xffffffffu, p, o);
+        const uint64_t y = __shfl_down_sync(0xffffffffu, x, o);
+        take_better(p, x, q, y);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) red[w] = ProbIdx{p, x};
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int i = 1; i < (int)(blockDim.x >> 5); ++i) take_better(p, x, red[i].p, red[i].x);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) argmax_partial_kernel(const cx<T> *__restrict__ state, uint64_t count, ProbIdx *out)
+{
+    __shared__ ProbIdx red[8];
+    constexpr uint32_t V = 16 / (uint32_t)sizeof(cx<T>);
+    double bp = -1.0;
+    uint64_t bx = ~0ull;
+    const uint64_t nvec = count / V, step = (uint64_t)gridDim.x * 256u;
+    for (uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x; i < nvec; i += step) {
+        const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + i * V);
+#pragma unroll
+        for (uint32_t j = 0; j < V; ++j) take_better(bp, bx, (double)prob_of(v.v[j]), i * V + j);
+    }
+    if (count < V && blockIdx.x == 0 && threadIdx.x == 0)   // a one-amplitude register
+        for (uint64_t x = 0; x < count; ++x) take_better(bp, bx, (double)prob_of(state[x]), x);
+    block_best(bp, bx, red);
+    if (threadIdx.x == 0) out[blockIdx.x] = ProbIdx{bp, bx};
+}
+
+__global__ void __launch_bounds__(256) argmax_final_kernel(const ProbIdx *__restrict__ part, uint32_t n_part, ProbIdx *out)
+{
+    __shared__ ProbIdx red[8];
+    double bp = -1.0;
+    uint64_t bx = ~0ull;
+    for (uint32_t i = threadIdx.x; i < n_part; i += 256u) take_better(bp, bx, part[i].p, part[i].x);
+    block_best(bp, bx, red);
+    if (threadIdx.x == 0) *out = ProbIdx{bp, bx};
+}
+
+int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, void *stream, uint64_t *launches)
+{
+    const uint64_t nvec = count / (prec == 0 ? 2 : 1);
+    uint32_t grid = (uint32_t)std::min<uint64_t>(READOUT_BLOCKS, (nvec + 255) / 256);
+    if (grid == 0) grid = 1;
+    ProbIdx *part = reinterpret_cast<ProbIdx *>(scratch);   // [0] = result, [1 ..] = per-block entries
+    if (prec == 0) argmax_partial_kernel<float><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<float> *)state, count, part + 1);
+    else argmax_partial_kernel<double><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<double> *)state, count, part + 1);
+    argmax_final_kernel<<<1, 256, 0, (cudaStream_t)stream>>>(part + 1, grid, part);
+    *launches += 2;
+    return (int)cudaGetLastError();
 }
 
 // ---- diagonal energy table: scatter c at index z, then in-place Walsh-Hadamard butterflies -------

@@ -17,6 +17,7 @@ struct GateLaunch {
 
 constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area
 constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
+constexpr uint32_t READOUT_BLOCKS = 148 * 8;   // grid of the read-out sweep: 8 blocks of 256 threads per SM
 constexpr uint32_t HDR_BYTES = 384;         // shared-memory header of the gate kernel
 constexpr uint32_t EXPECT_HDR_BYTES = 1024; // shared-memory header of the expectation kernel: holds the DPass copy
 
@@ -42,6 +43,8 @@ int launch_reduce(double *partial, uint32_t slots_per_b, double *E, int batch, v
 int launch_table_scatter(int prec, void *table, const uint64_t *z, const double *c, uint32_t count, void *stream,
                          uint64_t *launches);
 int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches);
+// Most probable basis state of `count` amplitudes; scratch: (READOUT_BLOCKS + 1) * 16 bytes, result {double p, uint64 x} at [0].
+int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, void *stream, uint64_t *launches);
 int kernels_init(void);   // opt-in shared memory sizes; returns the CUDA error
 
 }  // namespace gv

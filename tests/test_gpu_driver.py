@@ -118,3 +118,58 @@ def test_loop_follows_the_step_by_step_oracle(orc, n, D, budget):
     assert np.max(np.abs(hist - hist_o)) < 1e-8 * scale
     assert abs(res["E_best"] - E_o) < 1e-8 * scale
     assert np.max(np.abs(theta - th_o)) < 1e-6
+
+
+# ---- read-out (gvqe_argmax) -------------------------------------------------------------------
+def _check_argmax(x, p, p_ref, prec):
+    """x is a valid most-probable index of the oracle's distribution up to the precision of the stored amplitudes,
+    identical to the oracle's when the gap to the runner-up is larger than that."""
+    tol = 1e-12 if prec == "c128" else 2e-5 * float(p_ref.max()) + 1e-9
+    assert p_ref[x] >= p_ref.max() - tol
+    assert abs(p - p_ref[x]) <= tol
+    order = np.sort(p_ref)
+    if order[-1] - order[-2] > 2 * tol:
+        assert x == int(np.argmax(p_ref))
+
+
+@pytest.mark.parametrize("cfg,n,D,prec", [(1, 10, 3, "c128"), (2, 13, 2, "c128"), (3, 15, 2, "c64"), (4, 14, 2, "c64"),
+                                          (2, 3, 1, "c128"), (3, 1, 1, "c64")])
+def test_argmax_vs_oracle(orc, cfg, n, D, prec):
+    from oracle import readout_oracle as ro
+    w = make_workload(cfg, n=n, M=40, D=D, batch=3)
+    g = ctx(w, prec, in_flight=3)
+    g.energy_batch(w.params)
+    for slot in range(3):
+        p_ref = ro.probabilities(w.n, w.ops, w.params[slot])
+        x, p = g.argmax(slot)
+        _check_argmax(x, p, p_ref, prec)
+        psi = g.get_state(slot)                                    # the kernel's own decision on its own amplitudes
+        pk = (psi.real * psi.real + psi.imag * psi.imag)
+        assert x == int(np.argmax(pk)) and p == float(pk[x])
+
+
+@pytest.mark.parametrize("n,prec", [(12, "c128"), (26, "c64"), (25, "c128")])
+def test_argmax_product_state_closed_form(n, prec):
+    """Rotations only: bit q of x* is set exactly when sin^2(theta_q/2) > cos^2(theta_q/2) -- valid at sizes no host
+    evaluator reaches; the state spans many grid-stride rounds of the sweep."""
+    r = SplitMix64(100 + n)
+    theta = np.array([(2 * r.uniform() - 1) * 3.0 for _ in range(n)])
+    theta[np.abs(np.abs(theta) - np.pi / 2) < 0.05] += 0.2       # keep every qubit's decision away from the tie
+    g = gv.Gvqe(n, layout=dict(n_layers=0, entangler="cz", topology="linear"), precision=prec)
+    g.set_hamiltonian("Z" + "I" * (n - 1), [1.0])
+    g.alloc_workspace(1)
+    g.energy_batch(theta)
+    x, p = g.argmax(0)
+    s2, c2 = np.sin(theta / 2) ** 2, np.cos(theta / 2) ** 2
+    assert x == sum(1 << q for q in range(n) if s2[q] > c2[q])
+    assert abs(p - np.prod(np.maximum(s2, c2))) <= (1e-12 if prec == "c128" else 1e-5) * p
+    # basis state: RY(pi) on the bits of a pattern that includes the highest qubit
+    target = (1 << (n - 1)) | 0b1011
+    th = np.array([np.pi if (target >> q) & 1 else 0.0 for q in range(n)])
+    g.energy_batch(th)
+    x, p = g.argmax(0)
+    assert x == target and abs(p - 1.0) < 1e-5
+    g.energy_batch(np.zeros(n))                                    # |0...0>: every other probability is an exact 0
+    assert g.argmax(0) == (0, 1.0)
+    with pytest.raises(gv.GvqeError):
+        g.argmax(1)

@@ -233,3 +233,37 @@ def test_driver_oracle_separable_minimum_and_frozen_coordinates():
     th, E, hist, epochs, steps, reason = do.graph_vqe_minimize(energy, th0, masks, max_epochs=9, block_iters=0,
                                                                global_iters=0, epoch_patience=2)
     assert np.array_equal(th, th0) and epochs == 2 and reason == 1 and steps == 0
+
+
+# ---- pins of the read-out oracle (oracle/readout_oracle.py) -----------------------------------------------------------
+def test_readout_oracle_product_state_closed_form():
+    """RY(theta_q) on every qubit: p(x) = prod_q (cos^2 or sin^2)(theta_q / 2), so bit q of the most probable x is set
+    exactly when sin^2 > cos^2, and p(x*) is the product of the larger factors."""
+    from oracle import readout_oracle as ro
+    n = 9
+    r = SplitMix64(11)
+    theta = np.array([(2 * r.uniform() - 1) * 3.1 for _ in range(n)])
+    ops = [(0, q, -1, q) for q in range(n)]
+    x, p = ro.most_probable(n, ops, theta)
+    s2, c2 = np.sin(theta / 2) ** 2, np.cos(theta / 2) ** 2
+    assert x == sum(1 << q for q in range(n) if s2[q] > c2[q])
+    assert abs(p - np.prod(np.maximum(s2, c2))) < 1e-14
+    assert abs(ro.probabilities(n, ops, theta).sum() - 1.0) < 1e-13
+
+
+def test_readout_oracle_basis_state_and_tie():
+    """RY(pi) on chosen qubits prepares the basis state |x>: p = 1 there.  GHZ (RY(pi/2) on qubit 0, CNOT chain) has
+    two equal maxima at 0 and 2^n - 1 up to rounding; exact ties (RY(0) everywhere, Z-rotations only) go to the lowest x."""
+    from oracle import readout_oracle as ro
+    n = 6
+    target = 0b101101
+    ops = [(0, q, -1, q) for q in range(n)]
+    theta = np.array([np.pi if (target >> q) & 1 else 0.0 for q in range(n)])
+    x, p = ro.most_probable(n, ops, theta)
+    assert x == target and abs(p - 1.0) < 1e-14
+    ghz = [(0, 0, -1, 0)] + [(3, q + 1, q, -1) for q in range(n - 1)]
+    pr = ro.probabilities(n, ghz, np.array([np.pi / 2]))
+    assert abs(pr[0] - 0.5) < 1e-15 and abs(pr[-1] - 0.5) < 1e-15 and pr[1:-1].max() == 0.0
+    # an exact tie: X-rotation-free circuit on |0..0> plus one RY(pi/2) whose two branches are bit-identical in modulus
+    x, p = ro.most_probable(2, [(0, 1, -1, 0), (1, 1, -1, 1)], np.array([0.0, 0.7]))
+    assert x == 0 and abs(p - 1.0) < 1e-15
