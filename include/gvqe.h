@@ -117,6 +117,15 @@ gvqe_status gvqe_get_state(gvqe_ctx *ctx, int slot, void *host_out);
  * context's precision, each operation rounded separately.  One read-only sweep of the state on the GPU. */
 gvqe_status gvqe_argmax(gvqe_ctx *ctx, int slot, uint64_t *x, double *prob, void *cuda_stream);
 
+/* Shot sampling, PAPER.md:245, 256 ("this state is sampled"; 8192 shots): n_shots (<= 65536 per call) bitstrings
+ * distributed as |psi_x|^2 over the state in slot `slot`, by inversion of the cumulative distribution in index
+ * order: x[s] = the first x with sum_{y<=x} |psi_y|^2 > u[s] * Z, Z = sum_y |psi_y|^2.  The random numbers are the
+ * caller's: u: HOST, n_shots doubles in [0,1); x: HOST, n_shots results; *norm (HOST, optional) = Z.  Sums are fp64 in
+ * a fixed order (deterministic); a shot whose u * Z falls within rounding of a cumulative boundary may land on
+ * either neighbour. */
+gvqe_status gvqe_sample(gvqe_ctx *ctx, int slot, int n_shots, const double *u, uint64_t *x, double *norm,
+                        void *cuda_stream);
+
 /* Introspection of the compiled schedule (host; for tests and traffic accounting).
  * gvqe_schedule_info: number of fused gate blocks, number of off-diagonal passes, statevectors in flight.
  * gvqe_dump_schedule: writes a text description of every block/stage/op into buf (NUL-terminated, truncated to

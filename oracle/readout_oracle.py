@@ -26,3 +26,17 @@ def most_probable(n: int, ops, theta):
         if p[x] > p[best]:
             best = x
     return best, float(p[best])
+
+
+def sample(n: int, ops, theta, u):
+    """Shot sampling by inversion ("this state is sampled", 256: 8192 shots; reading R2): with the
+    cumulative distribution F(x) = sum_{y <= x} p(y) in index order and Z = F(2^n - 1), shot s is the first x with
+    F(x) > u_s Z.  The uniforms u_s in [0,1) are inputs.  Returns (x[len(u)], Z)."""
+    p = probabilities(n, ops, theta)
+    F = np.cumsum(p)                      # running sum in index order, fp64
+    Z = float(F[-1])
+    out = np.empty(len(u), dtype=np.uint64)
+    for s, us in enumerate(u):
+        t = float(us) * Z
+        out[s] = min(int(np.searchsorted(F, t, side="right")), len(F) - 1)   # first x with F[x] > t
+    return out, Z

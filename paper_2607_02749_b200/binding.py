@@ -22,7 +22,7 @@ STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "G
 EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
-           "gvqe_get_state", "gvqe_argmax", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
+           "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
            "gvqe_merge_small_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
@@ -80,6 +80,7 @@ def load():
     L.gvqe_param_shift_grad.argtypes = [vp, vp, vp, vp, vp, vp]
     L.gvqe_get_state.argtypes = [vp, i32, vp]
     L.gvqe_argmax.argtypes = [vp, i32, vp, vp, vp]
+    L.gvqe_sample.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     L.gvqe_schedule_info.argtypes = [vp, vp, vp, vp]
     L.gvqe_dump_schedule.argtypes = [vp, C.c_char_p, sz]
     L.gvqe_dump_schedule.restype = sz
@@ -229,6 +230,15 @@ class Gvqe:
         x, p = C.c_uint64(0), C.c_double(0.0)
         self._check(self._L.gvqe_argmax(self._h, int(slot), C.addressof(x), C.addressof(p), C.c_void_p(stream)))
         return int(x.value), p.value
+
+    def sample(self, u, slot: int = 0, stream: int = 0):
+        """(x[n_shots] uint64, Z): inverse-CDF samples of |psi|^2 in slot `slot` for the caller's uniforms u in [0,1)."""
+        uu = np.ascontiguousarray(u, dtype=np.float64).reshape(-1)
+        x = np.zeros(max(len(uu), 1), dtype=np.uint64)
+        z = C.c_double(0.0)
+        self._check(self._L.gvqe_sample(self._h, int(slot), len(uu), uu.ctypes.data, x.ctypes.data, C.addressof(z),
+                                        C.c_void_p(stream)))
+        return x[:len(uu)], z.value
 
     def schedule_info(self):
         a, b, c = C.c_int32(0), C.c_int32(0), C.c_int32(0)

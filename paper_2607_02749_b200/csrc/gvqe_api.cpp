@@ -280,7 +280,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, params_b, partial_b;
 };
@@ -311,6 +311,9 @@ Layout layout_of(const gvqe_ctx *c)
     L.dz = cv.take(c->H.diag_z.size() * 8);
     L.dc = cv.take(c->H.diag_c.size() * 8);
     L.readout = cv.take((size_t)(READOUT_BLOCKS + 1) * 16);
+    L.smass = cv.take((((size_t)1 << c->n_store) >> SAMPLE_CHUNK_LOG2) * 8 + 16);   // n_store >= 10 > chunk bits - 3
+    L.su = cv.take((size_t)SAMPLE_MAX_SHOTS * 8);
+    L.sx = cv.take((size_t)SAMPLE_MAX_SHOTS * 8);
     L.table = cv.take(c->tab_bytes() << c->n_store);
     L.fixed_end = cv.off;
     const uint64_t tiles = 1ull << (c->n_store - c->plan.k);
@@ -579,6 +582,36 @@ gvqe_status gvqe_argmax(gvqe_ctx *c, int slot, uint64_t *x, double *prob, void *
     if (e != cudaSuccess) return cuda_fail(c, e, "argmax D2H");
     *x = r.x;
     if (prob) *prob = r.p;
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_sample(gvqe_ctx *c, int slot, int n_shots, const double *u, uint64_t *x, double *norm, void *stream)
+{
+    if (!c || n_shots < 0 || (n_shots > 0 && (!u || !x))) return GVQE_ERR_INVALID_ARG;
+    if ((uint32_t)n_shots > SAMPLE_MAX_SHOTS) return fail(c, GVQE_ERR_INVALID_ARG, "sample: more than 65536 shots in one call");
+    if (c->dirty || !c->ws) return fail(c, GVQE_ERR_WORKSPACE, "sample: no energy call has run on this workspace");
+    if (slot < 0 || slot >= c->in_flight) return fail(c, GVQE_ERR_INVALID_ARG, "sample: slot out of range");
+    for (int s = 0; s < n_shots; ++s)
+        if (!(u[s] >= 0.0 && u[s] < 1.0)) return fail(c, GVQE_ERR_INVALID_ARG, "sample: uniforms must lie in [0, 1)");
+    const Layout L = layout_of(c);
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint64_t count = 1ull << c->n_user;
+    const uint64_t n_chunks = (count + (1u << SAMPLE_CHUNK_LOG2) - 1) >> SAMPLE_CHUNK_LOG2;
+    double *mass = (double *)(c->ws + L.smass), *total = mass + n_chunks;
+    double *u_dev = (double *)(c->ws + L.su);
+    uint64_t *x_dev = (uint64_t *)(c->ws + L.sx);
+    cudaError_t e = cudaSuccess;
+    if (n_shots) e = cudaMemcpyAsync(u_dev, u, (size_t)n_shots * 8, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "sample H2D");
+    const int ke = launch_sample(c->prec, (char *)c->d_states + L.state_b * (size_t)slot, count, mass, total, u_dev, x_dev,
+                                 (uint32_t)n_shots, st, &c->launches);
+    if (ke) return cuda_fail(c, ke, "sample launch");
+    if (n_shots) e = cudaMemcpyAsync(x, x_dev, (size_t)n_shots * 8, cudaMemcpyDeviceToHost, st);
+    double z = 0.0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&z, total, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "sample D2H");
+    if (norm) *norm = z;
     return GVQE_OK;
 }
 

@@ -360,6 +360,98 @@ int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, vo
     return (int)cudaGetLastError();
 }
 
+// ---- shot sampling ("this state is sampled", 256: 8192 shots) ---------------------
+// Inverse-CDF sampling from uniforms the caller supplies: x_s = the first x whose cumulative probability exceeds
+// u_s * Z, Z = sum_x |psi_x|^2.  Three kernels: probability mass of every chunk of 2^SAMPLE_CHUNK_LOG2 amplitudes
+// (fp64, fixed order), exclusive prefix over the chunks (one block, fixed order), then one warp per shot: binary
+// search over the chunk prefixes and a 32-wide running scan inside the chunk.  Deterministic.
+template <typename T>
+__global__ void __launch_bounds__(256) chunk_mass_kernel(const cx<T> *__restrict__ state, uint64_t count, uint32_t chunk_len,
+                                                         double *__restrict__ mass, uint64_t n_chunks)
+{
+    __shared__ double red[32];
+    for (uint64_t ci = blockIdx.x; ci < n_chunks; ci += gridDim.x) {
+        const cx<T> *p = state + ci * chunk_len;
+        const uint32_t len = (uint32_t)min((uint64_t)chunk_len, count - ci * chunk_len);
+        double v = 0.0;
+        for (uint32_t i = threadIdx.x; i < len; i += 256u) v += (double)prob_of(p[i]);
+        __syncthreads();   // red[] of the previous round has been read
+        const double s = block_sum(v, red);
+        if (threadIdx.x == 0) mass[ci] = s;
+    }
+}
+
+// In place: mass[i] <- sum_{j<i} mass[j]; *total <- sum of all.  One block; thread t owns a contiguous segment.
+__global__ void __launch_bounds__(1024) chunk_prefix_kernel(double *mass, uint64_t n_chunks, double *total)
+{
+    __shared__ double seg[1024];
+    const uint64_t per = (n_chunks + 1023) / 1024, lo = min(n_chunks, (uint64_t)threadIdx.x * per), hi = min(n_chunks, lo + per);
+    double s = 0.0;
+    for (uint64_t i = lo; i < hi; ++i) s += mass[i];
+    seg[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double run = 0.0;
+        for (int t = 0; t < 1024; ++t) { const double v = seg[t]; seg[t] = run; run += v; }
+        *total = run;
+    }
+    __syncthreads();
+    double run = seg[threadIdx.x];
+    for (uint64_t i = lo; i < hi; ++i) { const double v = mass[i]; mass[i] = run; run += v; }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) sample_kernel(const cx<T> *__restrict__ state, uint64_t count, uint32_t chunk_len,
+                                                     const double *__restrict__ prefix, uint64_t n_chunks,
+                                                     const double *__restrict__ total, const double *__restrict__ u,
+                                                     uint64_t *__restrict__ out, uint32_t n_shots)
+{
+    const uint32_t lane = threadIdx.x & 31u, shot = blockIdx.x * 8u + (threadIdx.x >> 5);
+    if (shot >= n_shots) return;
+    const double target = u[shot] * *total;
+    uint64_t lo = 0, hi = n_chunks;          // last chunk whose prefix is <= target
+    while (hi - lo > 1) {
+        const uint64_t mid = (lo + hi) >> 1;
+        if (prefix[mid] <= target) lo = mid; else hi = mid;
+    }
+    const uint64_t base = lo * chunk_len;
+    const uint32_t len = (uint32_t)min((uint64_t)chunk_len, count - base);
+    double run = prefix[lo];
+    uint64_t found = base + len - 1;         // rounding at the chunk end: the chunk's last amplitude
+    for (uint32_t i0 = 0; i0 < len; i0 += 32u) {
+        const uint32_t i = i0 + lane;
+        double v = i < len ? (double)prob_of(state[base + i]) : 0.0;
+        for (int o = 1; o < 32; o <<= 1) {   // inclusive scan over the 32 lanes, index order
+            const double w = __shfl_up_sync(0xffffffffu, v, o);
+            if ((int)lane >= o) v += w;
+        }
+        const unsigned hit = __ballot_sync(0xffffffffu, i < len && run + v > target);
+        if (hit) { found = base + i0 + (uint32_t)(__ffs(hit) - 1); break; }
+        run += __shfl_sync(0xffffffffu, v, 31);
+    }
+    if (lane == 0) out[shot] = found;
+}
+
+int launch_sample(int prec, const void *state, uint64_t count, double *mass, double *total, const double *u_dev,
+                  uint64_t *x_dev, uint32_t n_shots, void *stream, uint64_t *launches)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    const uint32_t chunk_len = 1u << SAMPLE_CHUNK_LOG2;
+    const uint64_t n_chunks = (count + chunk_len - 1) / chunk_len;
+    const uint32_t grid = (uint32_t)std::min<uint64_t>(n_chunks, READOUT_BLOCKS);
+    if (prec == 0) chunk_mass_kernel<float><<<grid, 256, 0, st>>>((const cx<float> *)state, count, chunk_len, mass, n_chunks);
+    else chunk_mass_kernel<double><<<grid, 256, 0, st>>>((const cx<double> *)state, count, chunk_len, mass, n_chunks);
+    chunk_prefix_kernel<<<1, 1024, 0, st>>>(mass, n_chunks, total);
+    *launches += 2;
+    if (n_shots) {
+        const uint32_t g2 = (n_shots + 7) / 8;
+        if (prec == 0) sample_kernel<float><<<g2, 256, 0, st>>>((const cx<float> *)state, count, chunk_len, mass, n_chunks, total, u_dev, x_dev, n_shots);
+        else sample_kernel<double><<<g2, 256, 0, st>>>((const cx<double> *)state, count, chunk_len, mass, n_chunks, total, u_dev, x_dev, n_shots);
+        ++*launches;
+    }
+    return (int)cudaGetLastError();
+}
+
 // ---- diagonal energy table: scatter c at index z, then in-place Walsh-Hadamard butterflies -------
 template <typename TT>
 __global__ void table_scatter_kernel(TT *table, const uint64_t *__restrict__ z, const double *__restrict__ c, uint32_t count)

@@ -18,6 +18,8 @@ struct GateLaunch {
 constexpr uint32_t EXPECT_TAB_CAP = 2048;   // complex entries of the shared-memory W-table area
 constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
 constexpr uint32_t READOUT_BLOCKS = 148 * 8;   // grid of the read-out sweep: 8 blocks of 256 threads per SM
+constexpr int SAMPLE_CHUNK_LOG2 = 12;            // shot sampling: probability mass is tabulated per 4096 amplitudes
+constexpr uint32_t SAMPLE_MAX_SHOTS = 1u << 16; // shots per gvqe_sample call (uniforms and results staged in the workspace)
 constexpr uint32_t HDR_BYTES = 384;         // shared-memory header of the gate kernel
 constexpr uint32_t EXPECT_HDR_BYTES = 1024; // shared-memory header of the expectation kernel: holds the DPass copy
 
@@ -45,6 +47,10 @@ int launch_table_scatter(int prec, void *table, const uint64_t *z, const double 
 int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches);
 // Most probable basis state of `count` amplitudes; scratch: (READOUT_BLOCKS + 1) * 16 bytes, result {double p, uint64 x} at [0].
 int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, void *stream, uint64_t *launches);
+// Inverse-CDF sampling: mass = ceil(count / 2^SAMPLE_CHUNK_LOG2) doubles (becomes the exclusive prefix), total = 1 double,
+// u_dev = n_shots uniforms in [0,1), x_dev = n_shots results.
+int launch_sample(int prec, const void *state, uint64_t count, double *mass, double *total, const double *u_dev,
+                  uint64_t *x_dev, uint32_t n_shots, void *stream, uint64_t *launches);
 int kernels_init(void);   // opt-in shared memory sizes; returns the CUDA error
 
 }  // namespace gv

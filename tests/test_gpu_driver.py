@@ -173,3 +173,62 @@ def test_argmax_product_state_closed_form(n, prec):
     assert g.argmax(0) == (0, 1.0)
     with pytest.raises(gv.GvqeError):
         g.argmax(1)
+
+
+# ---- shot sampling (gvqe_sample) ----------------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,D,prec", [(1, 10, 2, "c128"), (2, 14, 2, "c128"), (3, 15, 2, "c64"), (4, 13, 2, "c64"),
+                                          (2, 2, 1, "c128")])
+def test_sample_vs_oracle(orc, cfg, n, D, prec):
+    """Every shot is a valid inverse of the oracle's cumulative distribution (within the amplitude precision at the
+    boundaries); almost all shots are identical to the oracle's."""
+    from oracle import readout_oracle as ro
+    w = make_workload(cfg, n=n, M=30, D=D, batch=2)
+    g = ctx(w, prec, in_flight=2)
+    g.energy_batch(w.params)
+    r = SplitMix64(900 + n)
+    u = np.array([r.uniform() for _ in range(8192)])             # the paper's shot count
+    u[:3] = [0.0, 0.5, 1.0 - 2.0 ** -53]
+    for slot in range(2):
+        x, Z = g.sample(u, slot)
+        x_o, Z_o = ro.sample(w.n, w.ops, w.params[slot], u)
+        F = np.concatenate([[0.0], np.cumsum(ro.probabilities(w.n, w.ops, w.params[slot]))])
+        eps = 1e-12 if prec == "c128" else 1e-5
+        assert abs(Z - Z_o) <= eps
+        xi = x.astype(np.int64)
+        assert xi.min() >= 0 and xi.max() < (1 << w.n)
+        t = u * Z_o
+        assert np.all(F[xi] - eps <= t) and np.all(t <= F[xi + 1] + eps)
+        assert np.mean(x == x_o) > (0.999 if prec == "c128" else 0.98)
+        x2, _ = g.sample(u, slot)
+        assert np.array_equal(x, x2)                              # deterministic
+
+
+@pytest.mark.parametrize("n,prec", [(12, "c128"), (24, "c64")])
+def test_sample_quantiles_product_state(n, prec):
+    """Stratified uniforms: outcome counts equal S p(x) up to +-1 (closed-form p of a rotations-only circuit); at 24
+    qubits the shots are checked through their marginals: bit q is set in a fraction sin^2(theta_q/2) of the shots."""
+    r = SplitMix64(300 + n)
+    theta = np.array([(2 * r.uniform() - 1) * 3.0 for _ in range(n)])
+    g = gv.Gvqe(n, layout=dict(n_layers=0, entangler="cz", topology="linear"), precision=prec)
+    g.set_hamiltonian("Z" + "I" * (n - 1), [1.0])
+    g.alloc_workspace(1)
+    g.energy_batch(theta)
+    S = 65536
+    x, Z = g.sample((np.arange(S) + 0.5) / S, 0)
+    assert abs(Z - 1.0) < (1e-12 if prec == "c128" else 1e-5)
+    xi = x.astype(np.int64)
+    assert np.all(np.diff(xi) >= 0)
+    s2, c2 = np.sin(theta / 2) ** 2, np.cos(theta / 2) ** 2
+    if n <= 12:
+        p = np.ones(1 << n)
+        for q in range(n):
+            p *= np.where((np.arange(1 << n) >> q) & 1, s2[q], c2[q])
+        counts = np.bincount(xi, minlength=1 << n)
+        assert np.all(np.abs(counts - S * p) <= 1.0 + 1e-6)
+    for q in range(n):
+        assert abs(np.mean((xi >> q) & 1) - s2[q]) < 2e-3
+    with pytest.raises(gv.GvqeError):
+        g.sample([1.0], 0)
+    with pytest.raises(gv.GvqeError):
+        g.sample(np.zeros(65537), 0)
+    assert len(g.sample([], 0)[0]) == 0

@@ -267,3 +267,27 @@ def test_readout_oracle_basis_state_and_tie():
     # an exact tie: X-rotation-free circuit on |0..0> plus one RY(pi/2) whose two branches are bit-identical in modulus
     x, p = ro.most_probable(2, [(0, 1, -1, 0), (1, 1, -1, 1)], np.array([0.0, 0.7]))
     assert x == 0 and abs(p - 1.0) < 1e-15
+
+
+def test_readout_oracle_sampling_pins():
+    """One qubit after RY(theta): shot = 0 exactly when u < cos^2(theta/2).  A basis state: every shot is that state.
+    Stratified uniforms u_s = (s + 1/2)/S turn inversion into quantiles: every outcome x is drawn S p(x) times up to
+    +-1 (p from the product-state closed form)."""
+    from oracle import readout_oracle as ro
+    th = 1.1
+    u = np.array([0.0, 0.3, np.cos(th / 2) ** 2 - 1e-9, np.cos(th / 2) ** 2 + 1e-9, 0.999999])
+    x, Z = ro.sample(1, [(0, 0, -1, 0)], np.array([th]), u)
+    assert list(x) == [0, 0, 0, 1, 1] and abs(Z - 1.0) < 1e-15
+    n, target = 5, 0b10110
+    ops = [(0, q, -1, q) for q in range(n)]
+    x, Z = ro.sample(n, ops, np.array([np.pi if (target >> q) & 1 else 0.0 for q in range(n)]), np.linspace(1e-6, 0.999, 17))   # RY(pi) leaves ~1e-33 of mass elsewhere: u = 0 would land there
+    assert np.all(x == target)
+    r = SplitMix64(5)
+    theta = np.array([(2 * r.uniform() - 1) * 3.0 for _ in range(n)])
+    S = 4096
+    x, Z = ro.sample(n, ops, theta, (np.arange(S) + 0.5) / S)
+    s2, c2 = np.sin(theta / 2) ** 2, np.cos(theta / 2) ** 2
+    p = np.array([np.prod([s2[q] if (y >> q) & 1 else c2[q] for q in range(n)]) for y in range(1 << n)])
+    counts = np.bincount(x.astype(np.int64), minlength=1 << n)
+    assert np.all(np.abs(counts - S * p) <= 1.0 + 1e-9)
+    assert np.all(np.diff(x.astype(np.int64)) >= 0)              # inversion is monotone in u
