@@ -169,6 +169,11 @@ gvqe_status gvqe_louvain(int n, const double *w, double gamma, int32_t *communit
  * s_min qubits, the smallest such block (ties: lowest label) joins the block it shares the largest total weight
  * with (ties: lowest label).  community: in/out, relabelled by first appearance; *n_communities = new K. */
 gvqe_status gvqe_merge_small_blocks(int n, const double *w, int s_min, int32_t *community, int32_t *n_communities);
+/* The comparison partition of PAPER.md:229 ("geometric alternating offsets"): consecutive qubits in blocks of
+ * block_size, the block boundaries shifted by offset (0 <= offset < block_size): qubits [0, offset) form the first
+ * block when offset > 0, then [offset, offset + block_size), ...  Alternating the offset between epochs (e.g. 0 and
+ * block_size / 2) is the caller's loop.  community: n labels out, *n_communities = K. */
+gvqe_status gvqe_geometric_blocks(int n, int block_size, int offset, int32_t *community, int32_t *n_communities);
 /* theta_{B_i} (reading A11): mask[p] = 1 when parameter p drives a rotation on a qubit q with
  * community[q] == block, else 0.  mask: P bytes. */
 gvqe_status gvqe_block_param_mask(const gvqe_ctx *ctx, const int32_t *community, int32_t block, uint8_t *mask);

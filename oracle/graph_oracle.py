@@ -134,3 +134,11 @@ def block_param_mask(ops, n_params: int, community, block: int) -> np.ndarray:
         if kind in (0, 1) and param >= 0 and community[q0] == block:
             mask[param] = 1
     return mask
+
+
+def geometric_blocks(n: int, block_size: int, offset: int = 0):
+    """PAPER.md:229 "geometric alternating offsets" (reading G7): block boundaries at offset, offset + block_size, ...;
+    labels in qubit order."""
+    bounds = [b for b in range(offset, n, block_size)]
+    lab = [sum(1 for b in bounds if b <= q and b > 0) for q in range(n)]
+    return _first_appearance(lab), max(lab) + 1 if n else 0

@@ -24,7 +24,7 @@ EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
-           "gvqe_merge_small_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
+           "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
 
 class GvqeLayout(C.Structure):
@@ -94,6 +94,7 @@ def load():
     L.gvqe_louvain.argtypes = [i32, vp, C.c_double, vp, vp, vp]
     L.gvqe_merge_small_blocks.argtypes = [i32, vp, i32, vp, vp]
     L.gvqe_block_param_mask.argtypes = [vp, vp, i32, vp]
+    L.gvqe_geometric_blocks.argtypes = [i32, i32, i32, vp, vp]
     L.gvqe_graph_vqe_minimize.argtypes = [vp, C.POINTER(GvqeOptOptions), vp, vp, C.POINTER(GvqeOptResult), vp, i32, vp, vp]
     L.gvqe_last_error.argtypes = [vp]
     L.gvqe_last_error.restype = C.c_char_p
@@ -328,3 +329,10 @@ def merge_small_blocks(w, community, s_min: int):
     k = C.c_int32(0)
     _graph_check(load().gvqe_merge_small_blocks(w.shape[0], w.ctypes.data, int(s_min), c.ctypes.data, C.addressof(k)), "gvqe_merge_small_blocks")
     return c, k.value
+
+
+def geometric_blocks(n: int, block_size: int, offset: int = 0):
+    c = np.zeros(max(n, 1), dtype=np.int32)
+    k = C.c_int32(0)
+    _graph_check(load().gvqe_geometric_blocks(int(n), int(block_size), int(offset), c.ctypes.data, C.addressof(k)), "gvqe_geometric_blocks")
+    return c[:n], k.value

@@ -754,6 +754,14 @@ gvqe_status gvqe_merge_small_blocks(int n, const double *w, int s_min, int32_t *
     return GVQE_OK;
 }
 
+gvqe_status gvqe_geometric_blocks(int n, int block_size, int offset, int32_t *community, int32_t *n_communities)
+{
+    if (n < 1 || block_size < 1 || offset < 0 || offset >= block_size || !community) return GVQE_ERR_INVALID_ARG;
+    for (int q = 0; q < n; ++q) community[q] = q < offset ? 0 : (q - offset) / block_size + (offset > 0 ? 1 : 0);
+    if (n_communities) *n_communities = community[n - 1] + 1;
+    return GVQE_OK;
+}
+
 gvqe_status gvqe_block_param_mask(const gvqe_ctx *c, const int32_t *community, int32_t block, uint8_t *mask)
 {
     if (!c || !community || (c->P > 0 && !mask)) return GVQE_ERR_INVALID_ARG;

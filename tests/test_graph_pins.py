@@ -291,3 +291,17 @@ def test_readout_oracle_sampling_pins():
     counts = np.bincount(x.astype(np.int64), minlength=1 << n)
     assert np.all(np.abs(counts - S * p) <= 1.0 + 1e-9)
     assert np.all(np.diff(x.astype(np.int64)) >= 0)              # inversion is monotone in u
+
+
+def test_geometric_blocks_by_hand_and_library():
+    assert go.geometric_blocks(7, 3, 0) == ([0, 0, 0, 1, 1, 1, 2], 3)
+    assert go.geometric_blocks(7, 3, 1) == ([0, 1, 1, 1, 2, 2, 2], 3)
+    assert go.geometric_blocks(7, 3, 2) == ([0, 0, 1, 1, 1, 2, 2], 3)
+    assert go.geometric_blocks(4, 8, 0) == ([0, 0, 0, 0], 1)
+    for n in (1, 5, 16, 28):
+        for bs in (1, 2, 4, 5):
+            for off in range(bs):
+                lab, K = gb.geometric_blocks(n, bs, off)
+                assert (list(lab), K) == go.geometric_blocks(n, bs, off)
+    with pytest.raises(gv.GvqeError):
+        gb.geometric_blocks(5, 2, 2)
