@@ -319,14 +319,25 @@ __device__ __forceinline__ void block_best(double &p, uint64_t &x, ProbIdx *red)
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) argmax_partial_kernel(const cx<T> *__restrict__ state, uint64_t count, ProbIdx *out)
+__global__ void __launch_bounds__(256, 8) argmax_partial_kernel(const cx<T> *__restrict__ state, uint64_t count, ProbIdx *out)
 {
     __shared__ ProbIdx red[8];
     constexpr uint32_t V = 16 / (uint32_t)sizeof(cx<T>);
+    constexpr int U = 4;   // independent 16-byte loads in flight per thread (8 resident blocks per SM: one wave of 148 x 8)
     double bp = -1.0;
     uint64_t bx = ~0ull;
     const uint64_t nvec = count / V, step = (uint64_t)gridDim.x * 256u;
-    for (uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x; i < nvec; i += step) {
+    uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x;
+    for (; i + (U - 1) * step < nvec; i += U * step) {
+        vec16<T> v[U];
+#pragma unroll
+        for (int r = 0; r < U; ++r) v[r] = *reinterpret_cast<const vec16<T> *>(state + (i + r * step) * V);
+#pragma unroll
+        for (int r = 0; r < U; ++r)
+#pragma unroll
+            for (uint32_t j = 0; j < V; ++j) take_better(bp, bx, (double)prob_of(v[r].v[j]), (i + r * step) * V + j);
+    }
+    for (; i < nvec; i += step) {
         const vec16<T> v = *reinterpret_cast<const vec16<T> *>(state + i * V);
 #pragma unroll
         for (uint32_t j = 0; j < V; ++j) take_better(bp, bx, (double)prob_of(v.v[j]), i * V + j);
@@ -366,18 +377,33 @@ int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, vo
 // (fp64, fixed order), exclusive prefix over the chunks (one block, fixed order), then one warp per shot: binary
 // search over the chunk prefixes and a 32-wide running scan inside the chunk.  Deterministic.
 template <typename T>
-__global__ void __launch_bounds__(256) chunk_mass_kernel(const cx<T> *__restrict__ state, uint64_t count, uint32_t chunk_len,
-                                                         double *__restrict__ mass, uint64_t n_chunks)
+__global__ void __launch_bounds__(256, 6) chunk_mass_kernel(const cx<T> *__restrict__ state, uint64_t count, uint32_t chunk_len,
+                                                            double *__restrict__ mass, uint64_t n_chunks)
 {
-    __shared__ double red[32];
-    for (uint64_t ci = blockIdx.x; ci < n_chunks; ci += gridDim.x) {
+    // one warp per chunk (no block barrier): lane-local sums over 16-byte vectors, four loads in flight, then shuffles
+    constexpr uint32_t V = 16 / (uint32_t)sizeof(cx<T>);
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint64_t nwarps = (uint64_t)gridDim.x * 8u;
+    for (uint64_t ci = (uint64_t)blockIdx.x * 8u + (threadIdx.x >> 5); ci < n_chunks; ci += nwarps) {
         const cx<T> *p = state + ci * chunk_len;
         const uint32_t len = (uint32_t)min((uint64_t)chunk_len, count - ci * chunk_len);
         double v = 0.0;
-        for (uint32_t i = threadIdx.x; i < len; i += 256u) v += (double)prob_of(p[i]);
-        __syncthreads();   // red[] of the previous round has been read
-        const double s = block_sum(v, red);
-        if (threadIdx.x == 0) mass[ci] = s;
+        if (len == chunk_len) {
+            const uint32_t nv = chunk_len / V;   // a multiple of 128
+            for (uint32_t i = lane; i < nv; i += 128u) {
+                vec16<T> a[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) a[r] = *reinterpret_cast<const vec16<T> *>(p + (size_t)(i + 32u * r) * V);
+#pragma unroll
+                for (int r = 0; r < 4; ++r)
+#pragma unroll
+                    for (uint32_t j = 0; j < V; ++j) v += (double)prob_of(a[r].v[j]);
+            }
+        } else {
+            for (uint32_t i = lane; i < len; i += 32u) v += (double)prob_of(p[i]);
+        }
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) mass[ci] = v;
     }
 }
 
@@ -438,7 +464,7 @@ int launch_sample(int prec, const void *state, uint64_t count, double *mass, dou
     cudaStream_t st = (cudaStream_t)stream;
     const uint32_t chunk_len = 1u << SAMPLE_CHUNK_LOG2;
     const uint64_t n_chunks = (count + chunk_len - 1) / chunk_len;
-    const uint32_t grid = (uint32_t)std::min<uint64_t>(n_chunks, READOUT_BLOCKS);
+    const uint32_t grid = (uint32_t)std::min<uint64_t>((n_chunks + 7) / 8, READOUT_BLOCKS);
     if (prec == 0) chunk_mass_kernel<float><<<grid, 256, 0, st>>>((const cx<float> *)state, count, chunk_len, mass, n_chunks);
     else chunk_mass_kernel<double><<<grid, 256, 0, st>>>((const cx<double> *)state, count, chunk_len, mass, n_chunks);
     chunk_prefix_kernel<<<1, 1024, 0, st>>>(mass, n_chunks, total);
