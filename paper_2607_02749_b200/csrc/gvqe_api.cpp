@@ -3,6 +3,7 @@
 // the caller's workspace.  No CPU fallback: every energy is computed by the kernels in kernels.cu.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -530,12 +531,131 @@ gvqe_status gvqe_energy_batch(gvqe_ctx *c, const double *params, int B, double *
     return GVQE_OK;
 }
 
+// Shared-prefix evaluation of a parameter-shift set.  A shifted row differs from theta in one
+// parameter, so up to the fused block in which that parameter is first read its state IS the state of theta.  The base
+// state advances block by block in slot 0; before block j runs on it, the rows whose parameter enters at block j copy
+// it into the other slots and run blocks j.. and the expectation passes there.  Every row still sees the same kernels
+// on the same data as in gvqe_energy_batch, so the energies are bit-identical to the unshared evaluation.
+// Returns GVQE_ERR_UNSUPPORTED when the scheme does not apply (one slot, schedule bookkeeping missing): caller falls back.
+static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const std::vector<int> &idx, double *E_pm /* 2 per idx */,
+                                      double *E0, cudaStream_t st)
+{
+    gvqe_status s = ensure_ready(c, st);
+    if (s != GVQE_OK) return s;
+    const int P = c->P, F = c->in_flight, NB = (int)c->dev.blocks.size();
+    if (F < 2 || NB == 0 || c->prog.block_ops.size() != (size_t)NB) return GVQE_ERR_UNSUPPORTED;
+    // first launch that reads each parameter: -1 = the product-state kernel, j = fused block j, -2 = no gate
+    std::vector<int> first((size_t)P, -2);
+    for (int32_t q : c->px.rot_param) if (q >= 0 && q < P) first[q] = -1;
+    for (int j = 0; j < NB; ++j)
+        for (int oi : c->prog.block_ops[j]) {
+            const size_t gi = (size_t)oi + (size_t)c->px.n_ops;
+            if (gi >= c->ops.size()) return GVQE_ERR_UNSUPPORTED;
+            const int q = c->ops[gi].param;
+            if (q >= 0 && first[q] == -2) first[q] = j;
+        }
+    std::vector<std::vector<int>> group((size_t)NB + 1);   // [0] = product-state kernel, [j + 1] = block j; entries index idx
+    for (size_t a = 0; a < idx.size(); ++a) {
+        const int f = first[idx[a]];
+        if (f == -2) { E_pm[2 * a] = E_pm[2 * a + 1] = 0.0; continue; }   // the energy does not depend on it
+        group[(size_t)(f + 1)].push_back((int)a);
+    }
+    const Layout L = layout_of(c);
+    const uint64_t stride = L.state_b / c->amp_bytes();
+    const size_t S_bytes = c->amp_bytes() << c->n_store;
+    const uint32_t tiles = 1u << (c->n_store - c->plan.k);
+    const double half_pi = 1.57079632679489661923;
+    auto state_of = [&](int slot) { return (void *)((char *)c->d_states + L.state_b * (size_t)slot); };
+    auto cs_of = [&](int slot) { return (void *)((char *)c->d_cs + (size_t)slot * (size_t)P * c->amp_bytes()); };
+    auto blocks_from = [&](int j0, int slot, int nb) -> gvqe_status {
+        for (int j = j0; j < NB; ++j) {
+            const int ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j], c->dev.blocks[j].k, c->dev.blocks[j].smem_prog_bytes,
+                                             c->n_store, state_of(slot), stride, cs_of(slot), P, nb, st, &c->launches);
+            if (ke) return cuda_fail(c, ke, "gate block");
+        }
+        return GVQE_OK;
+    };
+    auto expect = [&](int slot, int nb) -> gvqe_status {
+        double *partial = c->d_partial + (size_t)slot * c->slots_per_b;
+        for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
+            const int ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat,
+                                              c->d_gtabs, c->d_rss, state_of(slot), stride, c->d_table, partial, c->slots_per_b,
+                                              (uint32_t)pi * tiles, nb, st, &c->launches);
+            if (ke) return cuda_fail(c, ke, "expectation pass");
+        }
+        const int ke = launch_reduce(partial, c->slots_per_b, c->d_E + slot, nb, st, &c->launches);
+        return ke ? cuda_fail(c, ke, "reduce") : GVQE_OK;
+    };
+    // base row: parameters and (cos, sin) in slot 0
+    cudaError_t e = cudaMemcpyAsync(c->d_params, params, (size_t)P * 8, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
+    int ke = launch_expand_params(c->prec, c->d_params, c->d_cs, (uint64_t)P, st, &c->launches);
+    if (ke) return cuda_fail(c, ke, "expand_params");
+    if (c->px.n_ops > 0 && (ke = launch_init_product(c->prec, c->pxd, c->d_states, stride, c->d_cs, P, 1, st, &c->launches)))
+        return cuda_fail(c, ke, "product-state init");
+    std::vector<double> rows((size_t)(F - 1) * P);
+    for (int g = 0; g <= NB; ++g) {
+        const int j0 = g - 1;   // -1: from the product-state kernel
+        std::vector<std::pair<int, int>> work;   // (entry of idx, 0 = plus / 1 = minus)
+        for (int a : group[g]) { work.push_back({a, 0}); work.push_back({a, 1}); }
+        for (size_t w0 = 0; w0 < work.size(); w0 += (size_t)(F - 1)) {
+            const int nb = (int)std::min(work.size() - w0, (size_t)(F - 1));
+            for (int r = 0; r < nb; ++r) {
+                for (int q = 0; q < P; ++q) rows[(size_t)r * P + q] = params[q];
+                rows[(size_t)r * P + idx[work[w0 + r].first]] += work[w0 + r].second ? -half_pi : half_pi;
+            }
+            e = cudaMemcpyAsync(c->d_params + P, rows.data(), (size_t)nb * P * 8, cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
+            if ((ke = launch_expand_params(c->prec, c->d_params + P, cs_of(1), (uint64_t)nb * P, st, &c->launches)))
+                return cuda_fail(c, ke, "expand_params");
+            if (j0 < 0) {
+                if ((ke = launch_init_product(c->prec, c->pxd, state_of(1), stride, cs_of(1), P, nb, st, &c->launches)))
+                    return cuda_fail(c, ke, "product-state init");
+            } else if (!(j0 == 0 && c->dev.blocks[0].source_zero)) {
+                for (int r = 0; r < nb; ++r) {
+                    e = cudaMemcpyAsync(state_of(1 + r), state_of(0), S_bytes, cudaMemcpyDeviceToDevice, st);
+                    if (e != cudaSuccess) return cuda_fail(c, e, "state copy");
+                }
+            }
+            if ((s = blocks_from(j0 < 0 ? 0 : j0, 1, nb)) != GVQE_OK || (s = expect(1, nb)) != GVQE_OK) return s;
+            std::vector<double> Et((size_t)nb);
+            e = cudaMemcpyAsync(Et.data(), c->d_E + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, st);
+            if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // rows / Et are reused by the next chunk
+            if (e != cudaSuccess) return cuda_fail(c, e, "E D2H");
+            for (int r = 0; r < nb; ++r) E_pm[2 * work[w0 + r].first + work[w0 + r].second] = Et[r];
+        }
+        if (j0 >= 0) {   // the base state advances by block j0
+            ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j0], c->dev.blocks[j0].k, c->dev.blocks[j0].smem_prog_bytes,
+                                   c->n_store, state_of(0), stride, cs_of(0), P, 1, st, &c->launches);
+            if (ke) return cuda_fail(c, ke, "gate block");
+        }
+    }
+    if ((s = expect(0, 1)) != GVQE_OK) return s;
+    e = cudaMemcpyAsync(E0, c->d_E, 8, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e == cudaSuccess ? GVQE_OK : cuda_fail(c, e, "E D2H");
+}
+
 gvqe_status gvqe_param_shift_grad(gvqe_ctx *c, const double *params, const uint8_t *mask, double *dE, double *E0, void *stream)
 {
     if (!c) return GVQE_ERR_INVALID_ARG;
     if (c->P > 0 && (!params || !mask || !dE)) return fail(c, GVQE_ERR_INVALID_ARG, "param_shift_grad: null input");
     std::vector<int> idx;
     for (int p = 0; p < c->P; ++p) if (mask[p]) idx.push_back(p);
+    for (int p = 0; p < c->P; ++p)
+        if (!std::isfinite(params[p])) return fail(c, GVQE_ERR_INVALID_ARG, "param_shift_grad: parameter is not finite");
+    if (!idx.empty() && env_int("GVQE_SHARED_PREFIX", 1) != 0) {
+        std::vector<double> Epm(2 * idx.size());
+        double e0 = 0.0;
+        const gvqe_status s = grad_shared_prefix(c, params, idx, Epm.data(), &e0, (cudaStream_t)stream);
+        if (s == GVQE_OK) {
+            for (int p = 0; p < c->P; ++p) dE[p] = 0.0;
+            for (size_t j = 0; j < idx.size(); ++j) dE[idx[j]] = 0.5 * (Epm[2 * j] - Epm[2 * j + 1]);   // Eq. 13
+            if (E0) *E0 = e0;
+            return GVQE_OK;
+        }
+        if (s != GVQE_ERR_UNSUPPORTED) return s;
+    }
     const int B = 2 * (int)idx.size() + 1;
     // Eq. 13: rows theta, theta +/- (pi/2) e_p for the masked p, ascending (reading A8)
     std::vector<double> rows((size_t)B * c->P), E((size_t)B);

@@ -232,3 +232,35 @@ def test_sample_quantiles_product_state(n, prec):
     with pytest.raises(gv.GvqeError):
         g.sample(np.zeros(65537), 0)
     assert len(g.sample([], 0)[0]) == 0
+
+
+# ---- shared-prefix parameter-shift sweeps ---------------------------------------------------------
+@pytest.mark.parametrize("cfg,n,D,prec,in_flight,prefix", [
+    (1, 10, 3, "c128", 16, None), (2, 16, 4, "c128", 8, None), (4, 15, 3, "c64", 8, "1"), (4, 16, 2, "c128", 3, "0"),
+    (3, 17, 3, "c64", 2, None), (4, 14, 2, "c64", 1, None), (2, 4, 2, "c128", 5, None)])
+def test_shared_prefix_gradient_is_bit_identical(orc, monkeypatch, cfg, n, D, prec, in_flight, prefix):
+    """gvqe_param_shift_grad with snapshots of the base state at the block boundaries returns exactly the numbers of
+    the plain evaluation of all 2|mask|+1 rows (each row sees the same kernels on the same data), with and without
+    the product-state prefix, for chunked groups and for a one-slot workspace (fallback); and both match the oracle."""
+    if prefix is not None:
+        monkeypatch.setenv("GVQE_PREFIX", prefix)
+    w = make_workload(cfg, n=n, M=60, D=D, batch=1)
+    g = ctx(w, prec, in_flight=in_flight)
+    r = SplitMix64(77 + n)
+    mask = np.array([1 if r.uniform() < 0.4 else 0 for _ in range(w.P)], dtype=np.uint8)
+    mask[0] = mask[w.P - 1] = 1                                   # first layer (prefix) and the last rotation layer
+    monkeypatch.setenv("GVQE_SHARED_PREFIX", "1")
+    l0 = g.launch_count()
+    dE, E0 = g.param_shift_grad(w.theta, mask)
+    l_shared = g.launch_count() - l0
+    monkeypatch.setenv("GVQE_SHARED_PREFIX", "0")
+    l0 = g.launch_count()
+    dE_plain, E0_plain = g.param_shift_grad(w.theta, mask)
+    l_plain = g.launch_count() - l0
+    assert E0 == E0_plain and np.array_equal(dE, dE_plain)
+    assert np.all(dE[mask == 0] == 0.0)
+    assert l_shared > 0 and l_plain > 0
+    dE_o, E0_o = orc.param_shift_grad(w.n, w.ops, w.theta, mask, w.paulis, w.coeffs)
+    scale = np.sum(np.abs(w.coeffs))
+    tol_ = 1e-10 * scale if prec == "c128" else 2e-5 * scale
+    assert abs(E0 - E0_o) <= tol_ and np.max(np.abs(dE - dE_o)) <= tol_
