@@ -230,6 +230,19 @@ def run_ours(args):
     stream.synchronize()
     ro_ms = r0.elapsed_time(r1) / n_ro
     ro_gbs = (8 if prec == "c64" else 16) * 2.0 ** w.n / (ro_ms * 1e-3) / 1e9
+    # whole parameter-shift sweep through gvqe_param_shift_grad (configs whose batch is a shift set): shared-prefix
+    # evaluation, host buffers, one untimed-region measurement of all 2|mask|+1 evaluations
+    sweep = None
+    if w.mask is not None:
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        g.param_shift_grad(w.theta, w.mask, stream.cuda_stream)
+        s1.record(stream)
+        stream.synchronize()
+        n_ev = 2 * int(w.mask.sum()) + 1
+        sweep = {"evaluations": n_ev, "seconds": s0.elapsed_time(s1) * 1e-3,
+                 "evals_per_s": n_ev / (s0.elapsed_time(s1) * 1e-3), "api": "gvqe_param_shift_grad",
+                 "shared_prefix": bool((8 if prec == "c64" else 16) * 2 ** max(w.n, 10) >= 16 << 20)}
     if rank != 0:
         return
     peak, peak_src = peaks()
@@ -257,6 +270,7 @@ def run_ours(args):
                         "avg_launch_ms": prof["expect_ms"] / max(prof["expect_launches"], 1)},
         "readout": {"kernel": "argmax_partial_kernel", "achieved": ro_gbs, "unit": "GB/s", "frac": ro_gbs / peak,
                     "ms_per_call": ro_ms, "note": "one state, includes the 16-byte D2H and the stream synchronise"},
+        "sweep": sweep,
         "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
     }
     print(json.dumps(line))

@@ -103,7 +103,10 @@ gvqe_status gvqe_energy_batch_device(gvqe_ctx *ctx, const double *params_dev, in
 /* Eq. 13 over the parameters with mask[p] != 0 (Eq. 11: the cluster's parameters).  params: HOST, P doubles;
  * mask: HOST, P bytes; dE: HOST, P doubles (0 where mask is 0); E0: HOST, optional (NULL allowed), receives
  * E(params).  The 2|mask|+1 evaluations run as one batch (row 0 = theta, rows 2j+1 / 2j+2 = +/- pi/2 on the
- * j-th masked parameter). */
+ * j-th masked parameter).  With more than one statevector in flight and states of at least 16 MiB (smaller ones are
+ * launch-bound; GVQE_SHARED_PREFIX=1 forces it) the rows are evaluated with shared prefixes: the
+ * state of theta advances block by block and a shifted row starts from the boundary at which its parameter is first
+ * read; the results are bit-identical to gvqe_energy_batch on the expanded rows (GVQE_SHARED_PREFIX=0 disables it). */
 gvqe_status gvqe_param_shift_grad(gvqe_ctx *ctx, const double *params, const uint8_t *mask, double *dE, double *E0,
                                   void *cuda_stream);
 

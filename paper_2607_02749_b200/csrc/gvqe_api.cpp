@@ -644,7 +644,9 @@ gvqe_status gvqe_param_shift_grad(gvqe_ctx *c, const double *params, const uint8
     for (int p = 0; p < c->P; ++p) if (mask[p]) idx.push_back(p);
     for (int p = 0; p < c->P; ++p)
         if (!std::isfinite(params[p])) return fail(c, GVQE_ERR_INVALID_ARG, "param_shift_grad: parameter is not finite");
-    if (!idx.empty() && env_int("GVQE_SHARED_PREFIX", 1) != 0) {
+    // shared prefixes pay when kernel time dominates launch overhead: states of >= 16 MiB unless forced (1) or disabled (0)
+    const int sp = env_int("GVQE_SHARED_PREFIX", -1);
+    if (!idx.empty() && (sp == 1 || (sp < 0 && (c->amp_bytes() << c->n_store) >= ((size_t)16 << 20)))) {
         std::vector<double> Epm(2 * idx.size());
         double e0 = 0.0;
         const gvqe_status s = grad_shared_prefix(c, params, idx, Epm.data(), &e0, (cudaStream_t)stream);
