@@ -2,7 +2,9 @@
 
 Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs may
 import this package.  The product (``paper_2607_02749_b200``) never does.  The arithmetic lives in plain C
-(``gvqe_oracle.c`` tier T0, ``gvqe_oracle_t1.c`` tier T1); this file only builds and marshals.
+(``gvqe_oracle.c`` tier T0, ``gvqe_oracle_t1.c`` tier T1); this file only builds and marshals.  Plain-Python oracles of
+what sits around the energy path: ``graph_oracle.py`` (Eq. 9, Eq. 10, Louvain, block merge, masks), ``driver_oracle.py``
+(the epoch loop, step by step) and ``readout_oracle.py`` (most probable bitstring, shot sampling by inversion).
 """
 from __future__ import annotations
 

@@ -1,9 +1,10 @@
-"""GPU tests of the host-side Graph-VQE loop (gvqe_graph_vqe_minimize).
+"""GPU tests of what round 1 built around the hot path, all through the C ABI:
 
-The loop is an iteration whose every energy and gradient comes from the CUDA kernels; it is checked by what the
-mathematics fixes: a separable problem with a closed-form minimum, the variational bound against the exact ground
-energy of the dense Hamiltonian (n <= 8), the returned energy re-evaluated by the oracle at the returned parameters,
-a vanishing oracle gradient at the returned point, and the bookkeeping (history, best-so-far, ablation)."""
+* the host-side Graph-VQE loop (gvqe_graph_vqe_minimize, NEXT-1): every energy and gradient comes from
+  the CUDA kernels; checked against its step-by-step oracle, a separable closed form, the variational bound against
+  the dense ground energy (n <= 8), the oracle's energy and gradient at the returned vector, and the bookkeeping;
+* the read-out (gvqe_argmax, gvqe_sample, NEXT-4) against oracle/readout_oracle.py and closed forms;
+* shared-prefix parameter-shift sweeps (NEXT-2): bit-identical to the plain evaluation."""
 import numpy as np
 import pytest
 
