@@ -5,8 +5,8 @@ G4-G6 of DESIGN.md: per epoch, warm start from theta*_best; every block minimise
 from that same vector with L-BFGS on parameter-shift gradients (Eq. 13); the block solutions are fused; a global
 refinement over all parameters follows; best-so-far and the epoch patience are updated.  Energies come from a
 callable `energy(rows[B,P]) -> E[B]` (the tests pass the complex128 oracle T0), so nothing here touches the library.
-Pins: tests/test_graph_pins.py::test_driver_oracle_* (quadratic with known minimiser, separable cosine closed form,
-Eq. 14 window by hand).
+Pins: tests/test_graph_pins.py::test_driver_oracle_* (search direction against the dense BFGS inverse-Hessian update and
+conjugacy / finite termination on a convex quadratic, separable cosine closed form, Eq. 14 window by hand).
 """
 from __future__ import annotations
 
@@ -31,6 +31,24 @@ def delta_max(hist, W):
     return max((abs(hist[t] - hist[t - 1]) for t in range(lo, len(hist))), default=0.0)
 
 
+def lbfgs_direction(g, S, Y):
+    """Search direction d = -H g of L-BFGS from the stored pairs (s_i, y_i), oldest first, by the two-loop recursion with
+    the initial matrix H0 = (s.y / y.y) I of the newest pair (H0 = I without pairs).  Pinned in tests/test_graph_pins.py
+    against the explicit dense BFGS inverse-Hessian update (reading G5: the optimiser details are the build's own;
+    PAPER.md:214, 225 only name SciPy's L-BFGS-B)."""
+    q = np.array(g, dtype=np.float64)
+    al = [0.0] * len(S)
+    for i in reversed(range(len(S))):
+        al[i] = float(S[i] @ q) / float(S[i] @ Y[i])
+        q = q - al[i] * Y[i]
+    if S:
+        q = q * (float(S[-1] @ Y[-1]) / float(Y[-1] @ Y[-1]))
+    for i in range(len(S)):
+        be = float(Y[i] @ q) / float(S[i] @ Y[i])
+        q = q + (al[i] - be) * S[i]
+    return -q
+
+
 def minimize_masked(energy, theta, mask, max_iters, *, tol, f_tol, window, patience, memory):
     """L-BFGS (two-loop recursion) on the masked coordinates, Armijo backtracking (c1 = 1e-4) over step lengths
     a0 * 2^-t tried four at a time; a0 = min(1, 1/|g|_inf) without curvature pairs, else 1.  Returns (theta, E, steps)."""
@@ -42,17 +60,7 @@ def minimize_masked(energy, theta, mask, max_iters, *, tol, f_tol, window, patie
         ginf = float(np.max(np.abs(g)))
         if ginf < 0.1 * f_tol:
             break
-        q = g.copy()
-        al = [0.0] * len(S)
-        for i in reversed(range(len(S))):
-            al[i] = float(S[i] @ q) / float(S[i] @ Y[i])
-            q = q - al[i] * Y[i]
-        if S:
-            q = q * (float(S[-1] @ Y[-1]) / float(Y[-1] @ Y[-1]))
-        for i in range(len(S)):
-            be = float(Y[i] @ q) / float(S[i] @ Y[i])
-            q = q + (al[i] - be) * S[i]
-        d = -q
+        d = lbfgs_direction(g, S, Y)
         dg = float(d @ g)
         if not dg < 0.0:
             S, Y = [], []

@@ -231,6 +231,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 sets[si] |= cg.first; members[si].push_back(cg.second);
             }
             for (size_t si = 0; si < sets.size(); ++si) {
+                if (plan.rss.size() >= 65536) break;   // DGroup::rs_id / the `hot` word hold 16 bits: further clusters take the lookup path
                 uint32_t regs = sets[si];
                 for (int b = 0; b < k && __builtin_popcount(regs) < RSB; ++b) regs |= 1u << b;   // pad with low bits
                 DRs rs; memset(&rs, 0, sizeof rs);

@@ -235,6 +235,57 @@ def test_driver_oracle_separable_minimum_and_frozen_coordinates():
     assert np.array_equal(th, th0) and epochs == 2 and reason == 1 and steps == 0
 
 
+def test_driver_oracle_search_direction_is_bfgs():
+    """The two-loop recursion must give d = -H_k g with H_k the dense BFGS inverse-Hessian update
+    H <- (I - rho s y^T) H (I - rho y s^T) + rho s s^T applied to the stored pairs, oldest first, from
+    H0 = (s.y / y.y) I of the newest pair (Nocedal & Wright, Alg. 7.4 / Eq. 6.17).  A sign or ordering slip in the
+    recursion fails this; steepest descent (what the restart falls back to) fails it too."""
+    from oracle import driver_oracle as do
+    rng = np.random.default_rng(11)
+    for dim, m in ((3, 1), (4, 2), (4, 3), (6, 5)):
+        A = rng.normal(size=(dim, dim))
+        A = A @ A.T + dim * np.eye(dim)                         # SPD Hessian: y = A s gives s.y > 0
+        S = [rng.normal(size=dim) for _ in range(m)]
+        Y = [A @ s_ for s_ in S]
+        g = rng.normal(size=dim)
+        H = (S[-1] @ Y[-1]) / (Y[-1] @ Y[-1]) * np.eye(dim)
+        for s_, y_ in zip(S, Y):
+            rho = 1.0 / (y_ @ s_)
+            V = np.eye(dim) - rho * np.outer(s_, y_)
+            H = V @ H @ V.T + rho * np.outer(s_, s_)
+        d = do.lbfgs_direction(g, S, Y)
+        assert np.allclose(d, -H @ g, rtol=1e-11, atol=1e-12), (dim, m)
+        assert d @ g < 0.0                                       # a descent direction
+        assert not np.allclose(d, -g, rtol=1e-3)                 # and not the steepest-descent one
+    assert np.array_equal(do.lbfgs_direction(np.array([1.0, -2.0]), [], []), np.array([-1.0, 2.0]))
+
+
+def test_driver_oracle_lbfgs_on_a_convex_quadratic():
+    """Exact line searches on f = x^T A x / 2 - b^T x with memory >= dimension: BFGS directions are A-conjugate and
+    the minimiser A^-1 b is reached in at most `dim` steps (textbook property; a wrong recursion loses both)."""
+    from oracle import driver_oracle as do
+    rng = np.random.default_rng(5)
+    dim = 5
+    A = rng.normal(size=(dim, dim))
+    A = A @ A.T + np.eye(dim)
+    b = rng.normal(size=dim)
+    x = rng.normal(size=dim)
+    g = A @ x - b
+    S, Y, D = [], [], []
+    for _ in range(dim):
+        d = do.lbfgs_direction(g, S, Y)
+        a = -(g @ d) / (d @ A @ d)                               # exact minimiser along d
+        s_ = a * d
+        x = x + s_
+        gn = A @ x - b
+        S.append(s_), Y.append(gn - g), D.append(d)
+        g = gn
+    assert np.linalg.norm(x - np.linalg.solve(A, b)) < 1e-8
+    for i in range(dim):
+        for j in range(i):
+            assert abs(D[i] @ A @ D[j]) < 1e-8 * np.sqrt((D[i] @ A @ D[i]) * (D[j] @ A @ D[j]))
+
+
 # ---- pins of the read-out oracle (oracle/readout_oracle.py) -----------------------------------------------------------
 def test_readout_oracle_product_state_closed_form():
     """RY(theta_q) on every qubit: p(x) = prod_q (cos^2 or sin^2)(theta_q / 2), so bit q of the most probable x is set

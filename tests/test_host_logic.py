@@ -34,11 +34,11 @@ def test_no_oracle_in_product():
                 assert "import oracle" not in src and "from oracle" not in src and "gvqe_oracle" not in src, f
 
 
-@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5, 6])
 def test_grouping_bit_exact_vs_oracle(orc, cfg):
     c = CONFIGS[cfg]
     w = make_workload(cfg, D=1, batch=1)            # full-size Hamiltonian, tiny circuit
-    g = gv.Gvqe(w.n, layout=dict(n_layers=1, entangler=w.entangler, topology=w.topology), precision="c64" if cfg > 2 else "c128")
+    g = gv.Gvqe(w.n, layout=dict(n_layers=1, entangler=w.entangler, topology=w.topology), precision="c128" if cfg in (1, 2, 6) else "c64")
     g.set_hamiltonian(w.paulis, w.coeffs)
     got = g.get_grouping(w.M)
     want = orc.grouping(w.n, w.paulis)
