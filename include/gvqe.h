@@ -68,6 +68,34 @@ gvqe_status gvqe_create(int n_qubits, const gvqe_layout *layout, gvqe_precision 
 /* Same from an explicit op list (host, n_ops entries; params are indices in [0, n_params)). */
 gvqe_status gvqe_create_ops(int n_qubits, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec,
                             gvqe_ctx **out);
+
+/* Schedule options: HOW the same energies are computed (the circuit is compiled once and reused).  Every
+ * field 0 = the library's default; results are identical up to floating-point reassociation whatever is chosen.  The
+ * library reads no environment variable; tests pass these to reach every code path at small sizes. */
+typedef struct {
+    int32_t tile_bits;        /* k: qubits of a shared-memory tile (default 13 complex64 / 12 complex128; up to 14) */
+    int32_t fixed_bits;       /* f: lowest qubits that are in every tile (default 4 / 3): 2^f contiguous amplitudes */
+    int32_t reg_bits;         /* R: register bits per stage (default 5 / 4) */
+    int32_t expect_tile_bits; /* tile bits of the expectation passes (default min(k, 13 / 12)) */
+    int32_t prefix;           /* write-only product-state kernel for the first layer: 0 = when it saves HBM
+                               * passes, 1 = never, 2 = whenever the circuit starts with a rotation layer */
+    int32_t register_stages;  /* expectation: flip-mask groups evaluated from registers: 0 = on, 1 = off */
+    int32_t shared_prefix;    /* gvqe_param_shift_grad: 0 = shared prefixes for states >= 16 MiB, 1 = never, 2 = always */
+    int32_t specialise;       /* gate kernels generated and compiled for the schedule at the first energy call (NVRTC):
+                               * 0 = for registers of >= 20 qubits when NVRTC is present, 1 = never (generic kernels),
+                               * 2 = whenever the schedule is supported; GVQE_ERR_UNSUPPORTED at the first energy call if
+                               * it is not or NVRTC is missing */
+    int32_t reserved[8];      /* must be 0 */
+} gvqe_options;
+/* gvqe_create / gvqe_create_ops with options (opt == NULL: defaults). */
+gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, const gvqe_options *opt,
+                            gvqe_ctx **out);
+gvqe_status gvqe_create_ops_opt(int n_qubits, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec,
+                                const gvqe_options *opt, gvqe_ctx **out);
+/* Source text of the specialised kernel of fused block `block` (0-based) as the library would compile it: written to
+ * buf (NUL-terminated, truncated to cap); returns the full length needed, 0 when the schedule has no such kernel.
+ * *smem_bytes (optional): its dynamic shared memory.  Host only (no GPU, no compiler). */
+size_t gvqe_kernel_source(const gvqe_ctx *ctx, int block, char *buf, size_t cap, int32_t *smem_bytes);
 int gvqe_num_params(const gvqe_ctx *ctx);
 int gvqe_num_qubits(const gvqe_ctx *ctx);
 
@@ -104,9 +132,9 @@ gvqe_status gvqe_energy_batch_device(gvqe_ctx *ctx, const double *params_dev, in
  * mask: HOST, P bytes; dE: HOST, P doubles (0 where mask is 0); E0: HOST, optional (NULL allowed), receives
  * E(params).  The 2|mask|+1 evaluations run as one batch (row 0 = theta, rows 2j+1 / 2j+2 = +/- pi/2 on the
  * j-th masked parameter).  With more than one statevector in flight and states of at least 16 MiB (smaller ones are
- * launch-bound; GVQE_SHARED_PREFIX=1 forces it) the rows are evaluated with shared prefixes: the
+ * launch-bound; gvqe_options.shared_prefix overrides) the rows are evaluated with shared prefixes: the
  * state of theta advances block by block and a shifted row starts from the boundary at which its parameter is first
- * read; the results are bit-identical to gvqe_energy_batch on the expanded rows (GVQE_SHARED_PREFIX=0 disables it). */
+ * read; the results are bit-identical to gvqe_energy_batch on the expanded rows. */
 gvqe_status gvqe_param_shift_grad(gvqe_ctx *ctx, const double *params, const uint8_t *mask, double *dE, double *E0,
                                   void *cuda_stream);
 

@@ -19,7 +19,7 @@ GVQE_C64, GVQE_C128 = 0, 1
 STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "GVQE_ERR_WORKSPACE",
                 "GVQE_ERR_UNSUPPORTED", "GVQE_ERR_CUDA"]
 
-EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
+EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
@@ -29,6 +29,13 @@ EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_num_params", "gvqe_num_qubits
 
 class GvqeLayout(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("entangler", C.c_int32), ("topology", C.c_int32), ("final_rot", C.c_int32)]
+
+
+class GvqeOptions(C.Structure):
+    """gvqe_options: how the same energies are computed (0 = library default for every field)."""
+    _fields_ = [("tile_bits", C.c_int32), ("fixed_bits", C.c_int32), ("reg_bits", C.c_int32), ("expect_tile_bits", C.c_int32),
+                ("prefix", C.c_int32), ("register_stages", C.c_int32), ("shared_prefix", C.c_int32), ("specialise", C.c_int32),
+                ("reserved", C.c_int32 * 8)]
 
 
 class GvqeOptOptions(C.Structure):
@@ -66,6 +73,10 @@ def load():
     vp, i32, u64, sz = C.c_void_p, C.c_int, C.c_uint64, C.c_size_t
     L.gvqe_create.argtypes = [i32, C.POINTER(GvqeLayout), i32, C.POINTER(vp)]
     L.gvqe_create_ops.argtypes = [i32, vp, i32, i32, i32, C.POINTER(vp)]
+    L.gvqe_create_opt.argtypes = [i32, C.POINTER(GvqeLayout), i32, C.POINTER(GvqeOptions), C.POINTER(vp)]
+    L.gvqe_create_ops_opt.argtypes = [i32, vp, i32, i32, i32, C.POINTER(GvqeOptions), C.POINTER(vp)]
+    L.gvqe_kernel_source.argtypes = [vp, i32, C.c_char_p, sz, vp]
+    L.gvqe_kernel_source.restype = sz
     L.gvqe_num_params.argtypes = [vp]
     L.gvqe_num_qubits.argtypes = [vp]
     L.gvqe_set_hamiltonian.argtypes = [vp, i32, C.c_char_p, vp]
@@ -112,19 +123,27 @@ class Gvqe:
     """One libgvqe context.  Method names mirror the C ABI without the gvqe_ prefix."""
 
     def __init__(self, n_qubits: int, *, layout: Optional[dict] = None, ops=None, n_params: Optional[int] = None,
-                 precision: str = "c128"):
+                 precision: str = "c128", options: Optional[dict] = None):
         self._L = load()
         self._h = C.c_void_p()
         self._ws = None
         prec = {"c64": GVQE_C64, "c128": GVQE_C128}[precision]
         self.precision = precision
+        opt = None
+        if options:
+            o_ = GvqeOptions()
+            for k_, v_ in options.items():
+                setattr(o_, k_, int(v_))   # unknown names raise AttributeError... ctypes structures accept only their fields
+                if k_ not in dict(GvqeOptions._fields_):
+                    raise GvqeError(GVQE_ERR_INVALID_ARG, f"unknown option {k_}")
+            opt = C.byref(o_)
         if layout is not None:
             lay = GvqeLayout(int(layout["n_layers"]), _ENT.get(layout["entangler"], layout["entangler"]),
                              _TOPO.get(layout["topology"], layout["topology"]), int(layout.get("final_rot", 1)))
-            st = self._L.gvqe_create(n_qubits, C.byref(lay), prec, C.byref(self._h))
+            st = self._L.gvqe_create_opt(n_qubits, C.byref(lay), prec, opt, C.byref(self._h))
         else:
             o = np.ascontiguousarray(np.asarray(ops, dtype=np.int32).reshape(-1, 4))
-            st = self._L.gvqe_create_ops(n_qubits, o.ctypes.data, len(o), int(n_params), prec, C.byref(self._h))
+            st = self._L.gvqe_create_ops_opt(n_qubits, o.ctypes.data, len(o), int(n_params), prec, opt, C.byref(self._h))
         if st != GVQE_OK:
             raise GvqeError(st, "gvqe_create failed")
         self.n = n_qubits
@@ -251,6 +270,16 @@ class Gvqe:
         buf = C.create_string_buffer(need + 1)
         self._L.gvqe_dump_schedule(self._h, buf, need + 1)
         return buf.value.decode()
+
+    def kernel_source(self, block: int):
+        """(source text, dynamic shared memory bytes) of the specialised kernel of fused block `block`, or None."""
+        sm = C.c_int32(0)
+        need = self._L.gvqe_kernel_source(self._h, int(block), None, 0, C.addressof(sm))
+        if need == 0:
+            return None
+        buf = C.create_string_buffer(need + 1)
+        self._L.gvqe_kernel_source(self._h, int(block), buf, need + 1, C.addressof(sm))
+        return buf.value.decode(), int(sm.value)
 
     def get_exec_order(self) -> np.ndarray:
         m = self._L.gvqe_get_exec_order(self._h, None, 0)

@@ -54,8 +54,7 @@ struct DStage {              // 68 bytes
     uint16_t op_begin, op_end;          // DOp entries (block-local)
     uint16_t cx_begin, cx_end;          // DCx entries (block-local): the trailing CNOT run
     uint16_t postbit[DEV_MAX_R];        // image of the unit vector of each register bit under the CNOT run (linear part)
-    uint8_t warp_sync_after;            // 1: the next stage's warps read only what the same warp wrote: __syncwarp suffices
-    uint8_t warp_sync_cx;               // 1: the CNOT-run write-back stays inside each warp's own footprint
+    uint8_t pad[2];
     uint32_t po_bytes[DEV_MAX_R];       // swizzled BYTE offset of each register bit: phys(1 << regbit) * sizeof(amplitude)
     uint32_t post_bytes[DEV_MAX_R];     // the same for postbit (write-back of a stage with a CNOT run)
 };

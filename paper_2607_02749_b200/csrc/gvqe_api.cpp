@@ -9,12 +9,14 @@
 #include <cstdlib>
 #include <cstring>
 #include <string>
+#include <thread>
 #include <utility>
 #include <vector>
 
 #include "../../include/gvqe.h"
 #include "graph.h"
 #include "hamiltonian.h"
+#include "jit.h"
 #include "kernels.h"
 #include "lower.h"
 #include "schedule.h"
@@ -25,11 +27,6 @@ namespace {
 constexpr int N_MIN_STORE = 10;   // smaller registers are padded with idle qubits (they stay |0>)
 constexpr int N_MAX = 34;
 inline size_t al256(size_t v) { return (v + 255) & ~(size_t)255; }
-int env_int(const char *name, int dflt)
-{
-    const char *s = getenv(name);
-    return (s && *s) ? atoi(s) : dflt;
-}
 }  // namespace
 
 struct gvqe_ctx {
@@ -61,6 +58,14 @@ struct gvqe_ctx {
     uint32_t slots_per_b = 0;
     uint64_t launches = 0;
     // profiling (gvqe_profile_enable): 4 events per chunk
+    gvqe_options opt{};
+    // schedule-specialised gate kernels (jit.h): generated at create, compiled and loaded at the first energy call
+    int jit_state = 0;          // 0 not tried, 1 loaded, -1 not used
+    int sm_count = 148;
+    int jit_per_cta = 1;        // work items per thread block of the specialised kernels (tuned on the B200)
+    std::vector<JitBlock> jit_blocks;
+    std::vector<JitModule *> jit_mods;
+    void *d_ry = nullptr;
     bool profiling = false;
     std::vector<cudaEvent_t> ev;
     double prof_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -78,7 +83,7 @@ gvqe_status cuda_fail(gvqe_ctx *c, int e, const char *what)
     return GVQE_ERR_CUDA;
 }
 
-gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_precision prec, gvqe_ctx **out)
+gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_precision prec, const gvqe_options *opt, gvqe_ctx **out)
 {
     if (!out) return GVQE_ERR_INVALID_ARG;
     *out = nullptr;
@@ -94,11 +99,19 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
     }
     gvqe_ctx *c = new gvqe_ctx();
     c->n_user = n; c->n_store = n < N_MIN_STORE ? N_MIN_STORE : n; c->prec = prec; c->P = n_params; c->ops = ops;
-    c->K = env_int("GVQE_K", prec == GVQE_C64 ? 13 : 12);
-    c->F = env_int("GVQE_F", prec == GVQE_C64 ? 4 : 3);
-    c->R = env_int("GVQE_R", prec == GVQE_C64 ? 5 : 4);
+    if (opt) {
+        c->opt = *opt;
+        bool bad = opt->tile_bits < 0 || opt->fixed_bits < 0 || opt->reg_bits < 0 || opt->expect_tile_bits < 0 || opt->prefix < 0 ||
+                   opt->prefix > 2 || opt->register_stages < 0 || opt->register_stages > 1 || opt->shared_prefix < 0 ||
+                   opt->shared_prefix > 2 || opt->specialise < 0 || opt->specialise > 2;
+        for (int32_t r : opt->reserved) bad = bad || r != 0;
+        if (bad) { delete c; return GVQE_ERR_INVALID_ARG; }
+    }
+    c->K = c->opt.tile_bits ? c->opt.tile_bits : (prec == GVQE_C64 ? 13 : 12);
+    c->F = c->opt.fixed_bits ? c->opt.fixed_bits : (prec == GVQE_C64 ? 4 : 3);
+    c->R = c->opt.reg_bits ? c->opt.reg_bits : (prec == GVQE_C64 ? 5 : 4);
     if (c->K > c->n_store) c->K = c->n_store;
-    c->KE = env_int("GVQE_KE", c->K > (prec == GVQE_C64 ? 13 : 12) ? (prec == GVQE_C64 ? 13 : 12) : c->K);
+    c->KE = c->opt.expect_tile_bits ? c->opt.expect_tile_bits : (c->K > (prec == GVQE_C64 ? 13 : 12) ? (prec == GVQE_C64 ? 13 : 12) : c->K);
     if (c->KE > c->n_store) c->KE = c->n_store;
     if (c->K < c->R + 5 || c->K > 14 || c->F < 1 || c->F >= c->K || c->K - c->R > 9) { delete c; return GVQE_ERR_INVALID_ARG; }
     std::string err;
@@ -109,15 +122,14 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
         delete c;
         return GVQE_ERR_UNSUPPORTED;
     }
-    const char *pf = getenv("GVQE_PREFIX");   // "0" = never, "1" = always when there is one, unset = by pass count
-    Prefix px = (pf && pf[0] == '0') || getenv("GVQE_NO_PREFIX") ? Prefix() : find_prefix(c->n_store, c->ops);
+    Prefix px = c->opt.prefix == 1 ? Prefix() : find_prefix(c->n_store, c->ops);
     if (px.n_ops > 0) {
         Program prog2; DevProgram dev2;
         const std::vector<HostOp> rest(c->ops.begin() + px.n_ops, c->ops.end());
         if (compile_program(c->n_store, rest, c->K, c->F, c->R, prog2, err, false) &&
             lower_program(prog2, (int)c->amp_bytes(), dev2, err)) {
             const size_t passes_plain = 2 * c->dev.blocks.size() - 1, passes_px = 1 + 2 * dev2.blocks.size();
-            if (passes_px < passes_plain || (pf && pf[0] == '1')) { c->px = px; c->prog = prog2; c->dev = dev2; }
+            if (passes_px < passes_plain || c->opt.prefix == 2) { c->px = px; c->prog = prog2; c->dev = dev2; }
         }
     }
     if (c->px.n_ops > 0) {   // execution order in terms of the caller's op list: prefix first, then the compiled rest
@@ -125,6 +137,17 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
         for (int i = 0; i < c->px.n_ops; ++i) eo.push_back(i);
         for (int e : c->prog.exec_order) eo.push_back(e + c->px.n_ops);
         c->prog.exec_order.swap(eo);
+    }
+    // specialised gate kernels: source only here (host work); compiled and loaded by ensure_ready on the device
+    {
+        std::string why;
+        const bool want = c->opt.specialise == 2 || (c->opt.specialise == 0 && c->n_store >= 20);
+        if (want && c->prog.blocks.size() == c->dev.blocks.size() && jit_supported(c->prog, c->prec, why)) {
+            c->jit_blocks.resize(c->prog.blocks.size());
+            for (size_t b = 0; b < c->prog.blocks.size(); ++b)
+                if (!jit_generate(c->prog, (int)b, c->prec, c->jit_blocks[b], why)) { c->jit_blocks.clear(); break; }
+        }
+        if (c->jit_blocks.empty()) c->jit_state = -1;
     }
     *out = c;
     return GVQE_OK;
@@ -135,6 +158,25 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
 extern "C" {
 
 gvqe_status gvqe_create(int n, const gvqe_layout *L, gvqe_precision prec, gvqe_ctx **out)
+{
+    return gvqe_create_opt(n, L, prec, nullptr, out);
+}
+
+gvqe_status gvqe_create_ops(int n, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec, gvqe_ctx **out)
+{
+    return gvqe_create_ops_opt(n, ops, n_ops, n_params, prec, nullptr, out);
+}
+
+size_t gvqe_kernel_source(const gvqe_ctx *c, int block, char *buf, size_t cap, int32_t *smem_bytes)
+{
+    if (!c || block < 0 || (size_t)block >= c->jit_blocks.size()) return 0;
+    const std::string &s = c->jit_blocks[(size_t)block].source;
+    if (smem_bytes) *smem_bytes = (int32_t)c->jit_blocks[(size_t)block].smem_bytes;
+    if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }
+    return s.size() + 1;
+}
+
+gvqe_status gvqe_create_opt(int n, const gvqe_layout *L, gvqe_precision prec, const gvqe_options *opt, gvqe_ctx **out)
 {
     if (!L || !out || n < 1 || n > N_MAX) return GVQE_ERR_INVALID_ARG;
     if (L->n_layers < 0 || L->n_layers > 4096 || (L->entangler != GVQE_OP_CZ && L->entangler != GVQE_OP_CNOT) ||
@@ -184,15 +226,16 @@ gvqe_status gvqe_create(int n, const gvqe_layout *L, gvqe_precision prec, gvqe_c
     }
     for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RY, q, -1, 2 * n * D + q});
     if (L->final_rot == 2) for (int q = 0; q < n; ++q) ops.push_back({GVQE_OP_RZ, q, -1, 2 * n * D + n + q});
-    return build_ctx(n, ops, 2 * n * D + n * L->final_rot, prec, out);
+    return build_ctx(n, ops, 2 * n * D + n * L->final_rot, prec, opt, out);
 }
 
-gvqe_status gvqe_create_ops(int n, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec, gvqe_ctx **out)
+gvqe_status gvqe_create_ops_opt(int n, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec, const gvqe_options *opt,
+                                gvqe_ctx **out)
 {
     if (n_ops < 0 || (n_ops > 0 && !ops)) return GVQE_ERR_INVALID_ARG;
     std::vector<HostOp> v((size_t)n_ops);
     for (int i = 0; i < n_ops; ++i) v[i] = HostOp{ops[i].kind, ops[i].q0, ops[i].q1, ops[i].param};
-    return build_ctx(n, v, n_params, prec, out);
+    return build_ctx(n, v, n_params, prec, opt, out);
 }
 
 int gvqe_num_params(const gvqe_ctx *c) { return c ? c->P : -1; }
@@ -201,7 +244,7 @@ int gvqe_num_qubits(const gvqe_ctx *c) { return c ? c->n_user : -1; }
 static gvqe_status after_hamiltonian(gvqe_ctx *c)
 {
     std::string err;
-    if (!plan_expectation(c->H, c->n_store, c->KE, c->F, EXPECT_UMAX, EXPECT_TAB_CAP, (int)c->amp_bytes(), c->plan, err)) {
+    if (!plan_expectation(c->H, c->n_store, c->KE, c->F, EXPECT_UMAX, EXPECT_TAB_CAP, (int)c->amp_bytes(), c->opt.register_stages == 0, c->plan, err)) {
         c->have_h = false;
         return fail(c, GVQE_ERR_UNSUPPORTED, err);
     }
@@ -283,7 +326,7 @@ struct Carve {
 struct Layout {
     size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
-    size_t state_b, cs_b, params_b, partial_b;
+    size_t state_b, cs_b, ry_b, params_b, partial_b;
 };
 
 Layout layout_of(const gvqe_ctx *c)
@@ -320,9 +363,10 @@ Layout layout_of(const gvqe_ctx *c)
     const uint64_t tiles = 1ull << (c->n_store - c->plan.k);
     L.state_b = al256(c->amp_bytes() << c->n_store);
     L.cs_b = al256((size_t)(c->P > 0 ? c->P : 1) * c->amp_bytes());
+    L.ry_b = c->jit_blocks.empty() ? 0 : al256((size_t)(c->P > 0 ? c->P : 1) * c->amp_bytes() * 2);   // {tan, scale, form, 0}
     L.params_b = al256((size_t)(c->P > 0 ? c->P : 1) * 8);
     L.partial_b = al256((size_t)tiles * c->plan.passes.size() * 8);
-    L.per_state = L.state_b + L.cs_b + L.params_b + L.partial_b + 256 /* E */;
+    L.per_state = L.state_b + L.cs_b + L.ry_b + L.params_b + L.partial_b + 256 /* E */;
     return L;
 }
 
@@ -346,6 +390,30 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
         const int ke = kernels_init();
         if (ke) return cuda_fail(c, ke, "kernel attribute setup");
         c->kernels_ready = true;
+    }
+    if (c->jit_state == 0) {   // compile the specialised gate kernels (NVRTC, in parallel) and load them on this device
+        std::string why;
+        bool ok = jit_runtime_available(why);
+        if (ok) {
+            int dev = 0, sms = 0;
+            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) c->sm_count = sms;
+            const size_t nbk = c->jit_blocks.size();
+            std::vector<std::string> errs(nbk);
+            c->jit_mods.assign(nbk, nullptr);
+            for (size_t b0 = 0; b0 < nbk; b0 += 8) {   // NVRTC is thread safe: eight blocks at a time
+                std::vector<std::thread> th;
+                for (size_t b = b0; b < nbk && b < b0 + 8; ++b)
+                    th.emplace_back([c, b, &errs] { c->jit_mods[b] = jit_load(c->jit_blocks[b], errs[b]); });
+                for (std::thread &t : th) t.join();
+            }
+            for (size_t b = 0; b < nbk; ++b) if (!c->jit_mods[b]) { ok = false; why = errs[b]; }
+        }
+        if (!ok) {
+            for (JitModule *m : c->jit_mods) jit_unload(m);
+            c->jit_mods.clear();
+            if (c->opt.specialise == 2) return fail(c, GVQE_ERR_UNSUPPORTED, "specialised kernels requested but unavailable: " + why);
+            c->jit_state = -1; c->jit_blocks.clear();
+        } else c->jit_state = 1;
     }
     const Layout L = layout_of(c);
     if (c->ws_bytes < L.fixed_end + L.per_state) {
@@ -378,6 +446,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     char *p = w + L.fixed_end;
     c->d_states = p; p += L.state_b * fit;
     c->d_cs = p; p += L.cs_b * fit;
+    c->d_ry = L.ry_b ? p : nullptr; p += L.ry_b * fit;
     c->d_params = (double *)p; p += L.params_b * fit;
     c->d_partial = (double *)p; p += L.partial_b * fit;
     c->d_E = (double *)p;
@@ -414,6 +483,17 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
 }  // namespace
 extern "C" gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out);
 namespace {
+// Fused block j over nb statevectors starting at `states` (their (cos,sin) / tangent rows at cs / ry).
+int gate_block(gvqe_ctx *c, size_t j, void *states, uint64_t stride, const void *cs, const void *ry, int nb, cudaStream_t st)
+{
+    if (c->jit_state == 1) {
+        ++c->launches;
+        return jit_launch(c->jit_mods[j], c->jit_blocks[j], states, stride, ry, cs, nb, c->P, c->jit_per_cta, st);
+    }
+    return launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j], c->dev.blocks[j].k, c->dev.blocks[j].smem_prog_bytes, c->n_store,
+                             states, stride, cs, c->P, nb, st, &c->launches);
+}
+
 gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_dev, cudaStream_t st)
 {
     const Layout L = layout_of(c);
@@ -424,9 +504,12 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
             double tmp[8];
             gvqe_profile_read(c, tmp);
         }
-        for (int i = 0; i < 4; ++i) if (cudaEventCreate(&e4[i]) != cudaSuccess) return cuda_fail(c, (int)cudaGetLastError(), "event create");
+        for (int i = 0; i < 4; ++i) {
+            if (cudaEventCreate(&e4[i]) != cudaSuccess) return cuda_fail(c, (int)cudaGetLastError(), "event create");
+            c->ev.push_back(e4[i]);   // owned by the context from here on: freed by profile_read / destroy on every path
+        }
     }
-    int ke = launch_expand_params(c->prec, params_dev, c->d_cs, (uint64_t)nb * c->P, st, &c->launches);
+    int ke = launch_expand_params(c->prec, params_dev, c->d_cs, c->jit_state == 1 ? c->d_ry : nullptr, (uint64_t)nb * c->P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->profiling) cudaEventRecord(e4[0], st);
     if (c->px.n_ops > 0) {
@@ -434,8 +517,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
         if (ke) return cuda_fail(c, ke, "product-state init");
     }
     for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
-        ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[bi], c->dev.blocks[bi].k, c->dev.blocks[bi].smem_prog_bytes,
-                               c->n_store, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
+        ke = gate_block(c, bi, c->d_states, stride, c->d_cs, c->d_ry, nb, st);
         if (ke) return cuda_fail(c, ke, "gate block");
     }
     if (c->profiling) cudaEventRecord(e4[1], st);
@@ -450,7 +532,6 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     if (ke) return cuda_fail(c, ke, "reduce");
     if (c->profiling) {
         cudaEventRecord(e4[3], st);
-        for (int i = 0; i < 4; ++i) c->ev.push_back(e4[i]);
         const double S = (double)(c->amp_bytes() << c->n_store);
         double gb = 0;
         for (const DBlock &b : c->dev.blocks) gb += (b.source_zero ? 1.0 : 2.0) * S * nb;
@@ -567,10 +648,11 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
     const double half_pi = 1.57079632679489661923;
     auto state_of = [&](int slot) { return (void *)((char *)c->d_states + L.state_b * (size_t)slot); };
     auto cs_of = [&](int slot) { return (void *)((char *)c->d_cs + (size_t)slot * (size_t)P * c->amp_bytes()); };
+    auto ry_of = [&](int slot) { return c->d_ry ? (void *)((char *)c->d_ry + (size_t)slot * (size_t)P * c->amp_bytes() * 2) : nullptr; };
+    const bool use_ry = c->jit_state == 1;
     auto blocks_from = [&](int j0, int slot, int nb) -> gvqe_status {
         for (int j = j0; j < NB; ++j) {
-            const int ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j], c->dev.blocks[j].k, c->dev.blocks[j].smem_prog_bytes,
-                                             c->n_store, state_of(slot), stride, cs_of(slot), P, nb, st, &c->launches);
+            const int ke = gate_block(c, (size_t)j, state_of(slot), stride, cs_of(slot), ry_of(slot), nb, st);
             if (ke) return cuda_fail(c, ke, "gate block");
         }
         return GVQE_OK;
@@ -589,7 +671,7 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
     // base row: parameters and (cos, sin) in slot 0
     cudaError_t e = cudaMemcpyAsync(c->d_params, params, (size_t)P * 8, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
-    int ke = launch_expand_params(c->prec, c->d_params, c->d_cs, (uint64_t)P, st, &c->launches);
+    int ke = launch_expand_params(c->prec, c->d_params, c->d_cs, use_ry ? c->d_ry : nullptr, (uint64_t)P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->px.n_ops > 0 && (ke = launch_init_product(c->prec, c->pxd, c->d_states, stride, c->d_cs, P, 1, st, &c->launches)))
         return cuda_fail(c, ke, "product-state init");
@@ -606,7 +688,7 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
             }
             e = cudaMemcpyAsync(c->d_params + P, rows.data(), (size_t)nb * P * 8, cudaMemcpyHostToDevice, st);
             if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
-            if ((ke = launch_expand_params(c->prec, c->d_params + P, cs_of(1), (uint64_t)nb * P, st, &c->launches)))
+            if ((ke = launch_expand_params(c->prec, c->d_params + P, cs_of(1), use_ry ? ry_of(1) : nullptr, (uint64_t)nb * P, st, &c->launches)))
                 return cuda_fail(c, ke, "expand_params");
             if (j0 < 0) {
                 if ((ke = launch_init_product(c->prec, c->pxd, state_of(1), stride, cs_of(1), P, nb, st, &c->launches)))
@@ -625,8 +707,7 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
             for (int r = 0; r < nb; ++r) E_pm[2 * work[w0 + r].first + work[w0 + r].second] = Et[r];
         }
         if (j0 >= 0) {   // the base state advances by block j0
-            ke = launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j0], c->dev.blocks[j0].k, c->dev.blocks[j0].smem_prog_bytes,
-                                   c->n_store, state_of(0), stride, cs_of(0), P, 1, st, &c->launches);
+            ke = gate_block(c, (size_t)j0, state_of(0), stride, cs_of(0), ry_of(0), 1, st);
             if (ke) return cuda_fail(c, ke, "gate block");
         }
     }
@@ -645,8 +726,8 @@ gvqe_status gvqe_param_shift_grad(gvqe_ctx *c, const double *params, const uint8
     for (int p = 0; p < c->P; ++p)
         if (!std::isfinite(params[p])) return fail(c, GVQE_ERR_INVALID_ARG, "param_shift_grad: parameter is not finite");
     // shared prefixes pay when kernel time dominates launch overhead: states of >= 16 MiB unless forced (1) or disabled (0)
-    const int sp = env_int("GVQE_SHARED_PREFIX", -1);
-    if (!idx.empty() && (sp == 1 || (sp < 0 && (c->amp_bytes() << c->n_store) >= ((size_t)16 << 20)))) {
+    const int sp = c->opt.shared_prefix;   // 0 auto, 1 never, 2 always
+    if (!idx.empty() && (sp == 2 || (sp == 0 && (c->amp_bytes() << c->n_store) >= ((size_t)16 << 20)))) {
         std::vector<double> Epm(2 * idx.size());
         double e0 = 0.0;
         const gvqe_status s = grad_shared_prefix(c, params, idx, Epm.data(), &e0, (cudaStream_t)stream);
@@ -899,6 +980,7 @@ void gvqe_destroy(gvqe_ctx *c)
 {
     if (!c) return;
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    for (JitModule *m : c->jit_mods) jit_unload(m);
     delete c;
 }
 

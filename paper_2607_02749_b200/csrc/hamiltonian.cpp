@@ -113,7 +113,7 @@ bool hamiltonian_from_masks(int n, int M, const uint64_t *xm, const uint64_t *zm
 }
 
 bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint32_t tab_cap, int amp_bytes,
-                      ExpectPlan &plan, std::string &err)
+                      bool register_stages, ExpectPlan &plan, std::string &err)
 {
     const int FB = amp_bytes == 8 ? 4 : 3;   // same fold as phys<T>() in kernels.cuh
     auto hphys = [FB](uint32_t j) { uint32_t p = j; for (int sh = FB; sh < 16; sh += FB) p ^= (j >> sh) & ((1u << FB) - 1u); return p; };
@@ -215,7 +215,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
         // evaluated with those bits as register bits (amplitudes and partners in registers, W broadcast)
         const int RSB = k - TB;
         std::vector<char> in_rs(gm.size(), 0);
-        if (RSB >= 2 && RSB <= DEV_MAX_R && !getenv("GVQE_NO_RS")) {
+        if (RSB >= 2 && RSB <= DEV_MAX_R && register_stages) {
             std::vector<uint32_t> sets; std::vector<std::vector<int>> members;
             std::vector<std::pair<uint32_t, int>> cand;
             for (int g : passG[p]) {

@@ -41,7 +41,8 @@ struct ExpectPlan {
 // n_store: qubits of the stored state; k/f: tile bits / fixed low tile bits; umax: largest table (bits);
 // tab_cap: complex entries of the shared-memory table area.
 // amp_bytes: 8 (complex64) or 16 (complex128): fixes the shared-memory swizzle and the byte offsets of the lookups.
+// register_stages: evaluate the groups that fit R local bits from registers (false: every group takes the lookup / direct path).
 bool plan_expectation(const Hamiltonian &H, int n_store, int k, int f, int umax, uint32_t tab_cap, int amp_bytes,
-                      ExpectPlan &plan, std::string &err);
+                      bool register_stages, ExpectPlan &plan, std::string &err);
 
 }  // namespace gv

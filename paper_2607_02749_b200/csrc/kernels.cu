@@ -9,14 +9,21 @@
 namespace gv {
 
 // ---- parameter expansion: (cos(theta/2), sin(theta/2)) in fp64, stored in working precision ----
+// Second output for the specialised gate kernels (jit.cpp): R_y(theta) = c [[1,-t],[t,1]] with t = s/c when |c| >= |s|
+// (form 0), else s [[t,-1],[1,t]] with t = c/s (form 1); {t, scale = c or s, form, 0} per parameter (Eq. 7).
+template <typename T> struct alignas(4 * sizeof(T)) ry4 { T t, sc, form, pad; };
 template <typename T>
-__global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *__restrict__ cs, uint64_t count)
+__global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *__restrict__ cs, ry4<T> *__restrict__ ry, uint64_t count)
 {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= count) return;
     double s, c;
     sincos(0.5 * params[i], &s, &c);
     cs[i] = cx<T>{(T)c, (T)s};
+    if (ry) {
+        const bool f0 = fabs(c) >= fabs(s);
+        ry[i] = ry4<T>{(T)(f0 ? s / c : c / s), (T)(f0 ? c : s), f0 ? T(0) : T(1), T(0)};
+    }
 }
 
 // ---- product-state prefix, write-only --------------------------------------------------------------
@@ -146,10 +153,10 @@ gate_block_kernel(const DevArrays da, const __grid_constant__ DBlock blk, cx<T> 
     uint32_t po[R], pj2 = 0;
     for (int s = (int)sb->lead_cx; s < ns; ++s) {
         if (gate_stage<T, R>(pv, pv.stages[s], (uint32_t)s, reinterpret_cast<unsigned char *>(tile), tid, xbase, amp, po, pj2)) {
-            if (pv.stages[s].warp_sync_cx) __syncwarp(); else __syncthreads();   // reads done before the permuted writes
+            __syncthreads();   // reads done before the permuted writes
             gate_stage_store<T, R>(reinterpret_cast<unsigned char *>(tile), pj2, po, amp);
         }
-        if (pv.stages[s].warp_sync_after) __syncwarp(); else __syncthreads();
+        __syncthreads();
     }
     tile_store_u<T, NLD>(tile, state, x0, tid, hi, sb->hip);
 }
@@ -556,13 +563,13 @@ int kernels_init(void)
     return e;
 }
 
-int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches)
+int launch_expand_params(int prec, const double *params, void *cs, void *ry, uint64_t count, void *stream, uint64_t *launches)
 {
     if (!count) return 0;
     const unsigned nb = (unsigned)((count + 255) / 256);
     cudaStream_t st = (cudaStream_t)stream;
-    if (prec == 0) expand_params_kernel<float><<<nb, 256, 0, st>>>(params, (cx<float> *)cs, count);
-    else expand_params_kernel<double><<<nb, 256, 0, st>>>(params, (cx<double> *)cs, count);
+    if (prec == 0) expand_params_kernel<float><<<nb, 256, 0, st>>>(params, (cx<float> *)cs, (ry4<float> *)ry, count);
+    else expand_params_kernel<double><<<nb, 256, 0, st>>>(params, (cx<double> *)cs, (ry4<double> *)ry, count);
     ++*launches;
     return (int)cudaGetLastError();
 }

@@ -10,17 +10,10 @@
 
 #include "devprog.h"
 
-#ifdef GVQE_EMU   // host emulation used only by developer probes; never part of the library build
-#define GV_DEV inline
-#define GV_UNROLL
-static inline int gv_popcll(uint64_t v) { return __builtin_popcountll(v); }
-static inline int gv_popc(uint32_t v) { return __builtin_popcount(v); }
-#else
 #define GV_DEV __device__ __forceinline__
 #define GV_UNROLL _Pragma("unroll")
 GV_DEV int gv_popcll(uint64_t v) { return __popcll(v); }
 GV_DEV int gv_popc(uint32_t v) { return __popc(v); }
-#endif
 
 namespace gv {
 
@@ -199,7 +192,6 @@ template <typename T> GV_DEV void ry_pair(cx<T> &u, cx<T> &v, T c, T s)
     u = cx<T>{c * a.x - s * b.x, c * a.y - s * b.y};
     v = cx<T>{s * a.x + c * b.x, s * a.y + c * b.y};
 }
-#ifndef GVQE_EMU
 // complex64: (re, im) is one packed f32x2 operand -- FMUL2/FFMA2 on sm_100a rotate a pair in 4 instructions
 template <> GV_DEV void ry_pair<float>(cx<float> &u, cx<float> &v, float c, float s)
 {
@@ -210,7 +202,6 @@ template <> GV_DEV void ry_pair<float>(cx<float> &u, cx<float> &v, float c, floa
     u = cx<float>{un.x, un.y};
     v = cx<float>{vn.x, vn.y};
 }
-#endif
 
 template <typename T, int R, int S> GV_DEV void ry_slot(cx<T> *a, T c, T s)
 {
@@ -240,14 +231,12 @@ template <typename T, int R> GV_DEV void ry_layer(cx<T> *a, const int16_t *ryl, 
 
 // Complex multiply a * w; for complex64 with the packed f32x2 pipe: a.x * (w.x, w.y) + a.y * (-w.y, w.x).
 template <typename T> GV_DEV cx<T> cmul_w(cx<T> a, cx<T> w, cx<T> wsw) { (void)wsw; return cmul(a, w); }
-#ifndef GVQE_EMU
 template <> GV_DEV cx<float> cmul_w<float>(cx<float> a, cx<float> w, cx<float> wsw)
 {
     const float2 r = __ffma2_rn(make_float2(a.y, a.y), make_float2(wsw.x, wsw.y),
                                 __fmul2_rn(make_float2(a.x, a.x), make_float2(w.x, w.y)));
     return cx<float>{r.x, r.y};
 }
-#endif
 
 // Thread-phase tables of the block's diagonal segments (one entry per call): the factor that is constant over a
 // thread's registers splits into (tile-constant x thread-index bits 0..3) and (thread-index bits 4..).  Built once
@@ -481,7 +470,6 @@ GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32
         cmb[i] = q.a; cmb[i + 1] = q.b; cmb[i + 2] = q.c; cmb[i + 3] = q.d;
     }
     T tr = T(0), ti = T(0);
-#ifndef GVQE_EMU
     if constexpr (sizeof(T) == 4) {
         // packed: accA += b.x * (a.x, a.y), accB += b.y * (a.y, a.x); Re = accA.x + accB.x, Im = accA.y - accB.y
         float2 accA = make_float2(0.f, 0.f), accB = make_float2(0.f, 0.f);
@@ -497,7 +485,6 @@ GV_DEV double group_accumulate_lut(const uint32_t *gt, uint32_t pm_bytes, uint32
         ti = accA.y - accB.y;
         return 2.0 * (double)(w.x * tr - w.y * ti);
     }
-#endif
     GV_UNROLL
     for (int i = 0; i < (1 << L); ++i) {
         const uint32_t ob = pjb ^ cmb[i];
@@ -517,7 +504,6 @@ template <> struct TopBit<0> { static constexpr int value = 0; };
 template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T> *w)
 {
     constexpr int PV = TopBit<M>::value;
-#ifndef GVQE_EMU
     if constexpr (sizeof(T) == 4) {
         // packed: accA += v.x * (w.x u.x, w.y u.y), accB += v.y * (w.x u.y, w.y u.x);
         // Re(w conj(v) u) summed = (accA.x - accA.y) + (accB.x + accB.y).  Two chains each.
@@ -538,7 +524,6 @@ template <typename T, int R, int M> GV_DEV T rs_pairs(const cx<T> *a, const cx<T
         const float2 sa = __fadd2_rn(accA[0], accA[1]), sb = __fadd2_rn(accB[0], accB[1]);
         return (sa.x - sa.y) + (sb.x + sb.y);
     }
-#endif
     T acc[4] = {T(0), T(0), T(0), T(0)};   // independent chains
     int n = 0;
     GV_UNROLL

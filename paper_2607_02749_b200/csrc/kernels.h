@@ -32,7 +32,8 @@ struct PrefixDev {   // device view of schedule.h Prefix
 };
 
 // prec: 0 = complex64 (float), 1 = complex128 (double)
-int launch_expand_params(int prec, const double *params, void *cs, uint64_t count, void *stream, uint64_t *launches);
+// ry: optional second table for the specialised gate kernels ({tan, scale, form, 0} per parameter, jit.cpp), or NULL
+int launch_expand_params(int prec, const double *params, void *cs, void *ry, uint64_t count, void *stream, uint64_t *launches);
 int launch_init_product(int prec, const PrefixDev &pd, void *states, uint64_t stride_amps, const void *cs, int P, int batch,
                         void *stream, uint64_t *launches);
 int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &block, int k, uint32_t smem_prog_bytes, int n,

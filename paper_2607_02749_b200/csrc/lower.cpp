@@ -2,7 +2,6 @@
 // slice would outgrow the shared-memory budget (same tile bits, one more HBM round trip; results unchanged).
 #include "lower.h"
 
-#include <cstdlib>
 #include <cstring>
 
 namespace gv {
@@ -213,27 +212,6 @@ bool lower_program(const Program &p, int scs_bytes, DevProgram &D, std::string &
                     }
                     db.e1_cx = hphys(alin(1u));
                     for (uint32_t i = 0; i < nld && i < 16; ++i) db.hip_cx[i] = hphys(alin(i * nthr * V));
-                }
-            }
-            {   // which stage boundaries need only a warp-level barrier: a warp's footprint in the tile is fixed by the
-                // local positions of its warp-index bits = the highest non-register local bits of the stage
-                // (measured: no gain on B200, and it cannot be race-checked on this pool -- kept behind GVQE_WARP_SYNC)
-                const bool enable = getenv("GVQE_WARP_SYNC") != nullptr;
-                const int nwb = B.k - p.R - 5;
-                auto warp_bits = [&](const DStage &st) {
-                    uint32_t regs = 0, wb = 0; int cnt = 0;
-                    for (int s2 = 0; s2 < p.R; ++s2) regs |= 1u << st.regbit[s2];
-                    for (int b2 = B.k - 1; b2 >= 0 && cnt < nwb; --b2) if (!(regs >> b2 & 1)) { wb |= 1u << b2; ++cnt; }
-                    return wb;
-                };
-                for (uint32_t si2 = 0; si2 < n_stages; ++si2) {
-                    DStage &st = D.stages[db.stage_off + si2];
-                    const uint32_t wb = warp_bits(st);
-                    bool cx_inside = true;
-                    for (uint32_t ci = st.cx_begin; ci < st.cx_end; ++ci) if (wb >> D.cxs[db.cx_off + ci].tl & 1) cx_inside = false;
-                    st.warp_sync_cx = (uint8_t)(cx_inside && enable ? 1 : 0);
-                    st.warp_sync_after = 0;
-                    if (enable && si2 + 1 < n_stages && cx_inside && warp_bits(D.stages[db.stage_off + si2 + 1]) == wb) st.warp_sync_after = 1;
                 }
             }
             {   // vector offsets of the tile load/store (kernels.cuh tile_load_u)
