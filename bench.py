@@ -165,8 +165,9 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfg, prec, rows = args.config, PREC_OF[args.config], ROWS_PER_STEP[args.config]
     w = make_workload(cfg)
+    options = {k: int(v) for k, v in (kv.split("=") for kv in args.opt)} or None   # gvqe_options overrides (tuning runs)
     g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
-                precision=prec)
+                precision=prec, options=options)
     g.set_hamiltonian(w.paulis, w.coeffs)
     g.alloc_workspace(rows, device=f"cuda:{local}")
     n_gate_blocks, n_passes, _ = g.schedule_info()
@@ -286,6 +287,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="FIELD=INT",
+                    help="gvqe_options field for this run (e.g. tiles_per_block=4, specialise=1); default: library defaults")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

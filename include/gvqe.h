@@ -85,7 +85,9 @@ typedef struct {
                                * 0 = for registers of >= 20 qubits when NVRTC is present, 1 = never (generic kernels),
                                * 2 = whenever the schedule is supported; GVQE_ERR_UNSUPPORTED at the first energy call if
                                * it is not or NVRTC is missing */
-    int32_t reserved[8];      /* must be 0 */
+    int32_t tiles_per_block;  /* specialised kernels: consecutive tiles one thread block works through (its per-block
+                               * set-up is paid once): 0 = default (tuned on the B200), else 1..4096 */
+    int32_t reserved[7];      /* must be 0 */
 } gvqe_options;
 /* gvqe_create / gvqe_create_ops with options (opt == NULL: defaults). */
 gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, const gvqe_options *opt,
@@ -96,6 +98,11 @@ gvqe_status gvqe_create_ops_opt(int n_qubits, const gvqe_op *ops, int n_ops, int
  * buf (NUL-terminated, truncated to cap); returns the full length needed, 0 when the schedule has no such kernel.
  * *smem_bytes (optional): its dynamic shared memory.  Host only (no GPU, no compiler). */
 size_t gvqe_kernel_source(const gvqe_ctx *ctx, int block, char *buf, size_t cap, int32_t *smem_bytes);
+/* Compiles every specialised kernel of the context with NVRTC for sm_100a (host only: needs the compiler library, no
+ * GPU; images are cached for the first energy call).  *n_kernels (optional): how many were compiled (0 when the
+ * context uses the generic kernels).  GVQE_ERR_UNSUPPORTED with the compiler's message when NVRTC is missing or a
+ * kernel does not compile.  Used by the build check. */
+gvqe_status gvqe_compile_kernels(gvqe_ctx *ctx, int32_t *n_kernels);
 int gvqe_num_params(const gvqe_ctx *ctx);
 int gvqe_num_qubits(const gvqe_ctx *ctx);
 

@@ -19,7 +19,7 @@ GVQE_C64, GVQE_C128 = 0, 1
 STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "GVQE_ERR_WORKSPACE",
                 "GVQE_ERR_UNSUPPORTED", "GVQE_ERR_CUDA"]
 
-EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
+EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
@@ -35,7 +35,7 @@ class GvqeOptions(C.Structure):
     """gvqe_options: how the same energies are computed (0 = library default for every field)."""
     _fields_ = [("tile_bits", C.c_int32), ("fixed_bits", C.c_int32), ("reg_bits", C.c_int32), ("expect_tile_bits", C.c_int32),
                 ("prefix", C.c_int32), ("register_stages", C.c_int32), ("shared_prefix", C.c_int32), ("specialise", C.c_int32),
-                ("reserved", C.c_int32 * 8)]
+                ("tiles_per_block", C.c_int32), ("reserved", C.c_int32 * 7)]
 
 
 class GvqeOptOptions(C.Structure):
@@ -77,6 +77,7 @@ def load():
     L.gvqe_create_ops_opt.argtypes = [i32, vp, i32, i32, i32, C.POINTER(GvqeOptions), C.POINTER(vp)]
     L.gvqe_kernel_source.argtypes = [vp, i32, C.c_char_p, sz, vp]
     L.gvqe_kernel_source.restype = sz
+    L.gvqe_compile_kernels.argtypes = [vp, vp]
     L.gvqe_num_params.argtypes = [vp]
     L.gvqe_num_qubits.argtypes = [vp]
     L.gvqe_set_hamiltonian.argtypes = [vp, i32, C.c_char_p, vp]
@@ -280,6 +281,12 @@ class Gvqe:
         buf = C.create_string_buffer(need + 1)
         self._L.gvqe_kernel_source(self._h, int(block), buf, need + 1, C.addressof(sm))
         return buf.value.decode(), int(sm.value)
+
+    def compile_kernels(self) -> int:
+        """NVRTC-compile every specialised kernel (no GPU needed); returns how many."""
+        k = C.c_int32(0)
+        self._check(self._L.gvqe_compile_kernels(self._h, C.addressof(k)))
+        return int(k.value)
 
     def get_exec_order(self) -> np.ndarray:
         m = self._L.gvqe_get_exec_order(self._h, None, 0)

@@ -62,7 +62,7 @@ struct gvqe_ctx {
     // schedule-specialised gate kernels (jit.h): generated at create, compiled and loaded at the first energy call
     int jit_state = 0;          // 0 not tried, 1 loaded, -1 not used
     int sm_count = 148;
-    int jit_per_cta = 1;        // work items per thread block of the specialised kernels (tuned on the B200)
+    int jit_per_cta = 8;        // work items per thread block of the specialised kernels (tuned on the B200)
     std::vector<JitBlock> jit_blocks;
     std::vector<JitModule *> jit_mods;
     void *d_ry = nullptr;
@@ -101,12 +101,13 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
     c->n_user = n; c->n_store = n < N_MIN_STORE ? N_MIN_STORE : n; c->prec = prec; c->P = n_params; c->ops = ops;
     if (opt) {
         c->opt = *opt;
-        bool bad = opt->tile_bits < 0 || opt->fixed_bits < 0 || opt->reg_bits < 0 || opt->expect_tile_bits < 0 || opt->prefix < 0 ||
+        bool bad = opt->tile_bits > 14 || opt->fixed_bits > 8 || opt->reg_bits > 5 || opt->expect_tile_bits > 14 || opt->tile_bits < 0 || opt->fixed_bits < 0 || opt->reg_bits < 0 || opt->expect_tile_bits < 0 || opt->prefix < 0 ||
                    opt->prefix > 2 || opt->register_stages < 0 || opt->register_stages > 1 || opt->shared_prefix < 0 ||
-                   opt->shared_prefix > 2 || opt->specialise < 0 || opt->specialise > 2;
+                   opt->shared_prefix > 2 || opt->specialise < 0 || opt->specialise > 2 || opt->tiles_per_block < 0 || opt->tiles_per_block > 4096;
         for (int32_t r : opt->reserved) bad = bad || r != 0;
         if (bad) { delete c; return GVQE_ERR_INVALID_ARG; }
     }
+    if (c->opt.tiles_per_block) c->jit_per_cta = c->opt.tiles_per_block;
     c->K = c->opt.tile_bits ? c->opt.tile_bits : (prec == GVQE_C64 ? 13 : 12);
     c->F = c->opt.fixed_bits ? c->opt.fixed_bits : (prec == GVQE_C64 ? 4 : 3);
     c->R = c->opt.reg_bits ? c->opt.reg_bits : (prec == GVQE_C64 ? 5 : 4);
@@ -174,6 +175,24 @@ size_t gvqe_kernel_source(const gvqe_ctx *c, int block, char *buf, size_t cap, i
     if (smem_bytes) *smem_bytes = (int32_t)c->jit_blocks[(size_t)block].smem_bytes;
     if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }
     return s.size() + 1;
+}
+
+gvqe_status gvqe_compile_kernels(gvqe_ctx *c, int32_t *n_kernels)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (n_kernels) *n_kernels = 0;
+    const size_t nbk = c->jit_blocks.size();
+    std::vector<std::string> errs(nbk);
+    std::vector<char> ok(nbk, 0);
+    for (size_t b0 = 0; b0 < nbk; b0 += 8) {
+        std::vector<std::thread> th;
+        for (size_t b = b0; b < nbk && b < b0 + 8; ++b)
+            th.emplace_back([c, b, &errs, &ok] { std::vector<char> img; ok[b] = jit_compile_only(c->jit_blocks[b], img, errs[b]) ? 1 : 0; });
+        for (std::thread &t : th) t.join();
+    }
+    for (size_t b = 0; b < nbk; ++b) if (!ok[b]) return fail(c, GVQE_ERR_UNSUPPORTED, errs[b]);
+    if (n_kernels) *n_kernels = (int32_t)nbk;
+    return GVQE_OK;
 }
 
 gvqe_status gvqe_create_opt(int n, const gvqe_layout *L, gvqe_precision prec, const gvqe_options *opt, gvqe_ctx **out)

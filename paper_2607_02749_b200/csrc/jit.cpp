@@ -484,8 +484,9 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
             const int cnt = half == 0 ? si.nlo : si.nhi, from = half == 0 ? 0 : si.nlo;
             if (half == 1 && cnt == 0) continue;
             if (half == 0 && cnt == 0) continue;
-            E("            if (tid >= %du && tid < %du) {   // segment %d, %s table", q * 16 + half * 8, q * 16 + half * 8 + (1 << cnt), q, half ? "high" : "low");
-            E("                const unsigned e = tid - %du;", q * 16 + half * 8);
+            const int tbase = (q * 16 + half * 8) % (int)NT;   // one thread per entry; segments 16 apart share threads (in turn)
+            E("            if (tid >= %du && tid < %du) {   // segment %d, %s table", tbase, tbase + (1 << cnt), q, half ? "high" : "low");
+            E("                const unsigned e = tid - %du;", tbase);
             E("                amp f = MK((real)1, (real)0);");
             for (int i = 0; i < cnt; ++i) {
                 const int sl = si.active[from + i];

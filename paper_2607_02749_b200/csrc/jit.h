@@ -33,7 +33,9 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
 // ---- run time (jit_rt.cpp): NVRTC through dlopen, module load and launch through the driver entry points -----------
 struct JitModule;   // one loaded kernel
 bool jit_runtime_available(std::string &why);
-// Compiles `blk.source` (cached per process by source text) and loads it on the current device.
+// Compiles `blk.source` to an sm_100a image (cached per process by source text); needs no device.
+bool jit_compile_only(const JitBlock &blk, std::vector<char> &cubin, std::string &err);
+// Compiles (or takes the cached image) and loads it on the current device.
 JitModule *jit_load(const JitBlock &blk, std::string &err);
 void jit_unload(JitModule *m);
 // Launch on `stream`: states (device), stride in amplitudes, ry / cs tables (device, per statevector row of P entries);

@@ -17,9 +17,9 @@ from tests.dense_ref import dense_hamiltonian
 pytestmark = pytest.mark.gpu
 
 
-def ctx(w, prec="c128", in_flight=16):
+def ctx(w, prec="c128", in_flight=16, options=None):
     g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
-                precision=prec)
+                precision=prec, options=options)
     g.set_hamiltonian(w.paulis, w.coeffs)
     g.alloc_workspace(in_flight)
     return g
@@ -236,25 +236,25 @@ def test_sample_quantiles_product_state(n, prec):
 
 
 # ---- shared-prefix parameter-shift sweeps ---------------------------------------------------------
-@pytest.mark.parametrize("cfg,n,D,prec,in_flight,prefix", [
-    (1, 10, 3, "c128", 16, None), (2, 16, 4, "c128", 8, None), (4, 15, 3, "c64", 8, "1"), (4, 16, 2, "c128", 3, "0"),
-    (3, 17, 3, "c64", 2, None), (4, 14, 2, "c64", 1, None), (2, 4, 2, "c128", 5, None)])
-def test_shared_prefix_gradient_is_bit_identical(orc, monkeypatch, cfg, n, D, prec, in_flight, prefix):
+@pytest.mark.parametrize("cfg,n,D,prec,in_flight,prefix,spec", [
+    (1, 10, 3, "c128", 16, 0, 0), (2, 16, 4, "c128", 8, 0, 0), (4, 15, 3, "c64", 8, 2, 0), (4, 16, 2, "c128", 3, 1, 0),
+    (3, 17, 3, "c64", 2, 0, 0), (4, 14, 2, "c64", 1, 0, 0), (2, 4, 2, "c128", 5, 0, 0),
+    (4, 15, 3, "c64", 8, 2, 2), (4, 16, 2, "c128", 3, 1, 2), (3, 17, 3, "c64", 4, 0, 2)])
+def test_shared_prefix_gradient_is_bit_identical(orc, cfg, n, D, prec, in_flight, prefix, spec):
     """gvqe_param_shift_grad with snapshots of the base state at the block boundaries returns exactly the numbers of
     the plain evaluation of all 2|mask|+1 rows (each row sees the same kernels on the same data), with and without
-    the product-state prefix, for chunked groups and for a one-slot workspace (fallback); and both match the oracle."""
-    if prefix is not None:
-        monkeypatch.setenv("GVQE_PREFIX", prefix)
+    the product-state prefix (gvqe_options.prefix), for chunked groups and for a one-slot workspace (fallback), with the
+    generic and with the schedule-specialised gate kernels (gvqe_options.specialise); and both match the oracle."""
     w = make_workload(cfg, n=n, M=60, D=D, batch=1)
-    g = ctx(w, prec, in_flight=in_flight)
     r = SplitMix64(77 + n)
     mask = np.array([1 if r.uniform() < 0.4 else 0 for _ in range(w.P)], dtype=np.uint8)
     mask[0] = mask[w.P - 1] = 1                                   # first layer (prefix) and the last rotation layer
-    monkeypatch.setenv("GVQE_SHARED_PREFIX", "1")
+    g = ctx(w, prec, in_flight=in_flight, options=dict(prefix=prefix, shared_prefix=2, specialise=spec))
     l0 = g.launch_count()
     dE, E0 = g.param_shift_grad(w.theta, mask)
     l_shared = g.launch_count() - l0
-    monkeypatch.setenv("GVQE_SHARED_PREFIX", "0")
+    del g
+    g = ctx(w, prec, in_flight=in_flight, options=dict(prefix=prefix, shared_prefix=1, specialise=spec))
     l0 = g.launch_count()
     dE_plain, E0_plain = g.param_shift_grad(w.theta, mask)
     l_plain = g.launch_count() - l0

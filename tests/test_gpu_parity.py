@@ -31,12 +31,12 @@ def assert_close(prec, E, E_ref, coeffs, what=""):
     assert not bad.any(), f"{what}: max |dE| = {np.max(np.abs(E - E_ref)):.3e}, first bad row {int(np.argmax(bad))}"
 
 
-def ctx_for(w, prec, in_flight=None, ops=False):
+def ctx_for(w, prec, in_flight=None, ops=False, options=None):
     if ops:
-        g = gv.Gvqe(w.n, ops=w.ops, n_params=w.P, precision=prec)
+        g = gv.Gvqe(w.n, ops=w.ops, n_params=w.P, precision=prec, options=options)
     else:
         g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
-                    precision=prec)
+                    precision=prec, options=options)
     g.set_hamiltonian(w.paulis, w.coeffs)
     g.alloc_workspace(in_flight or min(w.B, 64))
     return g
@@ -155,14 +155,14 @@ def test_embedding_on_high_qubits(orc, prec, n_big):
 
 # ---- randomised small cases: arbitrary op lists and Pauli strings, several tiles, ragged sizes ------------------------
 @pytest.mark.parametrize("seed", range(14))
-def test_random_circuits_and_paulis(orc, seed, monkeypatch):
+def test_random_circuits_and_paulis(orc, seed):
     n = 1 + seed
-    monkeypatch.setenv("GVQE_K", str(10 + seed % 3))            # n > k from n = 11 on: multi-tile and strided blocks
     prec = "c64" if seed % 2 else "c128"
     ops, P = random_ops(7000 + seed, n, 150)
     paulis, coeffs = random_paulis(8000 + seed, n, 80, min(n, 6))
     th = np.random.default_rng(seed).uniform(-math.pi, math.pi, (5, P))
-    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec)
+    # n > k from n = 11 on: multi-tile and strided blocks
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(tile_bits=10 + seed % 3))
     g.set_hamiltonian(paulis, coeffs)
     g.alloc_workspace(3)                                         # 5 rows in chunks of 3 + 2
     E = g.energy_batch(th)
@@ -318,20 +318,17 @@ def test_c64_vs_c128_at_28_qubits():
 
 
 @pytest.mark.parametrize("n,D,ent,topo,prec", [(14, 2, "cz", "ring", "c64"), (15, 2, "cnot", "ring", "c128"), (12, 1, "cnot", "linear", "c64")])
-def test_without_product_state_prefix(orc, n, D, ent, topo, prec, monkeypatch):
-    """The first layer is normally WRITTEN as a product state; with GVQE_NO_PREFIX the same circuit runs
-    through the generic blocks from |0...0>.  Both must match the oracle (and so each other)."""
+def test_without_product_state_prefix(orc, n, D, ent, topo, prec):
+    """The first layer is normally WRITTEN as a product state; with gvqe_options.prefix = 1 the same circuit
+    runs through the generic blocks from |0...0>.  Both must match the oracle (and so each other)."""
     ops = np.array(layout_ops(n, D, ent, topo, 1), dtype=np.int32)
     P = num_params(n, D, 1)
     paulis, coeffs = random_paulis(500 + n, n, 100, 5)
     th = np.random.default_rng(n).uniform(-math.pi, math.pi, (3, P))
     ref = orc.energy_batch(n, ops, th, paulis, coeffs)
     for no_prefix in (False, True):
-        monkeypatch.setenv("GVQE_PREFIX", "1")
-        if no_prefix:
-            monkeypatch.setenv("GVQE_PREFIX", "0")
-        monkeypatch.setenv("GVQE_K", "10")
-        g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo), precision=prec)
+        g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo), precision=prec,
+                    options=dict(prefix=1 if no_prefix else 2, tile_bits=10))
         assert ("prefix ops=0" in g.dump_schedule()) == no_prefix
         g.set_hamiltonian(paulis, coeffs)
         g.alloc_workspace(3)
@@ -340,17 +337,72 @@ def test_without_product_state_prefix(orc, n, D, ent, topo, prec, monkeypatch):
 
 
 @pytest.mark.parametrize("prec", ["c64", "c128"])
-def test_expectation_modes_agree(orc, prec, monkeypatch):
-    """The planner evaluates most community-local groups as register stages; GVQE_NO_RS sends every group through the
-    lookup / direct modes instead.  Both plans must match the oracle on the config-4 recipe (pooled flip masks)."""
+def test_expectation_modes_agree(orc, prec):
+    """The planner evaluates most community-local groups as register stages; gvqe_options.register_stages = 1 sends
+    every group through the lookup / direct modes instead.  Both plans must match the oracle on the config-4 recipe
+    (pooled flip masks)."""
     w = make_workload(4, n=15, M=1500, D=2, batch=3)
     ref = orc.energy_batch(w.n, w.ops, w.params, w.paulis, w.coeffs)
     for no_rs in (False, True):
-        if no_rs:
-            monkeypatch.setenv("GVQE_NO_RS", "1")
-        monkeypatch.setenv("GVQE_K", "11")
-        g = ctx_for(w, prec, 3)
+        g = ctx_for(w, prec, 3, options=dict(register_stages=1 if no_rs else 0, tile_bits=11))
         assert_close(prec, g.energy_batch(w.params), ref, w.coeffs, f"no_rs={no_rs}")
+
+
+# ---- schedule-specialised gate kernels (jit.cpp; PAPER.md:179 "JIT-compiled once and reused") ------------------------------
+@pytest.mark.parametrize("n,D,ent,topo,fr,prec,prefix", [
+    (14, 2, "cnot", "ring", 1, "c64", 1), (14, 2, "cnot", "ring", 1, "c64", 2), (15, 3, "cz", "linear", 1, "c64", 1),
+    (13, 2, "cz", "linear", 2, "c128", 2), (16, 2, "cnot", "ring", 1, "c128", 1), (17, 3, "cz", "ring", 2, "c64", 2),
+    (14, 2, "cnot", "full", 1, "c64", 1), (15, 3, "cnot", "sca", 2, "c128", 1), (16, 3, "cnot", "pairwise", 1, "c64", 2),
+    (18, 2, "cnot", "ring", 1, "c64", 0), (17, 2, "cz", "linear", 1, "c128", 0)])
+def test_specialised_gate_kernels(orc, n, D, ent, topo, fr, prec, prefix):
+    """gvqe_options.specialise = 2 forces the generated kernels at small sizes (by default they serve >= 20 qubits):
+    energies and amplitudes against the oracle, five rows in chunks of three so that a thread block meets several
+    statevectors; the generic kernels (specialise = 1) on the same inputs agree within the same tolerance."""
+    ops = np.array(layout_ops(n, D, ent, topo, fr), dtype=np.int32)
+    P = num_params(n, D, fr)
+    paulis, coeffs = random_paulis(900 + n, n, 100, 5)
+    th = np.random.default_rng(n).uniform(-math.pi, math.pi, (5, P))
+    th[1, :3] = [math.pi, -math.pi, 0.0]                            # exact quarter turns: cos = 0 up to rounding
+    ref = orc.energy_batch(n, ops, th, paulis, coeffs)
+    for spec in (2, 1):
+        g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo, final_rot=fr), precision=prec,
+                    options=dict(specialise=spec, prefix=prefix))
+        assert (g.kernel_source(0) is not None) == (spec == 2)
+        g.set_hamiltonian(paulis, coeffs)
+        g.alloc_workspace(3)
+        assert_close(prec, g.energy_batch(th), ref, coeffs, f"specialise={spec}")
+        assert np.max(np.abs(g.get_state(1) - orc.state(n, ops, th[4]))) < (1e-12 if prec == "c128" else 2e-5)
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_specialised_random_circuits(orc, seed):
+    n = 13 + seed % 4
+    prec = "c64" if seed % 2 else "c128"
+    ops, P = random_ops(7100 + seed, n, 160)
+    paulis, coeffs = random_paulis(8100 + seed, n, 60, 6)
+    th = np.random.default_rng(seed).uniform(-math.pi, math.pi, (4, P))
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(specialise=2))
+    g.set_hamiltonian(paulis, coeffs)
+    g.alloc_workspace(4)
+    assert_close(prec, g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, f"specialised random n={n}")
+    assert np.max(np.abs(g.get_state(3) - orc.state(n, ops, th[3]))) < (1e-12 if prec == "c128" else 2e-5)
+
+
+def test_generic_kernels_at_config3_size(orc):
+    """From 20 qubits on the specialised kernels are the default; the generic ones stay covered at that size too."""
+    w = make_workload(3)
+    idx = np.arange(0, w.M, 17)
+    pl = w.pauli_list()
+    sub_p, sub_c = "".join(pl[i] for i in idx).encode(), w.coeffs[idx]
+    psi = orc.state(w.n, w.ops, w.params[5])
+    ref = orc.energy_of_state(w.n, psi, sub_p, sub_c)
+    for spec in (1, 0):
+        g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology), precision="c64",
+                    options=dict(specialise=spec))
+        assert (g.kernel_source(0) is None) == (spec == 1)
+        g.set_hamiltonian(sub_p, sub_c)
+        g.alloc_workspace(8)
+        assert_close("c64", g.energy_batch(w.params[:8])[5:6], [ref], sub_c, f"cfg3 specialise={spec}")
 
 
 def test_long_op_list_splits_blocks(orc):

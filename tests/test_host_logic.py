@@ -61,8 +61,8 @@ def test_masks_api_equals_string_api(orc):
         assert np.array_equal(u, v)
 
 
-def _check_order(orc, n, ops, P, prec, seed):
-    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec)
+def _check_order(orc, n, ops, P, prec, seed, options=None):
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=options)
     order = g.get_exec_order()
     assert sorted(order.tolist()) == list(range(len(ops)))          # every op exactly once
     th = np.random.default_rng(seed).uniform(-math.pi, math.pi, max(P, 1))
@@ -80,11 +80,11 @@ def test_schedule_order_is_equivalent_random(orc, seed):
 
 @pytest.mark.parametrize("n,D,ent,topo,fr,prec", [(14, 3, "cz", "linear", 1, "c64"), (15, 3, "cnot", "ring", 1, "c64"),
                                                    (13, 2, "cnot", "linear", 2, "c128"), (16, 2, "cz", "ring", 2, "c128")])
-def test_schedule_order_is_equivalent_layered(orc, n, D, ent, topo, fr, prec, monkeypatch):
-    monkeypatch.setenv("GVQE_K", "10")                              # several tiles and high-qubit blocks at small n
+def test_schedule_order_is_equivalent_layered(orc, n, D, ent, topo, fr, prec):
     from workload import layout_ops, num_params
     ops = np.array(layout_ops(n, D, ent, topo, fr), dtype=np.int32)
-    _check_order(orc, n, ops, num_params(n, D, fr), prec, n)
+    # tile_bits = 10: several tiles and high-qubit blocks at small n
+    _check_order(orc, n, ops, num_params(n, D, fr), prec, n, options=dict(tile_bits=10))
 
 
 def test_layout_expansion_matches_generator():
@@ -154,3 +154,45 @@ def test_argument_errors():
         g.set_workspace(0, 1 << 20)
     with pytest.raises(gv.GvqeError):
         g.set_workspace(4096, 16)       # too small for one statevector
+
+
+def test_no_environment_knobs_in_the_library():
+    """SURVEY 5 "no global flags": schedule choices are gvqe_options fields, never environment variables."""
+    csrc = os.path.join(ROOT, "paper_2607_02749_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
+def test_options_are_validated_and_change_the_schedule():
+    lay = dict(n_layers=2, entangler="cnot", topology="ring")
+    a = gv.Gvqe(14, layout=lay, precision="c64")
+    b = gv.Gvqe(14, layout=lay, precision="c64", options=dict(tile_bits=10))
+    assert "k=13" in a.dump_schedule() and "k=10" in b.dump_schedule()
+    assert "prefix ops=0" in gv.Gvqe(14, layout=lay, precision="c64", options=dict(prefix=1)).dump_schedule()
+    assert "prefix ops=0" not in gv.Gvqe(14, layout=lay, precision="c64", options=dict(prefix=2)).dump_schedule()
+    for bad in (dict(prefix=3), dict(specialise=-1), dict(tile_bits=40), dict(shared_prefix=7)):
+        with pytest.raises(gv.GvqeError):
+            gv.Gvqe(14, layout=lay, precision="c64", options=bad)
+    with pytest.raises(gv.GvqeError):
+        gv.Gvqe(14, layout=lay, options=dict(no_such_option=1))
+
+
+@pytest.mark.parametrize("cfg,prec", [(3, "c64"), (3, "c128"), (4, "c64"), (5, "c64"), (6, "c128")])
+def test_specialised_kernels_generate_and_compile(cfg, prec):
+    """The bench configurations get one generated kernel per fused block (default from 20 qubits on); each compiles for
+    sm_100a with NVRTC on this machine (no GPU needed), uses cp.async tile loads and fits two thread blocks per SM."""
+    w = make_workload(cfg, M=40, batch=1)
+    g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology), precision=prec)
+    nb = g.schedule_info()[0] - (0 if "prefix ops=0" in g.dump_schedule() else 1)
+    srcs = [g.kernel_source(b) for b in range(nb)]
+    assert all(s is not None for s in srcs) and g.kernel_source(nb) is None
+    for src, smem in srcs:
+        assert "cp.async.cg.shared.global" in src and smem <= 113 * 1024
+    try:
+        assert g.compile_kernels() == nb
+    except gv.GvqeError as e:
+        if "libnvrtc not found" in str(e):
+            pytest.skip("NVRTC is not installed here")
+        raise
+    # small registers keep the generic kernels unless asked
+    assert gv.Gvqe(12, layout=dict(n_layers=1, entangler="cz", topology="linear")).kernel_source(0) is None
