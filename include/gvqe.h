@@ -94,10 +94,17 @@ gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precis
                             gvqe_ctx **out);
 gvqe_status gvqe_create_ops_opt(int n_qubits, const gvqe_op *ops, int n_ops, int n_params, gvqe_precision prec,
                                 const gvqe_options *opt, gvqe_ctx **out);
-/* Source text of the specialised kernel of fused block `block` (0-based) as the library would compile it: written to
- * buf (NUL-terminated, truncated to cap); returns the full length needed, 0 when the schedule has no such kernel.
+/* Source text of specialised kernel number `block` as the library would compile it: the fused gate blocks first
+ * (0-based, in execution order), then -- once a Hamiltonian is set -- the expectation passes; written to
+ * buf (NUL-terminated, truncated to cap); returns the full length needed, 0 when there is no such kernel.
  * *smem_bytes (optional): its dynamic shared memory.  Host only (no GPU, no compiler). */
 size_t gvqe_kernel_source(const gvqe_ctx *ctx, int block, char *buf, size_t cap, int32_t *smem_bytes);
+/* The arrays the specialised expectation kernels read from global memory, as host images (introspection for tests):
+ * which = 0: static W tables (double re, im per entry), 1: tile-dependent index patterns (4 x uint32: shared-memory byte
+ * offset, first term, last term + 1, 0), 2: terms (double re, im of c_k i^{nY}; uint64 z bits outside the tile; uint64
+ * local z mask for direct groups), 3: per pass (uint32 first table entry, first pattern, number of patterns).
+ * Copies min(cap, size) bytes into buf; returns the size in bytes (0: no specialised expectation kernels). */
+size_t gvqe_kernel_arrays(const gvqe_ctx *ctx, int which, void *buf, size_t cap);
 /* Compiles every specialised kernel of the context with NVRTC for sm_100a (host only: needs the compiler library, no
  * GPU; images are cached for the first energy call).  *n_kernels (optional): how many were compiled (0 when the
  * context uses the generic kernels).  GVQE_ERR_UNSUPPORTED with the compiler's message when NVRTC is missing or a

@@ -19,7 +19,7 @@ GVQE_C64, GVQE_C128 = 0, 1
 STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "GVQE_ERR_WORKSPACE",
                 "GVQE_ERR_UNSUPPORTED", "GVQE_ERR_CUDA"]
 
-EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
+EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_kernel_arrays", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
@@ -78,6 +78,8 @@ def load():
     L.gvqe_kernel_source.argtypes = [vp, i32, C.c_char_p, sz, vp]
     L.gvqe_kernel_source.restype = sz
     L.gvqe_compile_kernels.argtypes = [vp, vp]
+    L.gvqe_kernel_arrays.argtypes = [vp, i32, vp, sz]
+    L.gvqe_kernel_arrays.restype = sz
     L.gvqe_num_params.argtypes = [vp]
     L.gvqe_num_qubits.argtypes = [vp]
     L.gvqe_set_hamiltonian.argtypes = [vp, i32, C.c_char_p, vp]
@@ -281,6 +283,13 @@ class Gvqe:
         buf = C.create_string_buffer(need + 1)
         self._L.gvqe_kernel_source(self._h, int(block), buf, need + 1, C.addressof(sm))
         return buf.value.decode(), int(sm.value)
+
+    def kernel_arrays(self, which: int) -> np.ndarray:
+        """Host image (uint8 array) of what the specialised expectation kernels read from global memory (gvqe_kernel_arrays)."""
+        need = self._L.gvqe_kernel_arrays(self._h, int(which), None, 0)
+        buf = np.zeros(max(need, 1), dtype=np.uint8)
+        self._L.gvqe_kernel_arrays(self._h, int(which), buf.ctypes.data, need)
+        return buf[:need]
 
     def compile_kernels(self) -> int:
         """NVRTC-compile every specialised kernel (no GPU needed); returns how many."""

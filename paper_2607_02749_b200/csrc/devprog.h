@@ -118,7 +118,7 @@ struct DGroup {              // one flip mask (or a slice of its terms) inside a
     uint32_t gtab_off;       // offset of the group's static W table in the global table array (= batch base + tab_off)
     uint32_t batch_entries;  // table entries of the whole batch this group belongs to
     uint32_t batch_last;     // index of the last group of that batch
-    uint32_t pad_hot;
+    uint32_t uloc;           // table mode: the local bits that form the table index (ascending order = index bit order)
     uint64_t hot;            // what the group loop needs, one shared-memory read: mode (0 lookup, 1 register stage, 2 direct)
                              // | m_r << 2 | rs_id << 8 | tab_off << 24 | has tile-dependent terms << 63
     uint32_t ex_pack;        // ex[] packed 4 bits each (entry e at bits 4e)

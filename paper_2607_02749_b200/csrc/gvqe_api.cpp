@@ -66,6 +66,12 @@ struct gvqe_ctx {
     std::vector<JitBlock> jit_blocks;
     std::vector<JitModule *> jit_mods;
     void *d_ry = nullptr;
+    int jitx_state = -1;        // expectation passes: -1 not used, 0 generated (to be loaded), 1 loaded
+    std::vector<JitBlock> jitx_blocks;
+    std::vector<JitModule *> jitx_mods;
+    JitExpectData jitx;
+    std::vector<float> jitx_wst_f;
+    void *d_jwst = nullptr; void *d_jpats = nullptr; void *d_jterms = nullptr;
     bool profiling = false;
     std::vector<cudaEvent_t> ev;
     double prof_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -170,24 +176,47 @@ gvqe_status gvqe_create_ops(int n, const gvqe_op *ops, int n_ops, int n_params, 
 
 size_t gvqe_kernel_source(const gvqe_ctx *c, int block, char *buf, size_t cap, int32_t *smem_bytes)
 {
-    if (!c || block < 0 || (size_t)block >= c->jit_blocks.size()) return 0;
-    const std::string &s = c->jit_blocks[(size_t)block].source;
-    if (smem_bytes) *smem_bytes = (int32_t)c->jit_blocks[(size_t)block].smem_bytes;
+    if (!c || block < 0 || (size_t)block >= c->jit_blocks.size() + c->jitx_blocks.size()) return 0;
+    const JitBlock &jb = (size_t)block < c->jit_blocks.size() ? c->jit_blocks[(size_t)block] : c->jitx_blocks[(size_t)block - c->jit_blocks.size()];
+    const std::string &s = jb.source;
+    if (smem_bytes) *smem_bytes = (int32_t)jb.smem_bytes;
     if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }
     return s.size() + 1;
+}
+
+size_t gvqe_kernel_arrays(const gvqe_ctx *c, int which, void *buf, size_t cap)
+{
+    if (!c || c->jitx_blocks.empty()) return 0;
+    std::vector<uint32_t> pp;
+    const void *src = nullptr;
+    size_t bytes = 0;
+    switch (which) {
+    case 0: src = c->jitx.wst.data(); bytes = c->jitx.wst.size() * 8; break;
+    case 1: src = c->jitx.pats.data(); bytes = c->jitx.pats.size() * sizeof(JitExpectData::Pat); break;
+    case 2: src = c->jitx.terms.data(); bytes = c->jitx.terms.size() * sizeof(JitExpectData::Term); break;
+    case 3:
+        for (size_t p = 0; p < c->jitx.pass_wst_off.size(); ++p) { pp.push_back(c->jitx.pass_wst_off[p]); pp.push_back(c->jitx.pass_pat_off[p]); pp.push_back(c->jitx.pass_pat_cnt[p]); }
+        src = pp.data(); bytes = pp.size() * 4; break;
+    default: return 0;
+    }
+    if (buf && cap && bytes) memcpy(buf, src, bytes < cap ? bytes : cap);
+    return bytes;
 }
 
 gvqe_status gvqe_compile_kernels(gvqe_ctx *c, int32_t *n_kernels)
 {
     if (!c) return GVQE_ERR_INVALID_ARG;
     if (n_kernels) *n_kernels = 0;
-    const size_t nbk = c->jit_blocks.size();
+    std::vector<const JitBlock *> all;
+    for (const JitBlock &jb : c->jit_blocks) all.push_back(&jb);
+    for (const JitBlock &jb : c->jitx_blocks) all.push_back(&jb);
+    const size_t nbk = all.size();
     std::vector<std::string> errs(nbk);
     std::vector<char> ok(nbk, 0);
     for (size_t b0 = 0; b0 < nbk; b0 += 8) {
         std::vector<std::thread> th;
         for (size_t b = b0; b < nbk && b < b0 + 8; ++b)
-            th.emplace_back([c, b, &errs, &ok] { std::vector<char> img; ok[b] = jit_compile_only(c->jit_blocks[b], img, errs[b]) ? 1 : 0; });
+            th.emplace_back([&all, b, &errs, &ok] { std::vector<char> img; ok[b] = jit_compile_only(*all[b], img, errs[b]) ? 1 : 0; });
         for (std::thread &t : th) t.join();
     }
     for (size_t b = 0; b < nbk; ++b) if (!ok[b]) return fail(c, GVQE_ERR_UNSUPPORTED, errs[b]);
@@ -289,6 +318,21 @@ static gvqe_status after_hamiltonian(gvqe_ctx *c)
         }
         c->fwht_tiles.push_back(td); c->fwht_masks.push_back(mask);
     }
+    // specialised expectation kernels: same policy as the gate kernels (gvqe_options.specialise)
+    for (JitModule *m : c->jitx_mods) jit_unload(m);
+    c->jitx_mods.clear(); c->jitx_blocks.clear(); c->jitx = JitExpectData(); c->jitx_state = -1;
+    {
+        std::string why;
+        const bool want = c->opt.specialise == 2 || (c->opt.specialise == 0 && c->n_store >= 20);
+        if (want && jit_expect_supported(c->plan, c->n_store, c->prec, why)) {
+            c->jitx_blocks.resize(c->plan.passes.size());
+            bool ok = true;
+            for (size_t p = 0; p < c->plan.passes.size() && ok; ++p)
+                ok = jit_expect_generate(c->plan, c->n_store, c->prec, (int)p, c->jitx, c->jitx_blocks[p], why);
+            if (ok) c->jitx_state = 0;
+            else { c->jitx_blocks.clear(); c->jitx = JitExpectData(); }
+        }
+    }
     c->have_h = true; c->dirty = true;
     return GVQE_OK;
 }
@@ -343,7 +387,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, jwst, jpats, jterms, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, ry_b, params_b, partial_b;
 };
@@ -363,6 +407,9 @@ Layout layout_of(const gvqe_ctx *c)
     L.ryl = cv.take(d.ryl.size() * 2);
     L.cxs = cv.take(d.cxs.size() * sizeof(DCx));
     L.slut = cv.take(d.slut.size() * 4);
+    L.jwst = cv.take(c->jitx.wst.size() / 2 * c->amp_bytes());
+    L.jpats = cv.take(c->jitx.pats.size() * sizeof(JitExpectData::Pat));
+    L.jterms = cv.take(c->jitx.terms.size() * sizeof(JitExpectData::Term));
     L.px_begin = cv.take(c->px.rot_begin.size() * 4); L.px_kind = cv.take(c->px.rot_kind.size());
     L.px_param = cv.take(c->px.rot_param.size() * 4); L.px_t = cv.take(c->px.cx_t.size()); L.px_c = cv.take(c->px.cx_c.size());
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
@@ -410,29 +457,38 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
         if (ke) return cuda_fail(c, ke, "kernel attribute setup");
         c->kernels_ready = true;
     }
-    if (c->jit_state == 0) {   // compile the specialised gate kernels (NVRTC, in parallel) and load them on this device
-        std::string why;
+    // compile the specialised kernels (NVRTC, eight at a time: it is thread safe) and load them on this device
+    auto load_all = [c](const std::vector<JitBlock> &blocks, std::vector<JitModule *> &mods, std::string &why) {
         bool ok = jit_runtime_available(why);
-        if (ok) {
-            int dev = 0, sms = 0;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) c->sm_count = sms;
-            const size_t nbk = c->jit_blocks.size();
-            std::vector<std::string> errs(nbk);
-            c->jit_mods.assign(nbk, nullptr);
-            for (size_t b0 = 0; b0 < nbk; b0 += 8) {   // NVRTC is thread safe: eight blocks at a time
-                std::vector<std::thread> th;
-                for (size_t b = b0; b < nbk && b < b0 + 8; ++b)
-                    th.emplace_back([c, b, &errs] { c->jit_mods[b] = jit_load(c->jit_blocks[b], errs[b]); });
-                for (std::thread &t : th) t.join();
-            }
-            for (size_t b = 0; b < nbk; ++b) if (!c->jit_mods[b]) { ok = false; why = errs[b]; }
+        if (!ok) return false;
+        const size_t nbk = blocks.size();
+        std::vector<std::string> errs(nbk);
+        mods.assign(nbk, nullptr);
+        for (size_t b0 = 0; b0 < nbk; b0 += 8) {
+            std::vector<std::thread> th;
+            for (size_t b = b0; b < nbk && b < b0 + 8; ++b)
+                th.emplace_back([&blocks, &mods, b, &errs] { mods[b] = jit_load(blocks[b], errs[b]); });
+            for (std::thread &t : th) t.join();
         }
-        if (!ok) {
-            for (JitModule *m : c->jit_mods) jit_unload(m);
-            c->jit_mods.clear();
+        for (size_t b = 0; b < nbk; ++b) if (!mods[b]) { ok = false; why = errs[b]; }
+        if (!ok) { for (JitModule *m : mods) jit_unload(m); mods.clear(); }
+        return ok;
+    };
+    if (c->jit_state == 0) {
+        std::string why;
+        if (load_all(c->jit_blocks, c->jit_mods, why)) c->jit_state = 1;
+        else {
             if (c->opt.specialise == 2) return fail(c, GVQE_ERR_UNSUPPORTED, "specialised kernels requested but unavailable: " + why);
             c->jit_state = -1; c->jit_blocks.clear();
-        } else c->jit_state = 1;
+        }
+    }
+    if (c->jitx_state == 0) {
+        std::string why;
+        if (load_all(c->jitx_blocks, c->jitx_mods, why)) c->jitx_state = 1;
+        else {
+            if (c->opt.specialise == 2) return fail(c, GVQE_ERR_UNSUPPORTED, "specialised kernels requested but unavailable: " + why);
+            c->jitx_state = -1; c->jitx_blocks.clear(); c->jitx = JitExpectData();
+        }
     }
     const Layout L = layout_of(c);
     if (c->ws_bytes < L.fixed_end + L.per_state) {
@@ -453,6 +509,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.csidx = (const int32_t *)(w + L.csidx);
     c->gl.ryl = (const int16_t *)(w + L.ryl); c->gl.cxs = (const DCx *)(w + L.cxs);
     c->gl.slut = (const uint32_t *)(w + L.slut);
+    c->d_jwst = w + L.jwst; c->d_jpats = w + L.jpats; c->d_jterms = w + L.jterms;
     c->pxd.rot_begin = (const int32_t *)(w + L.px_begin); c->pxd.rot_kind = (const uint8_t *)(w + L.px_kind);
     c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
     c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
@@ -482,6 +539,11 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
         UP(c->d_wstat, c->wstat_f);
     } else UP(c->d_wstat, c->plan.wstat);
     UP(c->d_gtabs, c->plan.gtabs); UP(c->d_rss, c->plan.rss);
+    if (c->jitx_state == 1) {
+        if (c->prec == GVQE_C64) { c->jitx_wst_f.assign(c->jitx.wst.begin(), c->jitx.wst.end()); UP(c->d_jwst, c->jitx_wst_f); }
+        else UP(c->d_jwst, c->jitx.wst);
+        UP(c->d_jpats, c->jitx.pats); UP(c->d_jterms, c->jitx.terms);
+    }
     UP(c->d_diag_z, c->H.diag_z); UP(c->d_diag_c, c->H.diag_c);
 #undef UP
     // diagonal energy table: E(x) = sum_{Z-only k} c_k (-1)^{popcount(x & z_k)} = WHT of the scattered coefficients
@@ -513,6 +575,20 @@ int gate_block(gvqe_ctx *c, size_t j, void *states, uint64_t stride, const void 
                              states, stride, cs, c->P, nb, st, &c->launches);
 }
 
+// Expectation pass pi over nb statevectors starting at `states`; partial sums go to partial[b][slot_off + tile].
+int expect_pass(gvqe_ctx *c, size_t pi, const void *states, uint64_t stride, double *partial, uint32_t slot_off, int nb, cudaStream_t st)
+{
+    if (c->jitx_state == 1) {
+        ++c->launches;
+        const char *wst = (const char *)c->d_jwst + (size_t)c->jitx.pass_wst_off[pi] * c->amp_bytes();
+        const char *pats = (const char *)c->d_jpats + (size_t)c->jitx.pass_pat_off[pi] * sizeof(JitExpectData::Pat);
+        return jit_launch_expect(c->jitx_mods[pi], c->jitx_blocks[pi], states, stride, c->d_table, wst, pats, c->d_jterms, partial,
+                                 c->slots_per_b, slot_off, nb, c->jit_per_cta, st);
+    }
+    return launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat, c->d_gtabs,
+                              c->d_rss, states, stride, c->d_table, partial, c->slots_per_b, slot_off, nb, st, &c->launches);
+}
+
 gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_dev, cudaStream_t st)
 {
     const Layout L = layout_of(c);
@@ -542,8 +618,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     if (c->profiling) cudaEventRecord(e4[1], st);
     const uint32_t tiles = 1u << (c->n_store - c->plan.k);
     for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
-        ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat, c->d_gtabs, c->d_rss, c->d_states,
-                                stride, c->d_table, c->d_partial, c->slots_per_b, (uint32_t)pi * tiles, nb, st, &c->launches);
+        ke = expect_pass(c, pi, c->d_states, stride, c->d_partial, (uint32_t)pi * tiles, nb, st);
         if (ke) return cuda_fail(c, ke, "expectation pass");
     }
     if (c->profiling) cudaEventRecord(e4[2], st);
@@ -679,9 +754,7 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
     auto expect = [&](int slot, int nb) -> gvqe_status {
         double *partial = c->d_partial + (size_t)slot * c->slots_per_b;
         for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
-            const int ke = launch_expect_pass(c->prec, c->d_passes, (int)pi, c->plan.k, c->n_store, c->d_groups, c->d_terms, c->d_wstat,
-                                              c->d_gtabs, c->d_rss, state_of(slot), stride, c->d_table, partial, c->slots_per_b,
-                                              (uint32_t)pi * tiles, nb, st, &c->launches);
+            const int ke = expect_pass(c, pi, state_of(slot), stride, partial, (uint32_t)pi * tiles, nb, st);
             if (ke) return cuda_fail(c, ke, "expectation pass");
         }
         const int ke = launch_reduce(partial, c->slots_per_b, c->d_E + slot, nb, st, &c->launches);
@@ -1000,6 +1073,7 @@ void gvqe_destroy(gvqe_ctx *c)
     if (!c) return;
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     for (JitModule *m : c->jit_mods) jit_unload(m);
+    for (JitModule *m : c->jitx_mods) jit_unload(m);
     delete c;
 }
 

@@ -307,6 +307,7 @@ bool plan_expectation(const Hamiltonian &H, int n, int k, int f, int umax, uint3
                 }
                 ++batch_groups;
                 if (table) {
+                    dg.uloc = Uloc;
                     dg.ubits = (uint8_t)ubits; dg.n_uruns = (uint8_t)(nur < 3 ? nur : 3);
                     for (int r = 0; r < nur && r < 3; ++r) { dg.uruns[r].lpos = ur[r].gpos; dg.uruns[r].len = ur[r].len; dg.uruns[r].shift = ur[r].lpos; }
                     dg.tab_off = tab_used; tab_used += 1u << ubits;

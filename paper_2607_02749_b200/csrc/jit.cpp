@@ -17,6 +17,7 @@
 // R_z phases and CZ signs (Eq. 7; entangling layer PAPER.md:169) of a diagonal segment are one complex
 // factor per amplitude = (per-thread table entry) x (per-tile constant) x (small tables over the register bits).
 #include "jit.h"
+#include "jit_internal.h"
 
 #include <algorithm>
 #include <cstdarg>
@@ -28,26 +29,6 @@ namespace {
 
 constexpr int JIT_MAX_STAGES = 40;            // per block (code size)
 constexpr uint32_t JIT_SMEM_MAX = 113 * 1024;   // two thread blocks per SM
-
-struct Emit {
-    std::string s;
-    void operator()(const char *fmt, ...)
-    {
-        char buf[1024];
-        va_list ap;
-        va_start(ap, fmt);
-        vsnprintf(buf, sizeof buf, fmt, ap);
-        va_end(ap);
-        s += buf;
-        s += '\n';
-    }
-};
-
-struct Geo {
-    int k, R, TB, lv, prec;   // lv: log2(amplitudes per 16-byte unit)
-    uint32_t pu(uint32_t u) const { return u ^ ((u >> 3) & 7u) ^ ((u >> 6) & 7u) ^ ((u >> 9) & 7u); }
-    uint32_t off(uint32_t j) const { return (pu(j >> lv) << 4) | ((j & ((1u << lv) - 1u)) << 3); }
-};
 
 uint64_t scatter(const Block &B, uint32_t j)
 {
@@ -63,19 +44,7 @@ int lpos_of(const Block &B, int q)
     return -1;
 }
 
-// thread-index bit -> local bit, chosen so that the lanes of one shared-memory wavefront hit distinct banks
-void choose_thread_bits(const Geo &g, const Stage &S, int *tb)
-{
-    bool isreg[16] = {false};
-    for (int s = 0; s < g.R; ++s) isreg[S.regbit[s]] = true;
-    bool used[16] = {false};
-    int n = 0;
-    if (g.lv == 1 && !isreg[0]) { tb[n++] = 0; used[0] = true; }   // 8-byte accesses: the amplitude inside the unit varies fastest
-    for (int res = 0; res < 3; ++res)
-        for (int b = g.lv; b < g.k; ++b)
-            if (!isreg[b] && !used[b] && (b - g.lv) % 3 == res) { tb[n++] = b; used[b] = true; break; }
-    for (int b = 0; b < g.k; ++b) if (!isreg[b] && !used[b]) { tb[n++] = b; used[b] = true; }
-}
+void choose_thread_bits(const Geo &g, const Stage &S, int *tb) { choose_thread_bits_for(g, S.regbit, g.R, tb); }
 
 // affine map of the local index by a CNOT run: j -> A j ^ c(tile)
 struct CxMap {
@@ -98,18 +67,6 @@ CxMap cx_map(const Program &p, const Block &B, const Stage &S, int k)
         } else m.outside.push_back({(int)p.cxs[ci].cq, 1u << tl});
     }
     return m;
-}
-
-// emits "unsigned NAME = deposit of tid bits into local bits tb[]"
-void emit_deposit(Emit &E, const char *name, const int *tb, int TB)
-{
-    E("        unsigned %s = 0u;", name);
-    for (int i = 0; i < TB;) {
-        int len = 1;
-        while (i + len < TB && tb[i + len] == tb[i] + len) ++len;
-        E("        %s |= ((tid >> %d) & %uu) << %d;", name, i, (1u << len) - 1u, tb[i]);
-        i += len;
-    }
 }
 
 struct SegInfo {
@@ -367,7 +324,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     for (int s = s_first; s < ns; ++s) {
         const Stage &S = p.stages[B.stage_begin + s];
         E("    {   // stage %d: thread part of the shared-memory offset", s);
-        emit_deposit(E, "j", tbs[s].data(), TB);
+        emit_deposit(E, "        ", "j", tbs[s].data(), TB);
         E("        ((unsigned *)(smem + %u))[tid] = OFF(j);", o_sb[s]);
         if (S.cx_end > S.cx_begin) {
             const CxMap m = cx_map(p, B, S, k);

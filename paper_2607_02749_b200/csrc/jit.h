@@ -12,6 +12,7 @@
 #include <string>
 #include <vector>
 
+#include "hamiltonian.h"
 #include "schedule.h"
 
 namespace gv {
@@ -30,6 +31,19 @@ bool jit_supported(const Program &p, int prec, std::string &why);
 // Source of the kernel of block `bi`.  prec: 0 = complex64, 1 = complex128.
 bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string &err);
 
+// ---- expectation passes (jit_expect.cpp): one kernel per read-only pass of an ExpectPlan ------------------------------
+struct JitExpectData {   // host images of the arrays the kernels read from global memory (uploaded once per Hamiltonian)
+    struct Pat { uint32_t dst, begin, end, pad; };          // shared-memory byte offset of a table entry; its terms
+    struct Term { double cr, ci; uint64_t zout, pad; };     // c_k i^{nY}; z bits outside the tile; (direct groups: local z mask)
+    std::vector<double> wst;                                 // static W tables, (re, im) per entry, pass after pass
+    std::vector<Pat> pats;
+    std::vector<Term> terms;
+    std::vector<uint32_t> pass_wst_off, pass_pat_off, pass_pat_cnt;   // per pass: first entry / first pattern / patterns
+};
+bool jit_expect_supported(const ExpectPlan &plan, int n, int prec, std::string &why);
+// Appends pass `pi`'s arrays to `data` (call for pi = 0, 1, ... in order) and writes its kernel to `out`.
+bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExpectData &data, JitBlock &out, std::string &err);
+
 // ---- run time (jit_rt.cpp): NVRTC through dlopen, module load and launch through the driver entry points -----------
 struct JitModule;   // one loaded kernel
 bool jit_runtime_available(std::string &why);
@@ -42,5 +56,9 @@ void jit_unload(JitModule *m);
 // per_cta: consecutive (statevector, tile) work items one thread block handles (its setup is paid once per thread block).
 int jit_launch(JitModule *m, const JitBlock &blk, void *states, uint64_t stride, const void *ry, const void *cs, int nb, int P,
                int per_cta, void *stream);
+// Expectation pass: table = diagonal energy table, wst / pats = this pass's static tables and patterns, terms = all terms.
+int jit_launch_expect(JitModule *m, const JitBlock &blk, const void *states, uint64_t stride, const void *table, const void *wst,
+                      const void *pats, const void *terms, double *partial, uint32_t slots_per_b, uint32_t slot_off, int nb,
+                      int per_cta, void *stream);
 
 }  // namespace gv

@@ -1,0 +1,424 @@
+// jit_expect.cpp -- generator of the schedule-specialised expectation-pass kernels (see jit.h).  Pure host C++.
+//
+// One kernel per read-only pass over the state (Eq. 4, 6, 12: PAPER.md:135, 150, 216).  A thread
+// block works through consecutive (statevector, tile) items.  Per item: the tile arrives in shared memory by 16-byte
+// cp.async copies (same swizzled layout as the gate kernels), the tables of the groups whose terms carry Z / Y on
+// qubits outside the tile are refreshed, then every flip-mask group of the pass is evaluated with literal addresses:
+//   diagonal part   sum_x |psi_x|^2 E(x) over the thread's 16-byte units (first pass only);
+//   clusters        (planner: groups whose flip mask and in-tile z bits fit R local bits) the thread holds the 2^R
+//                   amplitudes of those bits; per pair (x, x^m), x with the pivot bit clear,
+//                   Re(conj(psi[x^m]) W(x) psi[x]) = a . (b.x (Wx,-Wy) + b.y (Wy,Wx)),  a = psi[x], b = psi[x^m]:
+//                   three packed operations per pair, W from a broadcast table read;
+//   table groups    W depends on thread bits only, constant over the thread's 2^L pairs:
+//                   Re(W sum conj(b) a) with two packed operations per pair;
+//   direct groups   (very wide terms) W summed term by term.
+// Tables: W_g(e) = sum_k c_k i^{nY_k} (-1)^{popcount(e & zu_k)} over the group's table index e.  The part of the terms
+// with all Z / Y inside the tile is built on the host.  A term with z bits outside the tile has a sign that depends on
+// the tile: per tile, D_p = sum of those terms' signed coefficients per distinct index pattern p (one thread per
+// pattern), then one warp per group turns D into sum_p D_p (-1)^{p.e} by Walsh-Hadamard butterflies: cost
+// (terms + E log E) per group and tile instead of (terms x E).
+#include <algorithm>
+#include <cstring>
+#include <map>
+
+#include "jit.h"
+#include "jit_internal.h"
+
+namespace gv {
+namespace {
+
+struct GInfo {
+    int mode = 0;                 // 0 table (lookup), 1 cluster (register stage), 2 direct
+    uint32_t E = 0;               // table entries
+    uint32_t tab_off = 0;         // byte offset of the final table in shared memory
+    uint32_t scr_off = 0;         // byte offset of the per-tile scratch (dynamic groups): complex entries
+    uint32_t wst_off = 0;         // entry offset of the static table in the pass's global array
+    bool dyn = false;
+    uint32_t pat_begin = 0, pat_end = 0;
+};
+
+}  // namespace
+
+bool jit_expect_supported(const ExpectPlan &plan, int n, int prec, std::string &why)
+{
+    const int K = prec == 0 ? 13 : 12;
+    if (plan.k != K || n < K) { why = "tile size differs from the specialised kernels"; return false; }
+    if (plan.passes.empty()) { why = "no pass"; return false; }
+    return true;
+}
+
+bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExpectData &data, JitBlock &out, std::string &err)
+{
+    if (pi < 0 || (size_t)pi >= plan.passes.size()) { err = "jit: bad pass"; return false; }
+    const DPass &P = plan.passes[pi];
+    Geo g;
+    g.k = P.k; g.lv = prec == 0 ? 1 : 0; g.prec = prec;
+    const int k = g.k;
+    const int TBITS = 8;                    // 256 threads
+    const int RS = k - TBITS;               // bits a thread holds: 5 (complex64) / 4 (complex128)
+    g.R = RS; g.TB = TBITS;
+    const uint32_t NT = 256, NR = 1u << RS;
+    const int V = 1 << g.lv;
+    const uint32_t NU = (1u << k) / V / NT;
+    const uint32_t AB = prec == 0 ? 8 : 16;
+    const char *TT = prec == 0 ? "float" : "double";
+    if (NU != 16) { err = "jit: unsupported geometry"; return false; }
+    Block B; memset(&B, 0, sizeof B);       // tile description in the gate generator's terms
+    B.k = P.k; B.n_runs = P.n_runs; memcpy(B.runs, P.runs, sizeof B.runs);
+    auto scatter = [&](uint32_t j) { uint64_t x = 0; for (int r = 0; r < B.n_runs; ++r) x |= (uint64_t)((j >> B.runs[r].lpos) & ((1u << B.runs[r].len) - 1u)) << B.runs[r].gpos; return x; };
+
+    // ---- groups: tables, static parts, dynamic patterns
+    const uint32_t g0 = P.group_begin, g1 = P.group_end;
+    std::vector<GInfo> gi(g1 - g0);
+    uint32_t sm = 0;
+    auto take = [&](uint32_t bytes) { const uint32_t o = sm; sm = (sm + bytes + 15u) & ~15u; return o; };
+    const uint32_t o_tile = take((uint32_t)AB << k);
+    const size_t wst_base = data.wst.size() / 2;
+    const size_t pat_base = data.pats.size();
+    for (uint32_t q = g0; q < g1; ++q) {
+        const DGroup &dg = plan.groups[q];
+        GInfo &G = gi[q - g0];
+        G.mode = dg.rs ? 1 : (dg.direct ? 2 : 0);
+        if (G.mode == 2) continue;
+        G.E = 1u << dg.ubits;
+        G.tab_off = take(G.E * 16u > G.E * AB && G.mode == 1 ? G.E * 16u : G.E * AB);   // clusters: 16-byte entries
+        G.dyn = dg.dyn_end > dg.term_begin;
+        G.scr_off = G.dyn ? (G.mode == 1 ? take(G.E * AB) : G.tab_off) : 0;
+        G.wst_off = (uint32_t)(data.wst.size() / 2 - wst_base);
+        for (uint32_t e = 0; e < G.E; ++e) {   // static part (terms with every Z / Y inside the tile)
+            double wr = 0.0, wi = 0.0;
+            for (uint32_t t = dg.dyn_end; t < dg.term_end; ++t) {
+                const DTerm &tm = plan.terms[t];
+                const int par = __builtin_popcount(e & tm.zu) & 1;
+                wr += par ? -tm.cr : tm.cr; wi += par ? -tm.ci : tm.ci;
+            }
+            data.wst.push_back(wr); data.wst.push_back(wi);
+        }
+        if (G.dyn) {   // tile-dependent terms by index pattern, input order inside a pattern (deterministic sums)
+            std::map<uint32_t, std::vector<uint32_t>> by_pat;
+            for (uint32_t t = dg.term_begin; t < dg.dyn_end; ++t) by_pat[plan.terms[t].zu & (G.E - 1u)].push_back(t);
+            G.pat_begin = (uint32_t)(data.pats.size() - pat_base);
+            for (auto &kv : by_pat) {
+                JitExpectData::Pat pt;
+                pt.dst = G.scr_off + kv.first * AB;
+                pt.begin = (uint32_t)data.terms.size();
+                for (uint32_t t : kv.second) {
+                    const DTerm &tm = plan.terms[t];
+                    data.terms.push_back(JitExpectData::Term{tm.cr, tm.ci, tm.zout, 0});
+                }
+                pt.end = (uint32_t)data.terms.size(); pt.pad = 0;
+                data.pats.push_back(pt);
+            }
+            G.pat_end = (uint32_t)(data.pats.size() - pat_base);
+        }
+    }
+    const uint32_t n_pats = (uint32_t)(data.pats.size() - pat_base);
+    const uint32_t o_red = take(64 * 8);
+    bool any_dyn = false;
+    for (const GInfo &G : gi) any_dyn = any_dyn || G.dyn;
+    data.pass_wst_off.push_back((uint32_t)wst_base);
+    data.pass_pat_off.push_back((uint32_t)pat_base);
+    data.pass_pat_cnt.push_back(n_pats);
+    if (sm > 220u * 1024u) { err = "jit: expectation pass needs too much shared memory"; return false; }
+
+    char name[64];
+    snprintf(name, sizeof name, "gvqe_expect_%d_%s", pi, prec == 0 ? "c64" : "c128");
+    Emit E;
+    E("// generated by libgvqe (jit_expect.cpp): expectation pass %d of %zu, n = %d, k = %d, %s; %u groups, %u tile-dependent patterns",
+      pi, plan.passes.size(), n, k, prec == 0 ? "complex64" : "complex128", g1 - g0, n_pats);
+    emit_common_prelude(E, prec, g.lv);
+    E("typedef %s tabt;", TT);
+    E("struct __align__(16) Pat { unsigned dst, begin, end, pad; };");
+    E("struct __align__(32) Term { double cr, ci; u64 zout, pad; };");
+    if (prec == 0) {
+        E("struct __align__(16) tw4 { float x, y, z, w; };   // (Wx, -Wy, Wy, Wx)");
+        E("__device__ __forceinline__ tw4 twfmt(amp w) { tw4 t; t.x = w.x; t.y = -w.y; t.z = w.y; t.w = w.x; return t; }");
+        // a . (b.x (Wx,-Wy) + b.y (Wy,Wx)) accumulated component-wise
+        E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const amp be = __ffma2_rn(MK(b.y, b.y), MK(t.z, t.w), __fmul2_rn(MK(b.x, b.x), MK(t.x, t.y))); acc = __ffma2_rn(a, be, acc); }");
+        E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1 = __ffma2_rn(MK(b.x, b.x), a, s1); s2 = __ffma2_rn(MK(b.y, b.y), a, s2); }");
+    } else {
+        E("typedef double2 tw4;");
+        E("__device__ __forceinline__ tw4 twfmt(amp w) { return w; }");
+        E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const double br = fma(t.y, b.y, t.x * b.x), bi = fma(-t.y, b.x, t.x * b.y); acc.x = fma(a.x, br, acc.x); acc.y = fma(a.y, bi, acc.y); }");
+        E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1.x = fma(b.x, a.x, s1.x); s1.y = fma(b.x, a.y, s1.y); s2.x = fma(b.y, a.x, s2.x); s2.y = fma(b.y, a.y, s2.y); }");
+    }
+    E("");
+    E("extern \"C\" __global__ void __launch_bounds__(%u, 2) %s(const amp *states, u64 stride, const tabt *table, const amp *wst, const Pat *pats, const Term *terms,", NT, name);
+    E("        double *partial, unsigned slots_per_b, unsigned slot_off, int nb, int per_cta)");
+    E("{");
+    E("    extern __shared__ __align__(128) unsigned char smem[];");
+    E("    unsigned char *tile = smem + %u;", o_tile);
+    E("    double *red = (double *)(smem + %u);", o_red);
+    E("    const unsigned tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5;");
+    E("    (void)lane; (void)warp; (void)pats; (void)terms; (void)table;");
+    // static tables of the groups without tile-dependent terms: once per thread block
+    for (uint32_t q = g0; q < g1; ++q) {
+        const GInfo &G = gi[q - g0];
+        if (G.mode == 2 || G.dyn) continue;
+        if (G.mode == 1) E("    for (unsigned e = tid; e < %uu; e += %uu) ((tw4 *)(smem + %u))[e] = twfmt(wst[%u + e]);", G.E, NT, G.tab_off, G.wst_off);
+        else E("    for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = wst[%u + e];", G.E, NT, G.tab_off, G.wst_off);
+    }
+    E("    const unsigned ld_off = OFF(tid << %d);", g.lv);
+    {
+        std::string sx = "    const u64 ld_x = 0ull";
+        for (int r = 0; r < B.n_runs; ++r) {
+            const int lp = B.runs[r].lpos, len = B.runs[r].len, gp = B.runs[r].gpos;
+            int lo = lp - g.lv, hi = lp + len - g.lv;
+            if (lo < 0) lo = 0;
+            if (hi > TBITS) hi = TBITS;
+            if (hi <= lo) continue;
+            char b[128];
+            snprintf(b, sizeof b, " | ((u64)((tid >> %d) & %uu) << %d)", lo, (1u << (hi - lo)) - 1u, gp + (lo + g.lv - lp));
+            sx += b;
+        }
+        sx += ";";
+        E("%s", sx.c_str());
+    }
+    E("    const u64 total = (u64)nb << %d;", n - k);
+    E("    const u64 w_begin = (u64)blockIdx.x * (u64)per_cta;");
+    E("    const u64 w_end = w_begin + (u64)per_cta < total ? w_begin + (u64)per_cta : total;");
+    E("    for (u64 w = w_begin; w < w_end; ++w) {");
+    E("        const int b = (int)(w >> %d);", n - k);
+    E("        const u64 tile_id = w & %lluull;", (unsigned long long)((1ull << (n - k)) - 1ull));
+    E("        const amp *state = states + (u64)b * stride;");
+    {
+        E("        u64 xbase = 0ull;");
+        int consumed = 0, gpos = 0;
+        for (int r = 0; r <= B.n_runs; ++r) {
+            const int gend = r < B.n_runs ? B.runs[r].gpos : n;
+            const int gap = gend - gpos;
+            if (gap > 0) {
+                E("        xbase |= ((tile_id >> %d) & %lluull) << %d;", consumed, (unsigned long long)((1ull << gap) - 1ull), gpos);
+                consumed += gap;
+            }
+            if (r < B.n_runs) gpos = B.runs[r].gpos + B.runs[r].len;
+        }
+    }
+    E("        const amp *gptr = state + (xbase | ld_x);");
+    std::vector<uint64_t> hi(NU);
+    std::vector<uint32_t> ci(NU);
+    for (uint32_t i = 0; i < NU; ++i) {
+        const uint32_t j = (NT * i) << g.lv;
+        hi[i] = scatter(j); ci[i] = g.off(j);
+    }
+    for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (ld_off ^ %uu), gptr + %lluull);", ci[i], (unsigned long long)hi[i]);
+    if (P.with_diag) {   // diagonal energies of the thread's units: issued under the tile copies
+        E("        const tabt *tptr = table + (xbase | ld_x);");
+        if (prec == 0) { for (uint32_t i = 0; i < NU; ++i) E("        const float2 tv%u = *(const float2 *)(tptr + %lluull);", i, (unsigned long long)hi[i]); }
+        else { for (uint32_t i = 0; i < NU; ++i) E("        const double tv%u = tptr[%lluull];", i, (unsigned long long)hi[i]); }
+    }
+    // ---- tile-dependent tables
+    if (any_dyn) {
+        for (uint32_t q = g0; q < g1; ++q) {
+            const GInfo &G = gi[q - g0];
+            if (!G.dyn) continue;
+            E("        for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = MK((real)0, (real)0);", G.E, NT, G.scr_off);
+        }
+        E("        __syncthreads();");
+        E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): signed sum of its terms", n_pats, NT);
+        E("            const Pat p = pats[i];");
+        E("            double sr = 0.0, si = 0.0;");
+        E("            for (unsigned t = p.begin; t < p.end; ++t) {");
+        E("                const Term tm = terms[t];");
+        E("                const bool neg = __popcll(xbase & tm.zout) & 1;");
+        E("                sr += neg ? -tm.cr : tm.cr; si += neg ? -tm.ci : tm.ci;");
+        E("            }");
+        E("            *(amp *)(smem + p.dst) = MK((real)sr, (real)si);");
+        E("        }");
+        E("        __syncthreads();");
+        int wi = 0;
+        for (uint32_t q = g0; q < g1; ++q) {
+            const GInfo &G = gi[q - g0];
+            if (!G.dyn) continue;
+            const DGroup &dg = plan.groups[q];
+            E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits, plus the static part", wi % 8, q - g0, (int)dg.ubits);
+            E("            amp *d = (amp *)(smem + %u);", G.scr_off);
+            for (int bit = 0; bit < (int)dg.ubits; ++bit) {
+                E("            for (unsigned i = lane; i < %uu; i += 32u) { const unsigned j = ((i >> %d) << %d) | (i & %uu); const amp u = d[j], v = d[j | %uu]; d[j] = MK(u.x + v.x, u.y + v.y); d[j | %uu] = MK(u.x - v.x, u.y - v.y); }",
+                  G.E / 2, bit, bit + 1, (1u << bit) - 1u, 1u << bit, 1u << bit);
+                E("            __syncwarp();");
+            }
+            if (G.mode == 1) E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; ((tw4 *)(smem + %u))[e] = twfmt(MK(d[e].x + s.x, d[e].y + s.y)); }", G.E, G.wst_off, G.tab_off);
+            else E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; d[e] = MK(d[e].x + s.x, d[e].y + s.y); }", G.E, G.wst_off);
+            E("        }");
+            ++wi;
+        }
+    }
+    E("        cp_wait();");
+    E("        __syncthreads();");
+    E("        double acc = 0.0;");
+    // ---- diagonal part
+    if (P.with_diag) {
+        E("        {   // sum |psi|^2 E(x) over the thread's units");
+        E("            real da = (real)0;");
+        for (uint32_t i = 0; i < NU; ++i) {
+            if (prec == 0) {
+                E("            { const float4 v = *(const float4 *)(tile + (ld_off ^ %uu)); da = fmaf(fmaf(v.x, v.x, v.y * v.y), tv%u.x, da); da = fmaf(fmaf(v.z, v.z, v.w * v.w), tv%u.y, da); }", ci[i], i, i);
+            } else {
+                E("            { const double2 v = *(const double2 *)(tile + (ld_off ^ %uu)); da = fma(fma(v.x, v.x, v.y * v.y), tv%u, da); }", ci[i], i);
+            }
+        }
+        E("            acc += (double)da;");
+        E("        }");
+    }
+    const uint32_t LOMASK = 0x70u;
+    // ---- clusters
+    std::map<int, std::vector<uint32_t>> clusters;   // rs_id -> groups
+    for (uint32_t q = g0; q < g1; ++q) if (gi[q - g0].mode == 1) clusters[plan.groups[q].rs_id].push_back(q);
+    for (auto &cl : clusters) {
+        const DRs &rs = plan.rss[(size_t)cl.first];
+        int tb[16];
+        choose_thread_bits_for(g, rs.regbit, RS, tb);
+        const bool wide = (g.lv == 1 && rs.regbit[0] == 0);
+        uint32_t cr[32];
+        bool vused[8] = {false};
+        for (uint32_t r = 0; r < NR; ++r) {
+            uint32_t j = 0;
+            for (int b = 0; b < RS; ++b) if (r >> b & 1) j |= 1u << rs.regbit[b];
+            cr[r] = g.off(j);
+            vused[(cr[r] & LOMASK) >> 4] = true;
+        }
+        E("        {   // ---- cluster %d: %zu groups from registers", cl.first, cl.second.size());
+        emit_deposit(E, "            ", "jt", tb, TBITS);
+        E("            const unsigned sb = OFF(jt);");
+        for (int v = 0; v < 8; ++v) if (vused[v]) E("            const unsigned char *const pv%d = tile + (sb ^ %uu);", v, (uint32_t)v << 4);
+        E("            amp a[%u];", NR);
+        if (wide) {
+            for (uint32_t r = 0; r < NR; r += 2)
+                E("            { const float4 v = *(const float4 *)(pv%u + %uu); a[%u] = MK(v.x, v.y); a[%u] = MK(v.z, v.w); }", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r, r + 1);
+        } else {
+            for (uint32_t r = 0; r < NR; ++r) E("            a[%u] = *(const amp *)(pv%u + %uu);", r, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK);
+        }
+        for (uint32_t q : cl.second) {
+            const DGroup &dg = plan.groups[q];
+            const GInfo &G = gi[q - g0];
+            const uint32_t mr = dg.m_r;
+            int pv = 31 - __builtin_clz(mr);
+            E("            {   // group %u: flip mask over the slots %u", q - g0, mr);
+            E("                const tw4 *W = (const tw4 *)(smem + %u);", G.tab_off);
+            E("                amp s = MK((real)0, (real)0);");
+            for (uint32_t r = 0; r < NR; ++r) {
+                if (r >> pv & 1) continue;
+                E("                pairw(s, a[%u], a[%u], W[%u]);", r, r ^ mr, r);
+            }
+            E("                acc += 2.0 * (double)(s.x + s.y);");
+            E("            }");
+        }
+        E("        }");
+    }
+    // ---- table groups
+    for (uint32_t q = g0; q < g1; ++q) {
+        const GInfo &G = gi[q - g0];
+        if (G.mode != 0) continue;
+        const DGroup &dg = plan.groups[q];
+        // register-like bits: the pivot and L loop bits outside the index bits, preferably outside the flip mask
+        const uint32_t m = dg.m_loc, U = dg.uloc;
+        const int pivot = 31 - __builtin_clz(m);
+        uint8_t ex[8]; int ne = 0;
+        uint32_t exmask = 1u << pivot;
+        for (int pass2 = 0; pass2 < 2 && __builtin_popcount(exmask) < RS; ++pass2)
+            for (int b = k - 1; b >= 0 && __builtin_popcount(exmask) < RS; --b) {
+                if ((exmask | U) >> b & 1) continue;
+                if (pass2 == 0 && (m >> b & 1)) continue;
+                exmask |= 1u << b;
+            }
+        if (__builtin_popcount(exmask) < RS) { err = "jit: no room for loop bits"; return false; }
+        for (int b = 0; b < k; ++b) if (exmask >> b & 1) ex[ne++] = (uint8_t)b;
+        int tb[16];
+        choose_thread_bits_for(g, ex, RS, tb);
+        int pslot = 0;
+        for (int i = 0; i < RS; ++i) if (ex[i] == pivot) pslot = i;
+        uint32_t mreg = 0;                         // flip mask over the register-like slots
+        for (int i = 0; i < RS; ++i) if (m >> ex[i] & 1) mreg |= 1u << i;
+        const uint32_t mthr = m & ~exmask;         // flip-mask bits that are thread bits: the partner lives in another thread
+        uint32_t cr[32];
+        for (uint32_t r = 0; r < NR; ++r) {
+            uint32_t j = 0;
+            for (int b = 0; b < RS; ++b) if (r >> b & 1) j |= 1u << ex[b];
+            cr[r] = g.off(j);
+        }
+        E("        {   // ---- group %u (table over %d thread bits), flip mask local 0x%x", q - g0, (int)dg.ubits, m);
+        emit_deposit(E, "            ", "jt", tb, TBITS);
+        E("            const unsigned sb = OFF(jt);");
+        {   // table index: the bits of jt at the positions of U, packed
+            std::string ux = "            const unsigned u = 0u";
+            int o = 0;
+            for (int b = 0; b < k; ++b) if (U >> b & 1) {
+                char bb[64];
+                snprintf(bb, sizeof bb, " | (((jt >> %d) & 1u) << %d)", b, o);
+                ux += bb; ++o;
+            }
+            E("%s;", ux.c_str());
+        }
+        E("            const amp wv = ((const amp *)(smem + %u))[u];", G.tab_off);
+        E("            amp s1 = MK((real)0, (real)0), s2 = s1;");
+        const bool wide = (g.lv == 1 && ex[0] == 0 && mthr == 0);
+        if (mthr == 0) {   // partners in the same thread
+            bool vused[8] = {false};
+            for (uint32_t r = 0; r < NR; ++r) vused[(cr[r] & LOMASK) >> 4] = true;
+            for (int v = 0; v < 8; ++v) if (vused[v]) E("            const unsigned char *const pv%d = tile + (sb ^ %uu);", v, (uint32_t)v << 4);
+            E("            amp a[%u];", NR);
+            if (wide) {
+                for (uint32_t r = 0; r < NR; r += 2)
+                    E("            { const float4 v = *(const float4 *)(pv%u + %uu); a[%u] = MK(v.x, v.y); a[%u] = MK(v.z, v.w); }", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r, r + 1);
+            } else {
+                for (uint32_t r = 0; r < NR; ++r) E("            a[%u] = *(const amp *)(pv%u + %uu);", r, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK);
+            }
+            for (uint32_t r = 0; r < NR; ++r) if (!(r >> pslot & 1)) E("            pairs(s1, s2, a[%u], a[%u]);", r, r ^ mreg);
+        } else {
+            E("            const unsigned sbm = sb ^ %uu;", g.off(mthr));
+            bool vu[8] = {false}, vm[8] = {false};
+            for (uint32_t r = 0; r < NR; ++r) if (!(r >> pslot & 1)) { vu[(cr[r] & LOMASK) >> 4] = true; vm[(cr[r ^ mreg] & LOMASK) >> 4] = true; }
+            for (int v = 0; v < 8; ++v) if (vu[v]) E("            const unsigned char *const pv%d = tile + (sb ^ %uu);", v, (uint32_t)v << 4);
+            for (int v = 0; v < 8; ++v) if (vm[v]) E("            const unsigned char *const pm%d = tile + (sbm ^ %uu);", v, (uint32_t)v << 4);
+            for (uint32_t r = 0; r < NR; ++r) {
+                if (r >> pslot & 1) continue;
+                const uint32_t rb = r ^ mreg;
+                E("            pairs(s1, s2, *(const amp *)(pv%u + %uu), *(const amp *)(pm%u + %uu));", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, (cr[rb] & LOMASK) >> 4, cr[rb] & ~LOMASK);
+            }
+        }
+        // sum conj(b) a = (s1.x + s2.y) + i (s1.y - s2.x);  2 Re(W sum)
+        E("            acc += 2.0 * (double)(wv.x * (s1.x + s2.y) - wv.y * (s1.y - s2.x));");
+        E("        }");
+    }
+    // ---- direct groups (terms too wide for a table): W summed term by term per pair
+    for (uint32_t q = g0; q < g1; ++q) {
+        const GInfo &G = gi[q - g0];
+        if (G.mode != 2) continue;
+        const DGroup &dg = plan.groups[q];
+        const int pivot = 31 - __builtin_clz(dg.m_loc);
+        E("        {   // ---- group %u, direct", q - g0);
+        E("            real part = (real)0;");
+        E("            for (unsigned i = tid; i < %uu; i += %uu) {", 1u << (k - 1), NT);
+        E("                const unsigned j = ((i >> %d) << %d) | (i & %uu);", pivot, pivot + 1, (1u << pivot) - 1u);
+        E("                const amp a = *(const amp *)(tile + OFF(j)), bb = *(const amp *)(tile + OFF(j ^ %uu));", dg.m_loc);
+        E("                double wr = 0.0, wi = 0.0;");
+        E("                for (unsigned t = %uu; t < %uu; ++t) { const Term tm = terms[t]; const bool neg = (__popcll(xbase & tm.zout) + __popc(j & (unsigned)tm.pad)) & 1; wr += neg ? -tm.cr : tm.cr; wi += neg ? -tm.ci : tm.ci; }",
+          (uint32_t)data.terms.size(), (uint32_t)(data.terms.size() + (dg.term_end - dg.term_begin)));
+        E("                const real tr = bb.x * a.x + bb.y * a.y, ti = bb.x * a.y - bb.y * a.x;");
+        E("                part += (real)wr * tr - (real)wi * ti;");
+        E("            }");
+        E("            acc += 2.0 * (double)part;");
+        E("        }");
+        for (uint32_t t = dg.term_begin; t < dg.term_end; ++t) {   // direct terms: local z mask rides in `pad`
+            const DTerm &tm = plan.terms[t];
+            data.terms.push_back(JitExpectData::Term{tm.cr, tm.ci, tm.zout, (uint64_t)tm.zu});
+        }
+    }
+    // ---- deterministic block sum
+    E("        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);");
+    E("        if (lane == 0) red[warp] = acc;");
+    E("        __syncthreads();");
+    E("        if (tid == 0) { double s = 0.0; for (int i = 0; i < %u; ++i) s += red[i]; partial[(u64)b * slots_per_b + slot_off + tile_id] = s; }", NT / 32);
+    E("        __syncthreads();   // tile, tables and red are reused by the next work item");
+    E("    }");
+    E("}");
+    out.name = name;
+    out.source.swap(E.s);
+    out.smem_bytes = sm;
+    out.threads = NT;
+    out.tiles_log2 = n - k;
+    return true;
+}
+
+}  // namespace gv

@@ -173,4 +173,18 @@ int jit_launch(JitModule *m, const JitBlock &blk, void *states, uint64_t stride,
     return r == CUDA_SUCCESS ? 0 : (int)cudaErrorLaunchFailure;
 }
 
+int jit_launch_expect(JitModule *m, const JitBlock &blk, const void *states, uint64_t stride, const void *table, const void *wst,
+                      const void *pats, const void *terms, double *partial, uint32_t slots_per_b, uint32_t slot_off, int nb,
+                      int per_cta, void *stream)
+{
+    if (!m || !m->fn || nb <= 0 || per_cta < 1) return (int)cudaErrorInvalidValue;
+    const uint64_t total = (uint64_t)nb << blk.tiles_log2;
+    const uint64_t grid64 = (total + (uint64_t)per_cta - 1) / (uint64_t)per_cta;
+    if (grid64 > 0x7fffffffull) return (int)cudaErrorInvalidValue;
+    const unsigned grid = (unsigned)grid64;
+    void *args[] = {&states, &stride, &table, &wst, &pats, &terms, &partial, &slots_per_b, &slot_off, &nb, &per_cta};
+    const CUresult r = driver().LaunchKernel(m->fn, grid, 1, 1, blk.threads, 1, 1, blk.smem_bytes, (CUstream)stream, args, nullptr);
+    return r == CUDA_SUCCESS ? 0 : (int)cudaErrorLaunchFailure;
+}
+
 }  // namespace gv
