@@ -35,6 +35,8 @@ struct GInfo {
     uint32_t wst_off = 0;         // entry offset of the static table in the pass's global array
     bool dyn = false;
     uint32_t pat_begin = 0, pat_end = 0;
+    std::vector<double> wr, wi;   // static table (host copy)
+    uint32_t zmask = 0;           // index bits any term of the group looks at
 };
 
 }  // namespace
@@ -81,8 +83,10 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         G.mode = dg.rs ? 1 : (dg.direct ? 2 : 0);
         if (G.mode == 2) continue;
         G.E = 1u << dg.ubits;
-        G.tab_off = take(G.E * 16u > G.E * AB && G.mode == 1 ? G.E * 16u : G.E * AB);   // clusters: 16-byte entries
         G.dyn = dg.dyn_end > dg.term_begin;
+        // clusters: 16-byte entries, and only when a term depends on the tile (otherwise W is a literal in the code)
+        if (G.mode == 0) G.tab_off = take(G.E * AB);
+        else if (G.dyn) G.tab_off = take(G.E * 16u);
         G.scr_off = G.dyn ? (G.mode == 1 ? take(G.E * AB) : G.tab_off) : 0;
         G.wst_off = (uint32_t)(data.wst.size() / 2 - wst_base);
         for (uint32_t e = 0; e < G.E; ++e) {   // static part (terms with every Z / Y inside the tile)
@@ -93,7 +97,9 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 wr += par ? -tm.cr : tm.cr; wi += par ? -tm.ci : tm.ci;
             }
             data.wst.push_back(wr); data.wst.push_back(wi);
+            G.wr.push_back(wr); G.wi.push_back(wi);
         }
+        for (uint32_t t = dg.term_begin; t < dg.term_end; ++t) G.zmask |= plan.terms[t].zu & (G.E - 1u);
         if (G.dyn) {   // tile-dependent terms by index pattern, input order inside a pattern (deterministic sums)
             std::map<uint32_t, std::vector<uint32_t>> by_pat;
             for (uint32_t t = dg.term_begin; t < dg.dyn_end; ++t) by_pat[plan.terms[t].zu & (G.E - 1u)].push_back(t);
@@ -136,11 +142,55 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // a . (b.x (Wx,-Wy) + b.y (Wy,Wx)) accumulated component-wise
         E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const amp be = __ffma2_rn(MK(b.y, b.y), MK(t.z, t.w), __fmul2_rn(MK(b.x, b.x), MK(t.x, t.y))); acc = __ffma2_rn(a, be, acc); }");
         E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1 = __ffma2_rn(MK(b.x, b.x), a, s1); s2 = __ffma2_rn(MK(b.y, b.y), a, s2); }");
+        // W known when the kernel is generated (constant bank, read through the uniform path -- no shared-memory traffic):
+        // complex W three packed operations, real W two, imaginary W three scalar ones
+        E("#define PAIRC(acc, a, b, t) { const amp be = __ffma2_rn(MK((b).y, (b).y), MK((t).z, (t).w), __fmul2_rn(MK((b).x, (b).x), MK((t).x, (t).y))); acc = __ffma2_rn((a), be, acc); }");
+        E("#define PAIRR(acc, a, b, t) { acc = __ffma2_rn((a), __fmul2_rn((b), MK((t).x, (t).x)), acc); }");
+        E("#define PAIRI(acci, a, b, t) { acci = fmaf((t).z, fmaf(-(a).y, (b).x, (a).x * (b).y), acci); }");
     } else {
         E("typedef double2 tw4;");
         E("__device__ __forceinline__ tw4 twfmt(amp w) { return w; }");
         E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const double br = fma(t.y, b.y, t.x * b.x), bi = fma(-t.y, b.x, t.x * b.y); acc.x = fma(a.x, br, acc.x); acc.y = fma(a.y, bi, acc.y); }");
         E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1.x = fma(b.x, a.x, s1.x); s1.y = fma(b.x, a.y, s1.y); s2.x = fma(b.y, a.x, s2.x); s2.y = fma(b.y, a.y, s2.y); }");
+        E("#define PAIRC(acc, a, b, t) { const double br = fma((t).y, (b).y, (t).x * (b).x), bi = fma(-(t).y, (b).x, (t).x * (b).y); acc.x = fma((a).x, br, acc.x); acc.y = fma((a).y, bi, acc.y); }");
+        E("#define PAIRR(acc, a, b, t) { acc.x = fma((a).x * (t).x, (b).x, acc.x); acc.y = fma((a).y * (t).x, (b).y, acc.y); }");
+        E("#define PAIRI(acci, a, b, t) { acci = fma((t).y, fma(-(a).y, (b).x, (a).x * (b).y), acci); }");
+    }
+    // W of the cluster groups without tile-dependent terms: entries (Wx, -Wy, Wy, Wx) (complex128: (Wx, Wy)) in constant memory
+    std::vector<std::pair<double, double>> wconst;
+    std::map<std::pair<double, double>, uint32_t> wconst_ix;
+    auto const_index = [&](double wx, double wy) {
+        const std::pair<double, double> key(wx, wy);
+        auto it = wconst_ix.find(key);
+        if (it != wconst_ix.end()) return it->second;
+        const uint32_t ix = (uint32_t)wconst.size();
+        wconst.push_back(key); wconst_ix[key] = ix;
+        return ix;
+    };
+    for (uint32_t q = g0; q < g1; ++q) {
+        const GInfo &G = gi[q - g0];
+        if (G.mode != 1 || G.dyn) continue;
+        for (uint32_t e = 0; e < G.E; ++e) {
+            const double wx = prec == 0 ? (double)(float)G.wr[e] : G.wr[e], wy = prec == 0 ? (double)(float)G.wi[e] : G.wi[e];
+            if (wx != 0.0 || wy != 0.0) const_index(wx, wy);
+        }
+    }
+    if (!wconst.empty()) {
+        if (wconst.size() * 16 > 60000) { err = "jit: too many constant table entries"; return false; }
+        std::string t = std::string("__constant__ ") + (prec == 0 ? "tw4" : "double2") + " WC[" + std::to_string(wconst.size()) + "] = {";
+        auto lit = [&](double v) {   // a floating literal that reads back to exactly v
+            char b2[48];
+            snprintf(b2, sizeof b2, prec == 0 ? "%.9g" : "%.17g", v);
+            std::string x = b2;
+            if (x.find_first_of(".en") == std::string::npos) x += ".0";
+            return prec == 0 ? x + "f" : x;
+        };
+        for (auto &w : wconst) {
+            if (prec == 0) t += "{" + lit(w.first) + ", " + lit(-w.second) + ", " + lit(w.second) + ", " + lit(w.first) + "}, ";
+            else t += "{" + lit(w.first) + ", " + lit(w.second) + "}, ";
+        }
+        t += "};";
+        E("%s", t.c_str());
     }
     E("");
     E("extern \"C\" __global__ void __launch_bounds__(%u, 2) %s(const amp *states, u64 stride, const tabt *table, const amp *wst, const Pat *pats, const Term *terms,", NT, name);
@@ -154,9 +204,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     // static tables of the groups without tile-dependent terms: once per thread block
     for (uint32_t q = g0; q < g1; ++q) {
         const GInfo &G = gi[q - g0];
-        if (G.mode == 2 || G.dyn) continue;
-        if (G.mode == 1) E("    for (unsigned e = tid; e < %uu; e += %uu) ((tw4 *)(smem + %u))[e] = twfmt(wst[%u + e]);", G.E, NT, G.tab_off, G.wst_off);
-        else E("    for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = wst[%u + e];", G.E, NT, G.tab_off, G.wst_off);
+        if (G.mode != 0 || G.dyn) continue;
+        E("    for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = wst[%u + e];", G.E, NT, G.tab_off, G.wst_off);
     }
     E("    const unsigned ld_off = OFF(tid << %d);", g.lv);
     {
@@ -294,14 +343,28 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             const GInfo &G = gi[q - g0];
             const uint32_t mr = dg.m_r;
             int pv = 31 - __builtin_clz(mr);
-            E("            {   // group %u: flip mask over the slots %u", q - g0, mr);
-            E("                const tw4 *W = (const tw4 *)(smem + %u);", G.tab_off);
+            E("            {   // group %u: flip mask over the slots %u%s", q - g0, mr, G.dyn ? " (table refreshed per tile)" : " (W literal)");
             E("                amp s = MK((real)0, (real)0);");
-            for (uint32_t r = 0; r < NR; ++r) {
-                if (r >> pv & 1) continue;
-                E("                pairw(s, a[%u], a[%u], W[%u]);", r, r ^ mr, r);
+            if (G.dyn) {
+                E("                const tw4 *W = (const tw4 *)(smem + %u);", G.tab_off);
+                for (uint32_t r = 0; r < NR; ++r) {
+                    if (r >> pv & 1) continue;
+                    E("                pairw(s, a[%u], a[%u], W[%u]);", r, r ^ mr, r & G.zmask);   // only the index bits a term looks at: equal reads merge
+                }
+                E("                acc += 2.0 * (double)(s.x + s.y);");
+            } else {
+                E("                real si = (real)0;");
+                for (uint32_t r = 0; r < NR; ++r) {
+                    if (r >> pv & 1) continue;
+                    const double wx = prec == 0 ? (double)(float)G.wr[r] : G.wr[r], wy = prec == 0 ? (double)(float)G.wi[r] : G.wi[r];
+                    if (wx == 0.0 && wy == 0.0) continue;
+                    const uint32_t ix = const_index(wx, wy);
+                    if (wy == 0.0) E("                PAIRR(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
+                    else if (wx == 0.0) E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
+                    else E("                PAIRC(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
+                }
+                E("                acc += 2.0 * (double)(s.x + s.y + si);");
             }
-            E("                acc += 2.0 * (double)(s.x + s.y);");
             E("            }");
         }
         E("        }");

@@ -14,11 +14,18 @@ struct Emit {
     void operator()(const char *fmt, ...)
     {
         char buf[1024];
-        va_list ap;
+        va_list ap, ap2;
         va_start(ap, fmt);
-        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_copy(ap2, ap);
+        const int need = vsnprintf(buf, sizeof buf, fmt, ap);
         va_end(ap);
-        s += buf;
+        if (need >= (int)sizeof buf) {   // long lines (constant arrays)
+            std::string big((size_t)need + 1, ' ');
+            vsnprintf(&big[0], big.size(), fmt, ap2);
+            big.resize((size_t)need);
+            s += big;
+        } else s += buf;
+        va_end(ap2);
         s += '\n';
     }
 };
