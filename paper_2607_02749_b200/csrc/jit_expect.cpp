@@ -142,6 +142,9 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // a . (b.x (Wx,-Wy) + b.y (Wy,Wx)) accumulated component-wise
         E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const amp be = __ffma2_rn(MK(b.y, b.y), MK(t.z, t.w), __fmul2_rn(MK(b.x, b.x), MK(t.x, t.y))); acc = __ffma2_rn(a, be, acc); }");
         E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1 = __ffma2_rn(MK(b.x, b.x), a, s1); s2 = __ffma2_rn(MK(b.y, b.y), a, s2); }");
+        // conj(b) a = (b.x a.x + b.y a.y, b.x a.y - b.y a.x)
+        E("__device__ __forceinline__ amp cjmul(amp a, amp b) { const amp p = __fmul2_rn(MK(b.x, b.x), a), q = __fmul2_rn(MK(b.y, b.y), a); return MK(p.x + q.y, p.y - q.x); }");
+        E("__device__ __forceinline__ amp cadd(amp a, amp b) { return __fadd2_rn(a, b); }");
         // W known when the kernel is generated (constant bank, read through the uniform path -- no shared-memory traffic):
         // complex W three packed operations, real W two, imaginary W three scalar ones
         E("#define PAIRC(acc, a, b, t) { const amp be = __ffma2_rn(MK((b).y, (b).y), MK((t).z, (t).w), __fmul2_rn(MK((b).x, (b).x), MK((t).x, (t).y))); acc = __ffma2_rn((a), be, acc); }");
@@ -152,6 +155,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("__device__ __forceinline__ tw4 twfmt(amp w) { return w; }");
         E("__device__ __forceinline__ void pairw(amp &acc, amp a, amp b, tw4 t) { const double br = fma(t.y, b.y, t.x * b.x), bi = fma(-t.y, b.x, t.x * b.y); acc.x = fma(a.x, br, acc.x); acc.y = fma(a.y, bi, acc.y); }");
         E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1.x = fma(b.x, a.x, s1.x); s1.y = fma(b.x, a.y, s1.y); s2.x = fma(b.y, a.x, s2.x); s2.y = fma(b.y, a.y, s2.y); }");
+        E("__device__ __forceinline__ amp cjmul(amp a, amp b) { return MK(fma(b.y, a.y, b.x * a.x), fma(-b.y, a.x, b.x * a.y)); }");
+        E("__device__ __forceinline__ amp cadd(amp a, amp b) { return MK(a.x + b.x, a.y + b.y); }");
         E("#define PAIRC(acc, a, b, t) { const double br = fma((t).y, (b).y, (t).x * (b).x), bi = fma(-(t).y, (b).x, (t).x * (b).y); acc.x = fma((a).x, br, acc.x); acc.y = fma((a).y, bi, acc.y); }");
         E("#define PAIRR(acc, a, b, t) { acc.x = fma((a).x * (t).x, (b).x, acc.x); acc.y = fma((a).y * (t).x, (b).y, acc.y); }");
         E("#define PAIRI(acci, a, b, t) { acci = fma((t).y, fma(-(a).y, (b).x, (a).x * (b).y), acci); }");
@@ -369,24 +374,33 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         }
         E("        }");
     }
-    // ---- table groups
-    for (uint32_t q = g0; q < g1; ++q) {
-        const GInfo &G = gi[q - g0];
-        if (G.mode != 0) continue;
-        const DGroup &dg = plan.groups[q];
-        // register-like bits: the pivot and L loop bits outside the index bits, preferably outside the flip mask
-        const uint32_t m = dg.m_loc, U = dg.uloc;
+    // ---- table groups: all slices of one flip mask share the thread's pair products
+    // A flip mask whose terms look at more in-tile z bits than a table can index was cut into slices by the planner
+    // (Eq. 12: any partition of the terms).  The amplitudes are read from shared memory ONCE per mask: the thread keeps
+    // rho_i = conj(b_i) a_i of its 2^L pairs; a slice whose index bits avoid the loop bits multiplies its W with the sum of
+    // all rho_i, one that uses j loop bits with 2^j partial sums.
+    std::map<uint32_t, std::vector<uint32_t>> by_mask;
+    for (uint32_t q = g0; q < g1; ++q) if (gi[q - g0].mode == 0) by_mask[plan.groups[q].m_loc].push_back(q);
+    for (auto &mg : by_mask) {
+        const uint32_t m = mg.first;
         const int pivot = 31 - __builtin_clz(m);
-        uint8_t ex[8]; int ne = 0;
+        uint32_t Uall = 0;
+        for (uint32_t q : mg.second) Uall |= plan.groups[q].uloc;
+        // loop bits: outside every slice's index bits when possible, else the bits the fewest slices look at
         uint32_t exmask = 1u << pivot;
-        for (int pass2 = 0; pass2 < 2 && __builtin_popcount(exmask) < RS; ++pass2)
-            for (int b = k - 1; b >= 0 && __builtin_popcount(exmask) < RS; --b) {
-                if ((exmask | U) >> b & 1) continue;
-                if (pass2 == 0 && (m >> b & 1)) continue;
-                exmask |= 1u << b;
+        while (__builtin_popcount(exmask) < RS) {
+            int best = -1, best_cost = 1 << 30;
+            for (int bb = k - 1; bb >= 0; --bb) {
+                if (exmask >> bb & 1) continue;
+                int cost = 0;
+                for (uint32_t q : mg.second) cost += (int)(plan.groups[q].uloc >> bb & 1) * 4;
+                cost += (int)(m >> bb & 1);            // prefer bits outside the flip mask
+                if (cost < best_cost) { best_cost = cost; best = bb; }
             }
-        if (__builtin_popcount(exmask) < RS) { err = "jit: no room for loop bits"; return false; }
-        for (int b = 0; b < k; ++b) if (exmask >> b & 1) ex[ne++] = (uint8_t)b;
+            exmask |= 1u << best;
+        }
+        uint8_t ex[8]; int ne = 0;
+        for (int bb = 0; bb < k; ++bb) if (exmask >> bb & 1) ex[ne++] = (uint8_t)bb;
         int tb[16];
         choose_thread_bits_for(g, ex, RS, tb);
         int pslot = 0;
@@ -394,27 +408,19 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         uint32_t mreg = 0;                         // flip mask over the register-like slots
         for (int i = 0; i < RS; ++i) if (m >> ex[i] & 1) mreg |= 1u << i;
         const uint32_t mthr = m & ~exmask;         // flip-mask bits that are thread bits: the partner lives in another thread
-        uint32_t cr[32];
+        uint32_t cr[32], jr[32];
         for (uint32_t r = 0; r < NR; ++r) {
             uint32_t j = 0;
-            for (int b = 0; b < RS; ++b) if (r >> b & 1) j |= 1u << ex[b];
-            cr[r] = g.off(j);
+            for (int bb = 0; bb < RS; ++bb) if (r >> bb & 1) j |= 1u << ex[bb];
+            jr[r] = j; cr[r] = g.off(j);
         }
-        E("        {   // ---- group %u (table over %d thread bits), flip mask local 0x%x", q - g0, (int)dg.ubits, m);
+        std::vector<uint32_t> pairs_r;             // register indices with the pivot slot clear
+        for (uint32_t r = 0; r < NR; ++r) if (!(r >> pslot & 1)) pairs_r.push_back(r);
+        const int np = (int)pairs_r.size();
+        E("        {   // ---- flip mask local 0x%x: %zu table slice(s)", m, mg.second.size());
         emit_deposit(E, "            ", "jt", tb, TBITS);
         E("            const unsigned sb = OFF(jt);");
-        {   // table index: the bits of jt at the positions of U, packed
-            std::string ux = "            const unsigned u = 0u";
-            int o = 0;
-            for (int b = 0; b < k; ++b) if (U >> b & 1) {
-                char bb[64];
-                snprintf(bb, sizeof bb, " | (((jt >> %d) & 1u) << %d)", b, o);
-                ux += bb; ++o;
-            }
-            E("%s;", ux.c_str());
-        }
-        E("            const amp wv = ((const amp *)(smem + %u))[u];", G.tab_off);
-        E("            amp s1 = MK((real)0, (real)0), s2 = s1;");
+        E("            amp rho[%d];", np);
         const bool wide = (g.lv == 1 && ex[0] == 0 && mthr == 0);
         if (mthr == 0) {   // partners in the same thread
             bool vused[8] = {false};
@@ -427,21 +433,45 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             } else {
                 for (uint32_t r = 0; r < NR; ++r) E("            a[%u] = *(const amp *)(pv%u + %uu);", r, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK);
             }
-            for (uint32_t r = 0; r < NR; ++r) if (!(r >> pslot & 1)) E("            pairs(s1, s2, a[%u], a[%u]);", r, r ^ mreg);
+            for (int i = 0; i < np; ++i) E("            rho[%d] = cjmul(a[%u], a[%u]);", i, pairs_r[i], pairs_r[i] ^ mreg);
         } else {
             E("            const unsigned sbm = sb ^ %uu;", g.off(mthr));
             bool vu[8] = {false}, vm[8] = {false};
-            for (uint32_t r = 0; r < NR; ++r) if (!(r >> pslot & 1)) { vu[(cr[r] & LOMASK) >> 4] = true; vm[(cr[r ^ mreg] & LOMASK) >> 4] = true; }
+            for (uint32_t r : pairs_r) { vu[(cr[r] & LOMASK) >> 4] = true; vm[(cr[r ^ mreg] & LOMASK) >> 4] = true; }
             for (int v = 0; v < 8; ++v) if (vu[v]) E("            const unsigned char *const pv%d = tile + (sb ^ %uu);", v, (uint32_t)v << 4);
             for (int v = 0; v < 8; ++v) if (vm[v]) E("            const unsigned char *const pm%d = tile + (sbm ^ %uu);", v, (uint32_t)v << 4);
-            for (uint32_t r = 0; r < NR; ++r) {
-                if (r >> pslot & 1) continue;
-                const uint32_t rb = r ^ mreg;
-                E("            pairs(s1, s2, *(const amp *)(pv%u + %uu), *(const amp *)(pm%u + %uu));", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, (cr[rb] & LOMASK) >> 4, cr[rb] & ~LOMASK);
+            for (int i = 0; i < np; ++i) {
+                const uint32_t r = pairs_r[i], rb = r ^ mreg;
+                E("            rho[%d] = cjmul(*(const amp *)(pv%u + %uu), *(const amp *)(pm%u + %uu));", i, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, (cr[rb] & LOMASK) >> 4, cr[rb] & ~LOMASK);
             }
         }
-        // sum conj(b) a = (s1.x + s2.y) + i (s1.y - s2.x);  2 Re(W sum)
-        E("            acc += 2.0 * (double)(wv.x * (s1.x + s2.y) - wv.y * (s1.y - s2.x));");
+        E("            real accm = (real)0;");
+        for (uint32_t q : mg.second) {
+            const DGroup &dg = plan.groups[q];
+            const GInfo &G = gi[q - g0];
+            const uint32_t U = dg.uloc;
+            auto compress_u = [&](uint32_t j) { uint32_t o = 0; int pos = 0; for (int bb = 0; bb < k; ++bb) if (U >> bb & 1) { if (j >> bb & 1) o |= 1u << pos; ++pos; } return o; };
+            {   // table index of the thread: the bits of jt at the positions of U, packed
+                std::string ux = "            { const unsigned u = 0u";
+                int o = 0;
+                for (int bb = 0; bb < k; ++bb) if (U >> bb & 1) {
+                    if (!(exmask >> bb & 1)) { char b2[64]; snprintf(b2, sizeof b2, " | (((jt >> %d) & 1u) << %d)", bb, o); ux += b2; }
+                    ++o;
+                }
+                E("%s;   // slice %u", ux.c_str(), q - g0);
+            }
+            E("              const amp *tabp = (const amp *)(smem + %u) + u;", G.tab_off);
+            std::map<uint32_t, std::vector<int>> classes;   // index contribution of the loop bits -> pairs
+            for (int i = 0; i < np; ++i) classes[compress_u(jr[pairs_r[i]])].push_back(i);
+            for (auto &cl : classes) {
+                std::string sum = "rho[" + std::to_string(cl.second[0]) + "]";
+                E("              { amp t = %s;", sum.c_str());
+                for (size_t z = 1; z < cl.second.size(); ++z) E("                t = cadd(t, rho[%d]);", cl.second[z]);
+                E("                const amp wv = tabp[%u]; accm = %s(wv.x, t.x, %s(-wv.y, t.y, accm)); }", cl.first, prec == 0 ? "fmaf" : "fma", prec == 0 ? "fmaf" : "fma");
+            }
+            E("            }");
+        }
+        E("            acc += 2.0 * (double)accm;");
         E("        }");
     }
     // ---- direct groups (terms too wide for a table): W summed term by term per pair
