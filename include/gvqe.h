@@ -99,6 +99,11 @@ gvqe_status gvqe_create_ops_opt(int n_qubits, const gvqe_op *ops, int n_ops, int
  * buf (NUL-terminated, truncated to cap); returns the full length needed, 0 when there is no such kernel.
  * *smem_bytes (optional): its dynamic shared memory.  Host only (no GPU, no compiler). */
 size_t gvqe_kernel_source(const gvqe_ctx *ctx, int block, char *buf, size_t cap, int32_t *smem_bytes);
+/* Facts about specialised kernel number `block` (numbering as gvqe_kernel_source): out[0] = 0 gate block / 1 expectation
+ * pass, out[1] = dynamic shared memory in bytes, out[2] = floating-point lane operations per amplitude and launch the
+ * schedule needs (2 per rotation in tangent form, 4 per complex phase factor, 6 / 4 / 3 per amplitude pair of a
+ * complex / real / imaginary W): the numerator of the ALU roofline, out[3] = 0.  GVQE_ERR_INVALID_ARG if no such kernel. */
+gvqe_status gvqe_kernel_info(const gvqe_ctx *ctx, int block, double *out);
 /* The arrays the specialised expectation kernels read from global memory, as host images (introspection for tests):
  * which = 0: static W tables (double re, im per entry), 1: tile-dependent index patterns (4 x uint32: shared-memory byte
  * offset, first term, last term + 1, 0), 2: terms (double re, im of c_k i^{nY}; uint64 z bits outside the tile; uint64
@@ -194,6 +199,10 @@ uint64_t gvqe_launch_count(const gvqe_ctx *ctx);
  *   [7] chunks recorded. */
 gvqe_status gvqe_profile_enable(gvqe_ctx *ctx, int on);
 gvqe_status gvqe_profile_read(gvqe_ctx *ctx, double *out);
+/* Per-launch device times of the recorded chunks, in execution order: [product-state kernel if the schedule has one],
+ * fused gate blocks, expectation passes.  mean_ms / min_ms / max_ms: HOST, cap doubles each (any may be NULL); returns
+ * the number of launches per chunk (-1 on a NULL context).  The spread between chunks is what min / max show. */
+int gvqe_profile_read_launches(gvqe_ctx *ctx, double *mean_ms, double *min_ms, double *max_ms, int cap);
 
 /* ---- Host-side Graph-VQE driver (north_star item 3: partitioning and the optimiser loop stay on the host as plain
  * C++).  These calls do no GPU work of their own; gvqe_graph_vqe_minimize obtains every energy and gradient through

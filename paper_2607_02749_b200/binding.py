@@ -19,11 +19,11 @@ GVQE_C64, GVQE_C128 = 0, 1
 STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "GVQE_ERR_WORKSPACE",
                 "GVQE_ERR_UNSUPPORTED", "GVQE_ERR_CUDA"]
 
-EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_kernel_arrays", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
+EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_kernel_info", "gvqe_kernel_arrays", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
-           "gvqe_profile_enable", "gvqe_profile_read", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
+           "gvqe_profile_enable", "gvqe_profile_read", "gvqe_profile_read_launches", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
            "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
 
@@ -78,6 +78,7 @@ def load():
     L.gvqe_kernel_source.argtypes = [vp, i32, C.c_char_p, sz, vp]
     L.gvqe_kernel_source.restype = sz
     L.gvqe_compile_kernels.argtypes = [vp, vp]
+    L.gvqe_kernel_info.argtypes = [vp, i32, vp]
     L.gvqe_kernel_arrays.argtypes = [vp, i32, vp, sz]
     L.gvqe_kernel_arrays.restype = sz
     L.gvqe_num_params.argtypes = [vp]
@@ -103,6 +104,7 @@ def load():
     L.gvqe_launch_count.restype = u64
     L.gvqe_profile_enable.argtypes = [vp, i32]
     L.gvqe_profile_read.argtypes = [vp, vp]
+    L.gvqe_profile_read_launches.argtypes = [vp, vp, vp, vp, i32]
     L.gvqe_interaction_graph.argtypes = [vp, vp]
     L.gvqe_modularity.argtypes = [i32, vp, vp, C.c_double, vp]
     L.gvqe_louvain.argtypes = [i32, vp, C.c_double, vp, vp, vp]
@@ -284,6 +286,13 @@ class Gvqe:
         self._L.gvqe_kernel_source(self._h, int(block), buf, need + 1, C.addressof(sm))
         return buf.value.decode(), int(sm.value)
 
+    def kernel_info(self, block: int):
+        """dict(kind='gate'|'expect', smem_bytes, fp_ops_per_amp) of specialised kernel `block`, or None."""
+        o = np.zeros(4, dtype=np.float64)
+        if self._L.gvqe_kernel_info(self._h, int(block), o.ctypes.data) != GVQE_OK:
+            return None
+        return dict(kind="gate" if o[0] == 0 else "expect", smem_bytes=int(o[1]), fp_ops_per_amp=float(o[2]))
+
     def kernel_arrays(self, which: int) -> np.ndarray:
         """Host image (uint8 array) of what the specialised expectation kernels read from global memory (gvqe_kernel_arrays)."""
         need = self._L.gvqe_kernel_arrays(self._h, int(which), None, 0)
@@ -311,6 +320,13 @@ class Gvqe:
         self._check(self._L.gvqe_profile_read(self._h, o.ctypes.data))
         keys = ["gate_ms", "gate_launches", "gate_bytes", "expect_ms", "expect_launches", "expect_bytes", "other_ms", "chunks"]
         return dict(zip(keys, o.tolist()))
+
+    def profile_read_launches(self):
+        """(mean_ms, min_ms, max_ms) arrays, one entry per launch of a chunk in execution order (see gvqe.h)."""
+        m = self._L.gvqe_profile_read_launches(self._h, None, None, None, 0)
+        a, b, c = (np.zeros(max(m, 1), dtype=np.float64) for _ in range(3))
+        self._L.gvqe_profile_read_launches(self._h, a.ctypes.data, b.ctypes.data, c.ctypes.data, m)
+        return a[:m], b[:m], c[:m]
 
     def launch_count(self) -> int:
         return int(self._L.gvqe_launch_count(self._h))

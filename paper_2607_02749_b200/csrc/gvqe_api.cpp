@@ -72,9 +72,14 @@ struct gvqe_ctx {
     JitExpectData jitx;
     std::vector<float> jitx_wst_f;
     void *d_jwst = nullptr; void *d_jpats = nullptr; void *d_jterms = nullptr;
+    int32_t *d_sweep_idx = nullptr; double *d_sweep_E = nullptr;
     bool profiling = false;
     std::vector<cudaEvent_t> ev;
     double prof_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    std::vector<cudaEvent_t> ev_fine;          // profiling: one event after every gate launch / expectation pass of a chunk
+    std::vector<double> prof_launch_ms;        // summed per launch index (prefix kernel, gate blocks, passes)
+    std::vector<double> prof_launch_min, prof_launch_max;
+    double prof_fine_chunks = 0;
     std::string err;
     size_t amp_bytes() const { return prec == GVQE_C64 ? 8 : 16; }
     size_t tab_bytes() const { return prec == GVQE_C64 ? 4 : 8; }
@@ -182,6 +187,15 @@ size_t gvqe_kernel_source(const gvqe_ctx *c, int block, char *buf, size_t cap, i
     if (smem_bytes) *smem_bytes = (int32_t)jb.smem_bytes;
     if (buf && cap) { const size_t m = s.size() < cap - 1 ? s.size() : cap - 1; memcpy(buf, s.data(), m); buf[m] = 0; }
     return s.size() + 1;
+}
+
+gvqe_status gvqe_kernel_info(const gvqe_ctx *c, int block, double *out)
+{
+    if (!c || !out || block < 0 || (size_t)block >= c->jit_blocks.size() + c->jitx_blocks.size()) return GVQE_ERR_INVALID_ARG;
+    const bool gate = (size_t)block < c->jit_blocks.size();
+    const JitBlock &jb = gate ? c->jit_blocks[(size_t)block] : c->jitx_blocks[(size_t)block - c->jit_blocks.size()];
+    out[0] = gate ? 0.0 : 1.0; out[1] = (double)jb.smem_bytes; out[2] = jb.fma_ops_per_amp; out[3] = 0.0;
+    return GVQE_OK;
 }
 
 size_t gvqe_kernel_arrays(const gvqe_ctx *c, int which, void *buf, size_t cap)
@@ -387,7 +401,7 @@ struct Carve {
 };
 
 struct Layout {
-    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, jwst, jpats, jterms, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
+    size_t blocks, stages, ops, segs, trzs, tczs, csidx, ryl, cxs, slut, jwst, jpats, jterms, sweep_idx, sweep_E, px_begin, px_kind, px_param, px_t, px_c, passes, groups, terms, wstat, gtabs, rss, dz, dc, readout, smass, su, sx, table, fixed_end;
     size_t per_state;   // state + cs row + params row + partial slots + E
     size_t state_b, cs_b, ry_b, params_b, partial_b;
 };
@@ -410,6 +424,8 @@ Layout layout_of(const gvqe_ctx *c)
     L.jwst = cv.take(c->jitx.wst.size() / 2 * c->amp_bytes());
     L.jpats = cv.take(c->jitx.pats.size() * sizeof(JitExpectData::Pat));
     L.jterms = cv.take(c->jitx.terms.size() * sizeof(JitExpectData::Term));
+    L.sweep_idx = cv.take((size_t)SWEEP_MAX_ROWS * 4);
+    L.sweep_E = cv.take((size_t)(SWEEP_MAX_ROWS + 1) * 8);
     L.px_begin = cv.take(c->px.rot_begin.size() * 4); L.px_kind = cv.take(c->px.rot_kind.size());
     L.px_param = cv.take(c->px.rot_param.size() * 4); L.px_t = cv.take(c->px.cx_t.size()); L.px_c = cv.take(c->px.cx_c.size());
     L.passes = cv.take(c->plan.passes.size() * sizeof(DPass));
@@ -510,6 +526,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->gl.ryl = (const int16_t *)(w + L.ryl); c->gl.cxs = (const DCx *)(w + L.cxs);
     c->gl.slut = (const uint32_t *)(w + L.slut);
     c->d_jwst = w + L.jwst; c->d_jpats = w + L.jpats; c->d_jterms = w + L.jterms;
+    c->d_sweep_idx = (int32_t *)(w + L.sweep_idx); c->d_sweep_E = (double *)(w + L.sweep_E);
     c->pxd.rot_begin = (const int32_t *)(w + L.px_begin); c->pxd.rot_kind = (const uint8_t *)(w + L.px_kind);
     c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
     c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
@@ -563,13 +580,15 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
 // One chunk of `nb` statevectors: parameters are already on the device (nb x P doubles).
 }  // namespace
 extern "C" gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out);
+extern "C" int gvqe_profile_read_launches(gvqe_ctx *c, double *mean_ms, double *min_ms, double *max_ms, int cap);
 namespace {
 // Fused block j over nb statevectors starting at `states` (their (cos,sin) / tangent rows at cs / ry).
-int gate_block(gvqe_ctx *c, size_t j, void *states, uint64_t stride, const void *cs, const void *ry, int nb, cudaStream_t st)
+int gate_block(gvqe_ctx *c, size_t j, void *states, uint64_t stride, const void *cs, const void *ry, int nb, cudaStream_t st,
+               const void *src = nullptr, uint64_t src_stride = 0)
 {
     if (c->jit_state == 1) {
         ++c->launches;
-        return jit_launch(c->jit_mods[j], c->jit_blocks[j], states, stride, ry, cs, nb, c->P, c->jit_per_cta, st);
+        return jit_launch(c->jit_mods[j], c->jit_blocks[j], states, stride, ry, cs, nb, c->P, c->jit_per_cta, st, src, src_stride);
     }
     return launch_gate_block(c->prec, c->R, c->gl, c->dev.blocks[j], c->dev.blocks[j].k, c->dev.blocks[j].smem_prog_bytes, c->n_store,
                              states, stride, cs, c->P, nb, st, &c->launches);
@@ -598,6 +617,7 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
         if (c->ev.size() >= 4096) {   // fold what has been recorded so far
             double tmp[8];
             gvqe_profile_read(c, tmp);
+            gvqe_profile_read_launches(c, nullptr, nullptr, nullptr, 0);
         }
         for (int i = 0; i < 4; ++i) {
             if (cudaEventCreate(&e4[i]) != cudaSuccess) return cuda_fail(c, (int)cudaGetLastError(), "event create");
@@ -607,19 +627,30 @@ gvqe_status run_chunk(gvqe_ctx *c, const double *params_dev, int nb, double *E_d
     int ke = launch_expand_params(c->prec, params_dev, c->d_cs, c->jit_state == 1 ? c->d_ry : nullptr, (uint64_t)nb * c->P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->profiling) cudaEventRecord(e4[0], st);
+    auto mark = [&]() {   // fine-grained profile: an event after every launch of the chunk
+        if (!c->profiling) return;
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        c->ev_fine.push_back(e);
+        cudaEventRecord(e, st);
+    };
+    mark();
     if (c->px.n_ops > 0) {
         ke = launch_init_product(c->prec, c->pxd, c->d_states, stride, c->d_cs, c->P, nb, st, &c->launches);
         if (ke) return cuda_fail(c, ke, "product-state init");
+        mark();
     }
     for (size_t bi = 0; bi < c->dev.blocks.size(); ++bi) {
         ke = gate_block(c, bi, c->d_states, stride, c->d_cs, c->d_ry, nb, st);
         if (ke) return cuda_fail(c, ke, "gate block");
+        mark();
     }
     if (c->profiling) cudaEventRecord(e4[1], st);
     const uint32_t tiles = 1u << (c->n_store - c->plan.k);
     for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
         ke = expect_pass(c, pi, c->d_states, stride, c->d_partial, (uint32_t)pi * tiles, nb, st);
         if (ke) return cuda_fail(c, ke, "expectation pass");
+        mark();
     }
     if (c->profiling) cudaEventRecord(e4[2], st);
     ke = launch_reduce(c->d_partial, c->slots_per_b, E_dev, nb, st, &c->launches);
@@ -751,18 +782,37 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
         }
         return GVQE_OK;
     };
-    auto expect = [&](int slot, int nb) -> gvqe_status {
+    auto expect = [&](int slot, int nb, double *E_dev) -> gvqe_status {
         double *partial = c->d_partial + (size_t)slot * c->slots_per_b;
         for (size_t pi = 0; pi < c->plan.passes.size(); ++pi) {
             const int ke = expect_pass(c, pi, state_of(slot), stride, partial, (uint32_t)pi * tiles, nb, st);
             if (ke) return cuda_fail(c, ke, "expectation pass");
         }
-        const int ke = launch_reduce(partial, c->slots_per_b, c->d_E + slot, nb, st, &c->launches);
+        const int ke = launch_reduce(partial, c->slots_per_b, E_dev, nb, st, &c->launches);
         return ke ? cuda_fail(c, ke, "reduce") : GVQE_OK;
     };
-    // base row: parameters and (cos, sin) in slot 0
+    // work items in processing order: boundary after boundary, per parameter the + and the - row
+    std::vector<std::pair<int, int>> work;              // (entry of idx, 0 = plus / 1 = minus)
+    std::vector<size_t> group_begin((size_t)NB + 2, 0);
+    for (int g = 0; g <= NB; ++g) {
+        group_begin[(size_t)g] = work.size();
+        for (int a : group[(size_t)g]) { work.push_back({a, 0}); work.push_back({a, 1}); }
+    }
+    group_begin[(size_t)NB + 1] = work.size();
+    // With the specialised kernels the whole sweep is enqueued without a host round trip: the shift codes go up once, the
+    // rows are formed on the device, the first block of a suffix READS the base state and writes the row's own buffer
+    // (no copy), the energies stay on the device until the end.  The generic kernels keep the chunk-by-chunk form.
+    const bool staged = use_ry && work.size() <= SWEEP_MAX_ROWS;
+    std::vector<int32_t> codes;
+    std::vector<double> Eall(work.size() + 1);
     cudaError_t e = cudaMemcpyAsync(c->d_params, params, (size_t)P * 8, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
+    if (staged && !work.empty()) {
+        codes.resize(work.size());
+        for (size_t i = 0; i < work.size(); ++i) codes[i] = (int32_t)(idx[(size_t)work[i].first] * 2 + work[i].second);
+        e = cudaMemcpyAsync(c->d_sweep_idx, codes.data(), codes.size() * 4, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "sweep codes H2D");
+    }
     int ke = launch_expand_params(c->prec, c->d_params, c->d_cs, use_ry ? c->d_ry : nullptr, (uint64_t)P, st, &c->launches);
     if (ke) return cuda_fail(c, ke, "expand_params");
     if (c->px.n_ops > 0 && (ke = launch_init_product(c->prec, c->pxd, c->d_states, stride, c->d_cs, P, 1, st, &c->launches)))
@@ -770,43 +820,64 @@ static gvqe_status grad_shared_prefix(gvqe_ctx *c, const double *params, const s
     std::vector<double> rows((size_t)(F - 1) * P);
     for (int g = 0; g <= NB; ++g) {
         const int j0 = g - 1;   // -1: from the product-state kernel
-        std::vector<std::pair<int, int>> work;   // (entry of idx, 0 = plus / 1 = minus)
-        for (int a : group[g]) { work.push_back({a, 0}); work.push_back({a, 1}); }
-        for (size_t w0 = 0; w0 < work.size(); w0 += (size_t)(F - 1)) {
-            const int nb = (int)std::min(work.size() - w0, (size_t)(F - 1));
-            for (int r = 0; r < nb; ++r) {
-                for (int q = 0; q < P; ++q) rows[(size_t)r * P + q] = params[q];
-                rows[(size_t)r * P + idx[work[w0 + r].first]] += work[w0 + r].second ? -half_pi : half_pi;
+        for (size_t w0 = group_begin[(size_t)g]; w0 < group_begin[(size_t)g + 1]; w0 += (size_t)(F - 1)) {
+            const int nb = (int)std::min(group_begin[(size_t)g + 1] - w0, (size_t)(F - 1));
+            if (staged) {
+                if ((ke = launch_shift_rows(c->d_params, c->d_sweep_idx + w0, c->d_params + P, P, nb, st, &c->launches)))
+                    return cuda_fail(c, ke, "shift rows");
+            } else {
+                for (int r = 0; r < nb; ++r) {
+                    for (int q = 0; q < P; ++q) rows[(size_t)r * P + q] = params[q];
+                    rows[(size_t)r * P + idx[(size_t)work[w0 + r].first]] += work[w0 + r].second ? -half_pi : half_pi;
+                }
+                e = cudaMemcpyAsync(c->d_params + P, rows.data(), (size_t)nb * P * 8, cudaMemcpyHostToDevice, st);
+                if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
             }
-            e = cudaMemcpyAsync(c->d_params + P, rows.data(), (size_t)nb * P * 8, cudaMemcpyHostToDevice, st);
-            if (e != cudaSuccess) return cuda_fail(c, e, "params H2D");
             if ((ke = launch_expand_params(c->prec, c->d_params + P, cs_of(1), use_ry ? ry_of(1) : nullptr, (uint64_t)nb * P, st, &c->launches)))
                 return cuda_fail(c, ke, "expand_params");
+            int j_first = j0 < 0 ? 0 : j0;
             if (j0 < 0) {
                 if ((ke = launch_init_product(c->prec, c->pxd, state_of(1), stride, cs_of(1), P, nb, st, &c->launches)))
                     return cuda_fail(c, ke, "product-state init");
             } else if (!(j0 == 0 && c->dev.blocks[0].source_zero)) {
-                for (int r = 0; r < nb; ++r) {
-                    e = cudaMemcpyAsync(state_of(1 + r), state_of(0), S_bytes, cudaMemcpyDeviceToDevice, st);
-                    if (e != cudaSuccess) return cuda_fail(c, e, "state copy");
+                if (use_ry) {   // block j0 out of place: reads the base state, writes the rows' buffers
+                    if ((ke = gate_block(c, (size_t)j0, state_of(1), stride, cs_of(1), ry_of(1), nb, st, state_of(0), 0)))
+                        return cuda_fail(c, ke, "gate block");
+                    j_first = j0 + 1;
+                } else {
+                    for (int r = 0; r < nb; ++r) {
+                        e = cudaMemcpyAsync(state_of(1 + r), state_of(0), S_bytes, cudaMemcpyDeviceToDevice, st);
+                        if (e != cudaSuccess) return cuda_fail(c, e, "state copy");
+                    }
                 }
             }
-            if ((s = blocks_from(j0 < 0 ? 0 : j0, 1, nb)) != GVQE_OK || (s = expect(1, nb)) != GVQE_OK) return s;
-            std::vector<double> Et((size_t)nb);
-            e = cudaMemcpyAsync(Et.data(), c->d_E + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, st);
-            if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // rows / Et are reused by the next chunk
-            if (e != cudaSuccess) return cuda_fail(c, e, "E D2H");
-            for (int r = 0; r < nb; ++r) E_pm[2 * work[w0 + r].first + work[w0 + r].second] = Et[r];
+            if ((s = blocks_from(j_first, 1, nb)) != GVQE_OK) return s;
+            if (staged) {
+                if ((s = expect(1, nb, c->d_sweep_E + w0)) != GVQE_OK) return s;
+            } else {
+                if ((s = expect(1, nb, c->d_E + 1)) != GVQE_OK) return s;
+                e = cudaMemcpyAsync(Eall.data() + w0, c->d_E + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, st);
+                if (e == cudaSuccess) e = cudaStreamSynchronize(st);   // rows / d_E are reused by the next chunk
+                if (e != cudaSuccess) return cuda_fail(c, e, "E D2H");
+            }
         }
         if (j0 >= 0) {   // the base state advances by block j0
             ke = gate_block(c, (size_t)j0, state_of(0), stride, cs_of(0), ry_of(0), 1, st);
             if (ke) return cuda_fail(c, ke, "gate block");
         }
     }
-    if ((s = expect(0, 1)) != GVQE_OK) return s;
-    e = cudaMemcpyAsync(E0, c->d_E, 8, cudaMemcpyDeviceToHost, st);
+    if (staged) {
+        if ((s = expect(0, 1, c->d_sweep_E + work.size())) != GVQE_OK) return s;
+        e = cudaMemcpyAsync(Eall.data(), c->d_sweep_E, (work.size() + 1) * 8, cudaMemcpyDeviceToHost, st);
+    } else {
+        if ((s = expect(0, 1, c->d_E)) != GVQE_OK) return s;
+        e = cudaMemcpyAsync(Eall.data() + work.size(), c->d_E, 8, cudaMemcpyDeviceToHost, st);
+    }
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    return e == cudaSuccess ? GVQE_OK : cuda_fail(c, e, "E D2H");
+    if (e != cudaSuccess) return cuda_fail(c, e, "E D2H");
+    for (size_t i = 0; i < work.size(); ++i) E_pm[2 * (size_t)work[i].first + (size_t)work[i].second] = Eall[i];
+    *E0 = Eall[work.size()];
+    return GVQE_OK;
 }
 
 gvqe_status gvqe_param_shift_grad(gvqe_ctx *c, const double *params, const uint8_t *mask, double *dE, double *E0, void *stream)
@@ -968,10 +1039,48 @@ gvqe_status gvqe_profile_enable(gvqe_ctx *c, int on)
     if (on) {
         for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
         c->ev.clear();
+        for (cudaEvent_t e : c->ev_fine) cudaEventDestroy(e);
+        c->ev_fine.clear(); c->prof_launch_ms.clear(); c->prof_fine_chunks = 0;
         for (double &v : c->prof_acc) v = 0.0;
     }
     c->profiling = on != 0;
     return GVQE_OK;
+}
+
+// folds the fine-grained events (1 + launches per chunk) into per-launch sums
+static void fold_fine(gvqe_ctx *c)
+{
+    const size_t per = 1 + (c->px.n_ops > 0 ? 1 : 0) + c->dev.blocks.size() + c->plan.passes.size();
+    if (c->prof_launch_ms.size() != per - 1) {
+        c->prof_launch_ms.assign(per - 1, 0.0); c->prof_launch_min.assign(per - 1, 1e300); c->prof_launch_max.assign(per - 1, 0.0);
+        c->prof_fine_chunks = 0;
+    }
+    for (size_t i = 0; i + per <= c->ev_fine.size(); i += per) {
+        if (cudaEventSynchronize(c->ev_fine[i + per - 1]) != cudaSuccess) break;
+        for (size_t j = 0; j + 1 < per; ++j) {
+            float ms = 0;
+            cudaEventElapsedTime(&ms, c->ev_fine[i + j], c->ev_fine[i + j + 1]);
+            c->prof_launch_ms[j] += ms;
+            if (ms < c->prof_launch_min[j]) c->prof_launch_min[j] = ms;
+            if (ms > c->prof_launch_max[j]) c->prof_launch_max[j] = ms;
+        }
+        c->prof_fine_chunks += 1;
+    }
+    for (cudaEvent_t e : c->ev_fine) cudaEventDestroy(e);
+    c->ev_fine.clear();
+}
+
+int gvqe_profile_read_launches(gvqe_ctx *c, double *mean_ms, double *min_ms, double *max_ms, int cap)
+{
+    if (!c) return -1;
+    fold_fine(c);
+    const int m = (int)c->prof_launch_ms.size();
+    for (int i = 0; i < m && i < cap; ++i) {
+        if (mean_ms) mean_ms[i] = c->prof_fine_chunks > 0 ? c->prof_launch_ms[(size_t)i] / c->prof_fine_chunks : 0.0;
+        if (min_ms) min_ms[i] = c->prof_fine_chunks > 0 ? c->prof_launch_min[(size_t)i] : 0.0;
+        if (max_ms) max_ms[i] = c->prof_launch_max[(size_t)i];
+    }
+    return m;
 }
 
 gvqe_status gvqe_profile_read(gvqe_ctx *c, double *out)
@@ -1072,6 +1181,7 @@ void gvqe_destroy(gvqe_ctx *c)
 {
     if (!c) return;
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    for (cudaEvent_t e : c->ev_fine) cudaEventDestroy(e);
     for (JitModule *m : c->jit_mods) jit_unload(m);
     for (JitModule *m : c->jitx_mods) jit_unload(m);
     delete c;

@@ -311,7 +311,10 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     }
     E("");
     // per_cta: work items (statevector, tile) one thread block handles, consecutive
-    E("extern \"C\" __global__ void __launch_bounds__(%u, 2) %s(amp *states, u64 stride, const ry4 *rytab, const amp *cstab, int nb, int Pn, int per_cta)", NT, name);
+    // src / src_stride: where the tiles are READ (normally = states / stride; a parameter-shift sweep reads the shared base
+    // state of theta, src_stride = 0, and writes the shifted rows' own buffers: SURVEY 8(f) NEXT-2)
+    E("extern \"C\" __global__ void __launch_bounds__(%u, 2) %s(amp *states, u64 stride, const ry4 *rytab, const amp *cstab, int nb, int Pn, int per_cta,", NT, name);
+    E("        const amp *src, u64 src_stride)");
     E("{");
     E("    extern __shared__ __align__(128) unsigned char smem[];");
     E("    unsigned char *tile = smem + %u;", o_tile);
@@ -319,7 +322,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     E("    amp *s_ry = (amp *)(smem + %u); real *s_sc = (real *)(smem + %u); amp *s_rz = (amp *)(smem + %u);", o_ry, o_sc, o_rz);
     E("    amp *s_tc = (amp *)(smem + %u); unsigned *s_tm = (unsigned *)(smem + %u); unsigned *s_rc = (unsigned *)(smem + %u);", o_tc, o_tm, o_rc);
     E("    real *s_scale = (real *)(smem + %u);", o_scale);
-    E("    (void)s_tc; (void)s_tm; (void)s_rc; (void)s_sc; (void)s_ry; (void)s_rz;");
+    E("    (void)s_tc; (void)s_tm; (void)s_rc; (void)s_sc; (void)s_ry; (void)s_rz; (void)src; (void)src_stride;");
     // ---- tables that depend on the thread index only
     for (int s = s_first; s < ns; ++s) {
         const Stage &S = p.stages[B.stage_begin + s];
@@ -389,6 +392,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         }
     }
     E("        amp *gptr = state + (xbase | ld_x);");
+    E("        const amp *gsrc = src + (u64)b * src_stride + (xbase | ld_x);");
     // ---- load phase
     std::vector<uint64_t> hi(NU);
     std::vector<uint32_t> ci(NU), ci_lead(NU);
@@ -417,9 +421,9 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
             oc += b;
         }
         E("%s;", oc.c_str());
-        for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (lead_o ^ %uu), gptr + %lluull);", ci_lead[i], (unsigned long long)hi[i]);
+        for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (lead_o ^ %uu), gsrc + %lluull);", ci_lead[i], (unsigned long long)hi[i]);
     } else {
-        for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (ld_off ^ %uu), gptr + %lluull);", ci[i], (unsigned long long)hi[i]);
+        for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (ld_off ^ %uu), gsrc + %lluull);", ci[i], (unsigned long long)hi[i]);
     }
     // ---- per-statevector setup
     E("        if (b != cur_b) {");
@@ -682,6 +686,18 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     E("        __syncthreads();   // the tile buffer is reused by the next work item");
     E("    }");
     E("}");
+    {   // arithmetic the block needs per amplitude (ALU roofline): rotations 2, every table / phase factor 4
+        double ops = 0.0;
+        for (int s2 = s_first; s2 < ns; ++s2)
+            for (int item : stage_items[s2]) {
+                if (item >= 0) { ops += 2.0; continue; }
+                const SegInfo &si = segs[-item - 1];
+                const bool any_ph = si.has_phth || si.has_tc || si.has_tm;
+                if (si.nlo > 0 || any_ph) ops += 4.0;
+                if (si.nhi > 0) ops += 4.0;
+            }
+        out.fma_ops_per_amp = ops;
+    }
     out.name = name;
     out.source.swap(E.s);
     out.smem_bytes = sm;

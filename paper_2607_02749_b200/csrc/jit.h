@@ -23,6 +23,9 @@ struct JitBlock {
     uint32_t smem_bytes = 0;   // dynamic shared memory per thread block
     uint32_t threads = 0;      // threads per thread block
     int tiles_log2 = 0;        // log2(tiles per statevector) = n - k
+    double fma_ops_per_amp = 0.0;   // FP lane operations (one FMA / MUL / ADD on one real) per amplitude and launch that the
+                                    // schedule needs: 2 per rotation (tangent form), 4 per complex factor, 6 / 4 / 3 per pair
+                                    // of a complex / real / imaginary W; what the ALU roofline in bench.py is counted in
 };
 
 // True when the generated kernels cover this program (tile and register sizes, stage counts, shared-memory budget).
@@ -54,8 +57,9 @@ JitModule *jit_load(const JitBlock &blk, std::string &err);
 void jit_unload(JitModule *m);
 // Launch on `stream`: states (device), stride in amplitudes, ry / cs tables (device, per statevector row of P entries);
 // per_cta: consecutive (statevector, tile) work items one thread block handles (its setup is paid once per thread block).
+// src (optional): statevector(s) the tiles are read from instead of `states` (src_stride 0: all rows read the same one).
 int jit_launch(JitModule *m, const JitBlock &blk, void *states, uint64_t stride, const void *ry, const void *cs, int nb, int P,
-               int per_cta, void *stream);
+               int per_cta, void *stream, const void *src = nullptr, uint64_t src_stride = 0);
 // Expectation pass: table = diagonal energy table, wst / pats = this pass's static tables and patterns, terms = all terms.
 int jit_launch_expect(JitModule *m, const JitBlock &blk, const void *states, uint64_t stride, const void *table, const void *wst,
                       const void *pats, const void *terms, double *partial, uint32_t slots_per_b, uint32_t slot_off, int nb,

@@ -127,6 +127,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     data.pass_pat_cnt.push_back(n_pats);
     if (sm > 220u * 1024u) { err = "jit: expectation pass needs too much shared memory"; return false; }
 
+    double ops_per_thread = 0.0;   // FP lane operations per thread and tile (ALU roofline)
     char name[64];
     snprintf(name, sizeof name, "gvqe_expect_%d_%s", pi, prec == 0 ? "c64" : "c128");
     Emit E;
@@ -355,6 +356,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 for (uint32_t r = 0; r < NR; ++r) {
                     if (r >> pv & 1) continue;
                     E("                pairw(s, a[%u], a[%u], W[%u]);", r, r ^ mr, r & G.zmask);   // only the index bits a term looks at: equal reads merge
+                    ops_per_thread += 6.0;
                 }
                 E("                acc += 2.0 * (double)(s.x + s.y);");
             } else {
@@ -364,9 +366,9 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                     const double wx = prec == 0 ? (double)(float)G.wr[r] : G.wr[r], wy = prec == 0 ? (double)(float)G.wi[r] : G.wi[r];
                     if (wx == 0.0 && wy == 0.0) continue;
                     const uint32_t ix = const_index(wx, wy);
-                    if (wy == 0.0) E("                PAIRR(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
-                    else if (wx == 0.0) E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
-                    else E("                PAIRC(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix);
+                    if (wy == 0.0) { E("                PAIRR(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 4.0; }
+                    else if (wx == 0.0) { E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 3.0; }
+                    else { E("                PAIRC(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 6.0; }
                 }
                 E("                acc += 2.0 * (double)(s.x + s.y + si);");
             }
@@ -445,6 +447,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 E("            rho[%d] = cjmul(*(const amp *)(pv%u + %uu), *(const amp *)(pm%u + %uu));", i, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, (cr[rb] & LOMASK) >> 4, cr[rb] & ~LOMASK);
             }
         }
+        ops_per_thread += 6.0 * np;   // conj(b) a: four multiplies and two adds per pair
         E("            real accm = (real)0;");
         for (uint32_t q : mg.second) {
             const DGroup &dg = plan.groups[q];
@@ -467,6 +470,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 std::string sum = "rho[" + std::to_string(cl.second[0]) + "]";
                 E("              { amp t = %s;", sum.c_str());
                 for (size_t z = 1; z < cl.second.size(); ++z) E("                t = cadd(t, rho[%d]);", cl.second[z]);
+                ops_per_thread += 2.0 * (double)(cl.second.size() - 1) + 2.0;
                 E("                const amp wv = tabp[%u]; accm = %s(wv.x, t.x, %s(-wv.y, t.y, accm)); }", cl.first, prec == 0 ? "fmaf" : "fma", prec == 0 ? "fmaf" : "fma");
             }
             E("            }");
@@ -506,6 +510,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     E("        __syncthreads();   // tile, tables and red are reused by the next work item");
     E("    }");
     E("}");
+    if (P.with_diag) ops_per_thread += 4.0 * NR;   // |psi|^2 E(x): three multiply-adds and one multiply per amplitude
+    out.fma_ops_per_amp = ops_per_thread / (double)NR;
     out.name = name;
     out.source.swap(E.s);
     out.smem_bytes = sm;

@@ -161,14 +161,15 @@ void jit_unload(JitModule *m)
 }
 
 int jit_launch(JitModule *m, const JitBlock &blk, void *states, uint64_t stride, const void *ry, const void *cs, int nb, int P,
-               int per_cta, void *stream)
+               int per_cta, void *stream, const void *src, uint64_t src_stride)
 {
+    if (!src) { src = states; src_stride = stride; }
     if (!m || !m->fn || nb <= 0 || per_cta < 1) return (int)cudaErrorInvalidValue;
     const uint64_t total = (uint64_t)nb << blk.tiles_log2;
     const uint64_t grid64 = (total + (uint64_t)per_cta - 1) / (uint64_t)per_cta;
     if (grid64 > 0x7fffffffull) return (int)cudaErrorInvalidValue;
     const unsigned grid = (unsigned)grid64;
-    void *args[] = {&states, &stride, &ry, &cs, &nb, &P, &per_cta};
+    void *args[] = {&states, &stride, &ry, &cs, &nb, &P, &per_cta, &src, &src_stride};
     const CUresult r = driver().LaunchKernel(m->fn, grid, 1, 1, blk.threads, 1, 1, blk.smem_bytes, (CUstream)stream, args, nullptr);
     return r == CUDA_SUCCESS ? 0 : (int)cudaErrorLaunchFailure;
 }

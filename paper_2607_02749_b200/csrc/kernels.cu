@@ -26,6 +26,23 @@ __global__ void expand_params_kernel(const double *__restrict__ params, cx<T> *_
     }
 }
 
+// ---- rows of a parameter-shift set (Eq. 13): row r = theta with +/- pi/2 on parameter code[r] >> 1 ----
+__global__ void __launch_bounds__(256) shift_rows_kernel(const double *__restrict__ theta, const int32_t *__restrict__ code,
+                                                         double *__restrict__ rows, int P)
+{
+    const int p = code[blockIdx.x] >> 1;
+    const double d = (code[blockIdx.x] & 1) ? -1.57079632679489661923 : 1.57079632679489661923;
+    for (int i = threadIdx.x; i < P; i += blockDim.x) rows[(size_t)blockIdx.x * P + i] = theta[i] + (i == p ? d : 0.0);
+}
+
+int launch_shift_rows(const double *theta, const int32_t *code, double *rows, int P, int n_rows, void *stream, uint64_t *launches)
+{
+    if (n_rows <= 0) return 0;
+    shift_rows_kernel<<<n_rows, 256, 0, (cudaStream_t)stream>>>(theta, code, rows, P);
+    ++*launches;
+    return (int)cudaGetLastError();
+}
+
 // ---- product-state prefix, write-only --------------------------------------------------------------
 // psi[y] = sign(y) * prod_q f_q[x_q],  x = A^-1 y  (A = the prefix's CNOT run, linear over GF(2); sign = its CZ run),
 // f_q = (rotations of qubit q)|0>.  The product comes from tables over 7-qubit groups; A^-1 y is split into the

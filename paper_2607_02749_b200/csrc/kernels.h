@@ -20,6 +20,7 @@ constexpr int EXPECT_UMAX = 8;              // largest single table: 2^8 entries
 constexpr uint32_t READOUT_BLOCKS = 148 * 8;   // grid of the read-out sweep: 8 blocks of 256 threads per SM
 constexpr int SAMPLE_CHUNK_LOG2 = 12;            // shot sampling: probability mass is tabulated per 4096 amplitudes
 constexpr uint32_t SAMPLE_MAX_SHOTS = 1u << 16; // shots per gvqe_sample call (uniforms and results staged in the workspace)
+constexpr uint32_t SWEEP_MAX_ROWS = 1u << 14;   // rows of one parameter-shift sweep staged in the workspace (codes in, energies out)
 constexpr uint32_t HDR_BYTES = 384;         // shared-memory header of the gate kernel
 constexpr uint32_t EXPECT_HDR_BYTES = 1024; // shared-memory header of the expectation kernel: holds the DPass copy
 
@@ -34,6 +35,8 @@ struct PrefixDev {   // device view of schedule.h Prefix
 // prec: 0 = complex64 (float), 1 = complex128 (double)
 // ry: optional second table for the specialised gate kernels ({tan, scale, form, 0} per parameter, jit.cpp), or NULL
 int launch_expand_params(int prec, const double *params, void *cs, void *ry, uint64_t count, void *stream, uint64_t *launches);
+// rows[r][:] = theta[:] with (code[r] & 1 ? -pi/2 : +pi/2) added to parameter code[r] >> 1 (all DEVICE pointers)
+int launch_shift_rows(const double *theta, const int32_t *code, double *rows, int P, int n_rows, void *stream, uint64_t *launches);
 int launch_init_product(int prec, const PrefixDev &pd, void *states, uint64_t stride_amps, const void *cs, int P, int batch,
                         void *stream, uint64_t *launches);
 int launch_gate_block(int prec, int R, const GateLaunch &g, const DBlock &block, int k, uint32_t smem_prog_bytes, int n,
