@@ -264,10 +264,16 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     }
     // ---- tile-dependent tables
     if (any_dyn) {
-        for (uint32_t q = g0; q < g1; ++q) {
-            const GInfo &G = gi[q - g0];
-            if (!G.dyn) continue;
-            E("        for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = MK((real)0, (real)0);", G.E, NT, G.scr_off);
+        {   // the scratch areas of the tile-dependent groups are contiguous ranges of 16-byte units: a few wide loops
+            std::vector<std::pair<uint32_t, uint32_t>> ranges;
+            for (uint32_t q = g0; q < g1; ++q) {
+                const GInfo &G = gi[q - g0];
+                if (!G.dyn) continue;
+                const uint32_t b0 = G.scr_off, b1 = (G.scr_off + G.E * AB + 15u) & ~15u;
+                if (!ranges.empty() && ranges.back().second == b0) ranges.back().second = b1; else ranges.push_back({b0, b1});
+            }
+            for (auto &rg : ranges)
+                E("        for (unsigned o = %uu + tid * 16u; o < %uu; o += %uu) *(unit16 *)(smem + o) = unit16{0u, 0u, 0u, 0u};", rg.first, rg.second, NT * 16);
         }
         E("        __syncthreads();");
         E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): signed sum of its terms", n_pats, NT);
@@ -286,15 +292,30 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             const GInfo &G = gi[q - g0];
             if (!G.dyn) continue;
             const DGroup &dg = plan.groups[q];
-            E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits, plus the static part", wi % 8, q - g0, (int)dg.ubits);
-            E("            amp *d = (amp *)(smem + %u);", G.scr_off);
-            for (int bit = 0; bit < (int)dg.ubits; ++bit) {
-                E("            for (unsigned i = lane; i < %uu; i += 32u) { const unsigned j = ((i >> %d) << %d) | (i & %uu); const amp u = d[j], v = d[j | %uu]; d[j] = MK(u.x + v.x, u.y + v.y); d[j | %uu] = MK(u.x - v.x, u.y - v.y); }",
-                  G.E / 2, bit, bit + 1, (1u << bit) - 1u, 1u << bit, 1u << bit);
-                E("            __syncwarp();");
+            // Walsh-Hadamard of the scattered pattern sums in registers: lane l holds entries [l EP, (l+1) EP); the rounds
+            // over the in-lane index bits are register butterflies, those over the lane bits take the partner by shuffle
+            // (new = partner + s mine, s = -1 on the lane with the bit set).  Then + static part, formatted for the readers.
+            const int ub = (int)dg.ubits, epl = ub > 5 ? ub - 5 : 0, EP = 1 << epl, nlb = ub - epl;
+            E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits, plus the static part", wi % 8, q - g0, ub);
+            E("            const amp *d = (const amp *)(smem + %u);", G.scr_off);
+            E("            const unsigned e0 = (lane & %uu) * %du;", (1u << nlb) - 1u, EP);
+            E("            amp v[%d];", EP);
+            for (int i = 0; i < EP; ++i) E("            v[%d] = d[e0 + %d];", i, i);
+            for (int bit = 0; bit < epl; ++bit)
+                for (int i = 0; i < EP; ++i) if (!(i >> bit & 1))
+                    E("            { const amp u = v[%d], w2 = v[%d]; v[%d] = MK(u.x + w2.x, u.y + w2.y); v[%d] = MK(u.x - w2.x, u.y - w2.y); }", i, i | (1 << bit), i, i | (1 << bit));
+            for (int lb = 0; lb < nlb; ++lb) {
+                E("            { const real sg = ((lane >> %d) & 1u) ? (real)-1 : (real)1;", lb);
+                for (int i = 0; i < EP; ++i)
+                    E("              { amp pz; pz.x = __shfl_xor_sync(0xffffffffu, v[%d].x, %d); pz.y = __shfl_xor_sync(0xffffffffu, v[%d].y, %d); v[%d] = MK(fma(sg, v[%d].x, pz.x), fma(sg, v[%d].y, pz.y)); }", i, 1 << lb, i, 1 << lb, i, i, i);
+                E("            }");
             }
-            if (G.mode == 1) E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; ((tw4 *)(smem + %u))[e] = twfmt(MK(d[e].x + s.x, d[e].y + s.y)); }", G.E, G.wst_off, G.tab_off);
-            else E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; d[e] = MK(d[e].x + s.x, d[e].y + s.y); }", G.E, G.wst_off);
+            E("            if (lane < %uu) {", 1u << nlb);
+            for (int i = 0; i < EP; ++i) {
+                if (G.mode == 1) E("                { const amp s = wst[%u + e0 + %d]; ((tw4 *)(smem + %u))[e0 + %d] = twfmt(MK(v[%d].x + s.x, v[%d].y + s.y)); }", G.wst_off, i, G.tab_off, i, i, i);
+                else E("                { const amp s = wst[%u + e0 + %d]; ((amp *)(smem + %u))[e0 + %d] = MK(v[%d].x + s.x, v[%d].y + s.y); }", G.wst_off, i, G.tab_off, i, i, i);
+            }
+            E("            }");
             E("        }");
             ++wi;
         }

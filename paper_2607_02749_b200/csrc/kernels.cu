@@ -55,7 +55,7 @@ __device__ __forceinline__ uint64_t prefix_ainv(const PrefixDev &pd, uint64_t y)
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256, 4)
 init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
 {
     __shared__ cx<T> f[40][2];
@@ -91,14 +91,26 @@ init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_
     const uint64_t ybase = ((uint64_t)blockIdx.x << pd.kk) | (uint64_t)(tid * V);
     const uint64_t xthr = prefix_ainv(pd, ybase);
     const uint64_t xe1 = prefix_ainv(pd, 1ull);
+    // Only the table groups whose index bits move with the vector number or the lane inside a vector need a lookup per
+    // amplitude; the product over the other groups is one factor per thread (the images of those y bits under A^-1 are
+    // the same for every thread: uniform branches).
+    uint64_t moving = V > 1 ? xe1 : 0ull;
+    for (uint32_t i = 0; i < nvec; ++i) moving |= xi[i];
+    cx<T> pc{T(1), T(0)};
+    uint32_t aff = 0;
+    for (int g = 0; g < ngrp; ++g) {
+        if ((moving >> (7 * g)) & 127ull) aff |= 1u << g;
+        else pc = cmul(pc, tab[g][(xthr >> (7 * g)) & 127ull]);
+    }
     for (uint32_t i = 0; i < nvec; ++i) {
         vec16<T> out;
 #pragma unroll
         for (uint32_t e = 0; e < V; ++e) {
             const uint64_t y = ybase | ((uint64_t)i * nthr * V) | e;
             const uint64_t x = xthr ^ xi[i] ^ (e ? xe1 : 0ull);
-            cx<T> p = tab[0][x & 127ull];
-            for (int g = 1; g < ngrp; ++g) p = cmul(p, tab[g][(x >> (7 * g)) & 127ull]);
+            cx<T> p = pc;
+            for (int g = 0; g < ngrp; ++g)
+                if (aff >> g & 1u) p = cmul(p, tab[g][(x >> (7 * g)) & 127ull]);
             int par = 0;
             for (int c = 0; c < pd.n_cz; ++c) par += __popcll(y & (y >> pd.cz_d[c]) & pd.cz_m[c]);
             out.v[e] = (par & 1) ? cneg(p) : p;
