@@ -296,6 +296,20 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             // over the in-lane index bits are register butterflies, those over the lane bits take the partner by shuffle
             // (new = partner + s mine, s = -1 on the lane with the bit set).  Then + static part, formatted for the readers.
             const int ub = (int)dg.ubits, epl = ub > 5 ? ub - 5 : 0, EP = 1 << epl, nlb = ub - epl;
+            if (prec == 1 && ub > 5) {   // complex128, large table: four 32-bit shuffles per entry cost more than the shared-memory butterflies (measured)
+                E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits (shared memory), plus the static part", wi % 8, q - g0, ub);
+                E("            amp *d = (amp *)(smem + %u);", G.scr_off);
+                for (int bit = 0; bit < ub; ++bit) {
+                    E("            for (unsigned i = lane; i < %uu; i += 32u) { const unsigned j = ((i >> %d) << %d) | (i & %uu); const amp u = d[j], v = d[j | %uu]; d[j] = MK(u.x + v.x, u.y + v.y); d[j | %uu] = MK(u.x - v.x, u.y - v.y); }",
+                      G.E / 2, bit, bit + 1, (1u << bit) - 1u, 1u << bit, 1u << bit);
+                    E("            __syncwarp();");
+                }
+                if (G.mode == 1) E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; ((tw4 *)(smem + %u))[e] = twfmt(MK(d[e].x + s.x, d[e].y + s.y)); }", G.E, G.wst_off, G.tab_off);
+                else E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; d[e] = MK(d[e].x + s.x, d[e].y + s.y); }", G.E, G.wst_off);
+                E("        }");
+                ++wi;
+                continue;
+            }
             E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits, plus the static part", wi % 8, q - g0, ub);
             E("            const amp *d = (const amp *)(smem + %u);", G.scr_off);
             E("            const unsigned e0 = (lane & %uu) * %du;", (1u << nlb) - 1u, EP);

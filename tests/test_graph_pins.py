@@ -356,3 +356,75 @@ def test_geometric_blocks_by_hand_and_library():
                 assert (list(lab), K) == go.geometric_blocks(n, bs, off)
     with pytest.raises(gv.GvqeError):
         gb.geometric_blocks(5, 2, 2)
+
+
+# ---- pins of the finite-shot estimator oracle (oracle/readout_oracle.energy_shots) -------------------
+def test_shot_oracle_settings_by_hand():
+    from oracle import readout_oracle as ro
+    settings, got = ro.measurement_groups(3, ["ZZI", "XIZ", "XZI", "YIZ", "IIZ", "XYI", "III"])
+    assert settings == [(0, 0), (1, 0), (1, 1), (3, 2)]              # (x_mask, y_mask) ascending; Z-only and identity first
+    assert got == [0, 1, 1, 2, 0, 3, 0]
+
+
+def test_shot_oracle_rotation_diagonalises_the_letters():
+    """After rotate_to_setting the probabilities weighted by (-1)^{popcount(x & support)} give the exact <P> of every term
+    of the setting (the definition of measuring in that basis); checked against the dense Kronecker expectation."""
+    import oracle
+    from oracle import readout_oracle as ro
+    from tests.dense_ref import dense_hamiltonian
+    n = 4
+    rng = np.random.default_rng(3)
+    psi = rng.normal(size=1 << n) + 1j * rng.normal(size=1 << n)
+    psi /= np.linalg.norm(psi)
+    for s in ["XIZY", "YYII", "ZIXZ", "IYZX", "XXXX", "ZZII"]:
+        xm = sum(1 << q for q, ch in enumerate(s) if ch in "XY")
+        ym = sum(1 << q for q, ch in enumerate(s) if ch == "Y")
+        supp = sum(1 << q for q, ch in enumerate(s) if ch != "I")
+        phi = ro.rotate_to_setting(n, psi, xm, ym)
+        assert abs(np.vdot(phi, phi).real - 1.0) < 1e-12
+        p = np.abs(phi) ** 2
+        est = sum(p[x] * (1 - 2 * (bin(x & supp).count("1") & 1)) for x in range(1 << n))
+        exact = np.vdot(psi, dense_hamiltonian(n, [s], [1.0]) @ psi).real
+        assert abs(est - exact) < 1e-12, s
+
+
+def test_shot_oracle_one_qubit_closed_form_and_rate():
+    """RY(theta)|0>, H = X: P(outcome 0 in the X basis) = (1 + sin theta) / 2.  Stratified uniforms give the estimate
+    within 1/S of sin theta; random uniforms give an error that shrinks like 1/sqrt(S) and the exact energy in the limit."""
+    from oracle import readout_oracle as ro
+    th = 0.7
+    ops = np.array([[0, 0, -1, 0]], dtype=np.int32)
+    for S in (10, 1000):
+        E, means, shots = ro.energy_shots(1, ops, [th], ["X"], [2.0], ((np.arange(S) + 0.5) / S).reshape(1, -1))
+        assert abs(E - 2.0 * np.sin(th)) <= 2.0 * (2.0 / S) + 1e-12
+        assert abs(np.mean(shots[0] == 0) - 0.5 * (1 + np.sin(th))) <= 1.0 / S + 1e-12
+    rms = {}
+    for S in (100, 10000):
+        errs = []
+        for rep in range(40):
+            u = np.random.default_rng(1000 * S + rep).uniform(size=(1, S))
+            E, _, _ = ro.energy_shots(1, ops, [th], ["X"], [2.0], u)
+            errs.append(E - 2.0 * np.sin(th))
+        rms[S] = float(np.sqrt(np.mean(np.square(errs))))
+    sigma = 2.0 * np.cos(th)                                      # std of one shot of 2 X: 2 sqrt(1 - sin^2)
+    assert 0.6 * sigma / 10 < rms[100] < 1.5 * sigma / 10 and 0.6 * sigma / 100 < rms[10000] < 1.5 * sigma / 100
+
+
+def test_shot_oracle_product_state_terms():
+    """Rotations only: <P> = prod_q f_q (closed form); each term's estimated mean lies within 5 standard errors."""
+    import math
+    from oracle import readout_oracle as ro
+    n, S = 5, 4000
+    rng = np.random.default_rng(8)
+    th = rng.uniform(-math.pi, math.pi, 2 * n)
+    ops = np.array([(0, q, -1, q) for q in range(n)] + [(1, q, -1, n + q) for q in range(n)], dtype=np.int32)
+    terms = ["ZIIZI", "XIIII", "IYIZI", "XYZII", "IIXXY", "ZZZZZ", "IIIII"]
+    cs = np.array([0.5, -1.0, 0.7, 0.3, -0.2, 1.1, 0.25])
+    settings, _ = ro.measurement_groups(n, terms)
+    E, means, _ = ro.energy_shots(n, ops, th, terms, cs, rng.uniform(size=(len(settings), S)))
+    for k, s in enumerate(terms):
+        v = 1.0
+        for q, ch in enumerate(s):
+            v *= {"I": 1.0, "Z": math.cos(th[q]), "X": math.sin(th[q]) * math.cos(th[n + q]), "Y": math.sin(th[q]) * math.sin(th[n + q])}[ch]
+        assert abs(means[k] - v) <= 5.0 * math.sqrt(max(1.0 - v * v, 1e-12) / S) + 1e-9, (s, means[k], v)
+    assert means[-1] == 1.0                                       # identity: +1 on every shot
