@@ -176,6 +176,20 @@ gvqe_status gvqe_argmax(gvqe_ctx *ctx, int slot, uint64_t *x, double *prob, void
 gvqe_status gvqe_sample(gvqe_ctx *ctx, int slot, int n_shots, const double *u, uint64_t *x, double *norm,
                         void *cuda_stream);
 
+/* Finite-shot energy estimate, PAPER.md:256 ("8192 measurement shots" per evaluation), 270 (shot-noise study).
+ * Measurement settings (reading R3): two terms share a setting when they carry the same X / Y letters on the same
+ * qubits; settings are numbered in ascending (x_mask, y_mask) order (Z-only and identity terms: setting 0 when present).
+ * gvqe_measurement_settings: *n_settings and, per term (HOST, n_terms entries, may be NULL), its setting.
+ * gvqe_energy_shots: for every setting the statevector of in-flight slot `slot` (as left by the last energy call) is
+ * copied into another slot, rotated into the setting's basis (H on the X qubits, H S^dagger on the Y qubits), n_shots
+ * bitstrings are drawn by inversion exactly as in gvqe_sample with the caller's uniforms u[setting * n_shots + s]
+ * (HOST, n_settings * n_shots doubles in [0,1)), and <P_k> is estimated as the mean of (-1)^{popcount(x & support_k)} over
+ * the shots of the term's setting.  *E_est = sum_k c_k <P_k>_est; term_means (HOST, optional, n_terms doubles).  Needs at
+ * least two statevectors in flight (GVQE_ERR_WORKSPACE otherwise); n_shots <= 65536.  The slot's own state is unchanged. */
+gvqe_status gvqe_measurement_settings(const gvqe_ctx *ctx, int32_t *n_settings, int32_t *setting_of_term);
+gvqe_status gvqe_energy_shots(gvqe_ctx *ctx, int slot, int n_shots, const double *u, double *E_est, double *term_means,
+                              void *cuda_stream);
+
 /* Introspection of the compiled schedule (host; for tests and traffic accounting).
  * gvqe_schedule_info: number of fused gate blocks, number of off-diagonal passes, statevectors in flight.
  * gvqe_dump_schedule: writes a text description of every block/stage/op into buf (NUL-terminated, truncated to

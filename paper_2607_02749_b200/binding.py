@@ -22,7 +22,7 @@ STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "G
 EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_kernel_info", "gvqe_kernel_arrays", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
-           "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
+           "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_measurement_settings", "gvqe_energy_shots", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_profile_read_launches", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
            "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
@@ -96,6 +96,8 @@ def load():
     L.gvqe_get_state.argtypes = [vp, i32, vp]
     L.gvqe_argmax.argtypes = [vp, i32, vp, vp, vp]
     L.gvqe_sample.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    L.gvqe_measurement_settings.argtypes = [vp, vp, vp]
+    L.gvqe_energy_shots.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     L.gvqe_schedule_info.argtypes = [vp, vp, vp, vp]
     L.gvqe_dump_schedule.argtypes = [vp, C.c_char_p, sz]
     L.gvqe_dump_schedule.restype = sz
@@ -264,6 +266,25 @@ class Gvqe:
         self._check(self._L.gvqe_sample(self._h, int(slot), len(uu), uu.ctypes.data, x.ctypes.data, C.addressof(z),
                                         C.c_void_p(stream)))
         return x[:len(uu)], z.value
+
+    def measurement_settings(self, n_terms: int):
+        """(n_settings, setting_of_term[n_terms]) of gvqe_measurement_settings."""
+        ns = C.c_int32(0)
+        got = np.zeros(max(n_terms, 1), dtype=np.int32)
+        self._check(self._L.gvqe_measurement_settings(self._h, C.addressof(ns), got.ctypes.data))
+        return int(ns.value), got[:n_terms]
+
+    def energy_shots(self, u, n_terms: int, slot: int = 0, stream: int = 0):
+        """(E_est, term_means[n_terms]) from u[n_settings, n_shots] uniforms in [0,1) (gvqe_energy_shots)."""
+        uu = np.ascontiguousarray(u, dtype=np.float64)
+        ns, _ = self.measurement_settings(n_terms)
+        if uu.ndim != 2 or uu.shape[0] != ns:
+            raise GvqeError(GVQE_ERR_INVALID_ARG, f"u must be [{ns}, n_shots]")
+        E = C.c_double(0.0)
+        means = np.zeros(max(n_terms, 1), dtype=np.float64)
+        self._check(self._L.gvqe_energy_shots(self._h, int(slot), uu.shape[1], uu.ctypes.data, C.addressof(E), means.ctypes.data,
+                                              C.c_void_p(stream)))
+        return E.value, means[:n_terms]
 
     def schedule_info(self):
         a, b, c = C.c_int32(0), C.c_int32(0), C.c_int32(0)

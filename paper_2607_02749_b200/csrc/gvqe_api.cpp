@@ -981,6 +981,87 @@ gvqe_status gvqe_sample(gvqe_ctx *c, int slot, int n_shots, const double *u, uin
     return GVQE_OK;
 }
 
+// measurement settings: distinct (x_mask, y_mask) in ascending order; returns the setting of every term
+static void settings_of(const gvqe_ctx *c, std::vector<std::pair<uint64_t, uint64_t>> &settings, std::vector<int32_t> &of_term)
+{
+    settings.clear();
+    for (const HostTerm &t : c->H.terms) settings.push_back({t.x, t.x & t.z});
+    std::sort(settings.begin(), settings.end());
+    settings.erase(std::unique(settings.begin(), settings.end()), settings.end());
+    of_term.resize(c->H.terms.size());
+    for (size_t k = 0; k < c->H.terms.size(); ++k) {
+        const std::pair<uint64_t, uint64_t> key(c->H.terms[k].x, c->H.terms[k].x & c->H.terms[k].z);
+        of_term[k] = (int32_t)(std::lower_bound(settings.begin(), settings.end(), key) - settings.begin());
+    }
+}
+
+gvqe_status gvqe_measurement_settings(const gvqe_ctx *c, int32_t *n_settings, int32_t *setting_of_term)
+{
+    if (!c) return GVQE_ERR_INVALID_ARG;
+    if (!c->have_h) return GVQE_ERR_NO_HAMILTONIAN;
+    std::vector<std::pair<uint64_t, uint64_t>> settings;
+    std::vector<int32_t> of_term;
+    settings_of(c, settings, of_term);
+    if (n_settings) *n_settings = (int32_t)settings.size();
+    if (setting_of_term) for (size_t k = 0; k < of_term.size(); ++k) setting_of_term[k] = of_term[k];
+    return GVQE_OK;
+}
+
+gvqe_status gvqe_energy_shots(gvqe_ctx *c, int slot, int n_shots, const double *u, double *E_est, double *term_means, void *stream)
+{
+    if (!c || !E_est || n_shots < 1 || !u) return GVQE_ERR_INVALID_ARG;
+    if ((uint32_t)n_shots > SAMPLE_MAX_SHOTS) return fail(c, GVQE_ERR_INVALID_ARG, "energy_shots: more than 65536 shots per setting");
+    if (c->dirty || !c->ws) return fail(c, GVQE_ERR_WORKSPACE, "energy_shots: no energy call has run on this workspace");
+    if (slot < 0 || slot >= c->in_flight) return fail(c, GVQE_ERR_INVALID_ARG, "energy_shots: slot out of range");
+    if (c->in_flight < 2) return fail(c, GVQE_ERR_WORKSPACE, "energy_shots: needs a second statevector in flight as scratch");
+    std::vector<std::pair<uint64_t, uint64_t>> settings;
+    std::vector<int32_t> of_term;
+    settings_of(c, settings, of_term);
+    const size_t NS = settings.size(), M = c->H.terms.size();
+    for (size_t i = 0; i < NS * (size_t)n_shots; ++i)
+        if (!(u[i] >= 0.0 && u[i] < 1.0)) return fail(c, GVQE_ERR_INVALID_ARG, "energy_shots: uniforms must lie in [0, 1)");
+    const Layout L = layout_of(c);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int scratch = (slot + 1) % c->in_flight;
+    char *src = (char *)c->d_states + L.state_b * (size_t)slot, *dst = (char *)c->d_states + L.state_b * (size_t)scratch;
+    const uint64_t count = 1ull << c->n_user;    // idle padding qubits stay |0>: the user's amplitudes are the first 2^n_user
+    const uint64_t n_chunks = (count + (1u << SAMPLE_CHUNK_LOG2) - 1) >> SAMPLE_CHUNK_LOG2;
+    double *mass = (double *)(c->ws + L.smass), *total = mass + n_chunks;
+    double *u_dev = (double *)(c->ws + L.su);
+    uint64_t *x_dev = (uint64_t *)(c->ws + L.sx);
+    std::vector<uint64_t> shots((size_t)n_shots);
+    std::vector<double> sum(M, 0.0);
+    for (size_t g = 0; g < NS; ++g) {
+        const uint64_t xm = settings[g].first, ym = settings[g].second;
+        const void *cur = src;
+        for (int q = 0; q < c->n_user; ++q) {   // the first rotation doubles as the copy into the scratch slot
+            if (!((xm >> q) & 1ull)) continue;
+            const int ke = launch_basis_rotate(c->prec, cur, dst, c->n_user, q, (int)((ym >> q) & 1ull), st, &c->launches);
+            if (ke) return cuda_fail(c, ke, "basis rotation");
+            cur = dst;
+        }
+        cudaError_t e = cudaMemcpyAsync(u_dev, u + g * (size_t)n_shots, (size_t)n_shots * 8, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "energy_shots H2D");
+        const int ke = launch_sample(c->prec, cur, count, mass, total, u_dev, x_dev, (uint32_t)n_shots, st, &c->launches);
+        if (ke) return cuda_fail(c, ke, "sample launch");
+        e = cudaMemcpyAsync(shots.data(), x_dev, (size_t)n_shots * 8, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return cuda_fail(c, e, "energy_shots D2H");
+        for (size_t k = 0; k < M; ++k) {
+            if ((size_t)of_term[k] != g) continue;
+            const uint64_t supp = c->H.terms[k].x | c->H.terms[k].z;
+            long plus = 0;
+            for (int s2 = 0; s2 < n_shots; ++s2) plus += (__builtin_popcountll(shots[(size_t)s2] & supp) & 1) ? -1 : 1;
+            sum[k] = (double)plus / (double)n_shots;
+        }
+    }
+    double E = 0.0;
+    for (size_t k = 0; k < M; ++k) E += c->H.terms[k].c * sum[k];
+    *E_est = E;
+    if (term_means) for (size_t k = 0; k < M; ++k) term_means[k] = sum[k];
+    return GVQE_OK;
+}
+
 gvqe_status gvqe_schedule_info(const gvqe_ctx *c, int32_t *nb, int32_t *np, int32_t *inflight)
 {
     if (!c) return GVQE_ERR_INVALID_ARG;

@@ -97,9 +97,9 @@ init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_
     uint64_t moving = V > 1 ? xe1 : 0ull;
     for (uint32_t i = 0; i < nvec; ++i) moving |= xi[i];
     cx<T> pc{T(1), T(0)};
-    uint32_t aff = 0;
+    int ga[5] = {0, 0, 0, 0, 0}, na = 0;   // the groups that need a lookup per amplitude (same for every thread)
     for (int g = 0; g < ngrp; ++g) {
-        if ((moving >> (7 * g)) & 127ull) aff |= 1u << g;
+        if ((moving >> (7 * g)) & 127ull) ga[na++] = g;
         else pc = cmul(pc, tab[g][(xthr >> (7 * g)) & 127ull]);
     }
     for (uint32_t i = 0; i < nvec; ++i) {
@@ -109,8 +109,9 @@ init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_
             const uint64_t y = ybase | ((uint64_t)i * nthr * V) | e;
             const uint64_t x = xthr ^ xi[i] ^ (e ? xe1 : 0ull);
             cx<T> p = pc;
-            for (int g = 0; g < ngrp; ++g)
-                if (aff >> g & 1u) p = cmul(p, tab[g][(x >> (7 * g)) & 127ull]);
+#pragma unroll
+            for (int a = 0; a < 5; ++a)
+                if (a < na) p = cmul(p, tab[ga[a]][(x >> (7 * ga[a])) & 127ull]);
             int par = 0;
             for (int c = 0; c < pd.n_cz; ++c) par += __popcll(y & (y >> pd.cz_d[c]) & pd.cz_m[c]);
             out.v[e] = (par & 1) ? cneg(p) : p;
@@ -511,6 +512,33 @@ int launch_sample(int prec, const void *state, uint64_t count, double *mass, dou
         else sample_kernel<double><<<g2, 256, 0, st>>>((const cx<double> *)state, count, chunk_len, mass, n_chunks, total, u_dev, x_dev, n_shots);
         ++*launches;
     }
+    return (int)cudaGetLastError();
+}
+
+// ---- measurement-basis change for shot sampling (reading R3) ------------------------------------------
+// dst = G_q src with G = H (X letter on qubit q) or H S^dagger (Y letter): (a, b) -> ((a + b') / sqrt 2, (a - b') / sqrt 2),
+// b' = b for X, b' = -i b for Y.  One thread per amplitude pair; src may equal dst (each pair is owned by one thread).
+template <typename T>
+__global__ void __launch_bounds__(256) basis_rotate_kernel(const cx<T> *src, cx<T> *dst, uint64_t pairs, int q, int is_y)
+{
+    const T r = (T)0.70710678118654752440;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < pairs; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t x = ((i >> q) << (q + 1)) | (i & ((1ull << q) - 1ull));
+        const cx<T> a = src[x];
+        cx<T> b = src[x | (1ull << q)];
+        if (is_y) b = cx<T>{b.y, -b.x};   // -i b
+        dst[x] = cx<T>{(a.x + b.x) * r, (a.y + b.y) * r};
+        dst[x | (1ull << q)] = cx<T>{(a.x - b.x) * r, (a.y - b.y) * r};
+    }
+}
+
+int launch_basis_rotate(int prec, const void *src, void *dst, int n, int q, int is_y, void *stream, uint64_t *launches)
+{
+    const uint64_t pairs = 1ull << (n - 1);
+    const unsigned grid = (unsigned)std::min<uint64_t>((pairs + 255) / 256, 148u * 16u);
+    if (prec == 0) basis_rotate_kernel<float><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<float> *)src, (cx<float> *)dst, pairs, q, is_y);
+    else basis_rotate_kernel<double><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<double> *)src, (cx<double> *)dst, pairs, q, is_y);
+    ++*launches;
     return (int)cudaGetLastError();
 }
 

@@ -55,6 +55,8 @@ int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, vo
 // u_dev = n_shots uniforms in [0,1), x_dev = n_shots results.
 int launch_sample(int prec, const void *state, uint64_t count, double *mass, double *total, const double *u_dev,
                   uint64_t *x_dev, uint32_t n_shots, void *stream, uint64_t *launches);
+// dst = (H or H S^dagger on qubit q) src over 2^n amplitudes (measurement basis of an X / Y letter); src may equal dst
+int launch_basis_rotate(int prec, const void *src, void *dst, int n, int q, int is_y, void *stream, uint64_t *launches);
 int kernels_init(void);   // opt-in shared memory sizes; returns the CUDA error
 
 }  // namespace gv

@@ -235,6 +235,55 @@ def test_sample_quantiles_product_state(n, prec):
     assert len(g.sample([], 0)[0]) == 0
 
 
+# ---- finite-shot energy estimate (gvqe_energy_shots) ----------------------------
+@pytest.mark.parametrize("cfg,n,D,prec", [(2, 9, 2, "c128"), (4, 12, 2, "c64"), (3, 14, 1, "c128"), (4, 15, 2, "c64")])
+def test_energy_shots_vs_oracle(orc, cfg, n, D, prec):
+    """Same uniforms, same settings: the library's shots are those of the oracle up to ties at cumulative boundaries, so every
+    term mean agrees within the fraction of shots that can differ, and the estimate approaches the exact energy."""
+    from oracle import readout_oracle as ro
+    w = make_workload(cfg, n=n, M=120, D=D, batch=2)
+    g = ctx(w, prec, in_flight=2)
+    g.energy_batch(w.params[:2])
+    pl = w.pauli_list()
+    settings, got = ro.measurement_groups(w.n, pl)
+    ns, got_lib = g.measurement_settings(w.M)
+    assert ns == len(settings) and got_lib.tolist() == got            # integer side: exact
+    S = 2000
+    u = np.random.default_rng(n).uniform(size=(ns, S))
+    E_ref, means_ref, _ = ro.energy_shots(w.n, w.ops, w.params[1], pl, w.coeffs, u)
+    E, means = g.energy_shots(u, w.M, slot=1)
+    slack = (3.0 if prec == "c64" else 0.0) / S                        # c64: a few shots may fall on the other side of a boundary
+    assert np.max(np.abs(means - means_ref)) <= 2.0 * slack + 1e-12
+    assert abs(E - E_ref) <= 2.0 * slack * np.sum(np.abs(w.coeffs)) + 1e-9
+    exact = orc.energy_batch(w.n, w.ops, w.params[1:2], w.paulis, w.coeffs)[0]
+    per_setting = np.zeros(ns)                                         # terms of one setting share shots: fully correlated
+    for k in range(w.M):
+        per_setting[got[k]] += abs(w.coeffs[k])
+    assert abs(E - exact) <= 6.0 * np.sqrt(np.sum(per_setting ** 2) / S)
+    assert np.array_equal(g.energy_batch(w.params[:2]), g.energy_batch(w.params[:2]))   # the slots were not disturbed for reuse
+    with pytest.raises(gv.GvqeError):
+        g.energy_shots(np.ones((ns, 4)), w.M, slot=0)                  # u = 1.0 is outside [0, 1)
+
+
+def test_energy_shots_one_qubit_closed_form():
+    """RY(theta)|0>, H = 2 X + 0.5 Z: stratified uniforms give each mean within 1/S of sin(theta) and cos(theta)."""
+    th, S = 0.7, 1000
+    g = gv.Gvqe(1, ops=np.array([[0, 0, -1, 0]], dtype=np.int32), n_params=1, precision="c128")
+    g.set_hamiltonian(b"X" + b"Z", [2.0, 0.5])
+    g.alloc_workspace(2)
+    g.energy_batch(np.array([[th], [0.0]]))
+    u = np.tile((np.arange(S) + 0.5) / S, (2, 1))
+    E, means = g.energy_shots(u, 2, slot=0)
+    assert abs(means[0] - np.sin(th)) <= 2.0 / S and abs(means[1] - np.cos(th)) <= 2.0 / S
+    assert abs(E - (2.0 * np.sin(th) + 0.5 * np.cos(th))) <= 5.0 / S
+    g1 = gv.Gvqe(1, ops=np.array([[0, 0, -1, 0]], dtype=np.int32), n_params=1, precision="c128")
+    g1.set_hamiltonian(b"X", [1.0])
+    g1.alloc_workspace(1)
+    g1.energy_batch(np.array([[th]]))
+    with pytest.raises(gv.GvqeError):                                  # one statevector in flight: no scratch slot
+        g1.energy_shots(u[:1], 1, slot=0)
+
+
 # ---- shared-prefix parameter-shift sweeps (SURVEY 8(f) NEXT-2) ---------------------------------------------------------
 @pytest.mark.parametrize("cfg,n,D,prec,in_flight,prefix,spec", [
     (1, 10, 3, "c128", 16, 0, 0), (2, 16, 4, "c128", 8, 0, 0), (4, 15, 3, "c64", 8, 2, 0), (4, 16, 2, "c128", 3, 1, 0),
