@@ -529,7 +529,7 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->d_sweep_idx = (int32_t *)(w + L.sweep_idx); c->d_sweep_E = (double *)(w + L.sweep_E);
     c->pxd.rot_begin = (const int32_t *)(w + L.px_begin); c->pxd.rot_kind = (const uint8_t *)(w + L.px_kind);
     c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
-    c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = c->n_store < 13 ? c->n_store : 13;
+    c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = std::min(c->n_store, c->prec == GVQE_C64 ? 15 : 14);   // amplitudes one thread block writes: its set-up (product tables) is paid once per 2^kk
     for (int i = 0; i < 4; ++i) { c->pxd.cz_d[i] = c->px.cz_d[i]; c->pxd.cz_m[i] = c->px.cz_m[i]; }
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
     c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs); c->d_rss = (DRs *)(w + L.rss);

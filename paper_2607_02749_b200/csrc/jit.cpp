@@ -44,7 +44,49 @@ int lpos_of(const Block &B, int q)
     return -1;
 }
 
-void choose_thread_bits(const Geo &g, const Stage &S, int *tb) { choose_thread_bits_for(g, S.regbit, g.R, tb); }
+// Thread-index bit -> local bit of a stage.  The lanes of one shared-memory wavefront (16 lanes of 8-byte accesses, 8 of
+// 16-byte ones) are the lowest thread-index bits: they are given the local bits for which the loads AND the stores of the
+// stage (the stores go through the CNOT map when the stage ends with a run) hit the most distinct bank groups; searched
+// exhaustively (at most C(9,4) subsets).  store_img: image of each local unit vector under the stage's CNOT run, or null.
+void choose_thread_bits(const Geo &g, const Stage &S, const uint32_t *store_img, int *tb)
+{
+    bool isreg[16] = {false};
+    for (int s = 0; s < g.R; ++s) isreg[S.regbit[s]] = true;
+    std::vector<int> free_bits;
+    for (int b = 0; b < g.k; ++b) if (!isreg[b]) free_bits.push_back(b);
+    const bool wide = g.lv == 0 || S.regbit[0] == 0;          // 16-byte accesses
+    const int L = wide ? 3 : 4, nl = 1 << L;
+    const int nf = (int)free_bits.size();
+    auto waves = [&](const std::vector<int> &lane_bits, bool through_map, bool wide_access) {
+        int count[16] = {0};
+        int worst = 0;
+        for (int l = 0; l < nl; ++l) {
+            uint32_t j = 0;
+            for (int i = 0; i < L; ++i) if (l >> i & 1) j ^= through_map ? store_img[lane_bits[i]] : (1u << lane_bits[i]);
+            const uint32_t o = g.off(j);
+            const int slot = wide_access ? (int)((o >> 4) & 7u) : (int)((o >> 3) & 15u);
+            worst = std::max(worst, ++count[slot]);
+        }
+        return worst;
+    };
+    std::vector<int> best;
+    int best_cost = 1 << 30;
+    std::vector<int> pick((size_t)L);
+    for (uint32_t mask = 0; mask < (1u << nf); ++mask) {
+        if (__builtin_popcount(mask) != L) continue;
+        int n = 0;
+        for (int i = 0; i < nf; ++i) if (mask >> i & 1) pick[(size_t)n++] = free_bits[(size_t)i];
+        // stores through a CNOT run are 8-byte accesses for complex64 (16 lanes): judged on the 8-byte banks with the L lanes we have
+        int cost = waves(pick, false, wide) * 4;
+        if (store_img) cost += waves(pick, true, g.lv == 0) * 4; else cost += waves(pick, false, wide) * 4;
+        for (int i = 0; i < L; ++i) cost += pick[(size_t)i] > 7 ? 1 : 0;   // mild preference for low bits (ties)
+        if (cost < best_cost) { best_cost = cost; best = pick; }
+    }
+    bool used[16] = {false};
+    int n = 0;
+    for (int b : best) { tb[n++] = b; used[b] = true; }
+    for (int b : free_bits) if (!used[b]) tb[n++] = b;
+}
 
 // affine map of the local index by a CNOT run: j -> A j ^ c(tile)
 struct CxMap {
@@ -138,7 +180,12 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     int last_seg = -1;
     for (int s = 0; s < ns; ++s) {
         const Stage &S = p.stages[B.stage_begin + s];
-        choose_thread_bits(g, S, tbs[s].data());
+        {
+            const bool cx = S.cx_end > S.cx_begin;
+            CxMap cm;
+            if (cx) cm = cx_map(p, B, S, k);
+            choose_thread_bits(g, S, cx ? cm.img : nullptr, tbs[s].data());
+        }
         auto tbit_of = [&](int lb) { for (int i = 0; i < TB; ++i) if (tbs[s][i] == lb) return i; return -1; };
         auto slot_of = [&](int lb) { for (int r = 0; r < R; ++r) if (S.regbit[r] == lb) return r; return -1; };
         for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {

@@ -395,17 +395,19 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 }
                 E("                acc += 2.0 * (double)(s.x + s.y);");
             } else {
-                E("                real si = (real)0;");
+                E("                real si = (real)0; amp s2 = MK((real)0, (real)0);");
+                int nem = 0;
                 for (uint32_t r = 0; r < NR; ++r) {
                     if (r >> pv & 1) continue;
                     const double wx = prec == 0 ? (double)(float)G.wr[r] : G.wr[r], wy = prec == 0 ? (double)(float)G.wi[r] : G.wi[r];
                     if (wx == 0.0 && wy == 0.0) continue;
                     const uint32_t ix = const_index(wx, wy);
-                    if (wy == 0.0) { E("                PAIRR(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 4.0; }
+                    const char *sa = (nem++ & 1) ? "s2" : "s";   // two accumulation chains
+                    if (wy == 0.0) { E("                PAIRR(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 4.0; }
                     else if (wx == 0.0) { E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 3.0; }
-                    else { E("                PAIRC(s, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 6.0; }
+                    else { E("                PAIRC(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 6.0; }
                 }
-                E("                acc += 2.0 * (double)(s.x + s.y + si);");
+                E("                acc += 2.0 * (double)((s.x + s.y) + (s2.x + s2.y) + si);");
             }
             E("            }");
         }
