@@ -87,7 +87,11 @@ typedef struct {
                                * it is not or NVRTC is missing */
     int32_t tiles_per_block;  /* specialised kernels: consecutive tiles one thread block works through (its per-block
                                * set-up is paid once): 0 = default (tuned on the B200), else 1..4096 */
-    int32_t reserved[7];      /* must be 0 */
+    int32_t blocks_per_sm;    /* specialised gate kernels: thread blocks resident per SM the kernels are compiled for
+                               * (register budget 65536 / (256 * blocks_per_sm)): 0 = default, else 2 or 3 */
+    int32_t staged_io;        /* specialised gate kernels: 0 = the first / last stage of a block exchanges its amplitudes with
+                               * global memory directly when it carries no CNOT run, 1 = every tile is staged in shared memory */
+    int32_t reserved[5];      /* must be 0 */
 } gvqe_options;
 /* gvqe_create / gvqe_create_ops with options (opt == NULL: defaults). */
 gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, const gvqe_options *opt,

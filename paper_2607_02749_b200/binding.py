@@ -35,7 +35,8 @@ class GvqeOptions(C.Structure):
     """gvqe_options: how the same energies are computed (0 = library default for every field)."""
     _fields_ = [("tile_bits", C.c_int32), ("fixed_bits", C.c_int32), ("reg_bits", C.c_int32), ("expect_tile_bits", C.c_int32),
                 ("prefix", C.c_int32), ("register_stages", C.c_int32), ("shared_prefix", C.c_int32), ("specialise", C.c_int32),
-                ("tiles_per_block", C.c_int32), ("reserved", C.c_int32 * 7)]
+                ("tiles_per_block", C.c_int32), ("blocks_per_sm", C.c_int32), ("staged_io", C.c_int32),
+                ("reserved", C.c_int32 * 5)]
 
 
 class GvqeOptOptions(C.Structure):

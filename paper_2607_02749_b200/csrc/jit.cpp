@@ -48,8 +48,10 @@ int lpos_of(const Block &B, int q)
 // 16-byte ones) are the lowest thread-index bits: they are given the local bits for which the loads AND the stores of the
 // stage (the stores go through the CNOT map when the stage ends with a run) hit the most distinct bank groups; searched
 // exhaustively (at most C(9,4) subsets).  store_img: image of each local unit vector under the stage's CNOT run, or null.
-void choose_thread_bits(const Geo &g, const Stage &S, const uint32_t *store_img, int *tb)
+void choose_thread_bits(const Geo &g, const Stage &S, const uint32_t *store_img, int *tb, bool direct_load = false, bool direct_store = false)
 {
+    // a stage that exchanges its amplitudes with global memory directly keeps the lowest free local bits in the lanes
+    // (whole 32-byte sectors per request); its global side does not count as shared-memory traffic
     bool isreg[16] = {false};
     for (int s = 0; s < g.R; ++s) isreg[S.regbit[s]] = true;
     std::vector<int> free_bits;
@@ -77,8 +79,17 @@ void choose_thread_bits(const Geo &g, const Stage &S, const uint32_t *store_img,
         int n = 0;
         for (int i = 0; i < nf; ++i) if (mask >> i & 1) pick[(size_t)n++] = free_bits[(size_t)i];
         // stores through a CNOT run are 8-byte accesses for complex64 (16 lanes): judged on the 8-byte banks with the L lanes we have
-        int cost = waves(pick, false, wide) * 4;
-        if (store_img) cost += waves(pick, true, g.lv == 0) * 4; else cost += waves(pick, false, wide) * 4;
+        int cost = direct_load ? 0 : waves(pick, false, wide) * 4;
+        if (direct_store) cost += 0;
+        else if (store_img) cost += waves(pick, true, g.lv == 0) * 4; else cost += waves(pick, false, wide) * 4;
+        if (direct_load || direct_store) {   // the lowest free bits in the lanes: a request is a run of whole 128-byte lines
+            const int need = L;
+            for (int i = 0; i < need && i < nf; ++i) {
+                bool in = false;
+                for (int x = 0; x < L; ++x) in = in || pick[(size_t)x] == free_bits[(size_t)i];
+                if (!in) cost += 64;
+            }
+        }
         for (int i = 0; i < L; ++i) cost += pick[(size_t)i] > 7 ? 1 : 0;   // mild preference for low bits (ties)
         if (cost < best_cost) { best_cost = cost; best = pick; }
     }
@@ -141,7 +152,7 @@ bool jit_supported(const Program &p, int prec, std::string &why)
     return true;
 }
 
-bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string &err)
+bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, JitBlock &out, std::string &err)
 {
     if (bi < 0 || (size_t)bi >= p.blocks.size()) { err = "jit: bad block"; return false; }
     const Block &B = p.blocks[bi];
@@ -172,6 +183,24 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         }
     }
     const int s_first = lead_cx ? 1 : 0;
+    // first / last stage straight from / to global memory (no staging of the tile in shared memory on that side):
+    // possible when the side carries no CNOT run (those are folded into shared-memory addresses)
+    // and when the stage's register bits lie above the lowest 128 bytes of the tile (bit 0 of a complex64 pair aside): the
+    // lanes then cover whole lines (measured: sector-sized requests run at half the rate of the staged copy or worse)
+    auto lines_ok = [&](const Stage &S) {
+        for (int r = 0; r < R; ++r) {
+            const int lb = S.regbit[r];
+            if (g.lv == 1 && r == 0 && lb == 0) continue;
+            if (lb < (g.lv == 1 ? 4 : 3)) return false;
+        }
+        return true;
+    };
+    bool direct_load = false, direct_store = false;
+    if (!staged_io && ns > 0) {
+        direct_load = !lead_cx && !B.source_zero && lines_ok(p.stages[B.stage_begin + s_first]);
+        const Stage &SL = p.stages[B.stage_begin + ns - 1];
+        direct_store = !(SL.cx_end > SL.cx_begin) && (ns - 1 >= s_first) && lines_ok(SL);
+    }
 
     // ---- per-stage geometry and segments
     std::vector<std::vector<int>> tbs((size_t)ns, std::vector<int>(16, 0));
@@ -184,7 +213,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
             const bool cx = S.cx_end > S.cx_begin;
             CxMap cm;
             if (cx) cm = cx_map(p, B, S, k);
-            choose_thread_bits(g, S, cx ? cm.img : nullptr, tbs[s].data());
+            choose_thread_bits(g, S, cx ? cm.img : nullptr, tbs[s].data(), direct_load && s == s_first, direct_store && s == ns - 1);
         }
         auto tbit_of = [&](int lb) { for (int i = 0; i < TB; ++i) if (tbs[s][i] == lb) return i; return -1; };
         auto slot_of = [&](int lb) { for (int r = 0; r < R; ++r) if (S.regbit[r] == lb) return r; return -1; };
@@ -360,7 +389,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     // per_cta: work items (statevector, tile) one thread block handles, consecutive
     // src / src_stride: where the tiles are READ (normally = states / stride; a parameter-shift sweep reads the shared base
     // state of theta, src_stride = 0, and writes the shifted rows' own buffers: SURVEY 8(f) NEXT-2)
-    E("extern \"C\" __global__ void __launch_bounds__(%u, 2) %s(amp *states, u64 stride, const ry4 *rytab, const amp *cstab, int nb, int Pn, int per_cta,", NT, name);
+    E("extern \"C\" __global__ void __launch_bounds__(%u, %d) %s(amp *states, u64 stride, const ry4 *rytab, const amp *cstab, int nb, int Pn, int per_cta,", NT, occupancy == 3 ? 3 : 2, name);
     E("        const amp *src, u64 src_stride)");
     E("{");
     E("    extern __shared__ __align__(128) unsigned char smem[];");
@@ -401,6 +430,18 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         sx += ";";
         E("%s", sx.c_str());
     }
+    auto emit_thread_global = [&](const char *nm, int s) {   // global offset (amplitudes) of the thread's part of the local index in stage s
+        std::string sx = std::string("    const u64 ") + nm + " = 0ull";
+        for (int i = 0; i < TB; ++i) {
+            char b[96];
+            snprintf(b, sizeof b, " | ((u64)((tid >> %d) & 1u) << %d)", i, __builtin_ctzll(scatter(B, 1u << tbs[s][i])));
+            sx += b;
+        }
+        sx += ";";
+        E("%s", sx.c_str());
+    };
+    if (direct_load) emit_thread_global("dl_x", s_first);
+    if (direct_store) emit_thread_global("ds_x", ns - 1);
     if (lead_cx) {
         E("    {   // leading CNOT run: thread part of the permuted destination");
         E("        unsigned ja = 0u;");
@@ -469,6 +510,20 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         }
         E("%s;", oc.c_str());
         for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (lead_o ^ %uu), gsrc + %lluull);", ci_lead[i], (unsigned long long)hi[i]);
+    } else if (direct_load) {
+        const Stage &S = p.stages[B.stage_begin + s_first];
+        const bool wide = (g.lv == 1 && S.regbit[0] == 0);
+        E("        amp a_in[%d];   // the first stage's amplitudes, straight from global memory", NR);
+        E("        {");
+        E("            const amp *gl = src + (u64)b * src_stride + (xbase | dl_x);");
+        for (int r = 0; r < NR; ++r) {
+            uint32_t j = 0;
+            for (int bb = 0; bb < R; ++bb) if (r >> bb & 1) j |= 1u << S.regbit[bb];
+            const unsigned long long go = (unsigned long long)scatter(B, j);
+            if (wide) { if (!(r & 1)) E("            { const float4 v = *(const float4 *)(gl + %lluull); a_in[%d] = MK(v.x, v.y); a_in[%d] = MK(v.z, v.w); }", go, r, r + 1); }
+            else E("            a_in[%d] = gl[%lluull];", r, go);
+        }
+        E("        }");
     } else {
         for (uint32_t i = 0; i < NU; ++i) E("        cp16(tile + (ld_off ^ %uu), gsrc + %lluull);", ci[i], (unsigned long long)hi[i]);
     }
@@ -553,7 +608,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         }
         E("        }");
     }
-    if (!B.source_zero) E("        cp_wait();");
+    if (!B.source_zero && !direct_load) E("        cp_wait();");
     E("        __syncthreads();");
     // ---- stages
     const uint32_t LOMASK = 0x70u;   // address bits the swizzle folds into: XOR there, plain addition everywhere else
@@ -573,8 +628,10 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         E("            const unsigned sb = ((const unsigned *)(smem + %u))[tid];", o_sb[s]);
         // address of register index r = [tile + (sb ^ low bits of its offset)] + the rest of its offset (an immediate)
         for (int v = 0; v < 8; ++v) if (vused[v]) E("            unsigned char *const pv%d = tile + (sb ^ %uu);", v, (uint32_t)v << 4);
-        E("            amp a[%d];", NR);
-        if (wide) {
+        if (direct_load && s == s_first) E("            amp (&a)[%d] = a_in;", NR);
+        else E("            amp a[%d];", NR);
+        if (direct_load && s == s_first) {
+        } else if (wide) {
             for (int r = 0; r < NR; r += 2)
                 E("            { const float4 v = *(const float4 *)(pv%u + %uu); a[%d] = MK(v.x, v.y); a[%d] = MK(v.z, v.w); }", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r, r + 1);
         } else {
@@ -662,7 +719,20 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
             }
             E("            }");
         }
-        if (!has_cx) {
+        if (direct_store && s == ns - 1) {   // results straight to global memory
+            E("            amp *gs = state + (xbase | ds_x);");
+            if (scale_at_store) {
+                E("            const real sc = *s_scale;");
+                for (int r = 0; r < NR; ++r) E("            a[%d] = scal(a[%d], sc);", r, r);
+            }
+            for (int r = 0; r < NR; ++r) {
+                uint32_t j = 0;
+                for (int bb = 0; bb < R; ++bb) if (r >> bb & 1) j |= 1u << S.regbit[bb];
+                const unsigned long long go = (unsigned long long)scatter(B, j);
+                if (wide) { if (!(r & 1)) E("            *(float4 *)(gs + %lluull) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", go, r, r, r + 1, r + 1); }
+                else E("            gs[%lluull] = a[%d];", go, r);
+            }
+        } else if (!has_cx) {
             if (wide) {
                 for (int r = 0; r < NR; r += 2)
                     E("            *(float4 *)(pv%u + %uu) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r, r, r + 1, r + 1);
@@ -720,6 +790,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
         E("        __syncthreads();");
     }
     // ---- store phase
+    if (!direct_store) {
     E("        {");
     if (scale_at_store) E("            const real sc = *s_scale;");
     for (uint32_t i = 0; i < NU; ++i) {
@@ -731,6 +802,7 @@ bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string
     }
     E("        }");
     E("        __syncthreads();   // the tile buffer is reused by the next work item");
+    }
     E("    }");
     E("}");
     {   // arithmetic the block needs per amplitude (ALU roofline): rotations 2, every table / phase factor 4

@@ -32,7 +32,10 @@ struct JitBlock {
 bool jit_supported(const Program &p, int prec, std::string &why);
 
 // Source of the kernel of block `bi`.  prec: 0 = complex64, 1 = complex128.
-bool jit_generate(const Program &p, int bi, int prec, JitBlock &out, std::string &err);
+// occupancy: thread blocks per SM the kernel is compiled for (0 = default).
+// staged_io: every tile goes through shared memory on both sides (otherwise the first / last stage of a block reads /
+// writes global memory directly when it carries no CNOT run).
+bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, JitBlock &out, std::string &err);
 
 // ---- expectation passes (jit_expect.cpp): one kernel per read-only pass of an ExpectPlan ------------------------------
 struct JitExpectData {   // host images of the arrays the kernels read from global memory (uploaded once per Hamiltonian)

@@ -151,6 +151,15 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("#define PAIRC(acc, a, b, t) { const amp be = __ffma2_rn(MK((b).y, (b).y), MK((t).z, (t).w), __fmul2_rn(MK((b).x, (b).x), MK((t).x, (t).y))); acc = __ffma2_rn((a), be, acc); }");
         E("#define PAIRR(acc, a, b, t) { acc = __ffma2_rn((a), __fmul2_rn((b), MK((t).x, (t).x)), acc); }");
         E("#define PAIRI(acci, a, b, t) { acci = fmaf((t).z, fmaf(-(a).y, (b).x, (a).x * (b).y), acci); }");
+        // shared-W forms: sums of a.b (real W), of the cross products (imaginary W), of b.x a and b.y a (complex W)
+        E("#define DOT0(a, b) __fmul2_rn((a), (b))");
+        E("#define DOT(p, a, b) { p = __ffma2_rn((a), (b), p); }");
+        E("#define WRE(acc, p, t) { acc = __ffma2_rn(p, MK((t).x, (t).x), acc); }");
+        E("#define CRS0(a, b) fmaf(-(a).y, (b).x, (a).x * (b).y)");
+        E("#define CRS(p, a, b) { p = fmaf(-(a).y, (b).x, fmaf((a).x, (b).y, p)); }");
+        E("#define WIM(acci, p, t) { acci = fmaf((t).z, p, acci); }");
+        E("#define PAIRS0(p1, p2, a, b) { p1 = __fmul2_rn(MK((b).x, (b).x), (a)); p2 = __fmul2_rn(MK((b).y, (b).y), (a)); }");
+        E("#define WCX(acc, p1, p2, t) { acc = __ffma2_rn(p1, MK((t).x, (t).y), acc); acc = __ffma2_rn(p2, MK((t).z, (t).w), acc); }");
     } else {
         E("typedef double2 tw4;");
         E("__device__ __forceinline__ tw4 twfmt(amp w) { return w; }");
@@ -161,6 +170,14 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("#define PAIRC(acc, a, b, t) { const double br = fma((t).y, (b).y, (t).x * (b).x), bi = fma(-(t).y, (b).x, (t).x * (b).y); acc.x = fma((a).x, br, acc.x); acc.y = fma((a).y, bi, acc.y); }");
         E("#define PAIRR(acc, a, b, t) { acc.x = fma((a).x * (t).x, (b).x, acc.x); acc.y = fma((a).y * (t).x, (b).y, acc.y); }");
         E("#define PAIRI(acci, a, b, t) { acci = fma((t).y, fma(-(a).y, (b).x, (a).x * (b).y), acci); }");
+        E("#define DOT0(a, b) MK((a).x * (b).x, (a).y * (b).y)");
+        E("#define DOT(p, a, b) { p.x = fma((a).x, (b).x, p.x); p.y = fma((a).y, (b).y, p.y); }");
+        E("#define WRE(acc, p, t) { acc.x = fma(p.x, (t).x, acc.x); acc.y = fma(p.y, (t).x, acc.y); }");
+        E("#define CRS0(a, b) fma(-(a).y, (b).x, (a).x * (b).y)");
+        E("#define CRS(p, a, b) { p = fma(-(a).y, (b).x, fma((a).x, (b).y, p)); }");
+        E("#define WIM(acci, p, t) { acci = fma((t).y, p, acci); }");
+        E("#define PAIRS0(p1, p2, a, b) { p1 = MK((b).x * (a).x, (b).x * (a).y); p2 = MK((b).y * (a).x, (b).y * (a).y); }");
+        E("#define WCX(acc, p1, p2, t) { acc.x = fma((t).x, p1.x + p2.y, acc.x); acc.y = fma((t).y, p2.x - p1.y, acc.y); }");
     }
     // W of the cluster groups without tile-dependent terms: entries (Wx, -Wy, Wy, Wx) (complex128: (Wx, Wy)) in constant memory
     std::vector<std::pair<double, double>> wconst;
@@ -232,9 +249,12 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     E("    const u64 total = (u64)nb << %d;", n - k);
     E("    const u64 w_begin = (u64)blockIdx.x * (u64)per_cta;");
     E("    const u64 w_end = w_begin + (u64)per_cta < total ? w_begin + (u64)per_cta : total;");
+    // work items in (tile, statevector) order: the diagonal table's tile stays in L2 for the rows that follow, and the
+    // tile-dependent tables (which do not depend on the state) are built once per tile
+    if (any_dyn) E("    u64 cur_tile = ~0ull;");
     E("    for (u64 w = w_begin; w < w_end; ++w) {");
-    E("        const int b = (int)(w >> %d);", n - k);
-    E("        const u64 tile_id = w & %lluull;", (unsigned long long)((1ull << (n - k)) - 1ull));
+    E("        const u64 tile_id = w / (u64)nb;");
+    E("        const int b = (int)(w - tile_id * (u64)nb);");
     E("        const amp *state = states + (u64)b * stride;");
     {
         E("        u64 xbase = 0ull;");
@@ -264,6 +284,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     }
     // ---- tile-dependent tables
     if (any_dyn) {
+        E("        if (tile_id != cur_tile) {");
+        E("        cur_tile = tile_id;");
         {   // the scratch areas of the tile-dependent groups are contiguous ranges of 16-byte units: a few wide loops
             std::vector<std::pair<uint32_t, uint32_t>> ranges;
             for (uint32_t q = g0; q < g1; ++q) {
@@ -333,6 +355,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             E("        }");
             ++wi;
         }
+        E("        }");
     }
     E("        cp_wait();");
     E("        __syncthreads();");
@@ -396,16 +419,46 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 E("                acc += 2.0 * (double)(s.x + s.y);");
             } else {
                 E("                real si = (real)0; amp s2 = MK((real)0, (real)0);");
-                int nem = 0;
+                // pairs whose W is the same number (index bits the group's terms do not read, equal table entries) are
+                // summed first and multiplied by W once
+                std::map<uint32_t, std::vector<uint32_t>> by_w;
+                std::vector<uint32_t> w_order;
                 for (uint32_t r = 0; r < NR; ++r) {
                     if (r >> pv & 1) continue;
                     const double wx = prec == 0 ? (double)(float)G.wr[r] : G.wr[r], wy = prec == 0 ? (double)(float)G.wi[r] : G.wi[r];
                     if (wx == 0.0 && wy == 0.0) continue;
                     const uint32_t ix = const_index(wx, wy);
+                    if (!by_w.count(ix)) w_order.push_back(ix);
+                    by_w[ix].push_back(r);
+                }
+                int nem = 0;
+                for (uint32_t ix : w_order) {
+                    const std::vector<uint32_t> &rs = by_w[ix];
+                    const double wx = wconst[ix].first, wy = wconst[ix].second;
                     const char *sa = (nem++ & 1) ? "s2" : "s";   // two accumulation chains
-                    if (wy == 0.0) { E("                PAIRR(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 4.0; }
-                    else if (wx == 0.0) { E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 3.0; }
-                    else { E("                PAIRC(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 6.0; }
+                    if (rs.size() == 1) {
+                        const uint32_t r = rs[0];
+                        if (wy == 0.0) { E("                PAIRR(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 4.0; }
+                        else if (wx == 0.0) { E("                PAIRI(si, a[%u], a[%u], WC[%u])", r, r ^ mr, ix); ops_per_thread += 3.0; }
+                        else { E("                PAIRC(%s, a[%u], a[%u], WC[%u])", sa, r, r ^ mr, ix); ops_per_thread += 6.0; }
+                        continue;
+                    }
+                    if (wy == 0.0) {
+                        E("                { amp p = DOT0(a[%u], a[%u]);", rs[0], rs[0] ^ mr);
+                        for (size_t i = 1; i < rs.size(); ++i) E("                  DOT(p, a[%u], a[%u])", rs[i], rs[i] ^ mr);
+                        E("                  WRE(%s, p, WC[%u]) }", sa, ix);
+                        ops_per_thread += 2.0 * (double)rs.size() + 2.0;
+                    } else if (wx == 0.0) {
+                        E("                { real p = CRS0(a[%u], a[%u]);", rs[0], rs[0] ^ mr);
+                        for (size_t i = 1; i < rs.size(); ++i) E("                  CRS(p, a[%u], a[%u])", rs[i], rs[i] ^ mr);
+                        E("                  WIM(si, p, WC[%u]) }", ix);
+                        ops_per_thread += 2.0 * (double)rs.size() + 1.0;
+                    } else {
+                        E("                { amp p1, p2; PAIRS0(p1, p2, a[%u], a[%u])", rs[0], rs[0] ^ mr);
+                        for (size_t i = 1; i < rs.size(); ++i) E("                  pairs(p1, p2, a[%u], a[%u]);", rs[i], rs[i] ^ mr);
+                        E("                  WCX(%s, p1, p2, WC[%u]) }", sa, ix);
+                        ops_per_thread += 4.0 * (double)rs.size() + 4.0;
+                    }
                 }
                 E("                acc += 2.0 * (double)((s.x + s.y) + (s2.x + s2.y) + si);");
             }

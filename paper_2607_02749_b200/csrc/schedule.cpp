@@ -287,9 +287,69 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
     BlockTake bt, best;
     bool first = true;
     const bool zero_first = from_zero;
+    // Every block is one read and one write of the whole state, so the number of blocks is what the tile choice
+    // minimises: a beam search over sequences of tile-bit sets (the greedy sequence is always among the beams' ancestors).
+    std::vector<uint64_t> plan;
+    if (n > k && !ops.empty()) {
+        struct Beam { std::vector<int> pending; std::vector<uint64_t> seq; int nd_left; };
+        auto nd_count = [&](const std::vector<int> &pd) { int c = 0; for (int i : pd) if (!is_diag(ops[i])) ++c; return c; };
+        const size_t WIDTH = 12;
+        std::vector<Beam> beams(1);
+        beams[0].pending = pending; beams[0].nd_left = nd_count(pending);
+        std::vector<char> gone(ops.size());
+        for (int level = 0; level < 4096 && plan.empty(); ++level) {
+            std::vector<Beam> next;
+            for (const Beam &b : beams) {
+                block_candidates(ops, b.pending, n, k, f, cand);
+                for (uint64_t T : cand) {
+                    block_take(ops, b.pending, T, n, bt);
+                    if (bt.taken.empty()) continue;
+                    Beam nb; nb.seq = b.seq; nb.seq.push_back(T);
+                    std::fill(gone.begin(), gone.end(), 0);
+                    for (int idx : bt.taken) gone[idx] = 1;
+                    for (int idx : b.pending) if (!gone[idx]) nb.pending.push_back(idx);
+                    nb.nd_left = b.nd_left - bt.n_nondiag;
+                    if (nb.pending.empty()) { plan = nb.seq; break; }
+                    next.push_back(std::move(nb));
+                }
+                if (!plan.empty()) break;
+            }
+            if (!plan.empty() || next.empty()) break;
+            std::stable_sort(next.begin(), next.end(), [](const Beam &x, const Beam &y) {
+                return x.nd_left != y.nd_left ? x.nd_left < y.nd_left : x.pending.size() < y.pending.size(); });
+            std::vector<Beam> keep;
+            for (Beam &b : next) {
+                bool dup = false;
+                for (const Beam &q : keep) if (q.pending == b.pending) { dup = true; break; }
+                if (!dup) keep.push_back(std::move(b));
+                if (keep.size() >= WIDTH) break;
+            }
+            beams.swap(keep);
+        }
+        // the greedy sequence (most non-diagonal ops per block) is what the search has to beat
+        std::vector<int> pd = pending;
+        size_t greedy_len = 0;
+        while (!pd.empty() && greedy_len < plan.size()) {
+            block_candidates(ops, pd, n, k, f, cand);
+            best.taken.clear(); best.n_nondiag = -1;
+            for (uint64_t T : cand) {
+                block_take(ops, pd, T, n, bt);
+                if (bt.n_nondiag > best.n_nondiag || (bt.n_nondiag == best.n_nondiag && bt.taken.size() > best.taken.size())) best = bt;
+            }
+            if (best.taken.empty()) break;
+            std::fill(gone.begin(), gone.end(), 0);
+            for (int idx : best.taken) gone[idx] = 1;
+            std::vector<int> np;
+            for (int idx : pd) if (!gone[idx]) np.push_back(idx);
+            pd.swap(np);
+            ++greedy_len;
+        }
+        if (pd.empty() && greedy_len <= plan.size()) plan.clear();
+    }
     while (!pending.empty() || first) {
         // ---- choose T
         block_candidates(ops, pending, n, k, f, cand);
+        if (P.blocks.size() < plan.size()) { cand.clear(); cand.push_back(plan[P.blocks.size()]); }
         uint64_t bestT = cand[0];
         best.taken.clear(); best.n_nondiag = -1;
         for (uint64_t T : cand) {

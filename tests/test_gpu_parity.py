@@ -364,13 +364,13 @@ def test_specialised_gate_kernels(orc, n, D, ent, topo, fr, prec, prefix):
     th = np.random.default_rng(n).uniform(-math.pi, math.pi, (5, P))
     th[1, :3] = [math.pi, -math.pi, 0.0]                            # exact quarter turns: cos = 0 up to rounding
     ref = orc.energy_batch(n, ops, th, paulis, coeffs)
-    for spec in (2, 1):
+    for spec, staged in ((2, 0), (2, 1), (1, 0)):   # staged_io = 1: every tile through shared memory on both sides
         g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo, final_rot=fr), precision=prec,
-                    options=dict(specialise=spec, prefix=prefix))
+                    options=dict(specialise=spec, prefix=prefix, staged_io=staged))
         assert (g.kernel_source(0) is not None) == (spec == 2)
         g.set_hamiltonian(paulis, coeffs)
         g.alloc_workspace(3)
-        assert_close(prec, g.energy_batch(th), ref, coeffs, f"specialise={spec}")
+        assert_close(prec, g.energy_batch(th), ref, coeffs, f"specialise={spec} staged_io={staged}")
         assert np.max(np.abs(g.get_state(1) - orc.state(n, ops, th[4]))) < (1e-12 if prec == "c128" else 2e-5)
 
 
@@ -381,7 +381,7 @@ def test_specialised_random_circuits(orc, seed):
     ops, P = random_ops(7100 + seed, n, 160)
     paulis, coeffs = random_paulis(8100 + seed, n, 60, 6)
     th = np.random.default_rng(seed).uniform(-math.pi, math.pi, (4, P))
-    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(specialise=2))
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(specialise=2, staged_io=seed // 3 % 2))
     g.set_hamiltonian(paulis, coeffs)
     g.alloc_workspace(4)
     assert_close(prec, g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, f"specialised random n={n}")

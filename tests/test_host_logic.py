@@ -170,7 +170,13 @@ def test_options_are_validated_and_change_the_schedule():
     assert "k=13" in a.dump_schedule() and "k=10" in b.dump_schedule()
     assert "prefix ops=0" in gv.Gvqe(14, layout=lay, precision="c64", options=dict(prefix=1)).dump_schedule()
     assert "prefix ops=0" not in gv.Gvqe(14, layout=lay, precision="c64", options=dict(prefix=2)).dump_schedule()
-    for bad in (dict(prefix=3), dict(specialise=-1), dict(tile_bits=40), dict(shared_prefix=7)):
+    # the first / last stage of a block goes straight to global memory unless staged_io = 1 asks for the staged copy
+    spec = dict(specialise=2, prefix=1)
+    direct = "".join(gv.Gvqe(16, layout=lay, precision="c64", options=spec).kernel_source(b)[0] for b in range(2))
+    staged = "".join(gv.Gvqe(16, layout=lay, precision="c64", options=dict(spec, staged_io=1)).kernel_source(b)[0] for b in range(2))
+    assert ("a_in[" in direct or "amp *gs =" in direct) and "a_in[" not in staged and "amp *gs =" not in staged
+    assert "__launch_bounds__(256, 3)" in gv.Gvqe(16, layout=lay, precision="c64", options=dict(spec, blocks_per_sm=3)).kernel_source(0)[0]
+    for bad in (dict(prefix=3), dict(specialise=-1), dict(tile_bits=40), dict(shared_prefix=7), dict(blocks_per_sm=4), dict(staged_io=2)):
         with pytest.raises(gv.GvqeError):
             gv.Gvqe(14, layout=lay, precision="c64", options=bad)
     with pytest.raises(gv.GvqeError):
