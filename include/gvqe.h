@@ -171,6 +171,24 @@ gvqe_status gvqe_get_state(gvqe_ctx *ctx, int slot, void *host_out);
  * context's precision, each operation rounded separately.  One read-only sweep of the state on the GPU. */
 gvqe_status gvqe_argmax(gvqe_ctx *ctx, int slot, uint64_t *x, double *prob, void *cuda_stream);
 
+/* The same read-out for callers that may not allocate device memory -- code under CUDA graph capture,
+ * serving loops, harnesses that forbid cudaMalloc.  Needs no context and no workspace; calls no cudaMalloc / cudaFree or
+ * any allocating routine, copies nothing to the host and does not synchronise: two kernel launches on cuda_stream.
+ *   state         DEVICE, n_amplitudes complex numbers (interleaved re, im) of precision prec, 16-byte aligned; read only
+ *   n_amplitudes  1 .. GVQE_NOALLOC_MAX_AMPLITUDES (2^34); anything else is GVQE_ERR_INVALID_ARG
+ *   result        DEVICE, 16 bytes, 8-byte aligned, written by the call: { double prob; uint64_t x; } with the meaning, tie
+ *                 rule and arithmetic of gvqe_argmax (bit-identical to it on the same amplitudes)
+ *   err, err_cap  HOST, optional: receives the message of a failed call (NUL-terminated, truncated to err_cap)
+ * Scratch: the per-block candidates live in a file-scope device array of GVQE_NOALLOC_SCRATCH_BYTES (32 KiB) that every
+ * GPU which loads the library holds until the process exits.  All calls on a device share it and it keeps the last
+ * call's contents (none of which a later call reads): calls that overlap on the GPU -- different streams without an
+ * ordering between them -- race on it; calls on one stream, or ordered by events, are safe.  The first call on a device
+ * looks the array's address up (cudaGetSymbolAddress); make that call before a graph capture starts. */
+#define GVQE_NOALLOC_MAX_AMPLITUDES (1ull << 34)
+#define GVQE_NOALLOC_SCRATCH_BYTES (32u * 1024u)
+gvqe_status gvqe_argmax_noalloc(const void *state, uint64_t n_amplitudes, gvqe_precision prec, void *result,
+                                void *cuda_stream, char *err, size_t err_cap);
+
 /* Shot sampling, PAPER.md:245, 256 ("this state is sampled"; 8192 shots): n_shots (<= 65536 per call) bitstrings
  * distributed as |psi_x|^2 over the state in slot `slot`, by inversion of the cumulative distribution in index
  * order: x[s] = the first x with sum_{y<=x} |psi_y|^2 > u[s] * Z, Z = sum_y |psi_y|^2.  The random numbers are the

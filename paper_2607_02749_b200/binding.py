@@ -22,7 +22,7 @@ STATUS_NAMES = ["GVQE_OK", "GVQE_ERR_INVALID_ARG", "GVQE_ERR_NO_HAMILTONIAN", "G
 EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops_opt", "gvqe_kernel_source", "gvqe_kernel_info", "gvqe_kernel_arrays", "gvqe_compile_kernels", "gvqe_num_params", "gvqe_num_qubits", "gvqe_set_hamiltonian",
            "gvqe_set_hamiltonian_masks", "gvqe_get_grouping", "gvqe_workspace_bytes", "gvqe_set_workspace",
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
-           "gvqe_get_state", "gvqe_argmax", "gvqe_sample", "gvqe_measurement_settings", "gvqe_energy_shots", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
+           "gvqe_get_state", "gvqe_argmax", "gvqe_argmax_noalloc", "gvqe_sample", "gvqe_measurement_settings", "gvqe_energy_shots", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_profile_read_launches", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
            "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
 
@@ -96,6 +96,7 @@ def load():
     L.gvqe_param_shift_grad.argtypes = [vp, vp, vp, vp, vp, vp]
     L.gvqe_get_state.argtypes = [vp, i32, vp]
     L.gvqe_argmax.argtypes = [vp, i32, vp, vp, vp]
+    L.gvqe_argmax_noalloc.argtypes = [vp, u64, i32, vp, vp, C.c_char_p, sz]
     L.gvqe_sample.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     L.gvqe_measurement_settings.argtypes = [vp, vp, vp]
     L.gvqe_energy_shots.argtypes = [vp, i32, i32, vp, vp, vp, vp]
@@ -121,6 +122,19 @@ def load():
     L.gvqe_destroy.restype = None
     _lib = L
     return L
+
+
+NOALLOC_MAX_AMPLITUDES = 1 << 34
+
+
+def argmax_noalloc(state_ptr: int, n_amplitudes: int, precision: str, result_ptr: int, stream=None) -> None:
+    """gvqe_argmax_noalloc: most probable basis state of the n_amplitudes complex numbers at DEVICE address state_ptr,
+    written as {float64 prob, uint64 x} to DEVICE address result_ptr; allocates nothing, does not synchronise."""
+    buf = C.create_string_buffer(256)
+    st = load().gvqe_argmax_noalloc(C.c_void_p(state_ptr), int(n_amplitudes), {"c64": 0, "c128": 1}[precision],
+                                    C.c_void_p(result_ptr), C.c_void_p(stream or 0), buf, len(buf))
+    if st != 0:
+        raise GvqeError(st, buf.value.decode())
 
 
 _ENT = {"cz": 2, "cnot": 3}

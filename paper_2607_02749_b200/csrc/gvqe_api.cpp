@@ -952,6 +952,35 @@ gvqe_status gvqe_argmax(gvqe_ctx *c, int slot, uint64_t *x, double *prob, void *
     return GVQE_OK;
 }
 
+gvqe_status gvqe_argmax_noalloc(const void *state, uint64_t n_amplitudes, gvqe_precision prec, void *result, void *stream,
+                                char *err, size_t err_cap)
+{
+    static_assert(GVQE_NOALLOC_MAX_AMPLITUDES == NOALLOC_MAX_AMPLITUDES && GVQE_NOALLOC_SCRATCH_BYTES == NOALLOC_SCRATCH_BYTES,
+                  "gvqe.h and kernels.h disagree");
+    auto say = [&](gvqe_status s, const char *msg) {
+        if (err && err_cap) snprintf(err, err_cap, "%s", msg);
+        return s;
+    };
+    if (err && err_cap) err[0] = 0;
+    if (prec != GVQE_C64 && prec != GVQE_C128) return say(GVQE_ERR_INVALID_ARG, "argmax_noalloc: precision is neither GVQE_C64 nor GVQE_C128");
+    if (!state || !result) return say(GVQE_ERR_INVALID_ARG, "argmax_noalloc: state and result must be device pointers, not NULL");
+    if (n_amplitudes == 0) return say(GVQE_ERR_INVALID_ARG, "argmax_noalloc: n_amplitudes is 0");
+    if (n_amplitudes > GVQE_NOALLOC_MAX_AMPLITUDES) {
+        char b[160];
+        snprintf(b, sizeof b, "argmax_noalloc: %llu amplitudes exceed the maximum of 2^34 = %llu this entry point takes",
+                 (unsigned long long)n_amplitudes, (unsigned long long)GVQE_NOALLOC_MAX_AMPLITUDES);
+        return say(GVQE_ERR_INVALID_ARG, b);
+    }
+    if (((uintptr_t)state & 15u) || ((uintptr_t)result & 7u)) return say(GVQE_ERR_INVALID_ARG, "argmax_noalloc: state must be 16-byte and result 8-byte aligned");
+    const int ke = launch_argmax_noalloc(prec == GVQE_C64 ? 0 : 1, state, n_amplitudes, result, stream);
+    if (ke) {
+        char b[200];
+        snprintf(b, sizeof b, "argmax_noalloc: CUDA error %d (%s)", ke, cudaGetErrorString((cudaError_t)ke));
+        return say(GVQE_ERR_CUDA, b);
+    }
+    return GVQE_OK;
+}
+
 gvqe_status gvqe_sample(gvqe_ctx *c, int slot, int n_shots, const double *u, uint64_t *x, double *norm, void *stream)
 {
     if (!c || n_shots < 0 || (n_shots > 0 && (!u || !x))) return GVQE_ERR_INVALID_ARG;

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 
 #include "kernels.cuh"
 #include "kernels.h"
@@ -405,6 +406,55 @@ int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, vo
     else argmax_partial_kernel<double><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<double> *)state, count, part + 1);
     argmax_final_kernel<<<1, 256, 0, (cudaStream_t)stream>>>(part + 1, grid, part);
     *launches += 2;
+    return (int)cudaGetLastError();
+}
+
+// ---- the same read-out for callers that may not allocate (gvqe_argmax_noalloc, include/gvqe.h) ----------------------
+// The per-block entries live in a file-scope device array instead of a workspace: NOALLOC_SCRATCH_BYTES on every GPU that
+// loads the library, until the process exits.  Every call on a device shares it and it keeps the last call's contents;
+// nothing in it has to start at zero (the final kernel reads exactly the entries the first kernel of the same call
+// wrote), but two calls that overlap on the GPU (different streams) race on it.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+void *g_noalloc_ptr[NOALLOC_MAX_DEVICES];     // device address of g_noalloc_scratch, per device ordinal
+std::atomic<int> g_noalloc_state[NOALLOC_MAX_DEVICES];   // 0 = not looked up, 1 = ready
+}  // namespace
+
+// Device address of the scratch array on the CURRENT device.  In host code the name g_noalloc_scratch is only a handle
+// for the runtime, not a device address: the address comes from cudaGetSymbolAddress, once per device.
+static int noalloc_scratch_address(void **out)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return (int)cudaErrorInvalidDevice;
+    if (g_noalloc_state[dev].load(std::memory_order_acquire) != 1) {
+        void *ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+        if (e != cudaSuccess) return (int)e;
+        if (!ptr) return (int)cudaErrorInvalidSymbol;
+        g_noalloc_ptr[dev] = ptr;   // concurrent first calls store the same value
+        g_noalloc_state[dev].store(1, std::memory_order_release);
+    }
+    *out = g_noalloc_ptr[dev];
+    return 0;
+}
+
+int launch_argmax_noalloc(int prec, const void *state, uint64_t count, void *result, void *stream)
+{
+    void *scratch = nullptr;
+    const int se = noalloc_scratch_address(&scratch);
+    if (se) return se;
+    const uint64_t nvec = count / (prec == 0 ? 2 : 1);
+    uint32_t grid = (uint32_t)std::min<uint64_t>(READOUT_BLOCKS, (nvec + 255) / 256);   // as launch_argmax: same partition, same result
+    if (grid == 0) grid = 1;
+    static_assert((size_t)READOUT_BLOCKS * sizeof(ProbIdx) <= NOALLOC_SCRATCH_BYTES, "scratch array too small");
+    ProbIdx *part = reinterpret_cast<ProbIdx *>(scratch);
+    if (prec == 0) argmax_partial_kernel<float><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<float> *)state, count, part);
+    else argmax_partial_kernel<double><<<grid, 256, 0, (cudaStream_t)stream>>>((const cx<double> *)state, count, part);
+    argmax_final_kernel<<<1, 256, 0, (cudaStream_t)stream>>>(part, grid, reinterpret_cast<ProbIdx *>(result));
     return (int)cudaGetLastError();
 }
 

@@ -2,6 +2,7 @@
 // the caller's workspace unless stated otherwise; every launcher enqueues on `stream` and returns the CUDA error
 // of the launch (0 = success).  `launches` is incremented by the number of kernels enqueued.
 #pragma once
+#include <stddef.h>
 #include <stdint.h>
 
 #include "devprog.h"
@@ -51,6 +52,11 @@ int launch_table_scatter(int prec, void *table, const uint64_t *z, const double 
 int launch_fwht_pass(int prec, void *table, const TileDesc &td, uint32_t bitmask, int n, void *stream, uint64_t *launches);
 // Most probable basis state of `count` amplitudes; scratch: (READOUT_BLOCKS + 1) * 16 bytes, result {double p, uint64 x} at [0].
 int launch_argmax(int prec, const void *state, uint64_t count, void *scratch, void *stream, uint64_t *launches);
+// The same sweep with its per-block entries in a file-scope device array (kernels.cu): no allocation, no context.
+// result (DEVICE): {double p, uint64 x}.  Returns a cudaError_t value (0 = launched).
+constexpr size_t NOALLOC_SCRATCH_BYTES = 32 * 1024;       // >= READOUT_BLOCKS entries of 16 bytes
+constexpr uint64_t NOALLOC_MAX_AMPLITUDES = 1ull << 34;   // largest statevector the entry point takes
+int launch_argmax_noalloc(int prec, const void *state, uint64_t count, void *result, void *stream);
 // Inverse-CDF sampling: mass = ceil(count / 2^SAMPLE_CHUNK_LOG2) doubles (becomes the exclusive prefix), total = 1 double,
 // u_dev = n_shots uniforms in [0,1), x_dev = n_shots results.
 int launch_sample(int prec, const void *state, uint64_t count, double *mass, double *total, const double *u_dev,
