@@ -31,10 +31,10 @@ struct GInfo {
     int mode = 0;                 // 0 table (lookup), 1 cluster (register stage), 2 direct
     uint32_t E = 0;               // table entries
     uint32_t tab_off = 0;         // byte offset of the final table in shared memory
-    uint32_t scr_off = 0;         // byte offset of the per-tile scratch (dynamic groups): complex entries
     uint32_t wst_off = 0;         // entry offset of the static table in the pass's global array
     bool dyn = false;
     uint32_t pat_begin = 0, pat_end = 0;
+    std::vector<uint32_t> pat_keys; // index pattern (z bits inside the group's index bits) of each of its patterns
     std::vector<double> wr, wi;   // static table (host copy)
     uint32_t zmask = 0;           // index bits any term of the group looks at
 };
@@ -87,7 +87,6 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // clusters: 16-byte entries, and only when a term depends on the tile (otherwise W is a literal in the code)
         if (G.mode == 0) G.tab_off = take(G.E * AB);
         else if (G.dyn) G.tab_off = take(G.E * 16u);
-        G.scr_off = G.dyn ? (G.mode == 1 ? take(G.E * AB) : G.tab_off) : 0;
         G.wst_off = (uint32_t)(data.wst.size() / 2 - wst_base);
         for (uint32_t e = 0; e < G.E; ++e) {   // static part (terms with every Z / Y inside the tile)
             double wr = 0.0, wi = 0.0;
@@ -106,7 +105,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             G.pat_begin = (uint32_t)(data.pats.size() - pat_base);
             for (auto &kv : by_pat) {
                 JitExpectData::Pat pt;
-                pt.dst = G.scr_off + kv.first * AB;
+                pt.dst = kv.first;
+                G.pat_keys.push_back(kv.first);
                 pt.begin = (uint32_t)data.terms.size();
                 for (uint32_t t : kv.second) {
                     const DTerm &tm = plan.terms[t];
@@ -120,6 +120,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     }
     const uint32_t n_pats = (uint32_t)(data.pats.size() - pat_base);
     const uint32_t o_red = take(64 * 8);
+    const uint32_t o_psum = take((n_pats ? n_pats : 1u) * AB);   // per-tile pattern sums S_p
     bool any_dyn = false;
     for (const GInfo &G : gi) any_dyn = any_dyn || G.dyn;
     data.pass_wst_off.push_back((uint32_t)wst_base);
@@ -146,6 +147,10 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // conj(b) a = (b.x a.x + b.y a.y, b.x a.y - b.y a.x)
         E("__device__ __forceinline__ amp cjmul(amp a, amp b) { const amp p = __fmul2_rn(MK(b.x, b.x), a), q = __fmul2_rn(MK(b.y, b.y), a); return MK(p.x + q.y, p.y - q.x); }");
         E("__device__ __forceinline__ amp cadd(amp a, amp b) { return __fadd2_rn(a, b); }");
+        E("__device__ __forceinline__ amp csub(amp a, amp b) { return MK(a.x - b.x, a.y - b.y); }");
+        E("__device__ __forceinline__ amp cneg(amp a) { return MK(-a.x, -a.y); }");
+        // sign flip by a sign-bit mask (0 or 0x80000000)
+        E("__device__ __forceinline__ amp sflip(amp a, unsigned sb) { return MK(__uint_as_float(__float_as_uint(a.x) ^ sb), __uint_as_float(__float_as_uint(a.y) ^ sb)); }");
         // W known when the kernel is generated (constant bank, read through the uniform path -- no shared-memory traffic):
         // complex W three packed operations, real W two, imaginary W three scalar ones
         E("#define PAIRC(acc, a, b, t) { const amp be = __ffma2_rn(MK((b).y, (b).y), MK((t).z, (t).w), __fmul2_rn(MK((b).x, (b).x), MK((t).x, (t).y))); acc = __ffma2_rn((a), be, acc); }");
@@ -167,6 +172,9 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("__device__ __forceinline__ void pairs(amp &s1, amp &s2, amp a, amp b) { s1.x = fma(b.x, a.x, s1.x); s1.y = fma(b.x, a.y, s1.y); s2.x = fma(b.y, a.x, s2.x); s2.y = fma(b.y, a.y, s2.y); }");
         E("__device__ __forceinline__ amp cjmul(amp a, amp b) { return MK(fma(b.y, a.y, b.x * a.x), fma(-b.y, a.x, b.x * a.y)); }");
         E("__device__ __forceinline__ amp cadd(amp a, amp b) { return MK(a.x + b.x, a.y + b.y); }");
+        E("__device__ __forceinline__ amp csub(amp a, amp b) { return MK(a.x - b.x, a.y - b.y); }");
+        E("__device__ __forceinline__ amp cneg(amp a) { return MK(-a.x, -a.y); }");
+        E("__device__ __forceinline__ amp sflip(amp a, unsigned sb) { return MK(__hiloint2double(__double2hiint(a.x) ^ (int)sb, __double2loint(a.x)), __hiloint2double(__double2hiint(a.y) ^ (int)sb, __double2loint(a.y))); }");
         E("#define PAIRC(acc, a, b, t) { const double br = fma((t).y, (b).y, (t).x * (b).x), bi = fma(-(t).y, (b).x, (t).x * (b).y); acc.x = fma((a).x, br, acc.x); acc.y = fma((a).y, bi, acc.y); }");
         E("#define PAIRR(acc, a, b, t) { acc.x = fma((a).x * (t).x, (b).x, acc.x); acc.y = fma((a).y * (t).x, (b).y, acc.y); }");
         E("#define PAIRI(acci, a, b, t) { acci = fma((t).y, fma(-(a).y, (b).x, (a).x * (b).y), acci); }");
@@ -284,20 +292,14 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     }
     // ---- tile-dependent tables
     if (any_dyn) {
+        // Tile-dependent tables, once per tile: T[e] = static[e] + sum over the group's index patterns p of S_p (-1)^{p.e},
+        // S_p = the signed sum of the pattern's terms for this tile.  A group has few patterns (its terms' z masks inside
+        // the index bits), so the sum is taken pattern by pattern instead of by a full Walsh-Hadamard transform: lane l
+        // holds the entries [l EP, (l + 1) EP); a pattern's sign over the lane bits is one parity, its S_p goes to the
+        // accumulator of its in-lane part, and a register Walsh-Hadamard over the in-lane bits (skipping what is known
+        // to be zero when the kernel is generated) finishes the entries.  No shuffles, no shared-memory butterflies.
         E("        if (tile_id != cur_tile) {");
         E("        cur_tile = tile_id;");
-        {   // the scratch areas of the tile-dependent groups are contiguous ranges of 16-byte units: a few wide loops
-            std::vector<std::pair<uint32_t, uint32_t>> ranges;
-            for (uint32_t q = g0; q < g1; ++q) {
-                const GInfo &G = gi[q - g0];
-                if (!G.dyn) continue;
-                const uint32_t b0 = G.scr_off, b1 = (G.scr_off + G.E * AB + 15u) & ~15u;
-                if (!ranges.empty() && ranges.back().second == b0) ranges.back().second = b1; else ranges.push_back({b0, b1});
-            }
-            for (auto &rg : ranges)
-                E("        for (unsigned o = %uu + tid * 16u; o < %uu; o += %uu) *(unit16 *)(smem + o) = unit16{0u, 0u, 0u, 0u};", rg.first, rg.second, NT * 16);
-        }
-        E("        __syncthreads();");
         E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): signed sum of its terms", n_pats, NT);
         E("            const Pat p = pats[i];");
         E("            double sr = 0.0, si = 0.0;");
@@ -306,7 +308,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("                const bool neg = __popcll(xbase & tm.zout) & 1;");
         E("                sr += neg ? -tm.cr : tm.cr; si += neg ? -tm.ci : tm.ci;");
         E("            }");
-        E("            *(amp *)(smem + p.dst) = MK((real)sr, (real)si);");
+        E("            ((amp *)(smem + %u))[i] = MK((real)sr, (real)si);", o_psum);
         E("        }");
         E("        __syncthreads();");
         int wi = 0;
@@ -314,44 +316,32 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             const GInfo &G = gi[q - g0];
             if (!G.dyn) continue;
             const DGroup &dg = plan.groups[q];
-            // Walsh-Hadamard of the scattered pattern sums in registers: lane l holds entries [l EP, (l+1) EP); the rounds
-            // over the in-lane index bits are register butterflies, those over the lane bits take the partner by shuffle
-            // (new = partner + s mine, s = -1 on the lane with the bit set).  Then + static part, formatted for the readers.
             const int ub = (int)dg.ubits, epl = ub > 5 ? ub - 5 : 0, EP = 1 << epl, nlb = ub - epl;
-            if (prec == 1 && ub > 5) {   // complex128, large table: four 32-bit shuffles per entry cost more than the shared-memory butterflies (measured)
-                E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits (shared memory), plus the static part", wi % 8, q - g0, ub);
-                E("            amp *d = (amp *)(smem + %u);", G.scr_off);
-                for (int bit = 0; bit < ub; ++bit) {
-                    E("            for (unsigned i = lane; i < %uu; i += 32u) { const unsigned j = ((i >> %d) << %d) | (i & %uu); const amp u = d[j], v = d[j | %uu]; d[j] = MK(u.x + v.x, u.y + v.y); d[j | %uu] = MK(u.x - v.x, u.y - v.y); }",
-                      G.E / 2, bit, bit + 1, (1u << bit) - 1u, 1u << bit, 1u << bit);
-                    E("            __syncwarp();");
-                }
-                if (G.mode == 1) E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; ((tw4 *)(smem + %u))[e] = twfmt(MK(d[e].x + s.x, d[e].y + s.y)); }", G.E, G.wst_off, G.tab_off);
-                else E("            for (unsigned e = lane; e < %uu; e += 32u) { const amp s = wst[%u + e]; d[e] = MK(d[e].x + s.x, d[e].y + s.y); }", G.E, G.wst_off);
-                E("        }");
-                ++wi;
-                continue;
+            E("        if (warp == %du%s) {   // group %u: %zu patterns over %d index bits", wi % 8, nlb < 5 ? (std::string(" && lane < ") + std::to_string(1u << nlb) + "u").c_str() : "", q - g0, G.pat_keys.size(), ub);
+            E("            const unsigned e0 = lane * %du;", EP);
+            E("            amp st[%d], A[%d];", EP, EP);
+            for (int i = 0; i < EP; ++i) E("            st[%d] = wst[%u + e0 + %d];", i, G.wst_off, i);
+            std::vector<char> nz((size_t)EP, 0);
+            for (size_t j = 0; j < G.pat_keys.size(); ++j) {
+                const uint32_t key = G.pat_keys[j], pl = key & (uint32_t)(EP - 1), ph = key >> epl;
+                std::string sx = "((const amp *)(smem + " + std::to_string(o_psum) + "))[" + std::to_string(G.pat_begin + j) + "]";
+                if (ph) sx = "sflip(" + sx + ", (unsigned)__popc(lane & " + std::to_string(ph) + "u) << 31)";
+                if (nz[pl]) E("            A[%u] = cadd(A[%u], %s);", pl, pl, sx.c_str());
+                else { E("            A[%u] = %s;", pl, sx.c_str()); nz[pl] = 1; }
             }
-            E("        if (warp == %du) {   // group %u: Walsh-Hadamard over its %d index bits, plus the static part", wi % 8, q - g0, ub);
-            E("            const amp *d = (const amp *)(smem + %u);", G.scr_off);
-            E("            const unsigned e0 = (lane & %uu) * %du;", (1u << nlb) - 1u, EP);
-            E("            amp v[%d];", EP);
-            for (int i = 0; i < EP; ++i) E("            v[%d] = d[e0 + %d];", i, i);
             for (int bit = 0; bit < epl; ++bit)
-                for (int i = 0; i < EP; ++i) if (!(i >> bit & 1))
-                    E("            { const amp u = v[%d], w2 = v[%d]; v[%d] = MK(u.x + w2.x, u.y + w2.y); v[%d] = MK(u.x - w2.x, u.y - w2.y); }", i, i | (1 << bit), i, i | (1 << bit));
-            for (int lb = 0; lb < nlb; ++lb) {
-                E("            { const real sg = ((lane >> %d) & 1u) ? (real)-1 : (real)1;", lb);
-                for (int i = 0; i < EP; ++i)
-                    E("              { amp pz; pz.x = __shfl_xor_sync(0xffffffffu, v[%d].x, %d); pz.y = __shfl_xor_sync(0xffffffffu, v[%d].y, %d); v[%d] = MK(fma(sg, v[%d].x, pz.x), fma(sg, v[%d].y, pz.y)); }", i, 1 << lb, i, 1 << lb, i, i, i);
-                E("            }");
-            }
-            E("            if (lane < %uu) {", 1u << nlb);
+                for (int i = 0; i < EP; ++i) {
+                    if (i >> bit & 1) continue;
+                    const int j = i | (1 << bit);
+                    if (nz[i] && nz[j]) E("            { const amp u = A[%d], v = A[%d]; A[%d] = cadd(u, v); A[%d] = csub(u, v); }", i, j, i, j);
+                    else if (nz[i]) { E("            A[%d] = A[%d];", j, i); nz[j] = 1; }
+                    else if (nz[j]) { E("            A[%d] = A[%d]; A[%d] = cneg(A[%d]);", i, j, j, j); nz[i] = 1; }
+                }
             for (int i = 0; i < EP; ++i) {
-                if (G.mode == 1) E("                { const amp s = wst[%u + e0 + %d]; ((tw4 *)(smem + %u))[e0 + %d] = twfmt(MK(v[%d].x + s.x, v[%d].y + s.y)); }", G.wst_off, i, G.tab_off, i, i, i);
-                else E("                { const amp s = wst[%u + e0 + %d]; ((amp *)(smem + %u))[e0 + %d] = MK(v[%d].x + s.x, v[%d].y + s.y); }", G.wst_off, i, G.tab_off, i, i, i);
+                std::string v = nz[i] ? "cadd(A[" + std::to_string(i) + "], st[" + std::to_string(i) + "])" : "st[" + std::to_string(i) + "]";
+                if (G.mode == 1) E("            ((tw4 *)(smem + %u))[e0 + %d] = twfmt(%s);", G.tab_off, i, v.c_str());
+                else E("            ((amp *)(smem + %u))[e0 + %d] = %s;", G.tab_off, i, v.c_str());
             }
-            E("            }");
             E("        }");
             ++wi;
         }
