@@ -532,6 +532,23 @@ gvqe_status ensure_ready(gvqe_ctx *c, cudaStream_t st)
     c->pxd.rot_param = (const int32_t *)(w + L.px_param); c->pxd.cx_t = (const uint8_t *)(w + L.px_t); c->pxd.cx_c = (const uint8_t *)(w + L.px_c);
     c->pxd.n_cx = (int)c->px.cx_t.size(); c->pxd.n_cz = c->px.n_cz; c->pxd.n = c->n_store; c->pxd.kk = std::min(c->n_store, c->prec == GVQE_C64 ? 15 : 14);   // amplitudes one thread block writes: its set-up (product tables) is paid once per 2^kk
     for (int i = 0; i < 4; ++i) { c->pxd.cz_d[i] = c->px.cz_d[i]; c->pxd.cz_m[i] = c->px.cz_m[i]; }
+    {   // images of the offset bits inside a thread block under A^-1 (A = the prefix's CNOT run), as compact indices
+        auto ainv = [&](uint64_t y) {
+            for (int i = (int)c->px.cx_t.size() - 1; i >= 0; --i) y ^= ((y >> c->px.cx_c[i]) & 1ull) << c->px.cx_t[i];
+            return y;
+        };
+        uint64_t img[16] = {0}, vary = 0;
+        for (int b = 0; b < c->pxd.kk; ++b) { img[b] = ainv(1ull << b); vary |= img[b]; }
+        c->pxd.vary = vary; c->pxd.n_vary = __builtin_popcountll(vary);
+        memset(c->pxd.vq, 0, sizeof c->pxd.vq);
+        int j = 0;
+        for (int q = 0; q < 64; ++q) if ((vary >> q) & 1ull) c->pxd.vq[j++] = (uint8_t)q;
+        for (int b = 0; b < 16; ++b) {
+            uint64_t ci = 0;
+            for (int t = 0; t < c->pxd.n_vary; ++t) ci |= ((img[b] >> c->pxd.vq[t]) & 1ull) << t;
+            c->pxd.cimg[b] = ci;
+        }
+    }
     c->d_passes = (DPass *)(w + L.passes); c->d_groups = (DGroup *)(w + L.groups); c->d_terms = (DTerm *)(w + L.terms);
     c->d_wstat = w + L.wstat; c->d_gtabs = (uint32_t *)(w + L.gtabs); c->d_rss = (DRs *)(w + L.rss);
     c->d_diag_z = (uint64_t *)(w + L.dz); c->d_diag_c = (double *)(w + L.dc);

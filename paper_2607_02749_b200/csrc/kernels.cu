@@ -55,14 +55,21 @@ __device__ __forceinline__ uint64_t prefix_ainv(const PrefixDev &pd, uint64_t y)
     return y;
 }
 
-template <typename T>
+// The x bits that differ among the 2^kk amplitudes of one thread block (pd.vary, m = pd.n_vary of them) are numbered
+// 0 .. m-1 ("compact index"); A^-1 is linear, so the compact index of an amplitude is the XOR of the images pd.cimg[b] of
+// the set bits b of its offset inside the thread block.  The product over those m qubits comes from NTAB tables of 256
+// entries (8 compact bits each) rebuilt by every thread block with its own x folded in; the product over the other
+// qubits is one constant per thread block, folded into table 0.  Per amplitude: NTAB lookups, NTAB - 1 multiplications.
+template <typename T, int NTAB>
 __global__ void __launch_bounds__(256, 4)
 init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_t stride, const cx<T> *cs_table, int P)
 {
     __shared__ cx<T> f[40][2];
-    __shared__ cx<T> tab[5][128];
-    __shared__ uint64_t xi[64];
+    __shared__ cx<T> tab[NTAB][256];
+    __shared__ uint64_t cxi[64];
+    __shared__ cx<T> pconst;
     constexpr uint32_t V = 16 / sizeof(cx<T>);
+    constexpr int LV = V == 2 ? 1 : 0;
     const uint32_t tid = threadIdx.x, nthr = blockDim.x;
     const cx<T> *cs = cs_table + (uint64_t)blockIdx.y * P;
     cx<T> *state = states + (uint64_t)blockIdx.y * stride;
@@ -78,43 +85,65 @@ init_product_kernel(const __grid_constant__ PrefixDev pd, cx<T> *states, uint64_
         }
         f[tid][0] = a; f[tid][1] = b;
     }
-    const uint32_t nvec = (1u << pd.kk) / V / nthr;   // vectors per thread
-    if (tid < nvec) xi[tid] = prefix_ainv(pd, (uint64_t)tid * nthr * V);
+    const uint32_t nvec = (1u << pd.kk) / V / nthr;   // vectors per thread (<= 64)
+    const int tbits = 31 - __clz(nthr);                // offset bits [LV, LV + tbits) belong to the thread, the ones above to the vector number
+    if (tid < nvec) {
+        uint64_t c = 0;
+        for (int b = 0; (1u << b) < nvec; ++b) if ((tid >> b) & 1u) c ^= pd.cimg[LV + tbits + b];
+        cxi[tid] = c;
+    }
+    const uint64_t xcta = prefix_ainv(pd, (uint64_t)blockIdx.x << pd.kk);   // x of the thread block's first amplitude
     __syncthreads();
-    const int ngrp = (n + 6) / 7;
-    for (uint32_t e = tid; e < (uint32_t)ngrp * 128u; e += nthr) {
-        const uint32_t g = e >> 7, v = e & 127u;
+    if (tid < 32) {   // product over the qubits whose x bit is the same for the whole thread block
         cx<T> p{T(1), T(0)};
-        for (int j = 0; j < 7 && (int)(7 * g) + j < n; ++j) p = cmul(p, f[7 * g + j][(v >> j) & 1u]);
+        for (int q = (int)tid; q < n; q += 32)
+            if (!((pd.vary >> q) & 1ull)) p = cmul(p, f[q][(xcta >> q) & 1ull]);
+        for (int o = 16; o > 0; o >>= 1) {
+            cx<T> r;
+            r.x = __shfl_xor_sync(0xffffffffu, p.x, o); r.y = __shfl_xor_sync(0xffffffffu, p.y, o);
+            p = cmul(p, r);
+        }
+        if (tid == 0) pconst = p;
+    }
+    __syncthreads();
+    for (uint32_t e = tid; e < (uint32_t)NTAB * 256u; e += nthr) {
+        const uint32_t g = e >> 8, v = e & 255u;
+        cx<T> p = g == 0 ? pconst : cx<T>{T(1), T(0)};
+        for (int j = 0; j < 8 && (int)(8 * g) + j < pd.n_vary; ++j) {
+            const int q = pd.vq[8 * g + j];
+            p = cmul(p, f[q][((xcta >> q) ^ (uint64_t)(v >> j)) & 1ull]);
+        }
         tab[g][v] = p;
     }
-    __syncthreads();
+    uint64_t cthr = 0;
+    for (int b = 0; b < tbits; ++b) if ((tid >> b) & 1u) cthr ^= pd.cimg[LV + b];
+    const uint64_t ce1 = V > 1 ? pd.cimg[0] : 0ull;
+    const bool e_low = (ce1 >> 8) == 0ull;   // the lane-in-vector bit moves table 0 only: the other factors are shared by the vector
     const uint64_t ybase = ((uint64_t)blockIdx.x << pd.kk) | (uint64_t)(tid * V);
-    const uint64_t xthr = prefix_ainv(pd, ybase);
-    const uint64_t xe1 = prefix_ainv(pd, 1ull);
-    // Only the table groups whose index bits move with the vector number or the lane inside a vector need a lookup per
-    // amplitude; the product over the other groups is one factor per thread (the images of those y bits under A^-1 are
-    // the same for every thread: uniform branches).
-    uint64_t moving = V > 1 ? xe1 : 0ull;
-    for (uint32_t i = 0; i < nvec; ++i) moving |= xi[i];
-    cx<T> pc{T(1), T(0)};
-    int ga[5] = {0, 0, 0, 0, 0}, na = 0;   // the groups that need a lookup per amplitude (same for every thread)
-    for (int g = 0; g < ngrp; ++g) {
-        if ((moving >> (7 * g)) & 127ull) ga[na++] = g;
-        else pc = cmul(pc, tab[g][(xthr >> (7 * g)) & 127ull]);
-    }
+    __syncthreads();
     for (uint32_t i = 0; i < nvec; ++i) {
         vec16<T> out;
+        const uint64_t c0 = cthr ^ cxi[i];
+        cx<T> rest{T(1), T(0)};
+        if (NTAB > 1 && e_low) {
+            rest = tab[1][(c0 >> 8) & 255ull];
+#pragma unroll
+            for (int g = 2; g < NTAB; ++g) rest = cmul(rest, tab[g][(c0 >> (8 * g)) & 255ull]);
+        }
 #pragma unroll
         for (uint32_t e = 0; e < V; ++e) {
             const uint64_t y = ybase | ((uint64_t)i * nthr * V) | e;
-            const uint64_t x = xthr ^ xi[i] ^ (e ? xe1 : 0ull);
-            cx<T> p = pc;
+            const uint64_t c = c0 ^ (e ? ce1 : 0ull);
+            cx<T> p = tab[0][c & 255ull];
+            if (NTAB > 1) {
+                if (e_low) p = cmul(p, rest);
+                else {
 #pragma unroll
-            for (int a = 0; a < 5; ++a)
-                if (a < na) p = cmul(p, tab[ga[a]][(x >> (7 * ga[a])) & 127ull]);
+                    for (int g = 1; g < NTAB; ++g) p = cmul(p, tab[g][(c >> (8 * g)) & 255ull]);
+                }
+            }
             int par = 0;
-            for (int c = 0; c < pd.n_cz; ++c) par += __popcll(y & (y >> pd.cz_d[c]) & pd.cz_m[c]);
+            for (int cz = 0; cz < pd.n_cz; ++cz) par += __popcll(y & (y >> pd.cz_d[cz]) & pd.cz_m[cz]);
             out.v[e] = (par & 1) ? cneg(p) : p;
         }
         *reinterpret_cast<vec16<T> *>(state + (ybase | ((uint64_t)i * nthr * V))) = out;
@@ -686,8 +715,21 @@ int launch_init_product(int prec, const PrefixDev &pd, void *states, uint64_t st
 {
     cudaStream_t st = (cudaStream_t)stream;
     dim3 grid((unsigned)(1ull << (pd.n - pd.kk)), (unsigned)batch);
-    if (prec == 0) init_product_kernel<float><<<grid, 256, 0, st>>>(pd, (cx<float> *)states, stride, (const cx<float> *)cs, P);
-    else init_product_kernel<double><<<grid, 256, 0, st>>>(pd, (cx<double> *)states, stride, (const cx<double> *)cs, P);
+    const int ntab = pd.n_vary <= 8 ? 1 : (pd.n_vary + 7) / 8;
+#define GV_INIT(NT)                                                                                                       \
+    do {                                                                                                                  \
+        if (prec == 0) init_product_kernel<float, NT><<<grid, 256, 0, st>>>(pd, (cx<float> *)states, stride, (const cx<float> *)cs, P);      \
+        else init_product_kernel<double, NT><<<grid, 256, 0, st>>>(pd, (cx<double> *)states, stride, (const cx<double> *)cs, P);             \
+    } while (0)
+    switch (ntab) {
+    case 1: GV_INIT(1); break;
+    case 2: GV_INIT(2); break;
+    case 3: GV_INIT(3); break;
+    case 4: GV_INIT(4); break;
+    case 5: GV_INIT(5); break;
+    default: return (int)cudaErrorInvalidConfiguration;
+    }
+#undef GV_INIT
     ++*launches;
     return (int)cudaGetLastError();
 }

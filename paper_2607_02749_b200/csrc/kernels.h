@@ -31,6 +31,12 @@ struct PrefixDev {   // device view of schedule.h Prefix
     int n_cx, n_cz, n, kk;   // kk: log2 of the amplitudes one thread block writes (contiguous)
     int cz_d[4];
     uint64_t cz_m[4];
+    // x = A^-1 y inside one thread block of 2^kk amplitudes: vary = the x bits that differ among them (n_vary <= 40 of them,
+    // numbered in ascending order: vq[j] = the j-th), cimg[b] = image of offset bit b < kk as a compact index over those bits
+    uint64_t vary;
+    int n_vary;
+    uint8_t vq[40];
+    uint64_t cimg[16];
 };
 
 // prec: 0 = complex64 (float), 1 = complex128 (double)
