@@ -186,6 +186,8 @@ def measure(cfg, args, options, rank, world, local, main):
     from workload import make_workload
 
     prec, rows = PREC_OF[cfg], ROWS_PER_STEP[cfg]
+    if main and getattr(args, "rows", 0) > 0:
+        rows = args.rows
     w = make_workload(cfg)
     g = gv.Gvqe(w.n, layout=dict(n_layers=w.D, entangler=w.entangler, topology=w.topology, final_rot=w.final_rot),
                 precision=prec, options=options)
@@ -384,6 +386,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--rows", type=int, default=0, help="statevectors in flight per step for --config (default: ROWS_PER_STEP)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra-configs", action="store_true", help="default config only: skip the 5a / 5b / 3 measurements")
     ap.add_argument("--opt", action="append", default=[], metavar="FIELD=INT",

@@ -91,7 +91,10 @@ typedef struct {
                                * (register budget 65536 / (256 * blocks_per_sm)): 0 = default, else 2 or 3 */
     int32_t staged_io;        /* specialised gate kernels: 0 = the first / last stage of a block exchanges its amplitudes with
                                * global memory directly when it carries no CNOT run, 1 = every tile is staged in shared memory */
-    int32_t reserved[5];      /* must be 0 */
+    int32_t mid_cnot;         /* specialised gate kernels: 0 = a CNOT whose target is a register qubit of its stage is applied in
+                               * registers and rotations may follow it in the same stage (fewer stages), 1 = every CNOT is
+                               * part of a stage's trailing run (the generic kernels' schedule) */
+    int32_t reserved[4];      /* must be 0 */
 } gvqe_options;
 /* gvqe_create / gvqe_create_ops with options (opt == NULL: defaults). */
 gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, const gvqe_options *opt,

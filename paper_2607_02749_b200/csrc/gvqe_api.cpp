@@ -34,6 +34,7 @@ struct gvqe_ctx {
     int K = 0, F = 0, R = 0, KE = 0;   // KE: tile bits of the expectation passes
     std::vector<HostOp> ops;
     Program prog;
+    Program prog_generic;   // when prog carries in-register CNOTs (specialised kernels only): the program dev was lowered from
     DevProgram dev;
     Prefix px;               // product-state prefix of the op list (written, not simulated)
     PrefixDev pxd{};
@@ -115,7 +116,8 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
         bool bad = opt->tile_bits > 14 || opt->fixed_bits > 8 || opt->reg_bits > 5 || opt->expect_tile_bits > 14 || opt->tile_bits < 0 || opt->fixed_bits < 0 || opt->reg_bits < 0 || opt->expect_tile_bits < 0 || opt->prefix < 0 ||
                    opt->prefix > 2 || opt->register_stages < 0 || opt->register_stages > 1 || opt->shared_prefix < 0 ||
                    opt->shared_prefix > 2 || opt->specialise < 0 || opt->specialise > 2 || opt->tiles_per_block < 0 || opt->tiles_per_block > 4096 ||
-                   (opt->blocks_per_sm != 0 && opt->blocks_per_sm != 2 && opt->blocks_per_sm != 3) || opt->staged_io < 0 || opt->staged_io > 1;
+                   (opt->blocks_per_sm != 0 && opt->blocks_per_sm != 2 && opt->blocks_per_sm != 3) || opt->staged_io < 0 || opt->staged_io > 1 ||
+                   opt->mid_cnot < 0 || opt->mid_cnot > 1;
         for (int32_t r : opt->reserved) bad = bad || r != 0;
         if (bad) { delete c; return GVQE_ERR_INVALID_ARG; }
     }
@@ -155,12 +157,30 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
     {
         std::string why;
         const bool want = c->opt.specialise == 2 || (c->opt.specialise == 0 && c->n_store >= 20);
+        if (want && c->opt.mid_cnot == 0) {   // the specialised kernels apply CNOTs on register qubits in registers: fewer stages
+            Program pj;
+            const std::vector<HostOp> rest(c->ops.begin() + c->px.n_ops, c->ops.end());
+            if (compile_program(c->n_store, rest, c->K, c->F, c->R, pj, err, c->px.n_ops == 0, true) && pj.blocks.size() == c->prog.blocks.size() &&
+                pj.stages.size() < c->prog.stages.size() && jit_supported(pj, c->prec, why)) {
+                if (c->px.n_ops > 0) {
+                    std::vector<int> eo;
+                    for (int i = 0; i < c->px.n_ops; ++i) eo.push_back(i);
+                    for (int e : pj.exec_order) eo.push_back(e + c->px.n_ops);
+                    pj.exec_order.swap(eo);
+                }
+                c->prog_generic = c->prog;   // c->dev (the generic kernels' program) stays the lowering of this one
+                c->prog = pj;
+            }
+        }
         if (want && c->prog.blocks.size() == c->dev.blocks.size() && jit_supported(c->prog, c->prec, why)) {
             c->jit_blocks.resize(c->prog.blocks.size());
             for (size_t b = 0; b < c->prog.blocks.size(); ++b)
                 if (!jit_generate(c->prog, (int)b, c->prec, c->opt.blocks_per_sm, c->opt.staged_io != 0, c->jit_blocks[b], why)) { c->jit_blocks.clear(); break; }
         }
-        if (c->jit_blocks.empty()) c->jit_state = -1;
+        if (c->jit_blocks.empty()) {
+            c->jit_state = -1;
+            if (!c->prog_generic.blocks.empty()) { c->prog = c->prog_generic; c->prog_generic = Program(); }
+        }
     }
     *out = c;
     return GVQE_OK;

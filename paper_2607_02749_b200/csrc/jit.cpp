@@ -220,6 +220,7 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
         for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
             const MicroOp &m = p.mops[oi];
             if (m.kind == MOP_RY) { idx_of(ryp, m.param); stage_items[s].push_back((int)oi); continue; }
+            if (m.kind == MOP_CX) { stage_items[s].push_back((int)oi); continue; }
             const DiagSeg &ds = p.segs[m.param];
             SegInfo si;
             si.stage = s;
@@ -268,7 +269,7 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
         const std::vector<int> &it = stage_items[st];
         ry_defer[st].assign(it.size(), -1);
         for (size_t i = 0; i < it.size(); ++i) {
-            if (it[i] < 0) continue;
+            if (it[i] < 0 || p.mops[it[i]].kind != MOP_RY) continue;
             const int sl = p.mops[it[i]].a;
             for (size_t j = i + 1; j < it.size(); ++j) {
                 if (it[j] >= 0) { if (p.mops[it[j]].a == sl) break; continue; }
@@ -637,8 +638,31 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
         } else {
             for (int r = 0; r < NR; ++r) E("            a[%d] = *(const amp *)(pv%u + %uu);", r, (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK);
         }
+        // logical register index (the amplitude's true index bits) -> name in a[]: a CNOT between two register qubits only
+        // renames; one whose control is a thread or tile bit swaps the target pairs where the control is set
+        std::vector<int> perm((size_t)NR);
+        for (int r = 0; r < NR; ++r) perm[(size_t)r] = r;
+        auto tbit_of_stage = [&](int lb) { for (int i = 0; i < TB; ++i) if (tbs[s][i] == lb) return i; return -1; };
         for (size_t ii = 0; ii < stage_items[s].size(); ++ii) {
             const int item = stage_items[s][ii];
+            if (item >= 0 && p.mops[item].kind == MOP_CX) {
+                const MicroOp &m = p.mops[item];
+                const int t = m.a;
+                if (m.c == CTL_REG) {
+                    E("            // CNOT target slot %d, control slot %d: renamed", t, m.b);
+                    for (int r = 0; r < NR; ++r) if ((r >> m.b & 1) && !(r >> t & 1)) std::swap(perm[(size_t)r], perm[(size_t)(r | (1 << t))]);
+                } else {
+                    const int lb = lpos_of(B, m.b);
+                    if (lb >= 0) E("            {   // CNOT target slot %d, control qubit %d (a thread bit)\n                const bool cxc = (tid >> %d) & 1u;", t, m.b, tbit_of_stage(lb));
+                    else E("            {   // CNOT target slot %d, control qubit %d (outside the tile)\n                const bool cxc = (xbase >> %d) & 1ull;", t, m.b, m.b);
+                    for (int r = 0; r < NR; ++r) if (!(r >> t & 1)) {
+                        const int i0 = perm[(size_t)r], i1 = perm[(size_t)(r | (1 << t))];
+                        E("                { const amp u = a[%d], v = a[%d]; a[%d] = cxc ? v : u; a[%d] = cxc ? u : v; }", i0, i1, i0, i1);
+                    }
+                    E("            }");
+                }
+                continue;
+            }
             if (item >= 0) {
                 const MicroOp &m = p.mops[item];
                 const int yi = idx_of(ryp, m.param), sl = m.a;
@@ -646,9 +670,9 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
                 E("            {   // R_y on slot %d (parameter %d)%s", sl, m.param, ry_defer[s][ii] >= 0 ? "; sine-form sign joins the next segment" : "");
                 E("                const amp q = s_ry[%d];", yi);
                 E("                if (q.y == (real)0) {");
-                for (int r = 0; r < NR; ++r) if (!(r >> sl & 1)) E("                    ryc(a[%d], a[%d], q.x);", r, r | (1 << sl));
+                for (int r = 0; r < NR; ++r) if (!(r >> sl & 1)) E("                    ryc(a[%d], a[%d], q.x);", perm[r], perm[r | (1 << sl)]);
                 E("                } else {");
-                for (int r = 0; r < NR; ++r) if (!(r >> sl & 1)) E("                    %s(a[%d], a[%d], q.x);", sine, r, r | (1 << sl));
+                for (int r = 0; r < NR; ++r) if (!(r >> sl & 1)) E("                    %s(a[%d], a[%d], q.x);", sine, perm[r], perm[r | (1 << sl)]);
                 E("                }");
                 E("            }");
                 continue;
@@ -690,9 +714,9 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
             if (nlo == 0) {
                 if (any_ph) {
                     E("                const tw t0 = twmake(ph);");
-                    for (int r = 0; r < NR; ++r) E("                a[%d] = %s(a[%d], t0);", r, (si.x_neg >> r & 1) ? "cmulTn" : "cmulT", r);
+                    for (int r = 0; r < NR; ++r) E("                a[%d] = %s(a[%d], t0);", perm[r], (si.x_neg >> r & 1) ? "cmulTn" : "cmulT", perm[r]);
                 } else if (si.x_neg) {
-                    for (int r = 0; r < NR; ++r) if (si.x_neg >> r & 1) E("                a[%d] = cneg(a[%d]);", r, r);
+                    for (int r = 0; r < NR; ++r) if (si.x_neg >> r & 1) E("                a[%d] = cneg(a[%d]);", perm[r], perm[r]);
                 }
             } else {
                 E("                tw tl[%d];", 1 << nlo);
@@ -707,14 +731,14 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
                 }
                 auto tidx = [&](int r, int from, int cnt) { int v = 0; for (int i = 0; i < cnt; ++i) if (r >> si.active[from + i] & 1) v |= 1 << i; return v; };
                 for (int r = 0; r < NR; ++r)
-                    E("                a[%d] = %s(a[%d], tl[%d]);", r, (si.x_neg >> r & 1) ? "cmulTn" : "cmulT", r, tidx(r, 0, nlo));
+                    E("                a[%d] = %s(a[%d], tl[%d]);", perm[r], (si.x_neg >> r & 1) ? "cmulTn" : "cmulT", perm[r], tidx(r, 0, nlo));
                 if (nhi > 0) {
                     E("                tw th[%d];", 1 << nhi);
                     for (int e = 0; e < (1 << nhi); ++e) {
                         E("                th[%d] = ((const tw *)(smem + %u))[%d];", e, o_tab[q], 8 + e);
                         if (flips_any && !sign_expr(e, nlo, nhi).empty()) E("                th[%d] = twscale(th[%d], %s);", e, e, sign_expr(e, nlo, nhi).c_str());
                     }
-                    for (int r = 0; r < NR; ++r) E("                a[%d] = cmulT(a[%d], th[%d]);", r, r, tidx(r, nlo, nhi));
+                    for (int r = 0; r < NR; ++r) E("                a[%d] = cmulT(a[%d], th[%d]);", perm[r], perm[r], tidx(r, nlo, nhi));
                 }
             }
             E("            }");
@@ -729,15 +753,15 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
                 uint32_t j = 0;
                 for (int bb = 0; bb < R; ++bb) if (r >> bb & 1) j |= 1u << S.regbit[bb];
                 const unsigned long long go = (unsigned long long)scatter(B, j);
-                if (wide) { if (!(r & 1)) E("            *(float4 *)(gs + %lluull) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", go, r, r, r + 1, r + 1); }
-                else E("            gs[%lluull] = a[%d];", go, r);
+                if (wide) { if (!(r & 1)) E("            *(float4 *)(gs + %lluull) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", go, perm[r], perm[r], perm[r + 1], perm[r + 1]); }
+                else E("            gs[%lluull] = a[%d];", go, perm[r]);
             }
         } else if (!has_cx) {
             if (wide) {
                 for (int r = 0; r < NR; r += 2)
-                    E("            *(float4 *)(pv%u + %uu) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r, r, r + 1, r + 1);
+                    E("            *(float4 *)(pv%u + %uu) = make_float4(a[%d].x, a[%d].y, a[%d].x, a[%d].y);", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, perm[r], perm[r], perm[r + 1], perm[r + 1]);
             } else {
-                for (int r = 0; r < NR; ++r) E("            *(amp *)(pv%u + %uu) = a[%d];", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, r);
+                for (int r = 0; r < NR; ++r) E("            *(amp *)(pv%u + %uu) = a[%d];", (cr[r] & LOMASK) >> 4, cr[r] & ~LOMASK, perm[r]);
             }
         } else {
             // trailing CNOT run: |j> -> |A j ^ c>; the amplitude of local index j_thread ^ j_r goes to
@@ -772,7 +796,7 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
                     bool v2[8] = {false};
                     for (int r = 0; r < NR; ++r) v2[((c2[r] ^ cv) & LOMASK) >> 4] = true;
                     for (int v = 0; v < 8; ++v) if (v2[v]) E("                unsigned char *const pw%d = tile + (sb2 ^ %uu);", v, (uint32_t)v << 4);
-                    for (int r = 0; r < NR; ++r) E("                *(amp *)(pw%u + %uu) = a[%d];", ((c2[r] ^ cv) & LOMASK) >> 4, (c2[r] ^ cv) & ~LOMASK, r);
+                    for (int r = 0; r < NR; ++r) E("                *(amp *)(pw%u + %uu) = a[%d];", ((c2[r] ^ cv) & LOMASK) >> 4, (c2[r] ^ cv) & ~LOMASK, perm[r]);
                     E("            }");
                 }
             } else {
@@ -783,7 +807,7 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
                     oc += bb;
                 }
                 E("%s;", oc.c_str());
-                for (int r = 0; r < NR; ++r) E("            *(amp *)(tile + (sb3 ^ %uu)) = a[%d];", c2[r], r);
+                for (int r = 0; r < NR; ++r) E("            *(amp *)(tile + (sb3 ^ %uu)) = a[%d];", c2[r], perm[r]);
             }
         }
         E("        }");
@@ -809,7 +833,7 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
         double ops = 0.0;
         for (int s2 = s_first; s2 < ns; ++s2)
             for (int item : stage_items[s2]) {
-                if (item >= 0) { ops += 2.0; continue; }
+                if (item >= 0) { if (p.mops[item].kind == MOP_RY) ops += 2.0; continue; }
                 const SegInfo &si = segs[-item - 1];
                 const bool any_ph = si.has_phth || si.has_tc || si.has_tm;
                 if (si.nlo > 0 || any_ph) ops += 4.0;

@@ -116,7 +116,7 @@ constexpr int MAX_SEG_OPS = 96;    // RZ + CZ entries merged into one diagonal s
 constexpr int MAX_STAGE_ND = 64;   // RY/CNOT micro-ops per stage
 constexpr int MAX_STAGE_SEG = 12;  // diagonal segments per stage
 
-struct StageItem { bool is_seg; int op; std::vector<int> seg_ops; };  // op / seg_ops index the block's op list
+struct StageItem { bool is_seg; int op; std::vector<int> seg_ops; bool mid_cx = false; };  // op / seg_ops index the block's op list; mid_cx: a CNOT applied in registers
 
 struct StageTake {
     std::vector<StageItem> items;
@@ -128,8 +128,10 @@ struct StageTake {
 
 // bops: the block's ops in execution order; L: positions (into bops) still to run; carry: pending diagonals.
 // Rset: register qubits (global ids).  flush_anywhere: allow a diagonal flush after a non-diagonal op of this stage.
+// mid_cx: a CNOT whose target is a register qubit is applied in registers where it stands (its control may be anywhere)
+// and rotations may follow it; without it a CNOT always starts the stage's trailing run.
 void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, const std::vector<int> &carry_in,
-                uint64_t Rset, bool flush_anywhere, StageTake &out)
+                uint64_t Rset, bool flush_anywhere, bool mid_cx, StageTake &out)
 {
     out.items.clear(); out.rest.clear(); out.n_nondiag = 0; out.n_seg = 0; out.has_cx = false;
     std::vector<int> pend = carry_in;
@@ -167,8 +169,9 @@ void stage_take(const std::vector<HostOp> &bops, const std::vector<int> &L, cons
                     pend.clear(); pend_touch = 0;
                 }
                 StageItem it; it.is_seg = false; it.op = pos;
+                it.mid_cx = o.kind == 3 && mid_cx && !out.has_cx && (Rset >> o.q0 & 1);
+                if (o.kind == 3 && !it.mid_cx) { out.has_cx = true; cx_touch |= (1ull << o.q0) | (1ull << o.q1); }
                 out.items.push_back(std::move(it)); ++out.n_nondiag;
-                if (o.kind == 3) { out.has_cx = true; cx_touch |= (1ull << o.q0) | (1ull << o.q1); }
             }
         } else {
             out.rest.push_back(pos);
@@ -265,7 +268,7 @@ Prefix find_prefix(int n, const std::vector<HostOp> &ops)
 }
 
 bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &P, std::string &err,
-                     bool from_zero)
+                     bool from_zero, bool mid_cx)
 {
     P = Program();
     if (n < 1 || n > 40) { err = "schedule: bad qubit count"; return false; }
@@ -384,6 +387,54 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
         std::vector<uint64_t> rc;
         StageTake st, sbest;
         uint32_t max_seg = 0;
+        // Every stage is one trip of the tile through shared memory: a beam search over (register set, flush mode)
+        // sequences looks for the fewest stages (ties: the greedy score summed); the greedy choice is always a candidate.
+        std::vector<std::pair<uint64_t, int>> stage_plan;
+        {
+            struct SB { std::vector<int> L, carry; std::vector<std::pair<uint64_t, int>> seq; double score; };
+            auto has_nd = [&](const std::vector<int> &v) { for (int pos : v) if (!is_diag(bops[pos])) return true; return false; };
+            const size_t WIDTH = 8;
+            std::vector<SB> beams(1);
+            beams[0].L = L; beams[0].score = 0.0;
+            bool found = false;
+            std::vector<std::pair<uint64_t, int>> best_seq;
+            double best_score = -1e30;
+            int best_extra = 2;
+            for (int depth = 0; depth < 64 && !found && has_nd(beams[0].L); ++depth) {
+                std::vector<SB> next;
+                for (const SB &b : beams) {
+                    if (!has_nd(b.L)) continue;
+                    stage_candidates(bops, b.L, T, k, R, rc);
+                    for (uint64_t rs : rc) for (int fa = 0; fa < 2; ++fa) {
+                        stage_take(bops, b.L, b.carry, rs, fa != 0, mid_cx, st);
+                        if (st.n_nondiag == 0) continue;
+                        SB nb2; nb2.L = st.rest; nb2.carry = st.carry; nb2.seq = b.seq; nb2.seq.push_back({rs, fa});
+                        nb2.score = b.score + st.n_nondiag - 0.1 * st.n_seg - 0.01 * conflict_penalty(T, rs, k);
+                        if (!has_nd(nb2.L)) {   // finished: maybe one closing stage for what is left of the diagonals
+                            const int extra = (nb2.L.empty() && (nb2.carry.empty() || !st.has_cx)) ? 0 : 1;
+                            if (extra < best_extra || (extra == best_extra && nb2.score > best_score)) { best_extra = extra; best_score = nb2.score; best_seq = nb2.seq; }
+                            found = true;
+                        } else next.push_back(std::move(nb2));
+                    }
+                }
+                if (found && best_extra == 1 && !next.empty()) {
+                    // a sequence one stage longer without a closing stage costs the same: keep what we have (fewer launches of code)
+                }
+                if (found || next.empty()) break;
+                std::stable_sort(next.begin(), next.end(), [](const SB &x, const SB &y) {
+                    return x.L.size() != y.L.size() ? x.L.size() < y.L.size() : x.score > y.score; });
+                std::vector<SB> keep;
+                for (SB &b : next) {
+                    bool dup = false;
+                    for (const SB &q : keep) if (q.L == b.L && q.carry == b.carry) { dup = true; break; }
+                    if (!dup) keep.push_back(std::move(b));
+                    if (keep.size() >= WIDTH) break;
+                }
+                beams.swap(keep);
+            }
+            if (found) stage_plan = best_seq;
+        }
+        size_t plan_pos = 0;
         while (!L.empty() || !carry.empty()) {
             bool any_nd = false;
             for (int pos : L) if (!is_diag(bops[pos])) { any_nd = true; break; }
@@ -399,13 +450,17 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
             } else {
                 stage_candidates(bops, L, T, k, R, rc);
                 double bscore = -1e30;
+                const bool planned = plan_pos < stage_plan.size();
+                if (planned) { rc.clear(); rc.push_back(stage_plan[plan_pos].first); }
                 for (uint64_t rs : rc) for (int fa = 0; fa < 2; ++fa) {
-                    stage_take(bops, L, carry, rs, fa != 0, st);
+                    if (planned && fa != stage_plan[plan_pos].second) continue;
+                    stage_take(bops, L, carry, rs, fa != 0, mid_cx, st);
                     if (st.n_nondiag == 0) continue;
                     const double score = st.n_nondiag - 0.1 * st.n_seg - 0.01 * conflict_penalty(T, rs, k);
                     if (score > bscore) { bscore = score; sbest = st; Rset = rs; }
                 }
                 if (bscore < -1e29) { err = "schedule: stage made no progress (internal)"; return false; }
+                ++plan_pos;
                 if (sbest.rest.empty() && !sbest.carry.empty() && !sbest.has_cx) {  // last stage of the block: flush what is pending
                     StageItem s; s.is_seg = true; s.op = -1; s.seg_ops = sbest.carry;
                     sbest.items.push_back(s); sbest.carry.clear();
@@ -447,7 +502,12 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                     const HostOp &o = bops[it.op];
                     P.exec_order.push_back(best.taken[it.op]);
                     if (o.kind == 0) { m.kind = MOP_RY; m.a = (uint8_t)slot_of(o.q0); m.param = o.param; }
-                    else { P.cxs.push_back(StageCx{(uint8_t)o.q0, (uint8_t)o.q1}); continue; }
+                    else if (it.mid_cx) {
+                        m.kind = MOP_CX; m.a = (uint8_t)slot_of(o.q0);
+                        const int cs = slot_of(o.q1);
+                        if (cs != 255) { m.b = (uint8_t)cs; m.c = CTL_REG; } else { m.b = (uint8_t)o.q1; m.c = CTL_FIXED; }
+                        m.param = -1;
+                    } else { P.cxs.push_back(StageCx{(uint8_t)o.q0, (uint8_t)o.q1}); continue; }
                 }
                 P.mops.push_back(m);
             }
@@ -496,6 +556,7 @@ std::string dump_program(const Program &p)
             for (uint32_t oi = S.op_begin; oi < S.op_end; ++oi) {
                 const MicroOp &m = p.mops[oi];
                 if (m.kind == MOP_RY) snprintf(buf, sizeof buf, " RY(s%d,p%d)", m.a, m.param);
+                else if (m.kind == MOP_CX) snprintf(buf, sizeof buf, m.c == CTL_REG ? " cx(s%d,c=s%d)" : " cx(s%d,c=q%d)", m.a, m.b);
                 else {
                     const DiagSeg &g = p.segs[m.param];
                     snprintf(buf, sizeof buf, " DIAG(#%d rz=%u cz=%u)", m.param, g.rz_end - g.rz_begin, g.cz_end - g.cz_begin);

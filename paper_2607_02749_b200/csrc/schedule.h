@@ -32,8 +32,11 @@ struct Program {
 
 // Compile.  Returns false and sets err on failure (never throws).
 // from_zero: the first block starts from |0...0> without reading (false when a product-state prefix wrote the state).
+// mid_cx: CNOTs whose target is a register qubit of the stage are applied in registers (MOP_CX micro-ops) and rotations
+// may follow them in the same stage -- fewer stages on CNOT ansaetze; only the specialised kernels (jit.cpp) run such
+// programs, the generic kernel needs mid_cx = false (every CNOT in a trailing run).
 bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R, Program &out, std::string &err,
-                     bool from_zero = true);
+                     bool from_zero = true, bool mid_cx = false);
 
 // Product-state prefix: the leading run of single-qubit rotations followed by the run of entanglers
 // that comes before the next rotation.  RZ RY |0> on every qubit is a product state, CZ multiplies it by a sign, a

@@ -364,13 +364,17 @@ def test_specialised_gate_kernels(orc, n, D, ent, topo, fr, prec, prefix):
     th = np.random.default_rng(n).uniform(-math.pi, math.pi, (5, P))
     th[1, :3] = [math.pi, -math.pi, 0.0]                            # exact quarter turns: cos = 0 up to rounding
     ref = orc.energy_batch(n, ops, th, paulis, coeffs)
-    for spec, staged in ((2, 0), (2, 1), (1, 0)):   # staged_io = 1: every tile through shared memory on both sides
+    # staged_io = 1: every tile through shared memory on both sides; mid_cnot = 1: every CNOT in a trailing run (the
+    # default applies CNOTs on register qubits in registers and lets rotations follow them in the same stage)
+    for spec, staged, mid in ((2, 0, 0), (2, 1, 0), (2, 0, 1), (1, 0, 0)):
         g = gv.Gvqe(n, layout=dict(n_layers=D, entangler=ent, topology=topo, final_rot=fr), precision=prec,
-                    options=dict(specialise=spec, prefix=prefix, staged_io=staged))
+                    options=dict(specialise=spec, prefix=prefix, staged_io=staged, mid_cnot=mid))
         assert (g.kernel_source(0) is not None) == (spec == 2)
+        if mid == 1 or spec == 1:
+            assert " cx(" not in g.dump_schedule()
         g.set_hamiltonian(paulis, coeffs)
         g.alloc_workspace(3)
-        assert_close(prec, g.energy_batch(th), ref, coeffs, f"specialise={spec} staged_io={staged}")
+        assert_close(prec, g.energy_batch(th), ref, coeffs, f"specialise={spec} staged_io={staged} mid_cnot={mid}")
         assert np.max(np.abs(g.get_state(1) - orc.state(n, ops, th[4]))) < (1e-12 if prec == "c128" else 2e-5)
 
 
