@@ -194,7 +194,7 @@ namespace {
 // local bit position of global qubit q inside tile-bit set T
 inline int local_pos(uint64_t T, int q) { return __builtin_popcountll(T & ((1ull << q) - 1)); }
 
-void stage_candidates(const std::vector<HostOp> &bops, const std::vector<int> &L, uint64_t T, int k, int R,
+void stage_candidates(const std::vector<HostOp> &bops, const std::vector<int> &L, uint64_t T, int k, int R, bool mid_cx,
                       std::vector<uint64_t> &cand)
 {
     cand.clear();
@@ -214,6 +214,22 @@ void stage_candidates(const std::vector<HostOp> &bops, const std::vector<int> &L
     }
     for (int p = 0; p < k && cnt < R; ++p) if (!(s >> tq[p] & 1)) { s |= 1ull << tq[p]; ++cnt; }
     if (std::find(cand.begin(), cand.end(), s) == cand.end()) cand.push_back(s);
+    if (!mid_cx) return;
+    // with CNOTs in registers their targets count as needed qubits too: the first R of them, and the same skipping the
+    // first one, two, ... (a stage that starts further down the dependency chain)
+    std::vector<int> order;
+    uint64_t seen = 0;
+    for (int pos : L) {
+        const HostOp &o = bops[pos];
+        if ((o.kind == 0 || o.kind == 3) && (T >> o.q0 & 1) && !(seen >> o.q0 & 1)) { seen |= 1ull << o.q0; order.push_back(o.q0); }
+    }
+    for (size_t p = 0; p < order.size() && p < 8; ++p) {
+        uint64_t w = 0; int c = 0;
+        for (size_t j = p; j < order.size() && c < R; ++j) { w |= 1ull << order[j]; ++c; }
+        for (size_t j = 0; j < p && c < R; ++j) { w |= 1ull << order[j]; ++c; }
+        for (int q = 0; q < k && c < R; ++q) if (!(w >> tq[q] & 1)) { w |= 1ull << tq[q]; ++c; }
+        if (std::find(cand.begin(), cand.end(), w) == cand.end()) cand.push_back(w);
+    }
 }
 
 // bank-conflict proxy for the swizzle phys = j ^ ((j >> 4) & 15): lanes vary the lowest 4 non-register local bits;
@@ -404,7 +420,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                 std::vector<SB> next;
                 for (const SB &b : beams) {
                     if (!has_nd(b.L)) continue;
-                    stage_candidates(bops, b.L, T, k, R, rc);
+                    stage_candidates(bops, b.L, T, k, R, mid_cx, rc);
                     for (uint64_t rs : rc) for (int fa = 0; fa < 2; ++fa) {
                         stage_take(bops, b.L, b.carry, rs, fa != 0, mid_cx, st);
                         if (st.n_nondiag == 0) continue;
@@ -448,7 +464,7 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                 sbest.items.push_back(s);
                 int cnt = 0; for (int q = 0; q < n && cnt < R; ++q) if (T >> q & 1) { Rset |= 1ull << q; ++cnt; }
             } else {
-                stage_candidates(bops, L, T, k, R, rc);
+                stage_candidates(bops, L, T, k, R, mid_cx, rc);
                 double bscore = -1e30;
                 const bool planned = plan_pos < stage_plan.size();
                 if (planned) { rc.clear(); rc.push_back(stage_plan[plan_pos].first); }
