@@ -314,3 +314,24 @@ def test_shared_prefix_gradient_is_bit_identical(orc, cfg, n, D, prec, in_flight
     scale = np.sum(np.abs(w.coeffs))
     tol_ = 1e-10 * scale if prec == "c128" else 2e-5 * scale
     assert abs(E0 - E0_o) <= tol_ and np.max(np.abs(dE - dE_o)) <= tol_
+
+
+def test_profile_read_launches_lists_every_kernel_of_a_chunk():
+    """gvqe_profile_enable / gvqe_profile_read_launches (what bench.py's per-kernel rooflines are measured with): one
+    entry per launch of an energy chunk in execution order -- prefix kernel (if any), gate blocks, expectation passes --
+    mean within [min, max], and their sums stay below the class totals of gvqe_profile_read."""
+    w = make_workload(3, n=20, M=200, D=2, batch=4)
+    g = ctx(w, "c64", in_flight=4)
+    g.energy_batch(w.params)
+    g.profile_enable(True)
+    for _ in range(3):
+        g.energy_batch(w.params)
+    mean, lo, hi = g.profile_read_launches()
+    tot = g.profile_read()
+    n_gate, n_pass, _ = g.schedule_info()
+    assert len(mean) == n_gate + n_pass and tot["chunks"] == 3
+    assert np.all(lo <= mean + 1e-9) and np.all(mean <= hi + 1e-9) and np.all(lo > 0.0)
+    # the class totals bracket a whole phase (launch gaps included), the per-launch figures only the kernels
+    assert 0.5 * tot["gate_ms"] <= mean[:n_gate].sum() * 3 <= 1.02 * tot["gate_ms"]
+    assert 0.5 * tot["expect_ms"] <= mean[n_gate:].sum() * 3 <= 1.02 * tot["expect_ms"]
+    g.profile_enable(False)

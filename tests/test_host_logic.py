@@ -202,3 +202,25 @@ def test_specialised_kernels_generate_and_compile(cfg, prec):
         raise
     # small registers keep the generic kernels unless asked
     assert gv.Gvqe(12, layout=dict(n_layers=1, entangler="cz", topology="linear")).kernel_source(0) is None
+
+
+def test_kernel_info_counts_the_schedules_arithmetic():
+    """gvqe_kernel_info: FP lane operations per amplitude of a generated gate kernel = 2 per rotation + 4 per complex
+    table factor of its diagonal segments (the numerator of bench.py's ALU roofline): at least 2 x its rotations, and
+    the blocks of one circuit together carry every R_y of the op list exactly once."""
+    import re
+    n, D = 20, 2
+    g = gv.Gvqe(n, layout=dict(n_layers=D, entangler="cnot", topology="ring"), precision="c64", options=dict(prefix=1))
+    nb = g.schedule_info()[0]
+    blocks = re.split(r"\nblock ", g.dump_schedule())[1:nb + 1]
+    total_ry = 0
+    for b in range(nb):
+        info = g.kernel_info(b)
+        n_ry = blocks[b].count(" RY(")
+        total_ry += n_ry
+        assert info["kind"] == "gate" and info["smem_bytes"] == g.kernel_source(b)[1]
+        assert info["fp_ops_per_amp"] >= 2.0 * n_ry and info["fp_ops_per_amp"] <= 2.0 * n_ry + 8.0 * (blocks[b].count(" DIAG(") + 1)
+    assert total_ry == n * (D + 1) and g.kernel_info(nb) is None
+    g.set_hamiltonian(["X" * 2 + "I" * (n - 2), "Z" * n], [0.5, 0.25])
+    x = g.kernel_info(nb)
+    assert x["kind"] == "expect" and x["fp_ops_per_amp"] > 0.0
