@@ -94,7 +94,10 @@ typedef struct {
     int32_t mid_cnot;         /* specialised gate kernels: 0 = a CNOT whose target is a register qubit of its stage is applied in
                                * registers and rotations may follow it in the same stage (fewer stages), 1 = every CNOT is
                                * part of a stage's trailing run (the generic kernels' schedule) */
-    int32_t reserved[4];      /* must be 0 */
+    int32_t interleave;       /* specialised gate kernels: thread blocks in groups of this many (a power of two <= 1024) take
+                               * neighbouring tiles at the same time: 0 = default (32, tuned on the B200), 1 = consecutive tiles per
+                               * thread block */
+    int32_t reserved[3];      /* must be 0 */
 } gvqe_options;
 /* gvqe_create / gvqe_create_ops with options (opt == NULL: defaults). */
 gvqe_status gvqe_create_opt(int n_qubits, const gvqe_layout *layout, gvqe_precision prec, const gvqe_options *opt,

@@ -36,7 +36,7 @@ class GvqeOptions(C.Structure):
     _fields_ = [("tile_bits", C.c_int32), ("fixed_bits", C.c_int32), ("reg_bits", C.c_int32), ("expect_tile_bits", C.c_int32),
                 ("prefix", C.c_int32), ("register_stages", C.c_int32), ("shared_prefix", C.c_int32), ("specialise", C.c_int32),
                 ("tiles_per_block", C.c_int32), ("blocks_per_sm", C.c_int32), ("staged_io", C.c_int32),
-                ("mid_cnot", C.c_int32), ("reserved", C.c_int32 * 4)]
+                ("mid_cnot", C.c_int32), ("interleave", C.c_int32), ("reserved", C.c_int32 * 3)]
 
 
 class GvqeOptOptions(C.Structure):

@@ -117,7 +117,8 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
                    opt->prefix > 2 || opt->register_stages < 0 || opt->register_stages > 1 || opt->shared_prefix < 0 ||
                    opt->shared_prefix > 2 || opt->specialise < 0 || opt->specialise > 2 || opt->tiles_per_block < 0 || opt->tiles_per_block > 4096 ||
                    (opt->blocks_per_sm != 0 && opt->blocks_per_sm != 2 && opt->blocks_per_sm != 3) || opt->staged_io < 0 || opt->staged_io > 1 ||
-                   opt->mid_cnot < 0 || opt->mid_cnot > 1;
+                   opt->mid_cnot < 0 || opt->mid_cnot > 1 ||
+                   opt->interleave < 0 || opt->interleave > 1024 || (opt->interleave & (opt->interleave - 1)) != 0;
         for (int32_t r : opt->reserved) bad = bad || r != 0;
         if (bad) { delete c; return GVQE_ERR_INVALID_ARG; }
     }
@@ -175,7 +176,7 @@ gvqe_status build_ctx(int n, const std::vector<HostOp> &ops, int n_params, gvqe_
         if (want && c->prog.blocks.size() == c->dev.blocks.size() && jit_supported(c->prog, c->prec, why)) {
             c->jit_blocks.resize(c->prog.blocks.size());
             for (size_t b = 0; b < c->prog.blocks.size(); ++b)
-                if (!jit_generate(c->prog, (int)b, c->prec, c->opt.blocks_per_sm, c->opt.staged_io != 0, c->jit_blocks[b], why)) { c->jit_blocks.clear(); break; }
+                if (!jit_generate(c->prog, (int)b, c->prec, c->opt.blocks_per_sm, c->opt.staged_io != 0, c->opt.interleave ? c->opt.interleave : 32, c->jit_blocks[b], why)) { c->jit_blocks.clear(); break; }
         }
         if (c->jit_blocks.empty()) {
             c->jit_state = -1;

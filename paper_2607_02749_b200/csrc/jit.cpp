@@ -152,7 +152,7 @@ bool jit_supported(const Program &p, int prec, std::string &why)
     return true;
 }
 
-bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, JitBlock &out, std::string &err)
+bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, int interleave, JitBlock &out, std::string &err)
 {
     if (bi < 0 || (size_t)bi >= p.blocks.size()) { err = "jit: bad block"; return false; }
     const Block &B = p.blocks[bi];
@@ -460,9 +460,16 @@ bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged
     }
     E("    int cur_b = -1;");
     E("    const u64 total = (u64)nb << %d;", n - k);
-    E("    const u64 w_begin = (u64)blockIdx.x * (u64)per_cta;");
-    E("    const u64 w_end = w_begin + (u64)per_cta < total ? w_begin + (u64)per_cta : total;");
-    E("    for (u64 w = w_begin; w < w_end; ++w) {");
+    // thread blocks in groups of IL take neighbouring tiles at the same time (their 128-byte pieces are adjacent in memory);
+    // a group that would run past the end falls back to consecutive tiles per thread block
+    const unsigned IL = interleave > 1 ? (unsigned)interleave : 1u;
+    E("    const u64 il_base = (u64)(blockIdx.x / %uu) * (u64)per_cta * %uull;", IL, IL);
+    E("    const bool il = il_base + (u64)per_cta * %uull <= total;", IL);
+    E("    const u64 w_first = il ? il_base + (u64)(blockIdx.x %% %uu) : (u64)blockIdx.x * (u64)per_cta;", IL);
+    E("    const u64 w_step = il ? %uull : 1ull;", IL);
+    E("    for (int it = 0; it < per_cta; ++it) {");
+    E("        const u64 w = w_first + (u64)it * w_step;");
+    E("        if (w >= total) break;");
     E("        const int b = (int)(w >> %d);", n - k);
     E("        const u64 tile_id = w & %lluull;", (unsigned long long)((1ull << (n - k)) - 1ull));
     E("        amp *state = states + (u64)b * stride;");

@@ -35,7 +35,8 @@ bool jit_supported(const Program &p, int prec, std::string &why);
 // occupancy: thread blocks per SM the kernel is compiled for (0 = default).
 // staged_io: every tile goes through shared memory on both sides (otherwise the first / last stage of a block reads /
 // writes global memory directly when it carries no CNOT run).
-bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, JitBlock &out, std::string &err);
+// interleave: thread blocks in groups of this many (a power of two) take neighbouring tiles at the same time (0, 1: off).
+bool jit_generate(const Program &p, int bi, int prec, int occupancy, bool staged_io, int interleave, JitBlock &out, std::string &err);
 
 // ---- expectation passes (jit_expect.cpp): one kernel per read-only pass of an ExpectPlan ------------------------------
 struct JitExpectData {   // host images of the arrays the kernels read from global memory (uploaded once per Hamiltonian)

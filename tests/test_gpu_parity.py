@@ -385,7 +385,7 @@ def test_specialised_random_circuits(orc, seed):
     ops, P = random_ops(7100 + seed, n, 160)
     paulis, coeffs = random_paulis(8100 + seed, n, 60, 6)
     th = np.random.default_rng(seed).uniform(-math.pi, math.pi, (4, P))
-    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(specialise=2, staged_io=seed // 3 % 2))
+    g = gv.Gvqe(n, ops=ops, n_params=P, precision=prec, options=dict(specialise=2, staged_io=seed // 3 % 2, interleave=(0, 1, 4)[seed % 3]))
     g.set_hamiltonian(paulis, coeffs)
     g.alloc_workspace(4)
     assert_close(prec, g.energy_batch(th), orc.energy_batch(n, ops, th, paulis, coeffs), coeffs, f"specialised random n={n}")
