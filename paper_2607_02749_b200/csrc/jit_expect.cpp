@@ -77,6 +77,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     const uint32_t o_tile = take((uint32_t)AB << k);
     const size_t wst_base = data.wst.size() / 2;
     const size_t pat_base = data.pats.size();
+    const size_t term_base = data.terms.size();   // the tile-dependent terms of this pass follow, pattern after pattern
     for (uint32_t q = g0; q < g1; ++q) {
         const DGroup &dg = plan.groups[q];
         GInfo &G = gi[q - g0];
@@ -121,6 +122,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     const uint32_t n_pats = (uint32_t)(data.pats.size() - pat_base);
     const uint32_t o_red = take(64 * 8);
     const uint32_t o_psum = take((n_pats ? n_pats : 1u) * AB);   // per-tile pattern sums S_p
+    const uint32_t n_pterms = (uint32_t)(data.terms.size() - term_base);
+    const uint32_t o_sv = take((n_pterms ? n_pterms : 1u) * 16u);     // per-tile signed coefficients of those terms (fp64 pairs)
     bool any_dyn = false;
     for (const GInfo &G : gi) any_dyn = any_dyn || G.dyn;
     data.pass_wst_off.push_back((uint32_t)wst_base);
@@ -300,14 +303,16 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // to be zero when the kernel is generated) finishes the entries.  No shuffles, no shared-memory butterflies.
         E("        if (tile_id != cur_tile) {");
         E("        cur_tile = tile_id;");
-        E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): signed sum of its terms", n_pats, NT);
+        E("        for (unsigned t = tid; t < %uu; t += %uu) {   // one thread per term: its coefficient with this tile's sign", n_pterms, NT);
+        E("            const Term tm = terms[%zuu + t];", term_base);
+        E("            const bool neg = __popcll(xbase & tm.zout) & 1;");
+        E("            ((double2 *)(smem + %u))[t] = make_double2(neg ? -tm.cr : tm.cr, neg ? -tm.ci : tm.ci);", o_sv);
+        E("        }");
+        E("        __syncthreads();");
+        E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): sum of its terms, in their order", n_pats, NT);
         E("            const Pat p = pats[i];");
         E("            double sr = 0.0, si = 0.0;");
-        E("            for (unsigned t = p.begin; t < p.end; ++t) {");
-        E("                const Term tm = terms[t];");
-        E("                const bool neg = __popcll(xbase & tm.zout) & 1;");
-        E("                sr += neg ? -tm.cr : tm.cr; si += neg ? -tm.ci : tm.ci;");
-        E("            }");
+        E("            for (unsigned t = p.begin; t < p.end; ++t) { const double2 v = ((const double2 *)(smem + %u))[t - %zuu]; sr += v.x; si += v.y; }", o_sv, term_base);
         E("            ((amp *)(smem + %u))[i] = MK((real)sr, (real)si);", o_psum);
         E("        }");
         E("        __syncthreads();");
@@ -584,10 +589,12 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     }
     // ---- deterministic block sum
     E("        for (int o = 16; o > 0; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);");
-    E("        if (lane == 0) red[warp] = acc;");
+    // one barrier per work item: it frees the tile and the tables for the next item and publishes the warps' sums, which
+    // alternate between two sets of slots (thread 0 has read a set long before it is written again, two items later)
+    E("        double *const redw = red + (unsigned)(w & 1ull) * %uu;", NT / 32);
+    E("        if (lane == 0) redw[warp] = acc;");
     E("        __syncthreads();");
-    E("        if (tid == 0) { double s = 0.0; for (int i = 0; i < %u; ++i) s += red[i]; partial[(u64)b * slots_per_b + slot_off + tile_id] = s; }", NT / 32);
-    E("        __syncthreads();   // tile, tables and red are reused by the next work item");
+    E("        if (tid == 0) { double s = 0.0; for (int i = 0; i < %u; ++i) s += redw[i]; partial[(u64)b * slots_per_b + slot_off + tile_id] = s; }", NT / 32);
     E("    }");
     E("}");
     if (P.with_diag) ops_per_thread += 4.0 * NR;   // |psi|^2 E(x): three multiply-adds and one multiply per amplitude
