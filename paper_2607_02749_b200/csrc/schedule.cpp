@@ -79,7 +79,7 @@ int count_runs(uint64_t T)
 
 // candidate tile-bit sets: [0,f) + every contiguous window of k-f qubits + "first needed" set
 void block_candidates(const std::vector<HostOp> &ops, const std::vector<int> &pending, int n, int k, int f,
-                      std::vector<uint64_t> &cand)
+                      std::vector<uint64_t> &cand, bool two_windows = false)
 {
     cand.clear();
     if (n <= k) { cand.push_back((1ull << n) - 1); return; }
@@ -103,6 +103,16 @@ void block_candidates(const std::vector<HostOp> &ops, const std::vector<int> &pe
             if (pass == 1 || adj) { T |= 1ull << q; ++cnt; }
         }
     if (count_runs(T) <= MAX_RUNS && std::find(cand.begin(), cand.end(), T) == cand.end()) cand.push_back(T);
+    if (!two_windows) return;
+    // two windows (h1 + h2 = h qubits): two fronts of a layered circuit advance in one block
+    for (int h1 = 2; h1 <= h - 2; ++h1) {
+        const int h2 = h - h1;
+        for (int a = f; a + h1 <= n; ++a)
+            for (int b = a + h1 + 1; b + h2 <= n; ++b) {
+                const uint64_t W = low | (((1ull << h1) - 1) << a) | (((1ull << h2) - 1) << b);
+                if (std::find(cand.begin(), cand.end(), W) == cand.end()) cand.push_back(W);
+            }
+    }
 }
 
 }  // namespace
@@ -310,16 +320,18 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
     // minimises: a beam search over sequences of tile-bit sets (the greedy sequence is always among the beams' ancestors).
     std::vector<uint64_t> plan;
     if (n > k && !ops.empty()) {
+      std::vector<char> gone(ops.size());
+      auto search = [&](bool two_windows) {
+        std::vector<uint64_t> plan;
         struct Beam { std::vector<int> pending; std::vector<uint64_t> seq; int nd_left; };
         auto nd_count = [&](const std::vector<int> &pd) { int c = 0; for (int i : pd) if (!is_diag(ops[i])) ++c; return c; };
         const size_t WIDTH = 12;
         std::vector<Beam> beams(1);
         beams[0].pending = pending; beams[0].nd_left = nd_count(pending);
-        std::vector<char> gone(ops.size());
         for (int level = 0; level < 4096 && plan.empty(); ++level) {
             std::vector<Beam> next;
             for (const Beam &b : beams) {
-                block_candidates(ops, b.pending, n, k, f, cand);
+                block_candidates(ops, b.pending, n, k, f, cand, two_windows);
                 for (uint64_t T : cand) {
                     block_take(ops, b.pending, T, n, bt);
                     if (bt.taken.empty()) continue;
@@ -344,6 +356,14 @@ bool compile_program(int n, const std::vector<HostOp> &ops, int k, int f, int R,
                 if (keep.size() >= WIDTH) break;
             }
             beams.swap(keep);
+        }
+        return plan;
+      };
+        // tile sets of one window first; two windows only when that saves a block (more runs per tile otherwise)
+        plan = search(false);
+        {
+            const std::vector<uint64_t> plan2 = search(true);
+            if (!plan2.empty() && (plan.empty() || plan2.size() < plan.size())) plan = plan2;
         }
         // the greedy sequence (most non-diagonal ops per block) is what the search has to beat
         std::vector<int> pd = pending;
