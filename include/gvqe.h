@@ -282,9 +282,13 @@ typedef struct {
     int32_t patience;       /* p_block = p_global of Eq. 14 (paper: 12) */
     int32_t epoch_patience; /* p_epoch (paper: 3) */
     int32_t lbfgs_memory;   /* correction pairs kept (>= 1) */
-    int32_t reserved;
-    double tol;             /* eps_tol of Eq. 14 and the epoch-level improvement threshold (paper: 1e-4) */
+    int32_t optimizer;      /* PAPER.md:221 "both derivative-free (COBYLA) and gradient-based (L-BFGS-B)": 0 = L-BFGS on
+                             * parameter-shift gradients, 1 = COBYLA (linear-approximation simplex method, no gradients;
+                             * block_iters / global_iters then bound the energy evaluations after the first simplex) */
+    double tol;             /* eps_tol of Eq. 14 and the epoch-level improvement threshold (paper: 1e-4); also COBYLA's
+                             * final trust-region radius rho_end (SciPy's tol) */
     double f_tol;           /* L-BFGS relative decrease tolerance; g_tol = 0.1 f_tol */
+    double rho_beg;         /* COBYLA: first trust-region radius in radians; 0 = 1.0 (SciPy's default rhobeg) */
 } gvqe_opt_options;
 
 typedef struct {
@@ -294,7 +298,7 @@ typedef struct {
 } gvqe_opt_result;
 
 /* Graph-VQE epochs: from theta*_best, every block minimises Eq. 11 over its own parameters
- * (L-BFGS, parameter-shift gradients, Eq. 13) starting from the same vector, the block solutions are fused, a
+ * (L-BFGS on parameter-shift gradients, Eq. 13, or COBYLA: opt->optimizer) starting from the same vector, the block solutions are fused, a
  * global refinement over all parameters follows, the best vector is kept, and the run stops after epoch_patience
  * epochs without an improvement larger than tol.  Blocks run one after another on this GPU (the paper's worker
  * pool is out of scope).  params: P doubles in/out; history (optional): energy before the first epoch and after
@@ -302,6 +306,17 @@ typedef struct {
 gvqe_status gvqe_graph_vqe_minimize(gvqe_ctx *ctx, const gvqe_opt_options *opt, const int32_t *community,
                                     double *params, gvqe_opt_result *result, double *history, int32_t history_cap,
                                     int32_t *history_len, void *cuda_stream);
+
+/* The derivative-free minimiser of the loop above on a caller-supplied function (HOST only, no GPU; used by the CPU
+ * tests to compare it with SciPy's COBYLA): minimises f over x (n doubles, in/out).  f(rows, B, out, user) receives B
+ * points of n coordinates (row-major, HOST) and writes out[B]; a non-zero return aborts.  rho_beg >= rho_end > 0: first
+ * and last trust-region radius; max_evals: evaluation budget.  *f_best (optional) = f at the returned x; counts
+ * (optional, 6 x int32): evaluations, trust-region steps, geometry steps, radius reductions, simplex rebuilds,
+ * improving steps.  *reason (optional): 0 = rho_end reached, 1 = evaluation budget.  The method: PAPER.md:214, 221 name
+ * COBYLA; Powell's linear-approximation method without constraints, see csrc/cobyla.cpp. */
+typedef int (*gvqe_batch_fn)(const double *rows, int32_t n_rows, double *out, void *user);
+gvqe_status gvqe_cobyla_minimize(int32_t n, double *x, double rho_beg, double rho_end, int32_t max_evals, gvqe_batch_fn f,
+                                 void *user, double *f_best, int32_t *counts, int32_t *reason);
 
 const char *gvqe_last_error(const gvqe_ctx *ctx);
 void gvqe_destroy(gvqe_ctx *ctx);

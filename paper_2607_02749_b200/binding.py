@@ -24,7 +24,7 @@ EXPORTS = ["gvqe_create", "gvqe_create_ops", "gvqe_create_opt", "gvqe_create_ops
            "gvqe_set_max_in_flight", "gvqe_energy_batch", "gvqe_energy_batch_device", "gvqe_param_shift_grad",
            "gvqe_get_state", "gvqe_argmax", "gvqe_argmax_noalloc", "gvqe_sample", "gvqe_measurement_settings", "gvqe_energy_shots", "gvqe_schedule_info", "gvqe_dump_schedule", "gvqe_get_exec_order", "gvqe_launch_count",
            "gvqe_profile_enable", "gvqe_profile_read", "gvqe_profile_read_launches", "gvqe_interaction_graph", "gvqe_modularity", "gvqe_louvain",
-           "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_last_error", "gvqe_destroy"]
+           "gvqe_merge_small_blocks", "gvqe_geometric_blocks", "gvqe_block_param_mask", "gvqe_graph_vqe_minimize", "gvqe_cobyla_minimize", "gvqe_last_error", "gvqe_destroy"]
 
 
 class GvqeLayout(C.Structure):
@@ -42,7 +42,11 @@ class GvqeOptions(C.Structure):
 class GvqeOptOptions(C.Structure):
     _fields_ = [("max_epochs", C.c_int32), ("block_iters", C.c_int32), ("global_iters", C.c_int32),
                 ("window", C.c_int32), ("patience", C.c_int32), ("epoch_patience", C.c_int32),
-                ("lbfgs_memory", C.c_int32), ("reserved", C.c_int32), ("tol", C.c_double), ("f_tol", C.c_double)]
+                ("lbfgs_memory", C.c_int32), ("optimizer", C.c_int32), ("tol", C.c_double), ("f_tol", C.c_double),
+                ("rho_beg", C.c_double)]
+
+
+_BATCH_FN = C.CFUNCTYPE(C.c_int, C.POINTER(C.c_double), C.c_int32, C.POINTER(C.c_double), C.c_void_p)
 
 
 class GvqeOptResult(C.Structure):
@@ -116,6 +120,7 @@ def load():
     L.gvqe_block_param_mask.argtypes = [vp, vp, i32, vp]
     L.gvqe_geometric_blocks.argtypes = [i32, i32, i32, vp, vp]
     L.gvqe_graph_vqe_minimize.argtypes = [vp, C.POINTER(GvqeOptOptions), vp, vp, C.POINTER(GvqeOptResult), vp, i32, vp, vp]
+    L.gvqe_cobyla_minimize.argtypes = [i32, vp, C.c_double, C.c_double, i32, _BATCH_FN, vp, vp, vp, vp]
     L.gvqe_last_error.argtypes = [vp]
     L.gvqe_last_error.restype = C.c_char_p
     L.gvqe_destroy.argtypes = [vp]
@@ -382,14 +387,16 @@ class Gvqe:
         return m[:self.P]
 
     def graph_vqe_minimize(self, params, community, *, max_epochs=10, block_iters=50, global_iters=50, window=40,
-                           patience=12, epoch_patience=3, lbfgs_memory=8, tol=1e-4, f_tol=1e-9, stream: int = 0):
-        """Returns (params_best, result dict, history array).  Defaults are the paper's settings."""
+                           patience=12, epoch_patience=3, lbfgs_memory=8, tol=1e-4, f_tol=1e-9, optimizer="lbfgs", rho_beg=0.0,
+                           stream: int = 0):
+        """Returns (params_best, result dict, history array).  Defaults are the paper's settings (PAPER.md:256);
+        optimizer: "lbfgs" or "cobyla" (PAPER.md:221)."""
         p = np.array(params, dtype=np.float64).reshape(-1)
         c = np.ascontiguousarray(community, dtype=np.int32)
         if len(p) != self.P or len(c) != self.n:
             raise GvqeError(GVQE_ERR_INVALID_ARG, "params / community size")
-        opt = GvqeOptOptions(max_epochs, block_iters, global_iters, window, patience, epoch_patience, lbfgs_memory, 0,
-                             tol, f_tol)
+        opt = GvqeOptOptions(max_epochs, block_iters, global_iters, window, patience, epoch_patience, lbfgs_memory,
+                             {"lbfgs": 0, "cobyla": 1}[optimizer], tol, f_tol, rho_beg)
         res = GvqeOptResult()
         hist = np.zeros(max_epochs + 1, dtype=np.float64)
         hl = C.c_int32(0)
@@ -401,6 +408,29 @@ class Gvqe:
 def _graph_check(st: int, what: str):
     if st != GVQE_OK:
         raise GvqeError(st, what)
+
+
+def cobyla_minimize(fun, x0, rho_beg: float = 1.0, rho_end: float = 1e-4, max_evals: int = 1000):
+    """gvqe_cobyla_minimize on a Python callable fun(rows[B, n]) -> values[B] (host only).  Returns (x, f_best, counts dict, reason)."""
+    x = np.array(x0, dtype=np.float64).reshape(-1)
+    n = len(x)
+
+    def cb(rows, B, out, _user):
+        try:
+            pts = np.ctypeslib.as_array(rows, shape=(B * max(n, 1),))[:B * n].reshape(B, n)
+            vals = np.asarray(fun(pts.copy()), dtype=np.float64).reshape(B)
+            for b in range(B):
+                out[b] = vals[b]
+            return 0
+        except Exception:
+            return 1
+
+    fb, reason = C.c_double(0.0), C.c_int32(0)
+    counts = (C.c_int32 * 6)()
+    _graph_check(load().gvqe_cobyla_minimize(n, x.ctypes.data, float(rho_beg), float(rho_end), int(max_evals), _BATCH_FN(cb), None,
+                                             C.addressof(fb), counts, C.addressof(reason)), "gvqe_cobyla_minimize")
+    names = ("evals", "trust_steps", "geometry_steps", "rho_reductions", "rebuilds", "improvements")
+    return x, fb.value, dict(zip(names, list(counts))), reason.value
 
 
 def modularity(w, community, gamma: float = 1.0) -> float:

@@ -12,9 +12,9 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libgvqe.so")
-SOURCES = ["schedule.cpp", "lower.cpp", "hamiltonian.cpp", "graph.cpp", "driver.cpp", "jit.cpp", "jit_expect.cpp", "jit_rt.cpp", "gvqe_api.cpp",
+SOURCES = ["schedule.cpp", "lower.cpp", "hamiltonian.cpp", "graph.cpp", "cobyla.cpp", "driver.cpp", "jit.cpp", "jit_expect.cpp", "jit_rt.cpp", "gvqe_api.cpp",
            "kernels.cu", "expect.cu"]
-HEADERS = ["program.h", "devprog.h", "schedule.h", "lower.h", "hamiltonian.h", "graph.h", "kernels.h", "kernels.cuh", "jit.h", "jit_internal.h",
+HEADERS = ["program.h", "devprog.h", "schedule.h", "lower.h", "hamiltonian.h", "graph.h", "cobyla.h", "kernels.h", "kernels.cuh", "jit.h", "jit_internal.h",
            os.path.join("..", "..", "include", "gvqe.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]

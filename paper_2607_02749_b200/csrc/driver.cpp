@@ -2,13 +2,14 @@
 // public C ABI only: every energy and gradient comes from gvqe_energy_batch / gvqe_param_shift_grad, i.e. from the
 // sm_100a kernels.  PAPER.md:207-212 (Eq. 11: block-restricted objective), 214 (global refinement from the fused
 // block solution), 221-225 (Eq. 13, L-BFGS with f_tol, g_tol = 0.1 f_tol), 229-235 (four steps per epoch, Eq. 14
-// window criterion, epoch patience, warm start from theta*_best).
+// window criterion, epoch patience, warm start from theta*_best); 214, 221: COBYLA as the derivative-free choice (cobyla.cpp).
 #include <algorithm>
 #include <cmath>
 #include <deque>
 #include <vector>
 
 #include "../../include/gvqe.h"
+#include "cobyla.h"
 
 namespace {
 
@@ -128,7 +129,72 @@ gvqe_status minimize_masked(Run &r, std::vector<double> &theta, const std::vecto
     return GVQE_OK;
 }
 
+// COBYLA on the coordinates with mask != 0, all others frozen (Eq. 11), reading G8.  The first
+// simplex is one batch of n_active + 1 rows; afterwards one energy per step.  The Eq. 14 window criterion watches the
+// best energy after every evaluation, as in the L-BFGS loop.
+gvqe_status cobyla_masked(Run &r, std::vector<double> &theta, const std::vector<uint8_t> &mask, int max_iters, double *E_out)
+{
+    const int P = r.P;
+    std::vector<int> idx;
+    for (int p = 0; p < P; ++p) if (mask[p]) idx.push_back(p);
+    const int na = (int)idx.size();
+    std::vector<double> x((size_t)na), rows, Et;
+    for (int a = 0; a < na; ++a) x[a] = theta[idx[a]];
+    gvqe_status st = GVQE_OK;
+    const gv::CobylaFn f = [&](const double *pts, int B, double *out) {
+        rows.resize((size_t)B * std::max(P, 1));
+        for (int b = 0; b < B; ++b) {
+            for (int p = 0; p < P; ++p) rows[(size_t)b * P + p] = theta[p];
+            for (int a = 0; a < na; ++a) rows[(size_t)b * P + idx[a]] = pts[(size_t)b * na + a];
+        }
+        st = gvqe_energy_batch(r.ctx, rows.data(), B, out, r.stream);
+        r.evals += B;
+        return st == GVQE_OK;
+    };
+    if (max_iters <= 0 || na == 0) {   // phase switched off: the energy of the vector as it stands
+        rows.assign(theta.begin(), theta.end());
+        st = gvqe_energy_batch(r.ctx, rows.data(), 1, E_out, r.stream);
+        r.evals += 1;
+        return st;
+    }
+    gv::CobylaTrace tr;
+    int calm = 0;
+    const int W = r.opt->window, patience = r.opt->patience;
+    const double tol = r.opt->tol;
+    tr.monitor = [&](const std::vector<double> &h) {
+        calm = delta_max(h, W) < tol && (int)h.size() > W ? calm + 1 : 0;
+        return calm >= patience;
+    };
+    const double rho_beg = r.opt->rho_beg > 0.0 ? r.opt->rho_beg : 1.0;
+    const double rho_end = std::min(r.opt->tol, rho_beg);
+    const int rc = gv::cobyla_minimize(na, x.data(), rho_beg, rho_end, na + 1 + std::max(0, max_iters), f, &tr);
+    if (rc == -2) return st != GVQE_OK ? st : GVQE_ERR_CUDA;
+    if (rc < 0) return GVQE_ERR_INVALID_ARG;
+    for (int a = 0; a < na; ++a) theta[idx[a]] = x[a];
+    r.steps += tr.improvements;
+    *E_out = tr.f_best;
+    return GVQE_OK;
+}
+
 }  // namespace
+
+extern "C" gvqe_status gvqe_cobyla_minimize(int32_t n, double *x, double rho_beg, double rho_end, int32_t max_evals,
+                                            gvqe_batch_fn f, void *user, double *f_best, int32_t *counts, int32_t *reason)
+{
+    if (n < 0 || (n > 0 && !x) || !f || !(rho_beg > 0.0) || !(rho_end > 0.0) || rho_end > rho_beg || max_evals < 1)
+        return GVQE_ERR_INVALID_ARG;
+    gv::CobylaTrace tr;
+    const gv::CobylaFn fn = [&](const double *rows, int B, double *out) { return f(rows, B, out, user) == 0; };
+    const int rc = gv::cobyla_minimize(n, x, rho_beg, rho_end, max_evals, fn, &tr);
+    if (rc < 0) return GVQE_ERR_INVALID_ARG;
+    if (f_best) *f_best = tr.f_best;
+    if (counts) {
+        counts[0] = tr.evals; counts[1] = tr.trust_steps; counts[2] = tr.geometry_steps; counts[3] = tr.rho_reductions;
+        counts[4] = tr.rebuilds; counts[5] = tr.improvements;
+    }
+    if (reason) *reason = rc;
+    return GVQE_OK;
+}
 
 extern "C" gvqe_status gvqe_graph_vqe_minimize(gvqe_ctx *ctx, const gvqe_opt_options *opt, const int32_t *community,
                                                double *params, gvqe_opt_result *result, double *history,
@@ -138,8 +204,10 @@ extern "C" gvqe_status gvqe_graph_vqe_minimize(gvqe_ctx *ctx, const gvqe_opt_opt
     const int P = gvqe_num_params(ctx), n = gvqe_num_qubits(ctx);
     if (P > 0 && !params) return GVQE_ERR_INVALID_ARG;
     if (opt->max_epochs < 1 || opt->block_iters < 0 || opt->global_iters < 0 || opt->window < 1 || opt->patience < 1 ||
-        opt->epoch_patience < 1 || !(opt->tol > 0.0) || !(opt->f_tol >= 0.0))
+        opt->epoch_patience < 1 || !(opt->tol > 0.0) || !(opt->f_tol >= 0.0) || opt->optimizer < 0 || opt->optimizer > 1 ||
+        !(opt->rho_beg >= 0.0))
         return GVQE_ERR_INVALID_ARG;
+    const auto minimize = opt->optimizer == 1 ? cobyla_masked : minimize_masked;
     int K = 0;
     for (int q = 0; q < n; ++q) {
         if (community[q] < 0 || community[q] >= n) return GVQE_ERR_INVALID_ARG;
@@ -166,12 +234,12 @@ extern "C" gvqe_status gvqe_graph_vqe_minimize(gvqe_ctx *ctx, const gvqe_opt_opt
         for (int b = 0; b < K; ++b) {   // every block starts from the same vector; its own coordinates are fused
             theta = best;
             double Eb = 0.0;
-            st = minimize_masked(r, theta, masks[b], opt->block_iters, &Eb);
+            st = minimize(r, theta, masks[b], opt->block_iters, &Eb);
             if (st != GVQE_OK) return st;
             for (int p = 0; p < P; ++p) if (masks[b][p]) fused[p] = theta[p];
         }
         double E = 0.0;
-        if (opt->global_iters > 0) st = minimize_masked(r, fused, all, opt->global_iters, &E);
+        if (opt->global_iters > 0) st = minimize(r, fused, all, opt->global_iters, &E);
         else { st = gvqe_energy_batch(ctx, fused.data(), 1, &E, stream); r.evals += 1; }
         if (st != GVQE_OK) return st;
         if (history && hl < history_cap) history[hl++] = E;

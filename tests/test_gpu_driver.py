@@ -71,6 +71,52 @@ def test_variational_bound_and_oracle_agreement(orc, use_global):
         assert np.max(np.abs(dE)) < 5e-2 * max(1.0, np.max(np.abs(w.coeffs)))
 
 
+def test_cobyla_separable_closed_form():
+    """PAPER.md:221 "derivative-free (COBYLA)": the same separable problem with optimizer = "cobyla"; every block is one
+    parameter, the fused block solutions are the optimum -sum |a_q| (rho_end = tol = 1e-6 bounds the distance to it)."""
+    n = 6
+    a = np.array([1.0, -0.5, 2.0, 0.25, -1.5, 0.75])
+    paulis = "".join("".join("Z" if j == q else "I" for j in range(n)) for q in range(n))
+    g = gv.Gvqe(n, layout=dict(n_layers=0, entangler="cz", topology="linear"), precision="c128")
+    g.set_hamiltonian(paulis, a)
+    g.alloc_workspace(16)
+    r = SplitMix64(7)
+    theta0 = np.array([(2 * r.uniform() - 1) * 2.5 for _ in range(n)])
+    theta, res, hist = g.graph_vqe_minimize(theta0, list(range(n)), max_epochs=2, block_iters=200, global_iters=0,
+                                            optimizer="cobyla", tol=1e-6)
+    assert res["n_blocks"] == n and res["steps"] > 0
+    assert abs(res["E_best"] + np.sum(np.abs(a))) < 1e-9
+    assert np.all(np.abs(np.cos(theta) + np.sign(a)) < 1e-9)
+    # the whole vector at once (global phase only) reaches it too
+    theta, res, hist = g.graph_vqe_minimize(theta0, [0] * n, max_epochs=1, block_iters=0, global_iters=2000,
+                                            optimizer="cobyla", tol=1e-5, patience=10 ** 6)
+    assert abs(res["E_best"] + np.sum(np.abs(a))) < 1e-7
+
+
+def test_cobyla_variational_bound_and_oracle_agreement(orc):
+    """cfg 2 recipe shrunk to 8 qubits, 2 layers, c128, optimizer = "cobyla" in both phases: energies go down, stay above
+    the dense ground energy, and the returned vector has the returned energy (oracle T0).  No gradients are evaluated:
+    the evaluation count is the simplex sizes plus one per step."""
+    w = make_workload(2, n=8, M=60, D=2, batch=1)
+    g = ctx(w, in_flight=64)
+    lab = [0, 0, 0, 0, 1, 1, 1, 1]
+    E0 = g.energy_batch(w.theta)[0]
+    theta, res, hist = g.graph_vqe_minimize(w.theta, lab, max_epochs=2, block_iters=150, global_iters=300,
+                                            optimizer="cobyla", tol=1e-4, rho_beg=0.5)
+    H = dense_hamiltonian(w.n, w.pauli_list(), w.coeffs)
+    e_min = float(np.linalg.eigvalsh(H)[0])
+    assert res["E_best"] >= e_min - 1e-9
+    assert res["E_best"] < E0 - 0.1 * abs(E0 - e_min)
+    assert abs(hist[0] - E0) < 1e-12 and abs(res["E_best"] - min(hist)) < 1e-12
+    E_o = orc.energy_batch(w.n, w.ops, theta.reshape(1, -1), w.paulis, w.coeffs)[0]
+    assert abs(E_o - res["E_best"]) <= 1e-10 * abs(E_o) + 1e-12 * np.sum(np.abs(w.coeffs))
+    m0, m1 = g.block_param_mask(lab, 0), g.block_param_mask(lab, 1)
+    per_epoch_max = (int(m0.sum()) + 1 + 150) + (int(m1.sum()) + 1 + 150) + (w.P + 1 + 300)
+    assert 1 + res["epochs"] <= res["energy_evals"] <= 1 + res["epochs"] * per_epoch_max
+    with pytest.raises(gv.GvqeError):
+        g.graph_vqe_minimize(w.theta, lab, optimizer="cobyla", rho_beg=-1.0)
+
+
 def test_block_phase_touches_only_block_parameters():
     """One epoch, one block iteration budget, no global phase, a partition with an empty complement: parameters of
     qubits outside every optimised block keep their start values (Eq. 11: theta outside B_i is constant)."""
