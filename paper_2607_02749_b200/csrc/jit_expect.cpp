@@ -298,9 +298,11 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         // Tile-dependent tables, once per tile: T[e] = static[e] + sum over the group's index patterns p of S_p (-1)^{p.e},
         // S_p = the signed sum of the pattern's terms for this tile.  A group has few patterns (its terms' z masks inside
         // the index bits), so the sum is taken pattern by pattern instead of by a full Walsh-Hadamard transform: lane l
-        // holds the entries [l EP, (l + 1) EP); a pattern's sign over the lane bits is one parity, its S_p goes to the
-        // accumulator of its in-lane part, and a register Walsh-Hadamard over the in-lane bits (skipping what is known
-        // to be zero when the kernel is generated) finishes the entries.  No shuffles, no shared-memory butterflies.
+        // holds the entries l + 32 i (the LOW five index bits are the lane: neighbouring lanes read and write neighbouring
+        // entries -- with the entries [l EP, (l + 1) EP) per lane every store of a warp fell into the same banks, 32
+        // wavefronts per STS.128); a pattern's sign over the lane bits is one parity, its S_p goes to the accumulator of
+        // its in-lane part (the high index bits), and a register Walsh-Hadamard over the in-lane bits (skipping what is
+        // known to be zero when the kernel is generated) finishes the entries.  No shuffles, no shared-memory butterflies.
         E("        if (tile_id != cur_tile) {");
         E("        cur_tile = tile_id;");
         E("        for (unsigned t = tid; t < %uu; t += %uu) {   // one thread per term: its coefficient with this tile's sign", n_pterms, NT);
@@ -323,12 +325,12 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
             const DGroup &dg = plan.groups[q];
             const int ub = (int)dg.ubits, epl = ub > 5 ? ub - 5 : 0, EP = 1 << epl, nlb = ub - epl;
             E("        if (warp == %du%s) {   // group %u: %zu patterns over %d index bits", wi % 8, nlb < 5 ? (std::string(" && lane < ") + std::to_string(1u << nlb) + "u").c_str() : "", q - g0, G.pat_keys.size(), ub);
-            E("            const unsigned e0 = lane * %du;", EP);
+            E("            const unsigned e0 = lane;");
             E("            amp st[%d], A[%d];", EP, EP);
-            for (int i = 0; i < EP; ++i) E("            st[%d] = wst[%u + e0 + %d];", i, G.wst_off, i);
+            for (int i = 0; i < EP; ++i) E("            st[%d] = wst[%u + e0 + %d];", i, G.wst_off, i << nlb);
             std::vector<char> nz((size_t)EP, 0);
             for (size_t j = 0; j < G.pat_keys.size(); ++j) {
-                const uint32_t key = G.pat_keys[j], pl = key & (uint32_t)(EP - 1), ph = key >> epl;
+                const uint32_t key = G.pat_keys[j], pl = key >> nlb, ph = key & ((1u << nlb) - 1u);
                 std::string sx = "((const amp *)(smem + " + std::to_string(o_psum) + "))[" + std::to_string(G.pat_begin + j) + "]";
                 if (ph) sx = "sflip(" + sx + ", (unsigned)__popc(lane & " + std::to_string(ph) + "u) << 31)";
                 if (nz[pl]) E("            A[%u] = cadd(A[%u], %s);", pl, pl, sx.c_str());
@@ -344,8 +346,8 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
                 }
             for (int i = 0; i < EP; ++i) {
                 std::string v = nz[i] ? "cadd(A[" + std::to_string(i) + "], st[" + std::to_string(i) + "])" : "st[" + std::to_string(i) + "]";
-                if (G.mode == 1) E("            ((tw4 *)(smem + %u))[e0 + %d] = twfmt(%s);", G.tab_off, i, v.c_str());
-                else E("            ((amp *)(smem + %u))[e0 + %d] = %s;", G.tab_off, i, v.c_str());
+                if (G.mode == 1) E("            ((tw4 *)(smem + %u))[e0 + %d] = twfmt(%s);", G.tab_off, i << nlb, v.c_str());
+                else E("            ((amp *)(smem + %u))[e0 + %d] = %s;", G.tab_off, i << nlb, v.c_str());
             }
             E("        }");
             ++wi;

@@ -5,6 +5,7 @@ Tolerances (BASELINE.json north_star; reading A13):
   complex64 : |dE| <= max(1e-4 |E_oracle|, 1e-5 sum|c_k|)
 Masks / grouping are bit-exact (tests/test_host_logic.py, CPU)."""
 import math
+import re
 import os
 
 import numpy as np
@@ -346,6 +347,22 @@ def test_expectation_modes_agree(orc, prec):
     for no_rs in (False, True):
         g = ctx_for(w, prec, 3, options=dict(register_stages=1 if no_rs else 0, tile_bits=11))
         assert_close(prec, g.energy_batch(w.params), ref, w.coeffs, f"no_rs={no_rs}")
+
+
+@pytest.mark.parametrize("cfg,n,M,prec", [(5, 22, 5000, "c64"), (6, 18, 3000, "c128"), (6, 20, 5000, "c128")])
+def test_tile_dependent_tables_over_many_index_bits(orc, cfg, n, M, prec):
+    """Config-5 recipes (weight <= 6, terms across communities) shrunk to sizes the oracle finishes: their table slices have
+    terms with z bits outside the tile and 6-8 index bits, so the specialised passes rebuild tables of 64-256 entries per tile
+    (lane = low five index bits, register Walsh-Hadamard over the others).  Random angles, three rows, against oracle T1 (the
+    full Hamiltonian; Eq. 6)."""
+    w = make_workload(cfg, n=n, M=M, D=2, batch=3)
+    g = ctx_for(w, prec, 3, options=dict(specialise=2))
+    nb, npass, _ = g.schedule_info()
+    bits = [int(x) for i in range(nb, nb + npass) for x in re.findall(r"patterns over (\d+) index bits", g.kernel_source(i)[0])]
+    assert max(bits) >= 7
+    E = g.energy_batch(w.params)
+    ref = np.array([orc.t1_energy_of_state(w.n, orc.state(w.n, w.ops, w.params[b]), w.paulis, w.coeffs) for b in range(3)])
+    assert_close(prec, E, ref, w.coeffs, f"cfg{cfg} n={n}")
 
 
 # ---- schedule-specialised gate kernels (jit.cpp; PAPER.md:179 "JIT-compiled once and reused") ------------------------------
