@@ -126,6 +126,20 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     const uint32_t o_sv = take((n_pterms ? n_pterms : 1u) * 16u);     // per-tile signed coefficients of those terms (fp64 pairs)
     bool any_dyn = false;
     for (const GInfo &G : gi) any_dyn = any_dyn || G.dyn;
+    // The pass's tile-dependent terms and index patterns do not change from tile to tile: staged in shared memory once per
+    // thread block when that keeps two thread blocks on an SM (else read from global memory per tile).  With one statevector
+    // per tile (configs 5a / 5b) the table set-up is on every work item's critical path, and the two dependent global loads
+    // (term, then pattern) were a quarter of a pass.
+    constexpr uint32_t SMEM_TWO_BLOCKS = (233472u / 2u) - 1024u;
+    bool staged = false;
+    uint32_t o_terms = 0, o_pats = 0;
+    if (any_dyn && n_pterms && n_pats) {
+        const uint32_t before = sm;
+        o_terms = take(n_pterms * 24u);
+        o_pats = take(n_pats * 16u);
+        if (sm <= SMEM_TWO_BLOCKS || before > SMEM_TWO_BLOCKS) staged = true;
+        else sm = before;
+    }
     data.pass_wst_off.push_back((uint32_t)wst_base);
     data.pass_pat_off.push_back((uint32_t)pat_base);
     data.pass_pat_cnt.push_back(n_pats);
@@ -141,6 +155,7 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
     E("typedef %s tabt;", TT);
     E("struct __align__(16) Pat { unsigned dst, begin, end, pad; };");
     E("struct __align__(32) Term { double cr, ci; u64 zout, pad; };");
+    E("struct __align__(8) TermS { double cr, ci; u64 zout; };   // a term as staged in shared memory");
     if (prec == 0) {
         E("struct __align__(16) tw4 { float x, y, z, w; };   // (Wx, -Wy, Wy, Wx)");
         E("__device__ __forceinline__ tw4 twfmt(amp w) { tw4 t; t.x = w.x; t.y = -w.y; t.z = w.y; t.w = w.x; return t; }");
@@ -241,6 +256,11 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         if (G.mode != 0 || G.dyn) continue;
         E("    for (unsigned e = tid; e < %uu; e += %uu) ((amp *)(smem + %u))[e] = wst[%u + e];", G.E, NT, G.tab_off, G.wst_off);
     }
+    if (staged) {
+        E("    for (unsigned t = tid; t < %uu; t += %uu) { const Term tm = terms[%zuu + t]; TermS ts; ts.cr = tm.cr; ts.ci = tm.ci; ts.zout = tm.zout; ((TermS *)(smem + %u))[t] = ts; }", n_pterms, NT, term_base, o_terms);
+        E("    for (unsigned i = tid; i < %uu; i += %uu) ((Pat *)(smem + %u))[i] = pats[i];", n_pats, NT, o_pats);
+        E("    __syncthreads();");
+    }
     E("    const unsigned ld_off = OFF(tid << %d);", g.lv);
     {
         std::string sx = "    const u64 ld_x = 0ull";
@@ -306,13 +326,15 @@ bool jit_expect_generate(const ExpectPlan &plan, int n, int prec, int pi, JitExp
         E("        if (tile_id != cur_tile) {");
         E("        cur_tile = tile_id;");
         E("        for (unsigned t = tid; t < %uu; t += %uu) {   // one thread per term: its coefficient with this tile's sign", n_pterms, NT);
-        E("            const Term tm = terms[%zuu + t];", term_base);
+        if (staged) E("            const TermS tm = ((const TermS *)(smem + %u))[t];", o_terms);
+        else E("            const Term tm = terms[%zuu + t];", term_base);
         E("            const bool neg = __popcll(xbase & tm.zout) & 1;");
         E("            ((double2 *)(smem + %u))[t] = make_double2(neg ? -tm.cr : tm.cr, neg ? -tm.ci : tm.ci);", o_sv);
         E("        }");
         E("        __syncthreads();");
         E("        for (unsigned i = tid; i < %uu; i += %uu) {   // one thread per (group, index pattern): sum of its terms, in their order", n_pats, NT);
-        E("            const Pat p = pats[i];");
+        if (staged) E("            const Pat p = ((const Pat *)(smem + %u))[i];", o_pats);
+        else E("            const Pat p = pats[i];");
         E("            double sr = 0.0, si = 0.0;");
         E("            for (unsigned t = p.begin; t < p.end; ++t) { const double2 v = ((const double2 *)(smem + %u))[t - %zuu]; sr += v.x; si += v.y; }", o_sv, term_base);
         E("            ((amp *)(smem + %u))[i] = MK((real)sr, (real)si);", o_psum);
